@@ -1,0 +1,345 @@
+// ORACLE — TEST INFRASTRUCTURE ONLY.
+//
+// A plain, slow, obviously-correct CPU statement of what the combinatorial Hamiltonian kernel of
+// arxiv 2601.21310 computes ("Evaluates Slater-Condon rules on integer representations of
+// configurations to construct the Hamiltonian connectivity graphs").  Only tests/, __graft_entry__.smoke()
+// and bench.py's cpu_baseline / --impl reference legs may load this file; the product path never does.
+// It shares no code with paper_2601_21310_b200/csrc (no headers, helpers, tables or constants).
+//
+// What it states (each function cites the passage it follows; readings Q1..Q16 are listed in DESIGN.md):
+//   * H = E_core + sum h_pq a+_p a_q + 1/2 sum (pq|rs) a+_p a+_r a_s a_q  on FCIDUMP-style integrals
+//     (PAPER.md:231, 256).  Determinant |D> = prod_{p in alpha, ascending} a+_{p,alpha}
+//     prod_{q in beta, ascending} a+_{q,beta} |0>   (reading Q1).
+//   * connected set, Eq. 1: every single and double excitation D' of D with H_{D'D} != 0.
+//   * heat-bath screening, Eq. 14 and the tau rule: the sorted lists + early exit of the
+//     paper reach exactly { D' : |H_{D'D}| >= tau }, so the oracle is that definition: enumerate every
+//     excitation, evaluate it, filter by magnitude.  No sorted lists, no early exit here.
+//   * H_VV in CSR, E_var Eq. 11, PT2 external term Eq. 13.
+//
+// Parity pins (tests/test_oracle_pins.py): P1 explicit second-quantised operator application, P2 dense FCI
+// eigenvalue bound, P3 bitwise symmetry, P4 eps=0 == unscreened, P5 closed-form counts, P6 PT2 = 0 on the
+// full space, P7 two-electron closed forms, P8 dense brute-force PT2, P9 sum rule, P10 spin-swap symmetry and
+// the textbook Epstein-Nesbet energy of a single reference.  Every function below is pinned by at least one.
+//
+// Build: g++ -O2 -std=c++17 -fopenmp -ffp-contract=off -shared -fPIC oracle.cpp -o liboracle.so
+#include <algorithm>
+#include <cmath>
+#include <cstdint>
+#include <cstring>
+#include <vector>
+#ifdef _OPENMP
+#include <omp.h>
+#endif
+
+namespace {
+
+typedef uint64_t u64;
+
+struct Integrals {
+  int n;
+  const double* h1;   // [n*n]
+  const double* eri;  // packed 8-fold, reading Q3
+  double e_core;
+};
+
+inline int64_t tri(int64_t x, int64_t y) { return x >= y ? x * (x + 1) / 2 + y : y * (y + 1) / 2 + x; }
+// chemist-notation (pq|rs)
+inline double eri(const Integrals& I, int p, int q, int r, int s) { return I.eri[tri(tri(p, q), tri(r, s))]; }
+inline double h(const Integrals& I, int p, int q) { return I.h1[p * I.n + q]; }
+inline bool occ(u64 w, int p) { return (w >> p) & 1ull; }
+
+struct Det { u64 a, b; };
+inline bool operator<(const Det& x, const Det& y) { return x.a != y.a ? x.a < y.a : x.b < y.b; }
+inline bool operator==(const Det& x, const Det& y) { return x.a == y.a && x.b == y.b; }
+
+// diag(D) = E_core + sum_{p occ} h_pp + 1/2 sum_{sigma,tau} sum_{p in sigma, q in tau} [(pp|qq) - delta (pq|qp)]
+double diagonal(const Integrals& I, Det d) {
+  double e = I.e_core;
+  for (int p = 0; p < I.n; ++p) {
+    if (occ(d.a, p)) e += h(I, p, p);
+    if (occ(d.b, p)) e += h(I, p, p);
+  }
+  double two = 0.0;
+  for (int p = 0; p < I.n; ++p)
+    for (int q = 0; q < I.n; ++q) {
+      if (occ(d.a, p) && occ(d.a, q)) two += eri(I, p, p, q, q) - eri(I, p, q, q, p);
+      if (occ(d.b, p) && occ(d.b, q)) two += eri(I, p, p, q, q) - eri(I, p, q, q, p);
+      if (occ(d.a, p) && occ(d.b, q)) two += eri(I, p, p, q, q);
+      if (occ(d.b, p) && occ(d.a, q)) two += eri(I, p, p, q, q);
+    }
+  return e + 0.5 * two;
+}
+
+// (-1)^(number of electrons of the same spin string strictly between orbitals i and a)   (reading Q1)
+int single_phase(u64 w, int i, int a) {
+  int lo = std::min(i, a), hi = std::max(i, a), c = 0;
+  for (int p = lo + 1; p < hi; ++p) c += occ(w, p);
+  return (c & 1) ? -1 : 1;
+}
+
+// single i -> a in the spin string `same` (other string `other`), evaluation order fixed by reading Q7:
+// h_ia, then ((ia|qq) - (iq|qa)) for same-spin occupied q ascending, then (ia|qq) for other-spin occupied q ascending.
+double single_value(const Integrals& I, u64 same, u64 other, int i, int a) {
+  double v = h(I, i, a);
+  for (int q = 0; q < I.n; ++q)
+    if (occ(same, q)) v = v + (eri(I, i, a, q, q) - eri(I, i, q, q, a));
+  for (int q = 0; q < I.n; ++q)
+    if (occ(other, q)) v = v + eri(I, i, a, q, q);
+  return v * single_phase(same, i, a);
+}
+
+// same-spin double i<j -> a<b: a+_a a+_b a_j a_i = (a+_b a_j)(a+_a a_i); value (ia|jb) - (ib|ja)  (reading Q7)
+double same_double_value(const Integrals& I, u64 w, int i, int j, int a, int b) {
+  int ph = single_phase(w, i, a);
+  u64 w1 = (w & ~(1ull << i)) | (1ull << a);
+  ph *= single_phase(w1, j, b);
+  return (eri(I, i, a, j, b) - eri(I, i, b, j, a)) * ph;
+}
+
+// opposite-spin double i(alpha)->a, j(beta)->b: value (ia|jb), phase = product of the two single phases
+double opp_double_value(const Integrals& I, Det d, int i, int a, int j, int b) {
+  return eri(I, i, a, j, b) * (single_phase(d.a, i, a) * single_phase(d.b, j, b));
+}
+
+struct Conn { Det d; double h; };
+
+// conn(D, tau) = { (D', H_{D'D}) : D' single or double excitation of D, |H| >= tau, H != 0 }  (Eq. 1, Eq. 14; Q5, Q6, Q8)
+// Also counts every orbital-valid excitation visited (closed-form pin P5).
+int64_t connections(const Integrals& I, Det d, double tau, std::vector<Conn>* out) {
+  const int n = I.n;
+  int64_t visited = 0;
+  auto keep = [&](Det x, double v) {
+    ++visited;
+    if (v != 0.0 && std::fabs(v) >= tau && out) out->push_back({x, v});
+  };
+  // singles
+  for (int i = 0; i < n; ++i) for (int a = 0; a < n; ++a) {
+    if (occ(d.a, i) && !occ(d.a, a)) keep({(d.a ^ (1ull << i)) | (1ull << a), d.b}, single_value(I, d.a, d.b, i, a));
+    if (occ(d.b, i) && !occ(d.b, a)) keep({d.a, (d.b ^ (1ull << i)) | (1ull << a)}, single_value(I, d.b, d.a, i, a));
+  }
+  // same-spin doubles
+  for (int i = 0; i < n; ++i) for (int j = i + 1; j < n; ++j)
+    for (int a = 0; a < n; ++a) for (int b = a + 1; b < n; ++b) {
+      if (occ(d.a, i) && occ(d.a, j) && !occ(d.a, a) && !occ(d.a, b))
+        keep({(d.a ^ (1ull << i) ^ (1ull << j)) | (1ull << a) | (1ull << b), d.b}, same_double_value(I, d.a, i, j, a, b));
+      if (occ(d.b, i) && occ(d.b, j) && !occ(d.b, a) && !occ(d.b, b))
+        keep({d.a, (d.b ^ (1ull << i) ^ (1ull << j)) | (1ull << a) | (1ull << b)}, same_double_value(I, d.b, i, j, a, b));
+    }
+  // opposite-spin doubles
+  for (int i = 0; i < n; ++i) if (occ(d.a, i))
+    for (int a = 0; a < n; ++a) if (!occ(d.a, a))
+      for (int j = 0; j < n; ++j) if (occ(d.b, j))
+        for (int b = 0; b < n; ++b) if (!occ(d.b, b))
+          keep({(d.a ^ (1ull << i)) | (1ull << a), (d.b ^ (1ull << j)) | (1ull << b)}, opp_double_value(I, d, i, a, j, b));
+  if (out) std::sort(out->begin(), out->end(), [](const Conn& x, const Conn& y) { return x.d < y.d; });
+  return visited;
+}
+
+// General Slater-Condon element <X|H|Y> found from the two bitstrings alone (used by the dense-matrix pins).
+double element(const Integrals& I, Det x, Det y) {
+  int da = __builtin_popcountll(x.a ^ y.a) / 2, db = __builtin_popcountll(x.b ^ y.b) / 2;
+  if (da + db == 0) return diagonal(I, y);
+  if (da + db > 2) return 0.0;
+  auto holes = [](u64 from, u64 to, int* o) { int k = 0; for (int p = 0; p < 64; ++p) if (occ(from, p) && !occ(to, p)) o[k++] = p; };
+  int ia[2], aa[2], ib[2], ab[2];
+  holes(y.a, x.a, ia); holes(x.a, y.a, aa); holes(y.b, x.b, ib); holes(x.b, y.b, ab);
+  if (da == 1 && db == 0) return single_value(I, y.a, y.b, ia[0], aa[0]);
+  if (da == 0 && db == 1) return single_value(I, y.b, y.a, ib[0], ab[0]);
+  if (da == 2) return same_double_value(I, y.a, ia[0], ia[1], aa[0], aa[1]);
+  if (db == 2) return same_double_value(I, y.b, ib[0], ib[1], ab[0], ab[1]);
+  return opp_double_value(I, y, ia[0], aa[0], ib[0], ab[0]);
+}
+
+// Partition function for multi-pass PT2 (reading Q14): class = low bits of the XOR of per-orbital 64-bit words
+// z_alpha[p] (p in alpha) and z_beta[q] (q in beta); the words are splitmix64(seed + index) written out here.
+u64 splitmix64(u64 x) {
+  x += 0x9E3779B97F4A7C15ull;
+  x = (x ^ (x >> 30)) * 0xBF58476D1CE4E5B9ull;
+  x = (x ^ (x >> 27)) * 0x94D049BB133111EBull;
+  return x ^ (x >> 31);
+}
+u64 zobrist(Det d) {
+  const u64 seed = 260121310ull;
+  u64 z = 0;
+  for (int p = 0; p < 64; ++p) {
+    if (occ(d.a, p)) z ^= splitmix64(seed + p);
+    if (occ(d.b, p)) z ^= splitmix64(seed + 64 + p);
+  }
+  return z;
+}
+
+struct Csr { std::vector<int64_t> row_ptr; std::vector<int32_t> col; std::vector<double> val; };
+
+}  // namespace
+
+extern "C" {
+
+double orc_diagonal(int n, const double* h1, const double* eri_, double e_core, const u64* det) {
+  Integrals I{n, h1, eri_, e_core};
+  return diagonal(I, {det[0], det[1]});
+}
+
+double orc_element(int n, const double* h1, const double* eri_, double e_core, const u64* x, const u64* y) {
+  Integrals I{n, h1, eri_, e_core};
+  return element(I, {x[0], x[1]}, {y[0], y[1]});
+}
+
+// One source's screened connection list, sorted by key.  Returns the number kept (may exceed cap; only cap are
+// written); *visited_out = number of orbital-valid excitations enumerated.
+int64_t orc_connections(int n, const double* h1, const double* eri_, double e_core, const u64* det, double tau,
+                        u64* keys_out, double* h_out, int64_t cap, int64_t* visited_out) {
+  Integrals I{n, h1, eri_, e_core};
+  std::vector<Conn> c;
+  int64_t vis = connections(I, {det[0], det[1]}, tau, &c);
+  if (visited_out) *visited_out = vis;
+  for (int64_t k = 0; k < (int64_t)c.size() && k < cap; ++k) {
+    keys_out[2 * k] = c[k].d.a; keys_out[2 * k + 1] = c[k].d.b; h_out[k] = c[k].h;
+  }
+  return (int64_t)c.size();
+}
+
+// Dense <D_r|H|D_c> over a list of determinants (dense-matrix pins only; O(nd^2) element() calls).
+void orc_dense(int n, const double* h1, const double* eri_, double e_core, const u64* dets, int64_t nd, double* out) {
+  Integrals I{n, h1, eri_, e_core};
+  const Det* S = reinterpret_cast<const Det*>(dets);
+#pragma omp parallel for schedule(dynamic, 8)
+  for (int64_t r = 0; r < nd; ++r)
+    for (int64_t c = 0; c < nd; ++c) out[r * nd + c] = element(I, S[r], S[c]);
+}
+
+u64 orc_zobrist(const u64* det) { return zobrist({det[0], det[1]}); }
+
+// ham_build (reading Q4): row i = {(i, diag(D_i))} U {(j, H) : (D_j, H) in conn(D_i, eps), D_j in S}, columns ascending.
+// Returns an opaque handle; read it with orc_csr_nnz / orc_csr_copy, free with orc_csr_free.
+void* orc_ham_build(int n, const double* h1, const double* eri_, double e_core, const u64* dets, int64_t nd, double eps) {
+  Integrals I{n, h1, eri_, e_core};
+  const Det* S = reinterpret_cast<const Det*>(dets);
+  std::vector<std::vector<std::pair<int32_t, double>>> rows(nd);
+#pragma omp parallel for schedule(dynamic, 16)
+  for (int64_t i = 0; i < nd; ++i) {
+    std::vector<Conn> c;
+    connections(I, S[i], eps, &c);
+    auto& r = rows[i];
+    r.push_back({(int32_t)i, diagonal(I, S[i])});
+    for (const Conn& x : c) {
+      const Det* it = std::lower_bound(S, S + nd, x.d);
+      if (it != S + nd && *it == x.d) r.push_back({(int32_t)(it - S), x.h});
+    }
+    std::sort(r.begin(), r.end(), [](auto& x, auto& y) { return x.first < y.first; });
+  }
+  Csr* m = new Csr;
+  m->row_ptr.assign(nd + 1, 0);
+  for (int64_t i = 0; i < nd; ++i) m->row_ptr[i + 1] = m->row_ptr[i] + (int64_t)rows[i].size();
+  m->col.reserve(m->row_ptr[nd]); m->val.reserve(m->row_ptr[nd]);
+  for (int64_t i = 0; i < nd; ++i) for (auto& e : rows[i]) { m->col.push_back(e.first); m->val.push_back(e.second); }
+  return m;
+}
+int64_t orc_csr_nnz(void* hnd) { return (int64_t)static_cast<Csr*>(hnd)->col.size(); }
+void orc_csr_copy(void* hnd, int64_t* row_ptr, int32_t* col, double* val) {
+  Csr* m = static_cast<Csr*>(hnd);
+  std::memcpy(row_ptr, m->row_ptr.data(), m->row_ptr.size() * sizeof(int64_t));
+  std::memcpy(col, m->col.data(), m->col.size() * sizeof(int32_t));
+  std::memcpy(val, m->val.data(), m->val.size() * sizeof(double));
+}
+void orc_csr_free(void* hnd) { delete static_cast<Csr*>(hnd); }
+
+// energy, Eq. 11: y = H psi, E = psi^T y / psi^T psi; accumulated in long double.
+void orc_energy(int64_t nd, const int64_t* row_ptr, const int32_t* col, const double* val, const double* psi,
+                double* e_out, double* norm2_out, double* y_out) {
+  long double num = 0, den = 0;
+  for (int64_t i = 0; i < nd; ++i) {
+    long double y = 0;
+    for (int64_t k = row_ptr[i]; k < row_ptr[i + 1]; ++k) y += (long double)val[k] * psi[col[k]];
+    if (y_out) y_out[i] = (double)y;
+    num += y * psi[i];
+    den += (long double)psi[i] * psi[i];
+  }
+  *e_out = (double)(num / den);
+  if (norm2_out) *norm2_out = (double)den;
+}
+
+// pt2, Eq. 13 second term with the screened sum of readings Q6, Q9, Q10:
+//   for each source i with psi_i != 0: tau_i = eps2/|psi_i| (0 when eps2 == 0); for (D_a, H) in conn(D_i, tau_i),
+//   D_a not in S: v_a += H psi_i.   dE = (1/psi^T psi) sum_a v_a^2 / (E_S - diag(D_a)).
+// Externals are processed partition by partition (class = zobrist & (n_parts-1), n_parts a power of two); only
+// classes in [part_begin, part_end) are accumulated by this call, so a caller can bound memory by looping over
+// class ranges and adding the results.  part_sums[n_parts] (may be NULL) receives each processed partition's
+// partial sum (already / psi^T psi).
+// Also returns sum_abs = sum |t_a| / psi^T psi and min_abs_den = min_a |E_S - H_aa| (conditioning report, Q11).
+void orc_pt2(int n, const double* h1, const double* eri_, double e_core, const u64* dets, int64_t nd,
+             const double* psi, double e_s, double eps2, int n_parts, int part_begin, int part_end,
+             double* pt2_out, int64_t* n_external_out,
+             int64_t* n_contrib_out, double* part_sums, double* sum_abs_out, double* min_abs_den_out) {
+  Integrals I{n, h1, eri_, e_core};
+  const Det* S = reinterpret_cast<const Det*>(dets);
+  long double norm2 = 0;
+  for (int64_t i = 0; i < nd; ++i) norm2 += (long double)psi[i] * psi[i];
+  long double total = 0, total_abs = 0;
+  double min_den = INFINITY;
+  int64_t n_ext = 0, n_contrib = 0;
+  // enumerate once per source, bucket the kept external contributions by partition
+  std::vector<std::vector<std::pair<Det, double>>> parts(n_parts);
+#ifdef _OPENMP
+  int nthreads = omp_get_max_threads();
+#else
+  int nthreads = 1;
+#endif
+  std::vector<std::vector<std::vector<std::pair<Det, double>>>> local(nthreads, parts);
+#pragma omp parallel
+  {
+#ifdef _OPENMP
+    int t = omp_get_thread_num();
+#else
+    int t = 0;
+#endif
+#pragma omp for schedule(dynamic, 8)
+    for (int64_t i = 0; i < nd; ++i) {
+      if (psi[i] == 0.0) continue;  // reading Q6
+      double tau = eps2 == 0.0 ? 0.0 : eps2 / std::fabs(psi[i]);
+      std::vector<Conn> c;
+      connections(I, S[i], tau, &c);
+      for (const Conn& x : c) {
+        if (std::binary_search(S, S + nd, x.d)) continue;  // P = C \ V
+        int cls = (int)(zobrist(x.d) & (u64)(n_parts - 1));
+        if (cls < part_begin || cls >= part_end) continue;
+        local[t][cls].push_back({x.d, x.h * psi[i]});
+      }
+    }
+  }
+  for (int p = part_begin; p < part_end; ++p) {
+    auto& v = parts[p];
+    for (int t = 0; t < nthreads; ++t) { v.insert(v.end(), local[t][p].begin(), local[t][p].end()); std::vector<std::pair<Det, double>>().swap(local[t][p]); }
+    n_contrib += (int64_t)v.size();
+    std::sort(v.begin(), v.end(), [](auto& x, auto& y) { return x.first < y.first || (x.first == y.first && x.second < y.second); });
+    long double psum = 0;
+    for (size_t k = 0; k < v.size();) {
+      size_t e = k;
+      long double va = 0;
+      while (e < v.size() && v[e].first == v[k].first) va += v[e++].second;
+      double den = e_s - diagonal(I, v[k].first);
+      long double t = va * va / den;
+      psum += t; total_abs += fabsl(t);
+      min_den = std::min(min_den, std::fabs(den));
+      ++n_ext;
+      k = e;
+    }
+    if (part_sums) part_sums[p] = (double)(psum / norm2);
+    total += psum;
+    std::vector<std::pair<Det, double>>().swap(v);
+  }
+  *pt2_out = (double)(total / norm2);
+  if (n_external_out) *n_external_out = n_ext;
+  if (n_contrib_out) *n_contrib_out = n_contrib;
+  if (sum_abs_out) *sum_abs_out = (double)(total_abs / norm2);
+  if (min_abs_den_out) *min_abs_den_out = min_den;
+}
+
+int orc_num_threads(void) {
+#ifdef _OPENMP
+  return omp_get_max_threads();
+#else
+  return 1;
+#endif
+}
+
+}  // extern "C"

@@ -1,0 +1,234 @@
+"""Pins P1-P10: the oracle checked against things other than itself.
+
+The paper prints no worked example of this path (no element, list or PT2 value; its energies need FCIDUMP files and
+trained amplitudes that are not available), so the pins are brute force, closed forms, invariants and library routines.
+"""
+import itertools
+from math import comb
+
+import numpy as np
+import pytest
+import scipy.sparse as sp
+
+from synth_inputs import make_problem, CONFIGS
+from helpers import full_space, dense_eri, small_integrals, second_quantised_dense
+
+
+# ---------------------------------------------------------------- P1: explicit second quantisation
+@pytest.mark.parametrize("n,na,nb,seed", [(4, 2, 2, 11), (5, 3, 2, 12), (5, 1, 3, 13), (6, 3, 3, 14)])
+def test_p1_slater_condon_equals_operator_application(orc, n, na, nb, seed):
+    h1, eri = small_integrals(n, seed)
+    dets = full_space(n, na, nb)
+    H_sq = second_quantised_dense(n, h1, dense_eri(n, eri), dets, e_core=0.37)
+    H_or = orc.dense(n, h1, eri, 0.37, dets)
+    assert np.allclose(H_or, H_sq, rtol=0, atol=1e-12)
+    assert np.abs(H_sq).max() > 0.5  # not vacuous
+    # signs matter: there must be negative and positive phases among equal-magnitude integrals
+    assert (H_sq < -1e-3).any() and (H_sq > 1e-3).any()
+
+
+def test_p1b_enumeration_equals_bitstring_difference(orc):
+    """connections() (enumerate excitations) against element() (difference of two bitstrings) on a full space."""
+    n, na, nb = 6, 3, 2
+    h1, eri = small_integrals(n, 21)
+    dets = full_space(n, na, nb)
+    H = orc.dense(n, h1, eri, 0.0, dets)
+    index = {(int(a), int(b)): k for k, (a, b) in enumerate(dets)}
+    for c, d in enumerate(dets):
+        keys, hv, visited = orc.connections(n, h1, eri, 0.0, d, 0.0)
+        col = np.zeros(len(dets))
+        for (a, b), v in zip(keys, hv):
+            col[index[(int(a), int(b))]] = v
+        ref = H[:, c].copy(); ref[c] = 0.0
+        assert np.array_equal(col, ref)
+        assert len(keys) == len(set(map(tuple, keys.tolist())))
+        assert all(tuple(keys[k]) < tuple(keys[k + 1]) for k in range(len(keys) - 1))  # sorted by (alpha, beta)
+
+
+# ---------------------------------------------------------------- P2: variational bound / library eigensolver
+def test_p2_energy_bounded_by_fci_ground_state(orc):
+    n, na, nb = 6, 3, 3
+    h1, eri = small_integrals(n, 31)
+    dets = full_space(n, na, nb)
+    assert len(dets) == 400
+    H = orc.dense(n, h1, eri, 0.1, dets)
+    w, V = np.linalg.eigh(H)
+    rng = np.random.default_rng(5)
+    for trial in range(5):
+        idx = np.sort(rng.choice(400, size=60, replace=False))
+        psi = rng.standard_normal(60)
+        rp, col, val = orc.ham_build(n, h1, eri, 0.1, dets[idx], 0.0)
+        e, n2 = orc.energy(rp, col, val, psi)
+        assert e >= w[0] - 1e-12
+        assert np.isclose(n2, psi @ psi, rtol=1e-14)
+        assert np.isclose(e, psi @ H[np.ix_(idx, idx)] @ psi / (psi @ psi), rtol=1e-12)
+    rp, col, val = orc.ham_build(n, h1, eri, 0.1, dets, 0.0)
+    e, _ = orc.energy(rp, col, val, V[:, 0])
+    assert np.isclose(e, w[0], rtol=1e-12)
+    # E_diag = lambda_min(H_VV) <= E_var
+    A = sp.csr_matrix((val, col, rp), shape=(400, 400)).toarray()
+    assert np.array_equal(A, H)  # CSR at eps=0 is the dense matrix (no exact zeros among stored entries)
+
+
+# ---------------------------------------------------------------- P3: Hermiticity, bitwise
+@pytest.mark.parametrize("eps", [0.0, 1e-3, 5e-2])
+def test_p3_csr_bitwise_symmetric(orc, eps):
+    p = make_problem("tiny", n_dets=600)
+    rp, col, val = orc.ham_build(p["n"], p["h1"], p["eri"], 0.0, p["dets"], eps)
+    A = sp.csr_matrix((val, col, rp), shape=(600, 600))
+    At = A.T.tocsr(); At.sort_indices()
+    assert np.array_equal(A.indptr, At.indptr) and np.array_equal(A.indices, At.indices)
+    assert np.array_equal(A.data, At.data)  # bit-for-bit (H_PV = H_VP^T)
+    for i in range(600):  # columns ascending, diagonal always present, screen respected
+        c = col[rp[i]:rp[i + 1]]; v = val[rp[i]:rp[i + 1]]
+        assert np.all(np.diff(c) > 0) and i in c
+        off = v[c != i]
+        assert np.all(np.abs(off) >= eps) and np.all(off != 0.0)
+
+
+# ---------------------------------------------------------------- P4 / P5: eps=0 == unscreened, closed-form counts
+@pytest.mark.parametrize("name", ["tiny", "h2o", "n2", "cr2"])
+def test_p5_visit_count_closed_form(orc, name):
+    c = CONFIGS[name]
+    n, na, nb = c["n"], c["na"], c["nb"]
+    expected = (na * (n - na) + nb * (n - nb) + comb(na, 2) * comb(n - na, 2) + comb(nb, 2) * comb(n - nb, 2)
+                + na * nb * (n - na) * (n - nb))
+    assert expected == {"tiny": 875, "h2o": 12635, "n2": 30723, "cr2": 404712}[name]
+    from synth_inputs import make_integrals, BASE_SEED
+    h1, eri = make_integrals(n, c["L"], BASE_SEED + c["index"], band=c["band"])
+    rng = np.random.default_rng(3)
+    for _ in range(2):
+        a = sum(1 << int(q) for q in rng.choice(n, na, replace=False))
+        b = sum(1 << int(q) for q in rng.choice(n, nb, replace=False))
+        keys, hv, visited = orc.connections(n, h1, eri, 0.0, np.array([a, b], dtype=np.uint64), 0.0)
+        assert visited == expected
+        assert len(keys) == expected  # P4: tau = 0 keeps everything (random integrals: no exact zeros)
+        keys2, hv2, _ = orc.connections(n, h1, eri, 0.0, np.array([a, b], dtype=np.uint64), 1e-2)
+        kept = np.abs(hv) >= 1e-2
+        assert np.array_equal(keys2, keys[kept]) and np.array_equal(hv2, hv[kept])
+
+
+# ---------------------------------------------------------------- P6: PT2 vanishes on the full space
+def test_p6_pt2_zero_on_full_space(orc):
+    n, na, nb = 6, 3, 2
+    h1, eri = small_integrals(n, 41)
+    dets = full_space(n, na, nb)
+    psi = np.random.default_rng(1).standard_normal(len(dets))
+    r = orc.pt2(n, h1, eri, 0.0, dets, psi, -3.0, 0.0)
+    assert r["pt2"] == 0.0 and r["n_external"] == 0 and r["n_contrib"] == 0
+
+
+# ---------------------------------------------------------------- P7: textbook closed forms
+def test_p7_two_electrons_two_orbitals(orc):
+    h1, eri = small_integrals(2, 51)
+    g = dense_eri(2, eri)
+    J = lambda p, q: g[p, p, q, q]
+    K = lambda p, q: g[p, q, q, p]
+    d11 = np.array([1, 1], dtype=np.uint64); d22 = np.array([2, 2], dtype=np.uint64)
+    assert np.isclose(orc.element(2, h1, eri, 0.0, d11, d11), 2 * h1[0, 0] + J(0, 0), rtol=1e-14)
+    assert np.isclose(orc.element(2, h1, eri, 0.0, d22, d22), 2 * h1[1, 1] + J(1, 1), rtol=1e-14)
+    assert orc.element(2, h1, eri, 0.0, d22, d11) == K(0, 1)
+    assert orc.element(2, h1, eri, 0.0, d11, d22) == K(0, 1)
+    # open-shell pair |1a 2b>, |2a 1b>: diagonal h11 + h22 + J12, coupling -K12 in this ordering... sign by P1;
+    # the singlet/triplet eigenvalues h11+h22+J12 +- K12 are convention-free:
+    d12 = np.array([1, 2], dtype=np.uint64); d21 = np.array([2, 1], dtype=np.uint64)
+    M = np.array([[orc.element(2, h1, eri, 0.0, x, y) for y in (d12, d21)] for x in (d12, d21)])
+    ev = np.linalg.eigvalsh(M)
+    base = h1[0, 0] + h1[1, 1] + J(0, 1)
+    assert np.allclose(sorted(ev), sorted([base - K(0, 1), base + K(0, 1)]), rtol=1e-13)
+
+
+def test_p7b_closed_shell_hf_energy(orc):
+    n, nocc = 7, 3
+    h1, eri = small_integrals(n, 52)
+    g = dense_eri(n, eri)
+    e = 0.25 + 2 * sum(h1[i, i] for i in range(nocc)) + sum(
+        2 * g[i, i, j, j] - g[i, j, j, i] for i in range(nocc) for j in range(nocc))
+    hf = np.array([(1 << nocc) - 1] * 2, dtype=np.uint64)
+    assert np.isclose(orc.diagonal(n, h1, eri, 0.25, hf), e, rtol=1e-14)
+
+
+# ---------------------------------------------------------------- P8 / P9: dense brute-force PT2 and the sum rule
+@pytest.mark.parametrize("eps2", [0.0, 1e-3, 2e-2])
+def test_p8_pt2_dense_brute_force(orc, eps2):
+    n, na, nb = 7, 3, 3
+    h1, eri = small_integrals(n, 61)
+    dets = full_space(n, na, nb)  # 1225
+    H = orc.dense(n, h1, eri, 0.0, dets)
+    rng = np.random.default_rng(8)
+    idx = np.sort(rng.choice(len(dets), size=150, replace=False))
+    psi = rng.standard_normal(150) * np.exp(-rng.random(150) * 4)
+    psi[7] = 0.0  # a source with zero amplitude generates nothing (reading Q6)
+    ext = np.setdiff1d(np.arange(len(dets)), idx)
+    HS = H[np.ix_(idx, idx)]
+    e_s = psi @ HS @ psi / (psi @ psi)
+    C = H[np.ix_(ext, idx)] * psi[None, :]          # H_ai psi_i
+    tau = np.where(psi != 0, eps2 / np.abs(np.where(psi != 0, psi, 1.0)), np.inf) if eps2 > 0 else np.zeros(150)
+    keep = (np.abs(H[np.ix_(ext, idx)]) >= tau[None, :]) & (H[np.ix_(ext, idx)] != 0) & (psi != 0)[None, :]
+    v = (C * keep).sum(axis=1)
+    touched = keep.any(axis=1)
+    ref = np.sum(v[touched] ** 2 / (e_s - np.diag(H)[ext][touched])) / (psi @ psi)
+    rp, col, val = orc.ham_build(n, h1, eri, 0.0, dets[idx], 0.0)
+    e_or, _ = orc.energy(rp, col, val, psi)
+    assert np.isclose(e_or, e_s, rtol=1e-13)
+    for n_parts in (1, 4):
+        r = orc.pt2(n, h1, eri, 0.0, dets[idx], psi, e_s, eps2, n_parts=n_parts)
+        assert r["n_external"] == int(touched.sum())
+        assert r["n_contrib"] == int(keep.sum())
+        assert np.isclose(r["pt2"], ref, rtol=1e-12)
+        assert np.isclose(r["part_sums"].sum(), ref, rtol=1e-12)
+    # partition ranges add up (the multi-pass bookkeeping, reading Q14)
+    parts = [orc.pt2(n, h1, eri, 0.0, dets[idx], psi, e_s, eps2, n_parts=4, part_begin=k, part_end=k + 1) for k in range(4)]
+    assert np.isclose(sum(x["pt2"] for x in parts), ref, rtol=1e-12)
+    assert sum(x["n_external"] for x in parts) == int(touched.sum())
+    if eps2 == 0.0:
+        # P9 sum rule: ||H[:,S] psi||^2 = ||H_SS psi||^2 + sum_a v_a^2
+        lhs = np.sum((H[:, idx] @ psi) ** 2)
+        assert np.isclose(lhs, np.sum((HS @ psi) ** 2) + np.sum(v ** 2), rtol=1e-12)
+
+
+# ---------------------------------------------------------------- P10: spin-swap symmetry, single-reference EN2
+def test_p10_spin_swap_invariance(orc):
+    p = make_problem("tiny", n_dets=300)
+    n, h1, eri = p["n"], p["h1"], p["eri"]
+    dets, psi = p["dets"], p["psi"] / np.linalg.norm(p["psi"][:300])
+    sw = dets[:, ::-1].copy()
+    order = np.lexsort((sw[:, 1], sw[:, 0]))
+    sw, psw = np.ascontiguousarray(sw[order]), psi[order]
+    out = []
+    for d, s in ((dets, psi), (sw, psw)):
+        rp, col, val = orc.ham_build(n, h1, eri, 0.0, d, 1e-4)
+        e, _ = orc.energy(rp, col, val, s)
+        r = orc.pt2(n, h1, eri, 0.0, d, s, e, 1e-5)
+        out.append((len(col), e, r["pt2"], r["n_external"], r["n_contrib"]))
+    assert out[0][0] == out[1][0] and out[0][3:] == out[1][3:]
+    assert np.isclose(out[0][1], out[1][1], rtol=1e-13) and np.isclose(out[0][2], out[1][2], rtol=1e-11)
+
+
+def test_p10b_single_reference_epstein_nesbet(orc):
+    n, na, nb = 6, 2, 3
+    h1, eri = small_integrals(n, 71)
+    dets = full_space(n, na, nb)
+    H = orc.dense(n, h1, eri, 0.0, dets)
+    hf = 0
+    e0 = H[hf, hf]
+    others = np.arange(len(dets)) != hf
+    ref = np.sum(H[others, hf] ** 2 / (e0 - np.diag(H)[others]))
+    r = orc.pt2(n, h1, eri, 0.0, dets[hf:hf + 1], np.array([1.0]), e0, 0.0)
+    assert np.isclose(r["pt2"], ref, rtol=1e-12)
+    assert r["n_external"] == int(np.count_nonzero(H[others, hf]))
+
+
+def test_zobrist_is_xor_of_orbital_words(orc):
+    """Reading Q14: class function is a XOR over occupied orbitals, so an excitation shifts it by a fixed delta."""
+    z = lambda a, b: orc.zobrist(np.array([a, b], dtype=np.uint64))
+    assert z(0b0111, 0b1011) ^ z(0b0110, 0b1011) == z(0b0001, 0) and z(0, 0) == 0
+    assert z(0b0101, 0b0011) == z(0b0001, 0) ^ z(0b0100, 0) ^ z(0, 0b0001) ^ z(0, 0b0010)
+    # splitmix64(seed + index) with seed 260121310, written out independently
+    def sm(x):
+        m = (1 << 64) - 1
+        x = (x + 0x9E3779B97F4A7C15) & m
+        x = ((x ^ (x >> 30)) * 0xBF58476D1CE4E5B9) & m
+        x = ((x ^ (x >> 27)) * 0x94D049BB133111EB) & m
+        return x ^ (x >> 31)
+    assert z(1 << 5, 0) == sm(260121310 + 5) and z(0, 1 << 9) == sm(260121310 + 64 + 9)
