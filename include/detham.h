@@ -1,0 +1,136 @@
+/* detham.h — C ABI of the B200-native combinatorial Hamiltonian kernel of arxiv 2601.21310.
+ *
+ * The library rebuilds on one GPU (sm_100a) the paper's "Discrete Combinatorial Kernel" (Layer 0:
+ * "Evaluates Slater-Condon rules on integer representations of configurations to construct the Hamiltonian
+ * connectivity graphs (H_VV, H_VP) ... exporting sparse operators in CSR format"), the host-resident SpMV
+ * v = H psi (Alg. 1 line 14 at PAPER.md:282), the variational energy E_var (Eq. 11) and
+ * the external Epstein-Nesbet PT2 term (Eq. 13 second term) with heat-bath screening
+ * (Eq. 14 and the tau rule).  The paper calls the variational set V; here it is S.
+ *
+ * Conventions
+ *  - Plain C, no exceptions cross the boundary; every call returns a dh_status.
+ *  - n_orb = number of SPATIAL orbitals, 1 <= n_orb <= 64.  A determinant is two uint64 words {alpha, beta}; bit p of a
+ *    word = spatial orbital p occupied in that spin string.  |D> = prod_{p in alpha, ascending} a+_{p alpha}
+ *    prod_{q in beta, ascending} a+_{q beta} |0>  (sign convention; reading Q1).
+ *  - Integrals: h1 fp64 [n_orb*n_orb] symmetric; eri fp64 packed 8-fold symmetric chemist-notation (pq|rs) at
+ *    eri[T(T(p,q), T(r,s))], T(x,y) = max(x,y)*(max(x,y)+1)/2 + min(x,y)  (reading Q3).
+ *  - "device" pointers are CUDA device memory on the current device; "host" pointers are ordinary host memory.
+ *    Inputs are BORROWED (the caller keeps ownership; `dets` must stay valid until the next detham_set_subspace or
+ *    detham_destroy).  Everything reachable through detham_csr is OWNED by the context.
+ *  - All work is enqueued on the stream given at creation; calls that return scalars to host memory synchronise that
+ *    stream before returning.
+ *  - Nothing is truncated or sorted silently: an unsorted S, a full hash table or an allocation failure is an error code.
+ *  - There is no CPU fallback: without a CUDA device every compute call returns DH_ECUDA.
+ */
+#ifndef DETHAM_H
+#define DETHAM_H
+
+#include <stdint.h>
+
+#ifdef __cplusplus
+extern "C" {
+#endif
+
+typedef struct detham_ctx detham_ctx; /* opaque; owns every device allocation it makes */
+
+typedef enum {
+  DH_OK = 0,
+  DH_EINVAL = 1,     /* bad argument (NULL, n_orb out of range, negative or NaN threshold, call order) */
+  DH_EUNSORTED = 2,  /* S not strictly ascending by (alpha, beta) (covers duplicates) */
+  DH_EPOPCOUNT = 3,  /* a determinant has the wrong electron count or a bit at or above n_orb */
+  DH_ENOMEM = 4,     /* device or host allocation failed */
+  DH_ETABLEFULL = 5, /* PT2 hash table overflowed with the configured capacity / partition count */
+  DH_ECUDA = 6       /* CUDA runtime error (no device, launch failure); see detham_last_cuda_error */
+} dh_status;
+
+/* Counters of the most recent calls (metrics). */
+typedef struct {
+  int64_t nnz;              /* stored entries of H_SS (diagonal included) */
+  int64_t build_generated;  /* excitations that passed the magnitude screen in ham_build (looked up in S) */
+  int64_t pt2_generated;    /* excitations that passed the screen in pt2 (members of S included) */
+  int64_t pt2_contrib;      /* contributions H_ai psi_i added to externals a not in S */
+  int64_t pt2_external;     /* distinct externals */
+  int32_t pt2_parts;        /* key partitions (passes) used by the last pt2 */
+  int32_t pt2_max_probe;    /* longest probe sequence seen */
+  int64_t pt2_table_slots;  /* slots of the hash table used by each pass */
+  double pt2_sum_abs;       /* sum_a |v_a^2 / (E_S - H_aa)| / psi^T psi  (conditioning report, reading Q11) */
+  double pt2_min_abs_den;   /* min_a |E_S - H_aa| */
+  /* device times (CUDA events on the context's stream) of the kernels of the last calls, milliseconds */
+  double ms_store;          /* set_subspace: validation + lookup-index build */
+  double ms_build_count;    /* ham_build pass 1 (enumerate + lookup, count rows) */
+  double ms_build_fill;     /* ham_build pass 2 (enumerate + lookup, write CSR) + row scan + row sort */
+  double ms_energy;         /* SpMV + fused reductions */
+  double ms_pt2_plan;       /* pt2 class histogram (pass planning), 0 when both table_slots and n_parts are configured */
+  double ms_pt2_accum;      /* pt2 member insert + enumerate/accumulate kernels, summed over passes */
+  double ms_pt2_scan;       /* pt2 table scan/clear + reductions, summed over passes */
+} detham_counters;
+
+/* Create a context: uploads the integrals, derives J_pq = (pp|qq), K_pq = (pq|qp), and builds the heat-bath lists
+ * ("we precompute a lookup table during initialization: for each pair of occupied spin-orbitals (i,j),
+ * the corresponding pairs of virtual orbitals (a,b) are sorted in descending order of the integral magnitude").
+ * h1 / eri: host OR device pointers (detected).  cuda_stream: a cudaStream_t cast to void*, NULL = default stream.
+ * Requires 1 <= n_orb <= 64, 0 <= n_alpha, n_beta <= n_orb, n_alpha + n_beta >= 1. */
+dh_status detham_create(detham_ctx** out, int n_orb, int n_alpha, int n_beta, const double* h1, const double* eri,
+                        double e_core, void* cuda_stream);
+
+/* Set the variational subspace S ("variational set V_k").  dets: DEVICE uint64 [n_dets][2] = {alpha, beta},
+ * strictly ascending as 128-bit numbers with alpha the high word; 1 <= n_dets < 2^31.  Validated on the device
+ * (DH_EUNSORTED / DH_EPOPCOUNT).  Builds the L2-resident lookup structure of the determinant store.  Invalidates any CSR. */
+dh_status detham_set_subspace(detham_ctx* ctx, const uint64_t* dets, int64_t n_dets);
+
+/* ham_build (Alg. 1 line 8: "Construct sparse Hamiltonian block H_VV"): CSR with row i =
+ * {(i, H_ii)} U {(j, H_ij) : D_j in S, D_j a single or double excitation of D_i, |H_ij| >= eps, H_ij != 0}, columns
+ * ascending (reading Q4).  eps >= 0.  *nnz_out (host, may be NULL) receives the number of stored entries. */
+dh_status detham_ham_build(detham_ctx* ctx, double eps, int64_t* nnz_out);
+
+/* Device pointers of the CSR built last: row_ptr int64 [n_dets+1], col int32 [nnz], val fp64 [nnz].  Valid until the next
+ * detham_ham_build / detham_set_subspace / detham_destroy.  DH_EINVAL if no CSR exists. */
+dh_status detham_csr(detham_ctx* ctx, const int64_t** row_ptr, const int32_t** col, const double** val);
+
+/* Copy the CSR built last into caller buffers (each HOST or DEVICE, detected; any may be NULL to skip):
+ * row_ptr int64 [n_dets+1], col int32 [nnz], val fp64 [nnz].  Synchronises the stream. */
+dh_status detham_csr_copy(detham_ctx* ctx, int64_t* row_ptr, int32_t* col, double* val);
+
+/* energy (Eq. 11; the SpMV of Alg. 1 line 14): y = H_SS psi, E_S = psi^T y / psi^T psi.
+ * psi: DEVICE fp64 [n_dets].  y_out: DEVICE fp64 [n_dets] or NULL.  e_out, norm2_out: HOST (norm2_out may be NULL). */
+dh_status detham_energy(detham_ctx* ctx, const double* psi, double* e_out, double* norm2_out, double* y_out);
+
+/* Configure pt2: table_slots = hash-table capacity in 32-byte slots (0 = choose from free device memory);
+ * n_parts = number of key partitions / passes, a power of two <= 1024 (0 = choose so that every partition fits). */
+dh_status detham_pt2_config(detham_ctx* ctx, int64_t table_slots, int n_parts);
+
+/* pt2 (Eq. 13 second term, screened per Eq. 14 / PAPER.md:227; readings Q6, Q9, Q10):
+ * for every source i with psi_i != 0, tau_i = eps2 / |psi_i| (0 if eps2 == 0); for every single or double excitation a
+ * of D_i with |H_ai| >= tau_i, H_ai != 0 and a not in S:  v_a += H_ai psi_i.
+ * Result  dE = (1 / psi^T psi) sum_a v_a^2 / (e_s - H_aa).  psi: DEVICE fp64 [n_dets]; outputs HOST (counts may be NULL). */
+dh_status detham_pt2(detham_ctx* ctx, const double* psi, double e_s, double eps2, double* pt2_out,
+                     int64_t* n_external_out, int64_t* n_contrib_out);
+
+/* Per-partition partial sums (already divided by psi^T psi) of the last detham_pt2; writes min(cap, n_parts) values to
+ * `out` (HOST) and the partition count to *n_parts_out. */
+dh_status detham_pt2_partials(detham_ctx* ctx, double* out, int cap, int* n_parts_out);
+
+/* Whole hot path from HOST buffers (the end-to-end entry): copies dets and psi to the device, then set_subspace ->
+ * ham_build(eps) -> energy -> pt2(E_S, eps2), and returns the scalars to host memory. */
+dh_status detham_solve_host(detham_ctx* ctx, const uint64_t* dets_host, const double* psi_host, int64_t n_dets,
+                            double eps, double eps2, double* e_out, double* pt2_out, int64_t* nnz_out,
+                            int64_t* n_external_out);
+
+/* Test hook: the full screened connection list of source `row` of S at cutoff tau (members of S and externals alike,
+ * diagonal excluded), sorted by key.  keys_out HOST uint64 [cap][2], h_out HOST fp64 [cap]; *n_out = number found
+ * (if > cap only cap entries are written and the call returns DH_EINVAL). */
+dh_status detham_connections(detham_ctx* ctx, int64_t row, double tau, uint64_t* keys_out, double* h_out, int64_t cap,
+                             int64_t* n_out);
+
+/* Test hook: H_aa for `m` arbitrary determinants (DEVICE uint64 [m][2]) into DEVICE fp64 [m]. */
+dh_status detham_diagonals(detham_ctx* ctx, const uint64_t* dets, int64_t m, double* out);
+
+dh_status detham_get_counters(detham_ctx* ctx, detham_counters* out);
+void detham_destroy(detham_ctx* ctx);
+const char* detham_strerror(dh_status s);
+const char* detham_last_cuda_error(detham_ctx* ctx); /* text of the last CUDA error seen by this context, "" if none */
+
+#ifdef __cplusplus
+}
+#endif
+#endif /* DETHAM_H */

@@ -1,0 +1,170 @@
+// Shared declarations of the detham CUDA library (sm_100a only).  Nothing here is used by oracle/.
+#pragma once
+#include <cuda_runtime.h>
+#include <stdint.h>
+
+#include <string>
+#include <vector>
+
+#include "detham.h"
+
+typedef unsigned long long u64;
+
+#define DH_WARP 32
+#define DH_MAX_ORB 64
+#define DH_MAX_PBITS 10  // up to 1024 key partitions
+
+// ---------------------------------------------------------------- heat-bath lists
+// Three families of segments, one segment per ordered/unordered orbital pair:
+//   family 0 (alpha-alpha), 1 (beta-beta): pair i<j, id = j(j-1)/2 + i; entries (a<b), a,b not in {i,j};
+//                                          value <ij||ab> = (ia|jb) - (ib|ja)
+//   family 2 (alpha-beta): pair (i alpha, j beta), id = i*n + j; entries (a != i, b != j); value (ia|jb)
+// Inside a segment the entries are grouped by key-partition class (Zobrist class of the pair (a,b) in that family's
+// spins) and, inside a class, sorted by |value| descending (ties: (a,b) ascending).  sub_off[seg * P + c] is the
+// start of class c of segment seg; sub_off[nseg * P] = total.
+struct HbLists {
+  int pbits = -1;            // P = 1 << pbits
+  int nseg = 0;
+  int64_t total = 0;
+  int* sub_off = nullptr;       // device int32 [nseg * P + 1]
+  double* val = nullptr;        // device fp64 [total]
+  unsigned short* ab = nullptr; // device u16 [total]: a | (b << 8)
+};
+
+struct detham_ctx {
+  int n = 0, na = 0, nb = 0;
+  double e_core = 0.0;
+  cudaStream_t stream = nullptr;
+  int device = 0;
+  int sm_count = 148;
+  std::string cuda_err;
+
+  // integral store (a2): L2-resident
+  double* h1 = nullptr;   // [n*n]
+  double* eri = nullptr;  // packed
+  int64_t n_eri = 0;
+  double* J = nullptr;    // [n*n]  (pp|qq)
+  double* JK = nullptr;   // [n*n]  (pp|qq) - (pq|qp)
+  double* hd = nullptr;   // [n]    h_pp
+
+  HbLists lists[DH_MAX_PBITS + 1];  // built on demand per partition count
+
+  // determinant store (a1)
+  const u64* dets = nullptr;  // borrowed, device [nd][2]
+  int64_t nd = 0;
+  u64* dets_owned = nullptr;  // only for detham_solve_host
+  double* psi_owned = nullptr;
+  int64_t owned_cap = 0;
+  u64* shash_key = nullptr;   // device [shash_cap][2], open addressing, EMPTY = {0,0}
+  int* shash_idx = nullptr;   // device [shash_cap]
+  int64_t shash_cap = 0;
+
+  // CSR H_SS (a6)
+  int64_t* row_ptr = nullptr;
+  int* col = nullptr;
+  double* val = nullptr;
+  int64_t nnz = -1;
+  int64_t csr_cap = 0;
+  int* row_cnt = nullptr;  // device int32 [nd]
+  int64_t row_cap = 0;
+
+  // pt2
+  int64_t cfg_table_slots = 0;
+  int cfg_parts = 0;
+  void* table = nullptr;
+  int64_t table_slots = 0;
+  std::vector<double> partials;
+
+  // scratch
+  double* red = nullptr;      // device reduction buffer
+  int64_t red_cap = 0;
+  u64* dcount = nullptr;      // device counters [64]
+  void* pinned = nullptr;     // pinned host scratch (4 KB)
+  int64_t* hist = nullptr;    // device int64 [1024] class histogram
+
+  detham_counters ctr{};
+  cudaEvent_t ev[8] = {};  // scratch events for the per-phase timers
+};
+
+// record ev[k] on the context's stream
+#define DH_TICK(ctx, k) DH_CUDA(ctx, cudaEventRecord((ctx)->ev[k], (ctx)->stream))
+inline double dh_elapsed(detham_ctx* c, int a, int b) { float ms = 0.f; cudaEventElapsedTime(&ms, c->ev[a], c->ev[b]); return (double)ms; }
+
+#define DH_CUDA(ctx, expr)                                                     \
+  do {                                                                         \
+    cudaError_t _e = (expr);                                                   \
+    if (_e != cudaSuccess) {                                                   \
+      (ctx)->cuda_err = std::string(#expr) + ": " + cudaGetErrorString(_e);    \
+      return _e == cudaErrorMemoryAllocation ? DH_ENOMEM : DH_ECUDA;           \
+    }                                                                          \
+  } while (0)
+
+// entry points implemented across the translation units
+dh_status dh_build_jk(detham_ctx* c);
+dh_status dh_get_lists(detham_ctx* c, int pbits, const HbLists** out);
+dh_status dh_ham_build(detham_ctx* c, double eps);
+dh_status dh_energy(detham_ctx* c, const double* psi, double* e_out, double* n2_out, double* y_out);
+dh_status dh_pt2(detham_ctx* c, const double* psi, double e_s, double eps2, double* out);
+dh_status dh_connections(detham_ctx* c, int64_t row, double tau, std::vector<u64>& keys, std::vector<double>& h);
+dh_status dh_diagonals(detham_ctx* c, const u64* dets, int64_t m, double* out);
+dh_status dh_build_shash(detham_ctx* c);
+dh_status dh_validate_subspace(detham_ctx* c, const u64* dets, int64_t nd);
+dh_status dh_ensure_red(detham_ctx* c, int64_t n);
+
+// ---------------------------------------------------------------- device helpers
+#ifdef __CUDACC__
+
+__host__ __device__ __forceinline__ int dh_tri(int x, int y) { return x >= y ? x * (x + 1) / 2 + y : y * (y + 1) / 2 + x; }
+
+// chemist (pq|rs) from the packed 8-fold array
+__device__ __forceinline__ double dh_eri(const double* __restrict__ eri, int p, int q, int r, int s) {
+  int pq = dh_tri(p, q), rs = dh_tri(r, s);
+  return __ldg(eri + (pq >= rs ? pq * (pq + 1) / 2 + rs : rs * (rs + 1) / 2 + pq));
+}
+
+// Key-partition words (reading Q14): word of spin-orbital index s (alpha p -> p, beta q -> 64 + q) is
+// splitmix64(260121310 + s); a determinant's word is the XOR over its occupied spin-orbitals.
+__host__ __device__ __forceinline__ u64 dh_zword(int s) {
+  u64 x = 260121310ull + (u64)s + 0x9E3779B97F4A7C15ull;
+  x = (x ^ (x >> 30)) * 0xBF58476D1CE4E5B9ull;
+  x = (x ^ (x >> 27)) * 0x94D049BB133111EBull;
+  return x ^ (x >> 31);
+}
+
+struct __align__(16) Key128 { u64 a, b; };
+
+__device__ __forceinline__ Key128 dh_cas128(void* addr, Key128 cmp, Key128 val) {
+  Key128 old;
+  asm volatile(
+      "{\n\t.reg .b128 c, v, o;\n\t"
+      "mov.b128 c, {%2, %3};\n\t"
+      "mov.b128 v, {%4, %5};\n\t"
+      "atom.relaxed.gpu.global.cas.b128 o, [%6], c, v;\n\t"
+      "mov.b128 {%0, %1}, o;\n\t}"
+      : "=l"(old.a), "=l"(old.b)
+      : "l"(cmp.a), "l"(cmp.b), "l"(val.a), "l"(val.b), "l"(addr)
+      : "memory");
+  return old;
+}
+
+// one 32-byte slot in one transaction (LDG.E.256), coherent at gpu scope (bypasses the non-coherent L1)
+__device__ __forceinline__ void dh_ld256(const void* p, u64& a, u64& b, u64& c, u64& d) {
+  asm volatile("ld.relaxed.gpu.global.v4.u64 {%0,%1,%2,%3}, [%4];" : "=l"(a), "=l"(b), "=l"(c), "=l"(d) : "l"(p) : "memory");
+}
+
+// streaming variants for the table scan (evict-first: the scan touches every slot exactly once)
+__device__ __forceinline__ void dh_ld256_cs(const void* p, u64& a, u64& b, u64& c, u64& d) {
+  asm volatile("ld.global.cs.v4.u64 {%0,%1,%2,%3}, [%4];" : "=l"(a), "=l"(b), "=l"(c), "=l"(d) : "l"(p) : "memory");
+}
+__device__ __forceinline__ void dh_st256_zero(void* p) {
+  asm volatile("st.global.cs.v4.u64 [%0], {%1,%1,%1,%1};" ::"l"(p), "l"(0ull) : "memory");
+}
+
+// (-1)^(electrons of word w strictly between orbitals x and y): returns 0 (even) or 1 (odd)
+__device__ __forceinline__ int dh_parity_between(u64 w, int x, int y) {
+  int lo = min(x, y), hi = max(x, y);
+  u64 m = ((1ull << hi) - 1ull) & ~((2ull << lo) - 1ull);
+  return __popcll(w & m) & 1;
+}
+
+#endif  // __CUDACC__

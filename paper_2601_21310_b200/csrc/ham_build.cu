@@ -1,0 +1,303 @@
+// Determinant store lookup (a1) and CSR H_SS construction (a6).  PAPER.md:206, 269.
+#include "enumerate.cuh"
+
+namespace {
+
+constexpr int kWarpsPerCta = 8;
+
+// ---------------------------------------------------------------- determinant store
+__global__ void validate_kernel(const u64* __restrict__ dets, int64_t nd, int n, int na, int nb, int* flags) {
+  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nd) return;
+  u64 a = dets[2 * t], b = dets[2 * t + 1];
+  u64 hi = n == 64 ? 0ull : ~((1ull << n) - 1ull);
+  if (__popcll(a) != na || __popcll(b) != nb || (a & hi) || (b & hi)) flags[1] = 1;
+  if (t > 0) {
+    u64 pa = dets[2 * t - 2], pb = dets[2 * t - 1];
+    if (!(pa < a || (pa == a && pb < b))) flags[0] = 1;
+  }
+}
+
+// L2-resident open-addressing index of S: slot = mulhi(z(D), cap), linear probing, EMPTY = {0,0}
+__global__ void shash_insert_kernel(const u64* __restrict__ dets, int64_t nd, u64* keys, int* idx, u64 cap) {
+  __shared__ u64 Z[128];
+  for (int t = threadIdx.x; t < 128; t += blockDim.x) Z[t] = dh_zword(t);
+  __syncthreads();
+  int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nd) return;
+  u64 a = dets[2 * t], b = dets[2 * t + 1];
+  u64 slot = __umul64hi(dh_zobrist(a, b, Z), cap);
+  for (;;) {
+    Key128 old = dh_cas128(keys + 2 * slot, Key128{0ull, 0ull}, Key128{a, b});
+    if (old.a == 0ull && old.b == 0ull) { idx[slot] = (int)t; return; }
+    if (++slot == cap) slot = 0;
+  }
+}
+
+__device__ __forceinline__ int shash_find(const u64* __restrict__ keys, const int* __restrict__ idx, u64 cap, u64 ka, u64 kb, u64 z) {
+  u64 slot = __umul64hi(z, cap);
+  for (;;) {
+    ulonglong2 k = __ldg(reinterpret_cast<const ulonglong2*>(keys) + slot);
+    if (k.x == ka && k.y == kb) return __ldg(idx + slot);
+    if (k.x == 0ull && k.y == 0ull) return -1;
+    if (++slot == cap) slot = 0;
+  }
+}
+
+// ---------------------------------------------------------------- CSR sinks
+struct BuildSink {
+  static constexpr bool kLookupFirst = true;
+  const u64* keys; const int* idx; u64 cap;
+  int* col; double* val;   // row destination (fill pass) or nullptr (count pass)
+  int count;               // warp-uniform running count of hits
+  u64 generated;           // per-lane count of screened candidates looked up
+  int lane;
+  int pre_tok;
+  __device__ __forceinline__ bool pre(u64 ka, u64 kb, u64 z) {
+    ++generated;
+    pre_tok = shash_find(keys, idx, cap, ka, kb, z);
+    return pre_tok >= 0;
+  }
+  __device__ __forceinline__ void emit(bool act, u64 ka, u64 kb, u64 z, double H, int kind, int, int, int, int, int) {
+    int tok = -1;
+    if (act) {
+      if (kind == 0) tok = pre_tok;
+      else { ++generated; tok = shash_find(keys, idx, cap, ka, kb, z); }
+    }
+    unsigned hit = __ballot_sync(0xffffffffu, tok >= 0);
+    if (hit) {
+      if (col != nullptr && tok >= 0) {
+        int pos = count + __popc(hit & ((1u << lane) - 1u));
+        col[pos] = tok;
+        val[pos] = H;
+      }
+      count += __popc(hit);
+    }
+  }
+};
+
+template <bool FILL>
+__global__ void __launch_bounds__(kWarpsPerCta * 32)
+build_kernel(EnumParams P, const u64* __restrict__ dets, int64_t nd, double eps, const u64* __restrict__ hkeys,
+             const int* __restrict__ hidx, u64 hcap, int* __restrict__ row_cnt, const int64_t* __restrict__ row_ptr,
+             int* __restrict__ col, double* __restrict__ val, u64* counters /* [0]=next row, [1]=generated */) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  CtaTables T = dh_cta_stage(P, smem);
+  WarpScratch* wsp = reinterpret_cast<WarpScratch*>(smem + ((dh_cta_table_bytes(P.n) + 15) & ~(size_t)15));
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  WarpScratch& ws = wsp[warp];
+  u64 gen = 0;
+  for (;;) {
+    u64 row = 0;
+    if (lane == 0) row = atomicAdd(counters, 1ull);
+    row = __shfl_sync(0xffffffffu, row, 0);
+    if ((int64_t)row >= nd) break;
+    const u64 da = dets[2 * row], db = dets[2 * row + 1];
+    dh_fill_occ(P, ws, da, db, lane);
+    BuildSink sink{hkeys, hidx, hcap, nullptr, nullptr, 0, 0ull, lane, -1};
+    int64_t base = 0;
+    if (FILL) {
+      base = row_ptr[row];
+      double e0 = dh_fill_U(P, T, ws, lane);
+      if (lane == 0) { col[base] = (int)row; val[base] = e0; }
+      sink.col = col + base; sink.val = val + base; sink.count = 1;
+    }
+    u64 zsrc = 0;
+    if (lane == 0) zsrc = dh_zobrist(da, db, T.Z);
+    zsrc = __shfl_sync(0xffffffffu, zsrc, 0);
+    dh_enumerate(P, T, ws, da, db, eps, zsrc, 0u, sink, lane);
+    if (!FILL && lane == 0) row_cnt[row] = sink.count + 1;
+    gen += sink.generated;
+    __syncwarp();
+  }
+  if (!FILL) {
+    for (int o = 16; o > 0; o >>= 1) gen += __shfl_xor_sync(0xffffffffu, gen, o);
+    if (lane == 0 && gen) atomicAdd(counters + 1, gen);
+  }
+}
+
+// exclusive scan of row counts -> row_ptr (single CTA, sequential over chunks; |S| < 2^31 so this is a few ms at most)
+__global__ void scan_rows_kernel(const int* __restrict__ cnt, int64_t nd, int64_t* __restrict__ row_ptr) {
+  __shared__ int64_t warp_tot[32];
+  __shared__ int64_t carry;
+  if (threadIdx.x == 0) carry = 0;
+  __syncthreads();
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  for (int64_t base = 0; base < nd; base += blockDim.x) {
+    int64_t t = base + threadIdx.x;
+    int64_t v = t < nd ? cnt[t] : 0, x = v;
+    for (int o = 1; o < 32; o <<= 1) { int64_t y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+    if (lane == 31) warp_tot[warp] = x;
+    __syncthreads();
+    if (warp == 0) {
+      int64_t w = lane < (blockDim.x >> 5) ? warp_tot[lane] : 0, s = w;
+      for (int o = 1; o < 32; o <<= 1) { int64_t y = __shfl_up_sync(0xffffffffu, s, o); if (lane >= o) s += y; }
+      warp_tot[lane] = s - w;
+    }
+    __syncthreads();
+    int64_t excl = carry + warp_tot[warp] + x - v;
+    if (t < nd) row_ptr[t] = excl;
+    __syncthreads();
+    if (threadIdx.x == blockDim.x - 1) carry = excl + v;
+    __syncthreads();
+  }
+  if (threadIdx.x == 0) row_ptr[nd] = carry;
+}
+
+// ---------------------------------------------------------------- per-row column sort
+// Bitonic network with ascending comparators only (virtual +inf padding stays at the tail).
+template <class Sync>
+__device__ __forceinline__ void bitonic_rows(int* c, double* v, int len, int tid, int nthr, Sync sync) {
+  int N = 2;
+  while (N < len) N <<= 1;
+  for (int k = 2; k <= N; k <<= 1)
+    for (int jj = k >> 1; jj > 0; jj >>= 1) {
+      for (int t = tid; t < N / 2; t += nthr) {
+        int blk = t / jj, off = t % jj, lo, hi;
+        if (jj == (k >> 1)) { lo = blk * k + off; hi = blk * k + k - 1 - off; }
+        else { lo = blk * 2 * jj + off; hi = lo + jj; }
+        if (hi < len) {
+          int cl = c[lo], ch = c[hi];
+          if (ch < cl) { double vl = v[lo], vh = v[hi]; c[lo] = ch; c[hi] = cl; v[lo] = vh; v[hi] = vl; }
+        }
+      }
+      sync();
+    }
+}
+
+constexpr int kSortWarpCap = 512;
+__global__ void __launch_bounds__(kWarpsPerCta * 32)
+sort_rows_warp_kernel(const int64_t* __restrict__ row_ptr, int64_t nd, int* __restrict__ col, double* __restrict__ val) {
+  __shared__ int sc[kWarpsPerCta][kSortWarpCap];
+  __shared__ double sv[kWarpsPerCta][kSortWarpCap];
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  int64_t row = (int64_t)blockIdx.x * kWarpsPerCta + warp;
+  if (row >= nd) return;
+  int64_t b = row_ptr[row];
+  int len = (int)(row_ptr[row + 1] - b);
+  if (len <= 1 || len > kSortWarpCap) return;
+  for (int t = lane; t < len; t += 32) { sc[warp][t] = col[b + t]; sv[warp][t] = val[b + t]; }
+  __syncwarp();
+  bitonic_rows(sc[warp], sv[warp], len, lane, 32, [] { __syncwarp(); });
+  for (int t = lane; t < len; t += 32) { col[b + t] = sc[warp][t]; val[b + t] = sv[warp][t]; }
+}
+
+// rows longer than kSortWarpCap: one CTA per row, sorted in place in global memory (L2)
+__global__ void __launch_bounds__(1024)
+sort_rows_cta_kernel(const int64_t* __restrict__ row_ptr, int64_t nd, int* __restrict__ col, double* __restrict__ val) {
+  for (int64_t row = blockIdx.x; row < nd; row += gridDim.x) {
+    int64_t b = row_ptr[row];
+    int len = (int)(row_ptr[row + 1] - b);
+    if (len <= kSortWarpCap) continue;
+    bitonic_rows(col + b, val + b, len, threadIdx.x, blockDim.x, [] { __syncthreads(); });
+  }
+}
+
+template <class K>
+dh_status set_smem(detham_ctx* c, K kernel, size_t bytes) {
+  DH_CUDA(c, cudaFuncSetAttribute(kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)bytes));
+  return DH_OK;
+}
+
+}  // namespace
+
+dh_status dh_validate_subspace(detham_ctx* c, const u64* dets, int64_t nd) {
+  int* flags = reinterpret_cast<int*>(c->dcount);
+  DH_CUDA(c, cudaMemsetAsync(flags, 0, 2 * sizeof(int), c->stream));
+  validate_kernel<<<(unsigned)((nd + 255) / 256), 256, 0, c->stream>>>(dets, nd, c->n, c->na, c->nb, flags);
+  DH_CUDA(c, cudaGetLastError());
+  int* h = reinterpret_cast<int*>(c->pinned);
+  DH_CUDA(c, cudaMemcpyAsync(h, flags, 2 * sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+  DH_CUDA(c, cudaStreamSynchronize(c->stream));
+  if (h[1]) return DH_EPOPCOUNT;
+  if (h[0]) return DH_EUNSORTED;
+  return DH_OK;
+}
+
+dh_status dh_build_shash(detham_ctx* c) {
+  int64_t cap = 1024;
+  while (cap < 2 * c->nd) cap <<= 1;
+  if (cap != c->shash_cap) {
+    if (c->shash_key) cudaFree(c->shash_key);
+    if (c->shash_idx) cudaFree(c->shash_idx);
+    c->shash_key = nullptr; c->shash_idx = nullptr; c->shash_cap = 0;
+    DH_CUDA(c, cudaMalloc(&c->shash_key, cap * 2 * sizeof(u64)));
+    DH_CUDA(c, cudaMalloc(&c->shash_idx, cap * sizeof(int)));
+    c->shash_cap = cap;
+  }
+  DH_CUDA(c, cudaMemsetAsync(c->shash_key, 0, cap * 2 * sizeof(u64), c->stream));
+  shash_insert_kernel<<<(unsigned)((c->nd + 255) / 256), 256, 0, c->stream>>>(c->dets, c->nd, c->shash_key, c->shash_idx, (u64)cap);
+  DH_CUDA(c, cudaGetLastError());
+  return DH_OK;
+}
+
+static EnumParams make_params(detham_ctx* c, const HbLists* L) {
+  EnumParams P;
+  P.n = c->n; P.na = c->na; P.nb = c->nb; P.pbits = L->pbits; P.nss = c->n * (c->n - 1) / 2;
+  P.h1 = c->h1; P.eri = c->eri; P.sub_off = L->sub_off; P.lval = L->val; P.lab = L->ab;
+  P.J = c->J; P.JK = c->JK; P.hd = c->hd; P.e_core = c->e_core;
+  return P;
+}
+EnumParams dh_make_params(detham_ctx* c, const HbLists* L) { return make_params(c, L); }
+
+dh_status dh_ham_build(detham_ctx* c, double eps) {
+  const HbLists* L = nullptr;
+  dh_status st = dh_get_lists(c, 0, &L);
+  if (st != DH_OK) return st;
+  EnumParams P = make_params(c, L);
+  const int64_t nd = c->nd;
+  if (c->row_cap < nd) {
+    if (c->row_cnt) cudaFree(c->row_cnt);
+    if (c->row_ptr) cudaFree(c->row_ptr);
+    c->row_cnt = nullptr; c->row_ptr = nullptr; c->row_cap = 0;
+    DH_CUDA(c, cudaMalloc(&c->row_cnt, nd * sizeof(int)));
+    DH_CUDA(c, cudaMalloc(&c->row_ptr, (nd + 1) * sizeof(int64_t)));
+    c->row_cap = nd;
+  }
+  c->nnz = -1;
+  size_t smem = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + kWarpsPerCta * sizeof(WarpScratch);
+  st = set_smem(c, build_kernel<false>, smem); if (st != DH_OK) return st;
+  st = set_smem(c, build_kernel<true>, smem); if (st != DH_OK) return st;
+  int64_t want = (nd + kWarpsPerCta - 1) / kWarpsPerCta;
+  int grid = (int)(want < (int64_t)c->sm_count * 4 ? want : (int64_t)c->sm_count * 4);
+  DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 8 * sizeof(u64), c->stream));
+  DH_TICK(c, 0);
+  build_kernel<false><<<grid, kWarpsPerCta * 32, smem, c->stream>>>(P, c->dets, nd, eps, c->shash_key, c->shash_idx,
+                                                                      (u64)c->shash_cap, c->row_cnt, nullptr, nullptr,
+                                                                      nullptr, c->dcount);
+  DH_CUDA(c, cudaGetLastError());
+  scan_rows_kernel<<<1, 1024, 0, c->stream>>>(c->row_cnt, nd, c->row_ptr);
+  DH_CUDA(c, cudaGetLastError());
+  DH_TICK(c, 1);
+  int64_t* h = reinterpret_cast<int64_t*>(c->pinned);
+  DH_CUDA(c, cudaMemcpyAsync(h, c->row_ptr + nd, sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
+  DH_CUDA(c, cudaMemcpyAsync(h + 1, c->dcount + 1, sizeof(u64), cudaMemcpyDeviceToHost, c->stream));
+  DH_CUDA(c, cudaStreamSynchronize(c->stream));
+  const int64_t nnz = h[0];
+  c->ctr.build_generated = h[1];
+  if (c->csr_cap < nnz) {
+    if (c->col) cudaFree(c->col);
+    if (c->val) cudaFree(c->val);
+    c->col = nullptr; c->val = nullptr; c->csr_cap = 0;
+    DH_CUDA(c, cudaMalloc(&c->col, nnz * sizeof(int)));
+    DH_CUDA(c, cudaMalloc(&c->val, nnz * sizeof(double)));
+    c->csr_cap = nnz;
+  }
+  DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 8 * sizeof(u64), c->stream));
+  DH_TICK(c, 2);
+  build_kernel<true><<<grid, kWarpsPerCta * 32, smem, c->stream>>>(P, c->dets, nd, eps, c->shash_key, c->shash_idx,
+                                                                     (u64)c->shash_cap, c->row_cnt, c->row_ptr, c->col,
+                                                                     c->val, c->dcount);
+  DH_CUDA(c, cudaGetLastError());
+  sort_rows_warp_kernel<<<(unsigned)((nd + kWarpsPerCta - 1) / kWarpsPerCta), kWarpsPerCta * 32, 0, c->stream>>>(c->row_ptr, nd, c->col, c->val);
+  DH_CUDA(c, cudaGetLastError());
+  sort_rows_cta_kernel<<<c->sm_count * 2, 1024, 0, c->stream>>>(c->row_ptr, nd, c->col, c->val);
+  DH_CUDA(c, cudaGetLastError());
+  DH_TICK(c, 3);
+  DH_CUDA(c, cudaEventSynchronize(c->ev[3]));
+  c->ctr.ms_build_count = dh_elapsed(c, 0, 1);
+  c->ctr.ms_build_fill = dh_elapsed(c, 2, 3);
+  c->nnz = nnz;
+  c->ctr.nnz = nnz;
+  return DH_OK;
+}

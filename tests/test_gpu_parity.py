@@ -1,0 +1,306 @@
+"""GPU parity: the CUDA path (through the C ABI) against the oracle, element by element, on the same seeded inputs.
+
+Bars (BASELINE.json north_star): connection lists bit-exact as sorted sets; E_S relative 1e-10; PT2 relative 1e-9
+(reordered summation allowed); counts exact.
+"""
+import numpy as np
+import pytest
+
+from synth_inputs import make_problem, make_integrals, CONFIGS
+from helpers import full_space, small_integrals
+
+pytestmark = pytest.mark.gpu
+
+E_TOL = 1e-10
+PT2_TOL = 1e-9
+
+
+@pytest.fixture(scope="module")
+def pkg():
+    import torch
+    assert torch.cuda.is_available(), "gpu tests need a CUDA device"
+    import __graft_entry__ as g
+    g.build()
+    import paper_2601_21310_b200 as m
+    return m
+
+
+def _ctx(pkg, p):
+    ctx = pkg.create(p["n"], p["na"], p["nb"], p["h1"], p["eri"], p["e_core"])
+    ctx.set_subspace(p["dets"])
+    return ctx
+
+
+def _psi(p):
+    import torch
+    return torch.from_numpy(np.ascontiguousarray(p["psi"])).cuda()
+
+
+def _check_csr(ctx, ref, rows=None):
+    rp, col, val = (t.cpu().numpy() for t in ctx.csr())
+    orp, ocol, oval = ref
+    assert np.array_equal(rp, orp)
+    assert np.array_equal(col, ocol)
+    nd = len(rp) - 1
+    rowid = np.repeat(np.arange(nd), np.diff(rp))
+    off = col != rowid
+    assert np.array_equal(val[off], oval[off])                      # off-diagonals: identical bits
+    assert np.allclose(val[~off], oval[~off], rtol=1e-13, atol=0)   # diagonal: summation order differs
+
+
+def _check_connections(ctx, orc, p, rows, taus):
+    for r in rows:
+        for tau in taus:
+            gk, gh = ctx.connections(int(r), tau)
+            ok, oh, _ = orc.connections(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"][r], tau)
+            assert np.array_equal(gk, ok), (r, tau, len(gk), len(ok))
+            assert np.array_equal(gh, oh)
+
+
+def _full_parity(pkg, orc, p, eps, eps2, parts=(0,), oracle_chunks=1):
+    ctx = _ctx(pkg, p)
+    psi = _psi(p)
+    nnz = ctx.ham_build(eps)
+    ref = orc.ham_build(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"], eps)
+    assert nnz == len(ref[1])
+    _check_csr(ctx, ref)
+    e, n2 = ctx.energy(psi)
+    e_ref, n2_ref = orc.energy(*ref, p["psi"])
+    assert abs(e - e_ref) <= E_TOL * abs(e_ref)
+    assert abs(n2 - n2_ref) <= 1e-13 * n2_ref
+    np_or = 16
+    o = [orc.pt2(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"], p["psi"], e_ref, eps2, n_parts=np_or,
+                 part_begin=k * np_or // oracle_chunks, part_end=(k + 1) * np_or // oracle_chunks) for k in range(oracle_chunks)]
+    o_pt2 = sum(x["pt2"] for x in o); o_ext = sum(x["n_external"] for x in o); o_con = sum(x["n_contrib"] for x in o)
+    o_parts = sum(x["part_sums"] for x in o)
+    o_abs = sum(x["sum_abs"] for x in o)
+    for n_parts in parts:
+        ctx.pt2_config(0, n_parts)
+        g_pt2, g_ext, g_con = ctx.pt2(psi, e_ref, eps2)
+        c = ctx.counters()
+        assert (g_ext, g_con) == (o_ext, o_con), (n_parts, g_ext, g_con, o_ext, o_con)
+        assert abs(g_pt2 - o_pt2) <= PT2_TOL * abs(o_pt2), (n_parts, g_pt2, o_pt2, o_abs / abs(o_pt2))
+        assert abs(c["pt2_sum_abs"] - o_abs) <= 1e-8 * o_abs
+        if n_parts == np_or:  # same partition function on both sides (reading Q14): partials agree class by class
+            gp = ctx.pt2_partials()
+            assert np.allclose(gp, o_parts, rtol=1e-8, atol=1e-12 * o_abs)
+    ctx.close()
+    return dict(nnz=nnz, e=e, pt2=o_pt2, n_ext=o_ext, n_con=o_con, cond=o_abs / abs(o_pt2))
+
+
+def test_tiny_full(pkg, orc):
+    p = make_problem("tiny")
+    r = _full_parity(pkg, orc, p, 0.0, 0.0, parts=(0, 1, 4, 16))
+    assert r["n_con"] > 1_000_000 and r["n_ext"] > 40_000
+    ctx = _ctx(pkg, p)
+    _check_connections(ctx, orc, p, [0, 1, 7, 999, 1999], [0.0, 1e-3, 3e-2, 0.5])
+    ctx.close()
+
+
+@pytest.mark.parametrize("eps,eps2", [(1e-3, 1e-4), (5e-2, 1e-2), (1e-5, 1e-7)])
+def test_tiny_screened(pkg, orc, eps, eps2):
+    _full_parity(pkg, orc, make_problem("tiny"), eps, eps2, parts=(0, 16))
+
+
+def test_h2o_shaped_full(pkg, orc):
+    p = make_problem("h2o")
+    r = _full_parity(pkg, orc, p, p["eps"], p["eps2"], parts=(0, 16), oracle_chunks=4)
+    assert r["n_con"] > 100_000_000
+    ctx = _ctx(pkg, p)
+    _check_connections(ctx, orc, p, [0, 5, 12345, 19999], [1e-5, 1e-3, 1e-1])
+    ctx.close()
+
+
+def _masked(p, n_keep, seed):
+    rng = np.random.default_rng(seed)
+    nd = len(p["psi"])
+    keep = np.unique(np.concatenate([[int(np.argmax(np.abs(p["psi"])))], rng.choice(nd, size=n_keep, replace=False)]))
+    m = np.zeros(nd)
+    m[keep] = 1.0
+    q = dict(p)
+    q["psi"] = p["psi"] * m
+    return q, keep
+
+
+def _masked_parity(pkg, orc, p, n_keep, seed, parts):
+    """Tier-2 parity: sources with psi_i = 0 generate nothing, so psi*mask on the FULL S and integrals
+    is an exact instance of the same problem whose oracle cost is n_keep sources."""
+    import torch
+    q, keep = _masked(p, n_keep, seed)
+    ctx = _ctx(pkg, p)
+    nnz = ctx.ham_build(p["eps"])
+    rp, col, val = (t.cpu().numpy() for t in ctx.csr())
+    dets = p["dets"]
+    keyidx = {(int(a), int(b)): k for k, (a, b) in enumerate(dets)} if len(dets) <= 200_000 else None
+    void = np.ascontiguousarray(dets).view(np.dtype((np.void, 16))).ravel() if keyidx is None else None
+    for r in keep[:: max(1, len(keep) // 40)]:
+        ok, oh, _ = orc.connections(p["n"], p["h1"], p["eri"], p["e_core"], dets[r], p["eps"])
+        gk, gh = ctx.connections(int(r), p["eps"])
+        assert np.array_equal(gk, ok) and np.array_equal(gh, oh)
+        # the row of H_SS = the members of S among the connections, plus the diagonal
+        if keyidx is not None:
+            idx = np.array([keyidx.get((int(a), int(b)), -1) for a, b in ok])
+        else:
+            # sorted S: binary search on (alpha, beta)
+            lo = np.searchsorted(dets[:, 0], ok[:, 0], side="left"); idx = np.full(len(ok), -1)
+            for t, (a, b) in enumerate(ok):
+                hi = np.searchsorted(dets[:, 0], a, side="right")
+                j = lo[t] + np.searchsorted(dets[lo[t]:hi, 1], b)
+                if j < hi and dets[j, 1] == b:
+                    idx[t] = j
+        members = idx >= 0
+        cols = np.concatenate([idx[members], [r]]); vals = np.concatenate([oh[members], [orc.diagonal(p["n"], p["h1"], p["eri"], p["e_core"], dets[r])]])
+        order = np.argsort(cols)
+        grow_c, grow_v = col[rp[r]:rp[r + 1]], val[rp[r]:rp[r + 1]]
+        assert np.array_equal(grow_c, cols[order])
+        offd = grow_c != r
+        assert np.array_equal(grow_v[offd], vals[order][offd])
+        assert np.allclose(grow_v[~offd], vals[order][~offd], rtol=1e-13)
+    psi = torch.from_numpy(q["psi"]).cuda()
+    e_s = -1.2345 + float(orc.diagonal(p["n"], p["h1"], p["eri"], p["e_core"], dets[keep[0]]))
+    o = orc.pt2(p["n"], p["h1"], p["eri"], p["e_core"], dets, q["psi"], e_s, p["eps2"], n_parts=16)
+    for n_parts in parts:
+        ctx.pt2_config(0, n_parts)
+        g_pt2, g_ext, g_con = ctx.pt2(psi, e_s, p["eps2"])
+        assert (g_ext, g_con) == (o["n_external"], o["n_contrib"])
+        assert abs(g_pt2 - o["pt2"]) <= PT2_TOL * max(abs(o["pt2"]), 1e-3 * o["sum_abs"]), (g_pt2, o)
+        if n_parts == 16:
+            assert np.allclose(ctx.pt2_partials(), o["part_sums"], rtol=1e-8, atol=1e-12 * o["sum_abs"])
+    ctx.close()
+    return nnz
+
+
+def test_n2_shaped_masked(pkg, orc):
+    p = make_problem("n2")
+    _masked_parity(pkg, orc, p, 400, 7, parts=(0, 16))
+
+
+def test_cr2_shaped_masked(pkg, orc):
+    p = make_problem("cr2")
+    nnz = _masked_parity(pkg, orc, p, 48, 9, parts=(0, 16))
+    assert nnz >= len(p["psi"])
+
+
+# ---------------------------------------------------------------- edge cases
+def test_single_determinant_hf(pkg, orc):
+    p = make_problem("tiny", n_dets=1)
+    p["psi"] = np.array([1.0])
+    r = _full_parity(pkg, orc, p, 0.0, 0.0, parts=(0, 4))
+    assert r["nnz"] == 1 and r["n_ext"] == 875
+
+
+@pytest.mark.parametrize("n,na,nb", [(6, 3, 1), (7, 1, 4), (5, 5, 2), (6, 0, 3), (9, 2, 2)])
+def test_unequal_spins_and_degenerate_strings(pkg, orc, n, na, nb):
+    h1, eri = small_integrals(n, 100 + n + na)
+    dets = full_space(n, na, nb)
+    rng = np.random.default_rng(n * 10 + na)
+    idx = np.sort(rng.choice(len(dets), size=max(1, len(dets) // 3), replace=False))
+    psi = rng.standard_normal(len(idx))
+    psi[0] = 0.0 if len(idx) > 2 else psi[0]
+    p = dict(n=n, na=na, nb=nb, h1=h1, eri=eri, e_core=0.3, dets=np.ascontiguousarray(dets[idx]), psi=psi)
+    _full_parity(pkg, orc, p, 1e-3, 1e-3, parts=(0, 2))
+    _full_parity(pkg, orc, p, 0.0, 0.0, parts=(0,))
+
+
+def test_full_space_has_no_externals(pkg, orc):
+    n, na, nb = 6, 3, 2
+    h1, eri = small_integrals(n, 77)
+    dets = full_space(n, na, nb)
+    p = dict(n=n, na=na, nb=nb, h1=h1, eri=eri, e_core=0.0, dets=dets, psi=np.random.default_rng(2).standard_normal(len(dets)))
+    import torch
+    ctx = _ctx(pkg, p)
+    ctx.ham_build(0.0)
+    e, _ = ctx.energy(_psi(p))
+    pt2, n_ext, n_con = ctx.pt2(_psi(p), e, 0.0)
+    assert (pt2, n_ext, n_con) == (0.0, 0, 0)
+    # E_S of the ground eigenvector = lambda_min of the dense matrix (library eigensolver)
+    H = orc.dense(n, h1, eri, 0.0, dets)
+    w, V = np.linalg.eigh(H)
+    e0, _ = ctx.energy(torch.from_numpy(np.ascontiguousarray(V[:, 0])).cuda())
+    assert abs(e0 - w[0]) <= 1e-12 * abs(w[0])
+    ctx.close()
+
+
+def test_orbital_index_63(pkg, orc):
+    """n = 64: bit 63 of both words in use (maximum size of the determinant store's key)."""
+    n, na, nb = 64, 2, 1
+    h1, eri = make_integrals(n, 6, 4242)
+    rng = np.random.default_rng(1)
+    dets = set()
+    dets.add(((1 << 63) | 1, 1 << 63)); dets.add((3, 1)); dets.add(((1 << 63) | (1 << 62), 1 << 62))
+    while len(dets) < 300:
+        a = rng.choice(n, 2, replace=False); b = rng.integers(0, n)
+        dets.add(((1 << int(a[0])) | (1 << int(a[1])), 1 << int(b)))
+    dets = np.array(sorted(dets), dtype=np.uint64)
+    p = dict(n=n, na=na, nb=nb, h1=h1, eri=eri, e_core=0.0, dets=dets, psi=rng.standard_normal(len(dets)))
+    _full_parity(pkg, orc, p, 1e-4, 1e-4, parts=(0, 8))
+    ctx = _ctx(pkg, p)
+    _check_connections(ctx, orc, p, [0, len(dets) - 1, len(dets) // 2], [0.0, 1e-2])
+    ctx.close()
+
+
+def test_eps_infinite_keeps_only_the_diagonal(pkg, orc):
+    p = make_problem("tiny", n_dets=300)
+    ctx = _ctx(pkg, p)
+    assert ctx.ham_build(float("inf")) == 300
+    rp, col, val = (t.cpu().numpy() for t in ctx.csr())
+    assert np.array_equal(col, np.arange(300))
+    ref = np.array([orc.diagonal(p["n"], p["h1"], p["eri"], 0.0, d) for d in p["dets"]])
+    assert np.allclose(val, ref, rtol=1e-13)
+    import torch
+    d = ctx.diagonals(torch.from_numpy(p["dets"].view(np.int64)).cuda()).cpu().numpy()
+    assert np.allclose(d, ref, rtol=1e-13)
+    ctx.close()
+
+
+def test_invalid_subspaces_are_errors(pkg):
+    p = make_problem("tiny", n_dets=100)
+    ctx = pkg.create(p["n"], p["na"], p["nb"], p["h1"], p["eri"], 0.0)
+    d = p["dets"].copy()
+    with pytest.raises(pkg.DethamError) as e:
+        ctx.set_subspace(d[::-1].copy())
+    assert e.value.status == "DH_EUNSORTED"
+    dup = d.copy(); dup[5] = dup[4]
+    with pytest.raises(pkg.DethamError) as e:
+        ctx.set_subspace(dup)
+    assert e.value.status == "DH_EUNSORTED"
+    bad = d.copy(); bad[-1, 0] = np.uint64((1 << 10) - 1)  # ten alpha electrons instead of five
+    with pytest.raises(pkg.DethamError) as e:
+        ctx.set_subspace(bad)
+    assert e.value.status == "DH_EPOPCOUNT"
+    hi = d.copy(); hi[-1, 1] = np.uint64(0b1111 | (1 << 20))  # right count, but orbital 20 >= n_orb = 10
+    with pytest.raises(pkg.DethamError) as e:
+        ctx.set_subspace(hi)
+    assert e.value.status == "DH_EPOPCOUNT"
+    with pytest.raises(pkg.DethamError):
+        ctx.ham_build(-1.0)
+    ctx.set_subspace(d)
+    with pytest.raises(pkg.DethamError):
+        ctx.ham_build(float("nan"))
+    ctx.close()
+
+
+def test_table_overflow_is_reported(pkg):
+    p = make_problem("tiny", n_dets=500)
+    ctx = _ctx(pkg, p)
+    ctx.pt2_config(1024, 1)  # far too small for ~4e4 externals
+    with pytest.raises(pkg.DethamError) as e:
+        ctx.pt2(_psi(p), -20.0, 0.0)
+    assert e.value.status == "DH_ETABLEFULL"
+    ctx.pt2_config(0, 0)  # and the context recovers
+    pt2, n_ext, _ = ctx.pt2(_psi(p), -20.0, 0.0)
+    assert n_ext > 1000 and np.isfinite(pt2)
+    ctx.close()
+
+
+def test_solve_host_end_to_end(pkg, orc):
+    p = make_problem("tiny", n_dets=800)
+    ctx = pkg.create(p["n"], p["na"], p["nb"], p["h1"], p["eri"], 0.0)
+    e, pt2, nnz, n_ext = ctx.solve_host(p["dets"], p["psi"], 1e-4, 1e-5)
+    ref = orc.ham_build(p["n"], p["h1"], p["eri"], 0.0, p["dets"], 1e-4)
+    e_ref, _ = orc.energy(*ref, p["psi"])
+    o = orc.pt2(p["n"], p["h1"], p["eri"], 0.0, p["dets"], p["psi"], e_ref, 1e-5)
+    assert nnz == len(ref[1]) and n_ext == o["n_external"]
+    assert abs(e - e_ref) <= E_TOL * abs(e_ref)
+    assert abs(pt2 - o["pt2"]) <= 10 * PT2_TOL * abs(o["pt2"])  # E_S differs by 1e-10 relative between the two sides
+    ctx.close()
