@@ -1,0 +1,294 @@
+#!/usr/bin/env python
+"""bench.py — one "step" = one pass of the whole hot path over one synthetic workload:
+determinant-store build -> ham_build(eps) -> energy -> pt2(E_S, eps2), all inside libdetham.so's CUDA kernels.
+
+  python bench.py [--gpus N] [--steps K] [--warmup W] [--workload tiny|h2o|n2|cr2|n2sweep] [--n-dets M] [--impl reference]
+
+Prints ONE JSON line (rank 0).  metric = evaluated (screen-passing) Slater-Condon elements per second over the whole
+step; `roofline` is for the dominant kernel (pt2_accumulate_kernel) with the algorithmic bytes of SURVEY.md 8(d);
+`cpu_baseline` is the oracle timed on a bounded sample of the same workload on the host cores.
+"""
+from __future__ import annotations
+
+import argparse
+import json
+import os
+import statistics
+import subprocess
+import sys
+import threading
+import time
+
+import numpy as np
+
+ROOT = os.path.dirname(os.path.abspath(__file__))
+if ROOT not in sys.path:
+    sys.path.insert(0, ROOT)
+
+METRIC = "hamiltonian_elements_per_sec"
+UNIT = "elements/s"
+DEFAULT_WORKLOAD = "h2o"
+
+
+def load_peaks():
+    path = os.path.join(ROOT, "MEASURED_PEAKS.json")
+    if os.path.exists(path):
+        with open(path) as f:
+            return float(json.load(f)["hbm_gbs"]), "measured (MEASURED_PEAKS.json hbm_gbs, burst copy)"
+    return 6650.0, "fallback (B200_PROFILING.md 6.65 TB/s)"
+
+
+class ClockSampler:
+    """nvidia-smi clocks / throttle reasons sampled DURING the timed region."""
+    Q = ("clocks.sm,clocks.max.sm,power.draw,clocks_event_reasons.hw_slowdown,clocks_event_reasons.hw_thermal_slowdown,"
+         "clocks_event_reasons.sw_thermal_slowdown,clocks_event_reasons.sw_power_cap")
+
+    def __init__(self, index=0):
+        self.index, self.rows, self.proc = index, [], None
+
+    def start(self):
+        try:
+            self.proc = subprocess.Popen(["nvidia-smi", f"--id={self.index}", f"--query-gpu={self.Q}",
+                                          "--format=csv,noheader,nounits", "-lms", "100"], stdout=subprocess.PIPE, text=True)
+            threading.Thread(target=self._read, daemon=True).start()
+        except Exception:
+            self.proc = None
+
+    def _read(self):
+        for line in self.proc.stdout:
+            self.rows.append([x.strip() for x in line.split(",")])
+
+    def stop(self):
+        if self.proc is None:
+            return {"sm_mhz": None, "sm_max_mhz": None, "reasons": ["nvidia-smi unavailable"]}
+        time.sleep(0.15)
+        self.proc.terminate()
+        sm, mx, reasons = [], None, set()
+        names = ["hw_slowdown", "hw_thermal_slowdown", "sw_thermal_slowdown", "sw_power_cap"]
+        for r in self.rows:
+            try:
+                sm.append(float(r[0])); mx = float(r[1])
+                for k, nm in enumerate(names):
+                    if r[3 + k].lower().startswith("active"):
+                        reasons.add(nm)
+            except Exception:
+                pass
+        return {"sm_mhz": statistics.median(sm) if sm else None, "sm_max_mhz": mx, "reasons": sorted(reasons),
+                "samples": len(sm)}
+
+
+def oracle_sample(p, m_sources, seed=1):
+    """The oracle, as it stands, on a bounded sample: `m_sources` sources of the same S (always including the largest
+    |psi|); ham_build restricted to those rows + energy + pt2 with psi masked to them.  Returns elements/s in the
+    metric's unit: elements = sum over sampled sources of |conn(D_i, eps)| + |conn(D_i, tau_i)| (counted untimed)."""
+    import oracle
+    nd = len(p["psi"])
+    rng = np.random.default_rng(seed)
+    keep = np.unique(np.concatenate([[int(np.argmax(np.abs(p["psi"])))], rng.choice(nd, size=min(m_sources, nd), replace=False)]))
+    mask = np.zeros(nd); mask[keep] = 1.0
+    psi_m = p["psi"] * mask
+    t0 = time.perf_counter()
+    rp, col, val = oracle.ham_build(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"], p["eps"], rows=keep)
+    e, _ = oracle.energy(rp, col, val, psi_m)
+    r = oracle.pt2(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"], psi_m, e - 1.0, p["eps2"], n_parts=1)
+    dt = time.perf_counter() - t0
+    elements = 0
+    for i in keep[: min(len(keep), 64)]:  # untimed: the metric's numerator for the sampled sources (extrapolated from 64)
+        tau = p["eps2"] / abs(p["psi"][i]) if p["eps2"] > 0 else 0.0
+        elements += len(oracle.connections(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"][i], p["eps"])[1])
+        elements += len(oracle.connections(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"][i], tau)[1])
+    elements = elements * len(keep) / min(len(keep), 64)
+    return dict(seconds=dt, elements=elements, sources=len(keep), threads=oracle.num_threads(), n_contrib=r["n_contrib"])
+
+
+def sample_size(p):
+    exc = {"tiny": 875, "h2o": 12635, "n2": 30723, "n2sweep": 30723, "cr2": 404712}[p["name"]]
+    # ~1.2e8 element visits (two enumerations per source) plus the serial sort + H_aa work is 10-30 s of oracle time
+    return int(max(16, min(len(p["psi"]), 6e7 / exc)))
+
+
+def run_reference(args, p):
+    """--impl reference: the oracle on the host cores; each step = one bounded sample of the workload."""
+    times, last = [], None
+    m = max(8, sample_size(p) // 4)
+    for it in range(args.warmup + args.steps):
+        last = oracle_sample(p, m, seed=it)
+        if it >= args.warmup:
+            times.append(last["seconds"])
+    ms = 1e3 * sum(times) / len(times)
+    value = last["elements"] / (ms * 1e-3)
+    sample = f"{last['sources']} of {len(p['psi'])} sources per step (ham_build rows + energy + pt2 with psi masked), full S and integrals"
+    return {"impl": "reference", "metric": METRIC, "value": value, "unit": UNIT, "n_gpus": args.gpus, "steps": args.steps,
+            "warmup": args.warmup, "ms_per_step": ms, "higher_is_better": True, "scaling": "weak", "vs_baseline": None,
+            "dtype": "f64", "data": "synthetic", "config": workload_config(p),
+            "cpu_baseline": {"value": value, "unit": UNIT, "cores": last["threads"], "kind": "oracle", "sample": sample},
+            "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
+
+
+def workload_config(p):
+    return {"workload": f"{p['name']}-shaped synthetic: n_orb={p['n']}, N_alpha+N_beta={p['na']}+{p['nb']}, |S|={len(p['psi'])}, "
+                        f"eps={p['eps']:g}, eps2={p['eps2']:g}",
+            "n_orb": p["n"], "n_dets": int(len(p["psi"])), "eps": p["eps"], "eps2": p["eps2"],
+            "l2": "flushed between timed steps (256 MiB write); PT2 table >> L2 anyway"}
+
+
+def main():
+    ap = argparse.ArgumentParser()
+    ap.add_argument("--gpus", type=int, default=1)
+    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--warmup", type=int, default=3)
+    ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
+    ap.add_argument("--workload", default=DEFAULT_WORKLOAD)
+    ap.add_argument("--n-dets", type=int, default=None)
+    ap.add_argument("--n-parts", type=int, default=0, help="pt2 key partitions (0 = planned by the library)")
+    ap.add_argument("--table-slots", type=int, default=0)
+    ap.add_argument("--no-cpu-baseline", action="store_true")
+    ap.add_argument("--no-e2e", action="store_true")
+    args = ap.parse_args()
+    args.warmup = max(args.warmup, 0)
+
+    rank = int(os.environ.get("RANK", "0"))
+    world = int(os.environ.get("WORLD_SIZE", "1"))
+    local_rank = int(os.environ.get("LOCAL_RANK", "0"))
+
+    from synth_inputs import make_problem
+    if args.impl == "reference":
+        if rank != 0:
+            return 0
+        p = make_problem(args.workload, n_dets=args.n_dets)
+        print(json.dumps(run_reference(args, p)))
+        return 0
+
+    import torch
+    import paper_2601_21310_b200 as pkg  # raises if libdetham.so is missing: there is no CPU fallback
+    if not torch.cuda.is_available():
+        raise SystemExit("bench.py: no CUDA device (the detham hot path has no CPU fallback)")
+    torch.cuda.set_device(local_rank)
+    dist = None
+    if world > 1:
+        import torch.distributed as dist
+        dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
+
+    p = make_problem(args.workload, n_dets=args.n_dets)
+    nd = len(p["psi"])
+    ctx = pkg.create(p["n"], p["na"], p["nb"], p["h1"], p["eri"], p["e_core"])
+    ctx.pt2_config(args.table_slots, args.n_parts)
+    dets_dev = torch.from_numpy(p["dets"].view(np.int64)).cuda()
+    psi_dev = torch.from_numpy(p["psi"]).cuda()
+    flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
+
+    def step():
+        ctx.set_subspace(dets_dev)
+        ctx.ham_build(p["eps"])
+        e, _ = ctx.energy(psi_dev)
+        pt2, n_ext, n_con = ctx.pt2(psi_dev, e, p["eps2"])
+        return e, pt2
+
+    def barrier():
+        torch.cuda.synchronize()
+        if dist is not None:
+            dist.barrier()
+        torch.cuda.synchronize()
+
+    for _ in range(args.warmup):
+        step()
+    sampler = ClockSampler(local_rank)
+    barrier()
+    sampler.start()
+    step_ms, phases = [], []
+    for _ in range(args.steps):
+        flush.fill_(1)
+        torch.cuda.synchronize()
+        t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+        t0.record()
+        e_s, pt2 = step()
+        t1.record()
+        torch.cuda.synchronize()
+        step_ms.append(t0.elapsed_time(t1))
+        phases.append(ctx.counters())
+    barrier()
+    clocks = sampler.stop()
+    total_ms = sum(step_ms)
+    if dist is not None:
+        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
+        dist.all_reduce(t, op=dist.ReduceOp.MAX)
+        total_ms = float(t.item())
+    ms_per_step = total_ms / args.steps
+    c = phases[-1]
+    elements = c["build_generated"] + c["pt2_generated"]
+    value = world * elements / (ms_per_step * 1e-3)
+
+    # ---- roofline of the dominant kernel (pt2_accumulate_kernel), algorithmic bytes per SURVEY.md 8(d)
+    peak, peak_src = load_peaks()
+    parts = max(1, c["pt2_parts"])
+    acc_ms = statistics.mean(x["ms_pt2_accum"] for x in phases) / parts  # average launch duration
+    bytes_accum_launch = (32.0 * c["pt2_contrib"] + 24.0 * nd * parts) / parts
+    achieved = bytes_accum_launch / (acc_ms * 1e-3) / 1e9
+    mean = lambda k: statistics.mean(x[k] for x in phases)
+    t_energy, t_pt2 = mean("ms_energy"), mean("ms_pt2_plan") + mean("ms_pt2_accum") + mean("ms_pt2_scan")
+    b_energy = 12.0 * c["nnz"] + 8.0 * (nd + 1) + 16.0 * nd
+    b_pt2 = 32.0 * c["pt2_contrib"] + 32.0 * c["pt2_external"] + 24.0 * nd
+    path_gbs = (b_energy + b_pt2) / ((t_energy + t_pt2) * 1e-3) / 1e9
+    roofline = {"bound": "hbm", "kernel": "pt2_accumulate_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+                "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
+                "bytes_per_launch": bytes_accum_launch, "launch_ms": acc_ms, "launches_per_step": parts,
+                "energy_plus_pt2_GBps": path_gbs, "energy_plus_pt2_frac": path_gbs / peak}
+    traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
+    if os.path.exists(traffic_file):
+        try:
+            tr = json.load(open(traffic_file)).get(args.workload)
+            if tr:
+                roofline["traffic"] = tr["dram_bytes_per_launch"]
+        except Exception:
+            pass
+
+    out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
+           "ms_per_step": ms_per_step, "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+           "data": "synthetic", "config": workload_config(p), "clocks": clocks, "roofline": roofline,
+           "phases_ms": {k: mean(k) for k in ("ms_store", "ms_build_count", "ms_build_fill", "ms_energy", "ms_pt2_plan",
+                                              "ms_pt2_accum", "ms_pt2_scan")},
+           "counters": {k: c[k] for k in ("nnz", "build_generated", "pt2_generated", "pt2_contrib", "pt2_external",
+                                          "pt2_parts", "pt2_max_probe", "pt2_table_slots", "pt2_sum_abs", "pt2_min_abs_den")},
+           "results": {"E_S": e_s, "PT2": pt2}, "es_pt2_wall_ms": mean("ms_build_count") + mean("ms_build_fill") + t_energy + t_pt2,
+           "stored_nnz_per_sec": c["nnz"] / ((mean("ms_build_count") + mean("ms_build_fill")) * 1e-3),
+           "gpu_launches": 7 + 2 + (1 if c["ms_pt2_plan"] > 0 else 0) + 2 + 4 * parts}
+
+    # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
+    if not args.no_e2e:
+        dets_pin = torch.from_numpy(p["dets"].view(np.int64)).pin_memory()
+        psi_pin = torch.from_numpy(p["psi"]).pin_memory()
+        dh, ph = dets_pin.numpy().view(np.uint64), psi_pin.numpy()
+        ctx.solve_host(dh, ph, p["eps"], p["eps2"])
+        e2e_ms = []
+        for _ in range(max(2, min(args.steps, 3))):
+            flush.fill_(1)
+            torch.cuda.synchronize()
+            t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+            t0.record()
+            ctx.solve_host(dh, ph, p["eps"], p["eps2"])
+            t1.record()
+            torch.cuda.synchronize()
+            e2e_ms.append(t0.elapsed_time(t1))
+        e2e_total = sum(e2e_ms) / len(e2e_ms)
+        if dist is not None:
+            t = torch.tensor([e2e_total], dtype=torch.float64, device="cuda")
+            dist.all_reduce(t, op=dist.ReduceOp.MAX)
+            e2e_total = float(t.item())
+        out["e2e"] = {"value": world * elements / (e2e_total * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 24 * nd,
+                      "d2h_bytes_per_step": 32, "ms_per_step": e2e_total}
+
+    if rank == 0 and world == 1 and not args.no_cpu_baseline:
+        s = oracle_sample(p, sample_size(p))
+        out["cpu_baseline"] = {"value": s["elements"] / s["seconds"], "unit": UNIT, "cores": s["threads"], "kind": "oracle",
+                               "sample": f"{s['sources']} of {nd} sources (ham_build rows + energy + pt2 with psi masked to them) "
+                                         f"on the full S and integrals, {s['seconds']:.1f} s; host has {os.cpu_count()} cpus"}
+    if rank == 0:
+        print(json.dumps(out))
+    ctx.close()
+    if dist is not None:
+        dist.destroy_process_group()
+    return 0
+
+
+if __name__ == "__main__":
+    sys.exit(main())

@@ -42,7 +42,7 @@ def lib():
         L.orc_zobrist.restype = C.c_uint64
         L.orc_zobrist.argtypes = [up]
         L.orc_ham_build.restype = C.c_void_p
-        L.orc_ham_build.argtypes = [C.c_int, dp, dp, C.c_double, up, C.c_int64, C.c_double]
+        L.orc_ham_build.argtypes = [C.c_int, dp, dp, C.c_double, up, C.c_int64, C.c_double, ip, C.c_int64]
         L.orc_csr_nnz.restype = C.c_int64
         L.orc_csr_nnz.argtypes = [C.c_void_p]
         L.orc_csr_copy.restype = None
@@ -121,11 +121,15 @@ def connections(n, h1, eri, e_core, det, tau):
         cap = int(m)
 
 
-def ham_build(n, h1, eri, e_core, dets, eps):
-    """CSR H_SS: (row_ptr int64 [|S|+1], col int32 [nnz], val fp64 [nnz])."""
+def ham_build(n, h1, eri, e_core, dets, eps, rows=None):
+    """CSR H_SS: (row_ptr int64 [|S|+1], col int32 [nnz], val fp64 [nnz]).  rows: optional subset of rows to build."""
     h1, eri, dets = _f64(h1), _f64(eri), _u64(dets)
     nd = dets.shape[0]
-    hnd = lib().orc_ham_build(n, _d(h1), _d(eri), e_core, _u(dets), nd, eps)
+    if rows is None:
+        hnd = lib().orc_ham_build(n, _d(h1), _d(eri), e_core, _u(dets), nd, eps, None, 0)
+    else:
+        rows = np.ascontiguousarray(rows, dtype=np.int64)
+        hnd = lib().orc_ham_build(n, _d(h1), _d(eri), e_core, _u(dets), nd, eps, _i(rows), rows.shape[0])
     nnz = lib().orc_csr_nnz(hnd)
     row_ptr = np.empty(nd + 1, dtype=np.int64)
     col = np.empty(nnz, dtype=np.int32)

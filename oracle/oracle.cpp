@@ -211,12 +211,16 @@ u64 orc_zobrist(const u64* det) { return zobrist({det[0], det[1]}); }
 
 // ham_build (reading Q4): row i = {(i, diag(D_i))} U {(j, H) : (D_j, H) in conn(D_i, eps), D_j in S}, columns ascending.
 // Returns an opaque handle; read it with orc_csr_nnz / orc_csr_copy, free with orc_csr_free.
-void* orc_ham_build(int n, const double* h1, const double* eri_, double e_core, const u64* dets, int64_t nd, double eps) {
+// `row_list` (may be NULL = all rows): build only the listed rows; the other rows are left empty (bounded-sample timing).
+void* orc_ham_build(int n, const double* h1, const double* eri_, double e_core, const u64* dets, int64_t nd, double eps,
+                    const int64_t* row_list, int64_t n_rows) {
   Integrals I{n, h1, eri_, e_core};
   const Det* S = reinterpret_cast<const Det*>(dets);
   std::vector<std::vector<std::pair<int32_t, double>>> rows(nd);
+  const int64_t n_do = row_list ? n_rows : nd;
 #pragma omp parallel for schedule(dynamic, 16)
-  for (int64_t i = 0; i < nd; ++i) {
+  for (int64_t k = 0; k < n_do; ++k) {
+    const int64_t i = row_list ? row_list[k] : k;
     std::vector<Conn> c;
     connections(I, S[i], eps, &c);
     auto& r = rows[i];
