@@ -1,6 +1,7 @@
 // C ABI entry points (include/detham.h): argument checks, context lifetime, host<->device plumbing.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <numeric>
@@ -47,6 +48,13 @@ dh_status detham_create(detham_ctx** out, int n_orb, int n_alpha, int n_beta, co
   auto fail = [&](dh_status s) { free_all(c); delete c; return s; };
   auto body = [&]() -> dh_status {
     DH_CUDA(c, cudaGetDevice(&c->device));
+    // The PT2 table is probed one 32-byte sector at a time at random addresses: ask L2 not to fetch neighbouring sectors.
+    // (A hint; DETHAM_L2_FETCH = 32 | 64 | 128 overrides it for tuning.)
+    {
+      size_t gran = 32;
+      if (const char* e = getenv("DETHAM_L2_FETCH")) { int v = atoi(e); if (v == 32 || v == 64 || v == 128) gran = (size_t)v; }
+      if (cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, gran) != cudaSuccess) cudaGetLastError();
+    }
     DH_CUDA(c, cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device));
     const int64_t n = n_orb, npair = n * (n + 1) / 2;
     c->n_eri = npair * (npair + 1) / 2;

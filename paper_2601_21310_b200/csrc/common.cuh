@@ -71,7 +71,7 @@ struct detham_ctx {
   // pt2
   int64_t cfg_table_slots = 0;
   int cfg_parts = 0;
-  void* table = nullptr;
+  void* table = nullptr;      // zero between calls (the scan clears what it reads)
   int64_t table_slots = 0;
   std::vector<double> partials;
 
@@ -166,5 +166,29 @@ __device__ __forceinline__ int dh_parity_between(u64 w, int x, int y) {
   u64 m = ((1ull << hi) - 1ull) & ~((2ull << lo) - 1ull);
   return __popcll(w & m) & 1;
 }
+
+// lookup in the L2-resident open-addressing index of S (built by shash_insert_kernel): index of (ka, kb) or -1
+__device__ __forceinline__ int dh_shash_find(const u64* __restrict__ keys, const int* __restrict__ idx, u64 cap, u64 ka, u64 kb, u64 z) {
+  u64 slot = __umul64hi(z, cap);
+  for (;;) {
+    ulonglong2 k = __ldg(reinterpret_cast<const ulonglong2*>(keys) + slot);
+    if (k.x == ka && k.y == kb) return __ldg(idx + slot);
+    if (k.x == 0ull && k.y == 0ull) return -1;
+    if (++slot == cap) slot = 0;
+  }
+}
+
+// 32-byte streaming store / load of one PT2 contribution record (evict-first: each is touched once)
+__device__ __forceinline__ void dh_st256_cs(void* p, u64 a, u64 b, u64 c, u64 d) {
+  asm volatile("st.global.cs.v4.u64 [%0], {%1,%2,%3,%4};" ::"l"(p), "l"(a), "l"(b), "l"(c), "l"(d) : "memory");
+}
+
+// hash of a 128-bit determinant key for the PT2 bins and tables (independent of the key-partition words)
+__device__ __forceinline__ u64 dh_keymix(u64 ka, u64 kb) {
+  u64 m = (ka * 0x9E3779B97F4A7C15ull) ^ (kb * 0xC2B2AE3D27D4EB4Full);
+  m ^= m >> 32; m *= 0xD6E8FEB86659FD93ull; m ^= m >> 32;
+  return m;
+}
+__device__ __forceinline__ u64 dh_keymix2(u64 m) { m = (m ^ (m >> 31)) * 0x94D049BB133111EBull; return m ^ (m >> 29); }
 
 #endif  // __CUDACC__

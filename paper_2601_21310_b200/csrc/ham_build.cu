@@ -34,16 +34,6 @@ __global__ void shash_insert_kernel(const u64* __restrict__ dets, int64_t nd, u6
   }
 }
 
-__device__ __forceinline__ int shash_find(const u64* __restrict__ keys, const int* __restrict__ idx, u64 cap, u64 ka, u64 kb, u64 z) {
-  u64 slot = __umul64hi(z, cap);
-  for (;;) {
-    ulonglong2 k = __ldg(reinterpret_cast<const ulonglong2*>(keys) + slot);
-    if (k.x == ka && k.y == kb) return __ldg(idx + slot);
-    if (k.x == 0ull && k.y == 0ull) return -1;
-    if (++slot == cap) slot = 0;
-  }
-}
-
 // ---------------------------------------------------------------- CSR sinks
 struct BuildSink {
   static constexpr bool kLookupFirst = true;
@@ -55,14 +45,14 @@ struct BuildSink {
   int pre_tok;
   __device__ __forceinline__ bool pre(u64 ka, u64 kb, u64 z) {
     ++generated;
-    pre_tok = shash_find(keys, idx, cap, ka, kb, z);
+    pre_tok = dh_shash_find(keys, idx, cap, ka, kb, z);
     return pre_tok >= 0;
   }
   __device__ __forceinline__ void emit(bool act, u64 ka, u64 kb, u64 z, double H, int kind, int, int, int, int, int) {
     int tok = -1;
     if (act) {
       if (kind == 0) tok = pre_tok;
-      else { ++generated; tok = shash_find(keys, idx, cap, ka, kb, z); }
+      else { ++generated; tok = dh_shash_find(keys, idx, cap, ka, kb, z); }
     }
     unsigned hit = __ballot_sync(0xffffffffu, tok >= 0);
     if (hit) {

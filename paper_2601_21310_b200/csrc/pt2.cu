@@ -1,6 +1,7 @@
 // pt2 (a8, a9): external-determinant deduplication in an HBM open-addressing hash on 128-bit keys and the
 // Epstein-Nesbet reduction (Eq. 13 second term; screening Eq. 14 / PAPER.md:219-227).
 #include <math.h>
+#include <stdlib.h>
 
 #include "enumerate.cuh"
 
@@ -17,6 +18,7 @@ struct __align__(32) Slot { u64 ka, kb; double v, haa; };
 
 __device__ __forceinline__ double member_flag() { return __longlong_as_double(0x7ff8000000000001ll); }
 
+
 // ---------------------------------------------------------------- class histogram (pass planning)
 struct CountSink {
   static constexpr bool kLookupFirst = true;  // singles are counted (upper bound) without being evaluated
@@ -28,8 +30,8 @@ struct CountSink {
 };
 
 __global__ void __launch_bounds__(kWarpsPerCta * 32)
-count_kernel(EnumParams P, const u64* __restrict__ dets, const double* __restrict__ psi, int64_t nd, double eps2,
-             u64* counters, u64* __restrict__ hist) {
+count_kernel(EnumParams P, const u64* __restrict__ dets, const double* __restrict__ psi, int64_t nd, int64_t stride,
+             double eps2, u64* counters, u64* __restrict__ hist) {
   extern __shared__ __align__(16) unsigned char smem[];
   CtaTables T = dh_cta_stage(P, smem);
   size_t off = (dh_cta_table_bytes(P.n) + 15) & ~(size_t)15;
@@ -43,7 +45,7 @@ count_kernel(EnumParams P, const u64* __restrict__ dets, const double* __restric
   for (;;) {
     u64 row = 0;
     if (lane == 0) row = atomicAdd(counters, 1ull);
-    row = __shfl_sync(0xffffffffu, row, 0);
+    row = __shfl_sync(0xffffffffu, row, 0) * (u64)stride;  // every stride-th source (stride 1 = exact histogram)
     if ((int64_t)row >= nd) break;
     const double p = psi[row];
     const u64 da = dets[2 * row], db = dets[2 * row + 1];
@@ -82,76 +84,308 @@ __global__ void member_insert_kernel(const u64* __restrict__ dets, int64_t nd, u
 }
 
 // ---------------------------------------------------------------- accumulate
-struct Pt2Sink {
-  static constexpr bool kLookupFirst = false;
-  Slot* table; u64 cap;
-  const CtaTables* T; const WarpScratch* ws; int n;
-  double psi, e0;
-  u64 gen, contrib;
-  int max_probe;
-  int* overflow;
-  __device__ __forceinline__ bool pre(u64, u64, u64) { return true; }
-  __device__ __forceinline__ void emit(bool act, u64 ka, u64 kb, u64 z, double H, int kind, int s, int i, int j, int a, int b) {
-    if (!act) return;
-    ++gen;
-    const double cval = H * psi;
-    u64 slot = __umul64hi(z, cap);
-    int probes = 0;
-    for (;;) {
-      Slot* sp = table + slot;
-      u64 k0, k1, vb, hb;
-      dh_ld256(sp, k0, k1, vb, hb);
-      if (k0 == ka && k1 == kb) {
-        if (vb != (u64)0x7ff8000000000001ull) { atomicAdd(&sp->v, cval); ++contrib; }  // not a member of S
-        break;
-      }
-      if (k0 == 0ull && k1 == 0ull) {
-        Key128 old = dh_cas128(sp, Key128{0ull, 0ull}, Key128{ka, kb});
-        if (old.a == 0ull && old.b == 0ull) {  // claimed: this thread also records H_aa
-          sp->haa = dh_excited_diag(*T, *ws, n, e0, kind, s, i, j, a, b);
-          atomicAdd(&sp->v, cval);
-          ++contrib;
-          break;
-        }
-        if (old.a == ka && old.b == kb) { atomicAdd(&sp->v, cval); ++contrib; break; }  // lost the race to the same key
-      }
-      if (++slot == cap) slot = 0;
-      if (++probes > kProbeLimit) { *overflow = 1; break; }
-    }
-    max_probe = max(max_probe, probes);
-  }
+// One warp per source determinant, one CTA per SM.  Per (source, pass):
+//   singles  - candidates of this pass's key class are compacted into a small queue and evaluated 32 at a time
+//              (reading Q5: every single is evaluated exactly, in the order of reading Q7);
+//   doubles  - phase A: every occupied pair (i,j) looks up its class sub-list and finds, by a galloping search on the
+//              magnitude-sorted values, the prefix with |value| >= tau (the paper's early exit, taken as
+//              a search instead of a walk); empty prefixes are dropped and the lengths prefix-summed;
+//              phase B: the concatenation of all prefixes is walked 32*kU entries at a time, so every lane holds an
+//              entry whatever the individual prefix lengths are, and each lane issues kU independent table probes
+//              before it waits on any of them.
+constexpr int kChunk = 256;     // occupied pairs per phase-A chunk
+// kAccWarps warps per CTA and kU table probes in flight per lane are template parameters of the kernel
+
+struct FlatScratch {
+  u64 zij[kChunk];               // partition word of the source with (i,j) removed
+  int pref[kChunk + 1];          // exclusive prefix of the kept lengths
+  int beg[kChunk];               // first list entry of the kept prefix
+  unsigned short meta[kChunk];   // fam << 12 | i << 6 | j
+  unsigned short sq[64];         // singles queue: s << 12 | i << 6 | a
 };
 
-__global__ void __launch_bounds__(kWarpsPerCta * 32)
+// entry meta: kind << 25 | s << 24 | i << 18 | j << 12 | a << 6 | b
+__device__ __forceinline__ unsigned pack_meta(int kind, int s, int i, int j, int a, int b) {
+  return ((unsigned)kind << 25) | ((unsigned)s << 24) | ((unsigned)i << 18) | ((unsigned)j << 12) | ((unsigned)a << 6) | (unsigned)b;
+}
+
+struct ProbeCtx {
+  Slot* table; u64 cap;
+  const CtaTables* T; const WarpScratch* ws; int n;
+  double e0;
+  unsigned contrib; int max_probe;
+  int* overflow;
+};
+
+__device__ __forceinline__ double meta_diag(const ProbeCtx& pc, unsigned m) {
+  return dh_excited_diag(*pc.T, *pc.ws, pc.n, pc.e0, (int)(m >> 25), (int)((m >> 24) & 1u), (int)((m >> 18) & 63u),
+                         (int)((m >> 12) & 63u), (int)((m >> 6) & 63u), (int)(m & 63u));
+}
+
+// Resolve up to U candidates per lane: all pending slots are loaded before any is examined, all needed CAS are issued
+// before any result is used.  A slot is {key, v, H_aa}; members of S carry the NaN flag in v and absorb nothing.
+template <int U>
+__device__ __forceinline__ void probe_batch(ProbeCtx& pc, const u64 (&ka)[U], const u64 (&kb)[U], const double (&cv)[U],
+                                            u64 (&slot)[U], const unsigned (&meta)[U], unsigned pend) {
+  if (!pend) return;
+  int probes = 0;
+  for (;;) {
+    u64 k0[U], k1[U], vb[U], hb[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u)
+      if ((pend >> u) & 1u) dh_ld256(pc.table + slot[u], k0[u], k1[u], vb[u], hb[u]);
+    unsigned cas = 0;
+#pragma unroll
+    for (int u = 0; u < U; ++u)
+      if ((pend >> u) & 1u) {
+        if (k0[u] == ka[u] && k1[u] == kb[u]) {
+          if (vb[u] != (u64)0x7ff8000000000001ull) { atomicAdd(&pc.table[slot[u]].v, cv[u]); ++pc.contrib; }
+          pend &= ~(1u << u);
+        } else if ((k0[u] | k1[u]) == 0ull) {
+          cas |= 1u << u;
+        } else if (++slot[u] == pc.cap) {
+          slot[u] = 0;
+        }
+      }
+    if (cas) {
+#pragma unroll
+      for (int u = 0; u < U; ++u)
+        if ((cas >> u) & 1u) {
+          Key128 old = dh_cas128(pc.table + slot[u], Key128{0ull, 0ull}, Key128{ka[u], kb[u]});
+          k0[u] = old.a; k1[u] = old.b;
+        }
+#pragma unroll
+      for (int u = 0; u < U; ++u)
+        if ((cas >> u) & 1u) {
+          if ((k0[u] | k1[u]) == 0ull) {  // claimed: this thread also records H_aa
+            pc.table[slot[u]].haa = meta_diag(pc, meta[u]);
+            atomicAdd(&pc.table[slot[u]].v, cv[u]); ++pc.contrib;
+            pend &= ~(1u << u);
+          } else if (k0[u] == ka[u] && k1[u] == kb[u]) {  // lost the race to the same key (never a member: those are pre-inserted)
+            atomicAdd(&pc.table[slot[u]].v, cv[u]); ++pc.contrib;
+            pend &= ~(1u << u);
+          } else if (++slot[u] == pc.cap) {
+            slot[u] = 0;
+          }
+        }
+    }
+    if (!pend) break;
+    if (++probes > kProbeLimit) { *pc.overflow = 1; break; }
+  }
+  pc.max_probe = max(pc.max_probe, probes);
+}
+
+// decode the triangular index t = y(y-1)/2 + x, x < y
+__device__ __forceinline__ void tri_decode(int t, int& x, int& y) {
+  y = (int)((1.0f + sqrtf(1.0f + 8.0f * (float)t)) * 0.5f);
+  while (y * (y - 1) / 2 > t) --y;
+  while ((y + 1) * y / 2 <= t) ++y;
+  x = t - y * (y - 1) / 2;
+}
+
+template <int kAccWarps, int kU>
+__global__ void __launch_bounds__(kAccWarps * 32, 1)
 pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* __restrict__ psi, int64_t nd, double eps2,
                       unsigned pass, Slot* table, u64 cap, u64* counters /* [0] next row [1] gen [2] contrib [3] max probe */,
                       int* overflow) {
   extern __shared__ __align__(16) unsigned char smem[];
   CtaTables T = dh_cta_stage(P, smem);
-  WarpScratch* wsp = reinterpret_cast<WarpScratch*>(smem + ((dh_cta_table_bytes(P.n) + 15) & ~(size_t)15));
+  size_t off = (dh_cta_table_bytes(P.n) + 15) & ~(size_t)15;
+  WarpScratch* wsp = reinterpret_cast<WarpScratch*>(smem + off);
+  FlatScratch* fsp = reinterpret_cast<FlatScratch*>(smem + off + kAccWarps * sizeof(WarpScratch));
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  const unsigned lt = (1u << lane) - 1u;
   WarpScratch& ws = wsp[warp];
-  Pt2Sink sink{table, cap, &T, &ws, P.n, 0.0, 0.0, 0ull, 0ull, 0, overflow};
+  FlatScratch& fs = fsp[warp];
+  const int n = P.n, na = P.na, nb = P.nb;
+  const unsigned pmask = (1u << P.pbits) - 1u;
+  const int NP = 1 << P.pbits;
+  const int nAA = na * (na - 1) / 2, nBB = nb * (nb - 1) / 2, npairs = nAA + nBB + na * nb;
+  const int nva = n - na, nvb = n - nb, tot_a = na * nva, tot_s = tot_a + nb * nvb;
+  ProbeCtx pc{table, cap, &T, &ws, n, 0.0, 0u, 0, overflow};
+  u64 gen_total = 0, contrib_total = 0;
   for (;;) {
     u64 row = 0;
     if (lane == 0) row = atomicAdd(counters, 1ull);
     row = __shfl_sync(0xffffffffu, row, 0);
     if ((int64_t)row >= nd) break;
+    if (*reinterpret_cast<volatile int*>(overflow)) break;
     const double p = psi[row];
     if (p == 0.0) continue;  // reading Q6: a source with zero amplitude generates nothing
     const double tau = eps2 == 0.0 ? 0.0 : __ddiv_rn(eps2, fabs(p));
     const u64 da = dets[2 * row], db = dets[2 * row + 1];
     dh_fill_occ(P, ws, da, db, lane);
-    sink.psi = p;
-    sink.e0 = dh_fill_U(P, T, ws, lane);
+    pc.e0 = dh_fill_U(P, T, ws, lane);
+    pc.contrib = 0u;
+    unsigned gen = 0u;
     u64 zsrc = 0;
     if (lane == 0) zsrc = dh_zobrist(da, db, T.Z);
     zsrc = __shfl_sync(0xffffffffu, zsrc, 0);
-    dh_enumerate(P, T, ws, da, db, tau, zsrc, pass, sink, lane);
-    __syncwarp();
+
+    // ---- singles
+    {
+      int qn = 0;
+      for (int t0 = 0; t0 < tot_s + 32; t0 += 32) {
+        const bool last = t0 >= tot_s;
+        if (!last) {
+          const int t = t0 + lane;
+          bool in = t < tot_s;
+          unsigned code = 0;
+          if (in) {
+            const int s = t >= tot_a ? 1 : 0, tt = s ? t - tot_a : t, nv = s ? nvb : nva;
+            const int i = ws.occ[s][tt / nv], a = ws.vir[s][tt % nv];
+            const u64 z = zsrc ^ T.Z[64 * s + i] ^ T.Z[64 * s + a];
+            in = ((unsigned)z & pmask) == pass;
+            code = ((unsigned)s << 12) | ((unsigned)i << 6) | (unsigned)a;
+          }
+          const unsigned m = __ballot_sync(0xffffffffu, in);
+          if (in) fs.sq[qn + __popc(m & lt)] = (unsigned short)code;
+          qn += __popc(m);
+          __syncwarp();
+        }
+        if (qn >= 32 || (last && qn > 0)) {
+          const int take = qn >= 32 ? 32 : qn;
+          u64 ka[1] = {da}, kb[1] = {db}, slot[1] = {0};
+          double cv[1] = {0.0};
+          unsigned meta[1] = {0u};
+          unsigned pend = 0u;
+          if (lane < take) {
+            const unsigned code = fs.sq[qn - take + lane];
+            const int s = (int)(code >> 12), i = (int)((code >> 6) & 63u), a = (int)(code & 63u);
+            const u64 w = s ? db : da;
+            const double v = dh_single_value(P, ws, w, s, i, a);
+            if (v != 0.0 && fabs(v) >= tau) {
+              const u64 nw = (w ^ (1ull << i)) | (1ull << a);
+              if (s == 0) ka[0] = nw; else kb[0] = nw;
+              const u64 z = zsrc ^ T.Z[64 * s + i] ^ T.Z[64 * s + a];
+              slot[0] = __umul64hi(z, cap);
+              cv[0] = v * p;
+              meta[0] = pack_meta(0, s, i, 0, a, 0);
+              pend = 1u;
+            }
+          }
+          __syncwarp();
+          qn -= take;
+          gen += pend;
+          probe_batch<1>(pc, ka, kb, cv, slot, meta, pend);
+        }
+      }
+    }
+
+    // ---- doubles
+    for (int qb = 0; qb < npairs; qb += kChunk) {
+      const int qe = min(npairs, qb + kChunk);
+      int cnt = 0, run = 0;
+      // phase A: kept prefix of every pair's class sub-list
+      for (int q0 = qb; q0 < qe; q0 += 32) {
+        const int q = q0 + lane;
+        int len = 0, beg = 0;
+        unsigned pm = 0;
+        u64 zij = 0;
+        if (q < qe) {
+          int fam, i, j, seg;
+          if (q < nAA) { int x, y; tri_decode(q, x, y); fam = 0; i = ws.occ[0][x]; j = ws.occ[0][y]; seg = j * (j - 1) / 2 + i; zij = zsrc ^ T.Z[i] ^ T.Z[j]; }
+          else if (q < nAA + nBB) { int x, y; tri_decode(q - nAA, x, y); fam = 1; i = ws.occ[1][x]; j = ws.occ[1][y]; seg = P.nss + j * (j - 1) / 2 + i; zij = zsrc ^ T.Z[64 + i] ^ T.Z[64 + j]; }
+          else { const int r = q - nAA - nBB; fam = 2; i = ws.occ[0][r / nb]; j = ws.occ[1][r % nb]; seg = 2 * P.nss + i * n + j; zij = zsrc ^ T.Z[i] ^ T.Z[64 + j]; }
+          const unsigned cls = ((unsigned)zij ^ pass) & pmask;
+          const int64_t so = (int64_t)seg * NP + cls;
+          beg = __ldg(P.sub_off + so);
+          const int end = __ldg(P.sub_off + so + 1);
+          int lo = beg, hi = end;
+          if (tau != 0.0) {  // first index whose |value| < tau: gallop from the head (most kept prefixes are short), then bisect
+            int pos = beg, step = 1;
+            while (pos < end && fabs(__ldg(P.lval + pos)) >= tau) { lo = pos + 1; pos += step; step <<= 1; }
+            hi = min(pos, end);
+            while (lo < hi) {
+              const int mid = (lo + hi) >> 1;
+              if (fabs(__ldg(P.lval + mid)) >= tau) lo = mid + 1; else hi = mid;
+            }
+          } else {
+            lo = end;
+          }
+          len = lo - beg;
+          pm = ((unsigned)fam << 12) | ((unsigned)i << 6) | (unsigned)j;
+        }
+        const unsigned m = __ballot_sync(0xffffffffu, len > 0);
+        int x = len;
+#pragma unroll
+        for (int o = 1; o < 32; o <<= 1) { int y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+        const int tot = __shfl_sync(0xffffffffu, x, 31);
+        if (len > 0) {
+          const int idx = cnt + __popc(m & lt);
+          fs.pref[idx] = run + x - len; fs.beg[idx] = beg; fs.meta[idx] = (unsigned short)pm; fs.zij[idx] = zij;
+        }
+        cnt += __popc(m);
+        run += tot;
+      }
+      if (lane == 0) fs.pref[cnt] = run;
+      __syncwarp();
+      // phase B: walk the concatenated prefixes
+      const int TT = run;
+      int qcur = 0;
+      for (int t0 = 0; t0 < TT; t0 += 32 * kU) {
+        u64 ka[kU], kb[kU], slot[kU];
+        double cv[kU];
+        unsigned meta[kU];
+        unsigned pend = 0u;
+#pragma unroll
+        for (int u = 0; u < kU; ++u) {
+          ka[u] = da; kb[u] = db; slot[u] = 0; cv[u] = 0.0; meta[u] = 0u;
+          const int tt = t0 + 32 * u;
+          if (tt < TT) {  // warp-uniform
+            const int pe = (qcur + lane < cnt) ? fs.pref[qcur + lane + 1] - tt : 0x7fffffff;  // end of pair qcur+lane, relative
+            const unsigned bm = __reduce_or_sync(0xffffffffu, pe < 32 ? (1u << pe) : 0u);
+            const int adv = __popc(__ballot_sync(0xffffffffu, pe <= 32));
+            const int myq = qcur + __popc(bm & ((2u << lane) - 1u));
+            qcur += adv;
+            const int t = tt + lane;
+            if (t < TT) {
+              const int k = fs.beg[myq] + (t - fs.pref[myq]);
+              const unsigned pm = fs.meta[myq];
+              double v = __ldg(P.lval + k);
+              const unsigned ab = __ldg(P.lab + k);
+              const int a = (int)(ab & 0xFFu), b = (int)(ab >> 8);
+              const int fam = (int)(pm >> 12), i = (int)((pm >> 6) & 63u), j = (int)(pm & 63u);
+              const u64 zij = fs.zij[myq];
+              bool act = v != 0.0;
+              if (fam < 2) {
+                const u64 w = fam ? db : da;
+                act = act && !((w >> a) & 1ull) && !((w >> b) & 1ull);
+                if (act) {
+                  const u64 nw = (w ^ (1ull << i) ^ (1ull << j)) | (1ull << a) | (1ull << b);
+                  if (fam == 0) ka[u] = nw; else kb[u] = nw;
+                  const u64 z = zij ^ T.Z[64 * fam + a] ^ T.Z[64 * fam + b];
+                  // a+_a a+_b a_j a_i = (a+_b a_j)(a+_a a_i): phase(i->a on w) * phase(j->b on w with i->a applied)
+                  const int par = dh_parity_between(w, i, a) ^ dh_parity_between((w ^ (1ull << i)) | (1ull << a), j, b);
+                  if (par) v = -v;
+                  slot[u] = __umul64hi(z, cap);
+                  meta[u] = pack_meta(1, fam, i, j, a, b);
+                }
+              } else {
+                act = act && !((da >> a) & 1ull) && !((db >> b) & 1ull);
+                if (act) {
+                  ka[u] = (da ^ (1ull << i)) | (1ull << a);
+                  kb[u] = (db ^ (1ull << j)) | (1ull << b);
+                  const u64 z = zij ^ T.Z[a] ^ T.Z[64 + b];
+                  if (dh_parity_between(da, i, a) ^ dh_parity_between(db, j, b)) v = -v;
+                  slot[u] = __umul64hi(z, cap);
+                  meta[u] = pack_meta(2, 0, i, j, a, b);
+                }
+              }
+              if (act) { cv[u] = v * p; pend |= 1u << u; }
+            }
+          }
+        }
+        gen += __popc(pend);
+        probe_batch<kU>(pc, ka, kb, cv, slot, meta, pend);
+      }
+      __syncwarp();
+    }
+    gen_total += gen;
+    contrib_total += pc.contrib;
   }
-  u64 g = sink.gen, ct = sink.contrib;
-  int mp = sink.max_probe;
+  u64 g = gen_total, ct = contrib_total;
+  int mp = pc.max_probe;
   for (int o = 16; o > 0; o >>= 1) {
     g += __shfl_xor_sync(0xffffffffu, g, o);
     ct += __shfl_xor_sync(0xffffffffu, ct, o);
@@ -168,16 +402,26 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
 __global__ void __launch_bounds__(256)
 pt2_scan_kernel(Slot* table, u64 cap, double e_s, double* __restrict__ part /* [grid][4]: sum, sum_abs, min_den, count */) {
   double sum = 0.0, sabs = 0.0, mden = INFINITY, cnt = 0.0;
-  for (u64 t = (u64)blockIdx.x * blockDim.x + threadIdx.x; t < cap; t += (u64)gridDim.x * blockDim.x) {
-    struct { u64 x, y, z, w; } q;
-    dh_ld256_cs(table + t, q.x, q.y, q.z, q.w);
-    if (q.x | q.y) {
-      if (q.z != (u64)0x7ff8000000000001ull) {
-        double v = __longlong_as_double((long long)q.z), den = e_s - __longlong_as_double((long long)q.w);
-        double term = v * v / den;
-        sum += term; sabs += fabs(term); mden = fmin(mden, fabs(den)); cnt += 1.0;
+  constexpr int V = 4;  // independent 32-byte loads in flight per thread
+  const u64 stride = (u64)gridDim.x * blockDim.x;
+  for (u64 t0 = (u64)blockIdx.x * blockDim.x + threadIdx.x; t0 < cap; t0 += V * stride) {
+    u64 x[V], y[V], z[V], w[V];
+#pragma unroll
+    for (int k = 0; k < V; ++k) {
+      x[k] = y[k] = z[k] = w[k] = 0ull;
+      const u64 t = t0 + k * stride;
+      if (t < cap) dh_ld256_cs(table + t, x[k], y[k], z[k], w[k]);
+    }
+#pragma unroll
+    for (int k = 0; k < V; ++k) {
+      if (x[k] | y[k]) {
+        if (z[k] != (u64)0x7ff8000000000001ull) {
+          double v = __longlong_as_double((long long)z[k]), den = e_s - __longlong_as_double((long long)w[k]);
+          double term = v * v / den;
+          sum += term; sabs += fabs(term); mden = fmin(mden, fabs(den)); cnt += 1.0;
+        }
+        dh_st256_zero(table + t0 + k * stride);
       }
-      dh_st256_zero(table + t);
     }
   }
   __shared__ double sh[4][8];
@@ -274,73 +518,43 @@ static dh_status ensure_table(detham_ctx* c, int64_t slots) {
   if (c->table) cudaFree(c->table);
   c->table = nullptr; c->table_slots = 0;
   DH_CUDA(c, cudaMalloc(&c->table, (size_t)slots * sizeof(Slot)));
-  DH_CUDA(c, cudaMemsetAsync(c->table, 0, (size_t)slots * sizeof(Slot), c->stream));
+  DH_CUDA(c, cudaMemsetAsync(c->table, 0, (size_t)slots * sizeof(Slot), c->stream));  // the scan keeps it zero afterwards
   c->table_slots = slots;
   return DH_OK;
 }
 
-dh_status dh_pt2(detham_ctx* c, const double* psi, double e_s, double eps2, double* out) {
+// One attempt at the whole PT2 with 2^pbits key partitions and a table of `slots` slots.  `adapt`: after pass 0 the
+// capacity used by the later passes is shrunk to (distinct keys of pass 0) / load, which cuts the scan traffic when the
+// table was sized from the contribution count (an upper bound of the distinct keys).
+static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, double eps2, int pbits, int64_t slots, bool adapt,
+                             double load, double* out) {
   const int64_t nd = c->nd;
-  const size_t smem_base = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + kWarpsPerCta * sizeof(WarpScratch);
-  int64_t want = (nd + kWarpsPerCta - 1) / kWarpsPerCta;
-  const int grid = (int)(want < (int64_t)c->sm_count * 4 ? want : (int64_t)c->sm_count * 4);
-  dh_status st;
-  u64* hp = reinterpret_cast<u64*>(c->pinned);
-
-  // ---- plan: partition count and table capacity
-  int pbits = 0;
-  int64_t slots = c->cfg_table_slots;
-  c->ctr.ms_pt2_plan = 0.0;
-  if (c->cfg_parts > 0) { while ((1 << pbits) < c->cfg_parts) ++pbits; }
-  if (c->cfg_parts == 0 || slots == 0) {
-    const HbLists* L0 = nullptr;
-    st = dh_get_lists(c, 0, &L0); if (st != DH_OK) return st;
-    EnumParams P0 = dh_make_params(c, L0);
-    size_t smem = smem_base + kFine * sizeof(unsigned);
-    DH_CUDA(c, cudaFuncSetAttribute(count_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-    DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 8 * sizeof(u64), c->stream));
-    DH_CUDA(c, cudaMemsetAsync(c->hist, 0, kFine * sizeof(u64), c->stream));
-    DH_TICK(c, 0);
-    count_kernel<<<grid, kWarpsPerCta * 32, smem, c->stream>>>(P0, c->dets, psi, nd, eps2, c->dcount, reinterpret_cast<u64*>(c->hist));
-    DH_CUDA(c, cudaGetLastError());
-    DH_TICK(c, 1);
-    std::vector<u64> hist(kFine);
-    DH_CUDA(c, cudaMemcpyAsync(hist.data(), c->hist, kFine * sizeof(u64), cudaMemcpyDeviceToHost, c->stream));
-    DH_CUDA(c, cudaStreamSynchronize(c->stream));
-    c->ctr.ms_pt2_plan = dh_elapsed(c, 0, 1);
-    size_t free_b = 0, total_b = 0;
-    DH_CUDA(c, cudaMemGetInfo(&free_b, &total_b));
-    int64_t max_slots = (int64_t)(((double)free_b + (double)c->table_slots * sizeof(Slot)) * 0.92 / sizeof(Slot));
-    if (slots > 0) max_slots = slots;
-    auto max_class = [&](int pb) {
-      u64 m = 0;
-      for (int cl = 0; cl < (1 << pb); ++cl) { u64 s = 0; for (int f = cl; f < kFine; f += (1 << pb)) s += hist[f]; if (s > m) m = s; }
-      return (int64_t)m;
-    };
-    if (c->cfg_parts == 0) {
-      pbits = 0;
-      while (pbits < DH_MAX_PBITS && (double)max_class(pbits) > 0.7 * (double)max_slots) ++pbits;
-      if ((double)max_class(pbits) > 0.7 * (double)max_slots) return DH_ETABLEFULL;
-    }
-    if (slots == 0) {
-      int64_t need = (int64_t)((double)max_class(pbits) / 0.5) + 1024;
-      slots = need < max_slots ? need : max_slots;
-    }
-  }
-  st = ensure_table(c, slots); if (st != DH_OK) return st;
+  dh_status st = ensure_table(c, slots); if (st != DH_OK) return st;
   Slot* table = reinterpret_cast<Slot*>(c->table);
-
   const HbLists* L = nullptr;
   st = dh_get_lists(c, pbits, &L); if (st != DH_OK) return st;
   EnumParams P = dh_make_params(c, L);
-  DH_CUDA(c, cudaFuncSetAttribute(pt2_accumulate_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem_base));
+  // launch shape: (warps per CTA, probes in flight per lane); DETHAM_PT2_VARIANT selects another one for tuning
+  using AccKernel = void (*)(EnumParams, const u64*, const double*, int64_t, double, unsigned, Slot*, u64, u64*, int*);
+  struct Variant { int warps, u; AccKernel k; };
+  static const Variant variants[] = {{16, 1, pt2_accumulate_kernel<16, 1>}, {16, 2, pt2_accumulate_kernel<16, 2>},
+                                     {12, 4, pt2_accumulate_kernel<12, 4>}, {8, 4, pt2_accumulate_kernel<8, 4>}};
+  int vi = 0;
+  if (const char* e = getenv("DETHAM_PT2_VARIANT")) { int v = atoi(e); if (v >= 0 && v < (int)(sizeof(variants) / sizeof(variants[0]))) vi = v; }
+  const int warps = variants[vi].warps;
+  AccKernel acc_kernel = variants[vi].k;
+  const size_t smem = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + warps * (sizeof(WarpScratch) + sizeof(FlatScratch));
+  DH_CUDA(c, cudaFuncSetAttribute(acc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int64_t want = (nd + warps - 1) / warps;
+  const int grid = (int)(want < (int64_t)c->sm_count ? want : (int64_t)c->sm_count);
 
   const int nparts = 1 << pbits;
-  const int sgrid = (int)(((slots + 255) / 256) < (int64_t)c->sm_count * 16 ? ((slots + 255) / 256) : (int64_t)c->sm_count * 16);
-  st = dh_ensure_red(c, 4 * ((int64_t)sgrid + 64) + 4 * (int64_t)(nparts + 1)); if (st != DH_OK) return st;
+  const int sgrid_max = c->sm_count * 16;
+  st = dh_ensure_red(c, 4 * ((int64_t)sgrid_max + 64) + 4 * (int64_t)(nparts + 1)); if (st != DH_OK) return st;
   double* results = c->red;                        // [nparts + 1][4]; row nparts = psi^T psi
   double* part = c->red + 4 * (int64_t)(nparts + 1);
   int* overflow = reinterpret_cast<int*>(c->dcount + 8);
+  u64* hp = reinterpret_cast<u64*>(c->pinned);
   DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 32 * sizeof(u64), c->stream));
 
   norm2_kernel<<<64, 256, 0, c->stream>>>(psi, nd, part);
@@ -349,22 +563,31 @@ dh_status dh_pt2(detham_ctx* c, const double* psi, double e_s, double eps2, doub
 
   u64 gen = 0, contrib = 0, max_probe = 0;
   double ms_accum = 0.0, ms_scan = 0.0;
+  int64_t cap = slots;
   for (int pass = 0; pass < nparts; ++pass) {
+    const int64_t sblocks = (cap + 1023) / 1024;
+    const int sgrid = (int)(sblocks < sgrid_max ? sblocks : sgrid_max);
     DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 4 * sizeof(u64), c->stream));
     DH_TICK(c, 2);
-    member_insert_kernel<<<(unsigned)((nd + 255) / 256), 256, 0, c->stream>>>(c->dets, nd, (unsigned)(nparts - 1), (unsigned)pass, table, (u64)slots, overflow);
-    pt2_accumulate_kernel<<<grid, kWarpsPerCta * 32, smem_base, c->stream>>>(P, c->dets, psi, nd, eps2, (unsigned)pass, table, (u64)slots, c->dcount, overflow);
+    member_insert_kernel<<<(unsigned)((nd + 255) / 256), 256, 0, c->stream>>>(c->dets, nd, (unsigned)(nparts - 1), (unsigned)pass, table, (u64)cap, overflow);
+    acc_kernel<<<grid, warps * 32, smem, c->stream>>>(P, c->dets, psi, nd, eps2, (unsigned)pass, table, (u64)cap, c->dcount, overflow);
     DH_TICK(c, 3);
-    pt2_scan_kernel<<<sgrid, 256, 0, c->stream>>>(table, (u64)slots, e_s, part);
+    pt2_scan_kernel<<<sgrid, 256, 0, c->stream>>>(table, (u64)cap, e_s, part);
     final_reduce4_kernel<<<1, 256, 0, c->stream>>>(part, sgrid, results + 4 * pass);
     DH_CUDA(c, cudaGetLastError());
     DH_TICK(c, 4);
     DH_CUDA(c, cudaMemcpyAsync(hp, c->dcount, 4 * sizeof(u64), cudaMemcpyDeviceToHost, c->stream));
     DH_CUDA(c, cudaMemcpyAsync(hp + 4, overflow, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(c, cudaMemcpyAsync(hp + 8, results + 4 * pass, 4 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     DH_CUDA(c, cudaStreamSynchronize(c->stream));
     ms_accum += dh_elapsed(c, 2, 3); ms_scan += dh_elapsed(c, 3, 4);
     gen += hp[1]; contrib += hp[2]; if (hp[3] > max_probe) max_probe = hp[3];
     if (*reinterpret_cast<int*>(hp + 4)) return DH_ETABLEFULL;  // the scan above already cleared the table
+    if (adapt && pass == 0 && nparts > 1) {
+      const double u0 = reinterpret_cast<double*>(hp + 8)[3] + (double)nd / nparts;  // distinct externals + members of one class
+      const double need = (u0 + 8.0 * sqrt(u0) + 1024.0) / load;
+      if (need < (double)cap) cap = (int64_t)need;
+    }
   }
   std::vector<double> res(4 * (size_t)(nparts + 1));
   DH_CUDA(c, cudaMemcpyAsync(res.data(), results, res.size() * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
@@ -388,6 +611,78 @@ dh_status dh_pt2(detham_ctx* c, const double* psi, double e_s, double eps2, doub
   c->ctr.ms_pt2_accum = ms_accum;
   c->ctr.ms_pt2_scan = ms_scan;
   return DH_OK;
+}
+
+dh_status dh_pt2(detham_ctx* c, const double* psi, double e_s, double eps2, double* out) {
+  const int64_t nd = c->nd;
+  dh_status st;
+  double load = 0.5;  // target load factor of the table (DETHAM_PT2_LOAD overrides; tuning knob)
+  if (const char* e = getenv("DETHAM_PT2_LOAD")) { double v = atof(e); if (v >= 0.05 && v <= 0.9) load = v; }
+  // Random 32-byte accesses fall off a cliff once their footprint exceeds what the GPU's TLBs cover: measured on B200,
+  // 36 G sectors/s up to 64 GB, 29 at 80 GB, 17 at 96 GB, 8.7 at 160 GB (profiles/r1_microbench.md).  More passes over a
+  // smaller table beat fewer passes over a bigger one, so the table never exceeds this many bytes unless configured.
+  double max_table_gb = 60.0;
+  if (const char* e = getenv("DETHAM_PT2_MAX_TABLE_GB")) { double v = atof(e); if (v >= 0.001 && v <= 4096.0) max_table_gb = v; }
+
+  // ---- plan: partition count and table capacity
+  int pbits = 0;
+  int64_t slots = c->cfg_table_slots;
+  const bool auto_parts = c->cfg_parts == 0, auto_slots = slots == 0;
+  c->ctr.ms_pt2_plan = 0.0;
+  if (!auto_parts) { while ((1 << pbits) < c->cfg_parts) ++pbits; }
+  int64_t max_slots = slots;
+  if (auto_parts || auto_slots) {
+    // class histogram of the contributions: exact for small inputs, else from every stride-th source (scaled, +10 %);
+    // it only sizes the table - an underestimate is caught by the overflow flag and retried with more partitions
+    const HbLists* L0 = nullptr;
+    st = dh_get_lists(c, 0, &L0); if (st != DH_OK) return st;
+    EnumParams P0 = dh_make_params(c, L0);
+    const size_t smem = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + kWarpsPerCta * sizeof(WarpScratch) + kFine * sizeof(unsigned);
+    const int64_t stride = nd <= 32768 ? 1 : nd / 16384;
+    const int64_t ns = (nd + stride - 1) / stride;
+    int64_t want = (ns + kWarpsPerCta - 1) / kWarpsPerCta;
+    const int grid = (int)(want < (int64_t)c->sm_count * 4 ? want : (int64_t)c->sm_count * 4);
+    DH_CUDA(c, cudaFuncSetAttribute(count_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 8 * sizeof(u64), c->stream));
+    DH_CUDA(c, cudaMemsetAsync(c->hist, 0, kFine * sizeof(u64), c->stream));
+    DH_TICK(c, 0);
+    count_kernel<<<grid, kWarpsPerCta * 32, smem, c->stream>>>(P0, c->dets, psi, nd, stride, eps2, c->dcount, reinterpret_cast<u64*>(c->hist));
+    DH_CUDA(c, cudaGetLastError());
+    DH_TICK(c, 1);
+    std::vector<u64> hist(kFine);
+    DH_CUDA(c, cudaMemcpyAsync(hist.data(), c->hist, kFine * sizeof(u64), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(c, cudaStreamSynchronize(c->stream));
+    c->ctr.ms_pt2_plan = dh_elapsed(c, 0, 1);
+    const double scale = stride == 1 ? 1.0 : 1.1 * (double)stride;
+    size_t free_b = 0, total_b = 0;
+    DH_CUDA(c, cudaMemGetInfo(&free_b, &total_b));
+    max_slots = (int64_t)(((double)free_b + (double)c->table_slots * sizeof(Slot)) * 0.92 / sizeof(Slot));
+    const int64_t tlb_slots = (int64_t)(max_table_gb * 1e9 / sizeof(Slot));
+    if (max_slots > tlb_slots) max_slots = tlb_slots;
+    if (!auto_slots) max_slots = slots;
+    auto max_class = [&](int pb) {
+      u64 m = 0;
+      for (int cl = 0; cl < (1 << pb); ++cl) { u64 s = 0; for (int f = cl; f < kFine; f += (1 << pb)) s += hist[f]; if (s > m) m = s; }
+      return (double)m * scale + 64.0;
+    };
+    if (auto_parts) {
+      // contributions bound the distinct keys from above; 0.9 of the slots at worst (all distinct) still terminates,
+      // and the typical duplication keeps the real load well below that
+      pbits = 0;
+      while (pbits < DH_MAX_PBITS && max_class(pbits) > 0.9 * (double)max_slots) ++pbits;
+      if (max_class(pbits) > 0.9 * (double)max_slots) return DH_ETABLEFULL;
+    }
+    if (auto_slots) {
+      int64_t need = (int64_t)(max_class(pbits) / load) + 1024;
+      slots = need < max_slots ? need : max_slots;
+    }
+  }
+  for (;;) {
+    st = pt2_attempt(c, psi, e_s, eps2, pbits, slots, auto_slots, load, out);
+    if (st != DH_ETABLEFULL || !auto_parts || pbits >= DH_MAX_PBITS) return st;
+    ++pbits;  // the plan was too optimistic: halve the keys per pass and start over
+    if (auto_slots) slots = max_slots;
+  }
 }
 
 dh_status dh_connections(detham_ctx* c, int64_t row, double tau, std::vector<u64>& keys, std::vector<double>& h) {
