@@ -57,8 +57,9 @@ typedef struct {
   double pt2_min_abs_den;   /* min_a |E_S - H_aa| */
   /* device times (CUDA events on the context's stream) of the kernels of the last calls, milliseconds */
   double ms_store;          /* set_subspace: validation + lookup-index build */
-  double ms_build_count;    /* ham_build pass 1 (enumerate + lookup, count rows) */
-  double ms_build_fill;     /* ham_build pass 2 (enumerate + lookup, write CSR) + row scan + row sort */
+  double ms_build_count;    /* ham_build enumeration pass (enumerate + lookup, hits appended to an arena) + row scan;
+                               includes the exact-size rerun when the arena of the previous build was too small */
+  double ms_build_fill;     /* ham_build arena -> CSR copy + per-row column sort */
   double ms_energy;         /* SpMV + fused reductions */
   double ms_pt2_plan;       /* pt2 class histogram (pass planning), 0 when both table_slots and n_parts are configured */
   double ms_pt2_accum;      /* pt2 member insert + enumerate/accumulate kernels, summed over passes */

@@ -67,6 +67,11 @@ struct detham_ctx {
   int64_t csr_cap = 0;
   int* row_cnt = nullptr;  // device int32 [nd]
   int64_t row_cap = 0;
+  int* acol = nullptr;     // build arena: hits in warp order, copied to col/val once the row offsets are known
+  double* aval = nullptr;
+  int64_t arena_cap = 0;   // entries
+  void* segs = nullptr;    // arena segments
+  int64_t seg_cap = 0;
 
   // pt2
   int64_t cfg_table_slots = 0;

@@ -35,14 +35,55 @@ __global__ void shash_insert_kernel(const u64* __restrict__ dets, int64_t nd, u6
 }
 
 // ---------------------------------------------------------------- CSR sinks
+// Single-pass build: every warp appends the (column, value) hits of its rows to an arena in blocks of kBlk entries
+// reserved with one atomic each; a row's hits form one or more segments {row, offset in row, arena offset, count}.
+// After the pass the row counts are scanned and the segments copied to their CSR positions.  If the arena (sized from
+// the previous build) is too small the pass keeps counting, and the host reruns it with the exact size.
+constexpr int kBlk = 1024;
+struct Seg { int row, local, cnt, pad; int64_t off; };
+
 struct BuildSink {
   static constexpr bool kLookupFirst = true;
   const u64* keys; const int* idx; u64 cap;
-  int* col; double* val;   // row destination (fill pass) or nullptr (count pass)
-  int count;               // warp-uniform running count of hits
+  int* acol; double* aval; int64_t arena_cap;
+  u64* cursors;            // [2] arena cursor, [3] segment cursor
+  Seg* segs; int64_t seg_cap; int* overflow;
+  int row;
+  int count;               // warp-uniform running count of the row's hits
+  int64_t wpos, wend;      // warp-uniform write window in the arena (wpos < 0: arena exhausted, count only)
+  int64_t seg_start; int seg_local;
   u64 generated;           // per-lane count of screened candidates looked up
   int lane;
   int pre_tok;
+  __device__ __forceinline__ void close_seg() {
+    const int64_t m = wpos - seg_start;
+    if (wpos >= 0 && m > 0 && lane == 0) {
+      u64 s = atomicAdd(cursors + 3, 1ull);
+      if ((int64_t)s < seg_cap) segs[s] = Seg{row, seg_local, (int)m, 0, seg_start};
+      else *overflow = 1;
+    }
+  }
+  __device__ __forceinline__ void begin_row(int r) { row = r; count = 0; seg_start = wpos; seg_local = 0; }
+  __device__ __forceinline__ void end_row() { close_seg(); }
+  __device__ __forceinline__ void put(bool has, int tok, double H) {
+    const unsigned hit = __ballot_sync(0xffffffffu, has);
+    if (!hit) return;
+    const int h = __popc(hit);
+    if (wpos >= 0 && wpos + h > wend) {  // block full: close the segment and reserve the next block
+      close_seg();
+      u64 b = 0;
+      if (lane == 0) b = atomicAdd(cursors + 2, (u64)kBlk);
+      b = __shfl_sync(0xffffffffu, b, 0);
+      if ((int64_t)b + kBlk > arena_cap) { wpos = -1; if (lane == 0) *overflow = 1; }
+      else { wpos = (int64_t)b; wend = wpos + kBlk; }
+      seg_start = wpos; seg_local = count;
+    }
+    if (wpos >= 0) {
+      if (has) { const int64_t pos = wpos + __popc(hit & ((1u << lane) - 1u)); acol[pos] = tok; aval[pos] = H; }
+      wpos += h;
+    }
+    count += h;
+  }
   __device__ __forceinline__ bool pre(u64 ka, u64 kb, u64 z) {
     ++generated;
     pre_tok = dh_shash_find(keys, idx, cap, ka, kb, z);
@@ -54,29 +95,21 @@ struct BuildSink {
       if (kind == 0) tok = pre_tok;
       else { ++generated; tok = dh_shash_find(keys, idx, cap, ka, kb, z); }
     }
-    unsigned hit = __ballot_sync(0xffffffffu, tok >= 0);
-    if (hit) {
-      if (col != nullptr && tok >= 0) {
-        int pos = count + __popc(hit & ((1u << lane) - 1u));
-        col[pos] = tok;
-        val[pos] = H;
-      }
-      count += __popc(hit);
-    }
+    put(tok >= 0, tok, H);
   }
 };
 
-template <bool FILL>
 __global__ void __launch_bounds__(kWarpsPerCta * 32)
 build_kernel(EnumParams P, const u64* __restrict__ dets, int64_t nd, double eps, const u64* __restrict__ hkeys,
-             const int* __restrict__ hidx, u64 hcap, int* __restrict__ row_cnt, const int64_t* __restrict__ row_ptr,
-             int* __restrict__ col, double* __restrict__ val, u64* counters /* [0]=next row, [1]=generated */) {
+             const int* __restrict__ hidx, u64 hcap, int* __restrict__ row_cnt, int* acol, double* aval, int64_t arena_cap,
+             Seg* segs, int64_t seg_cap, u64* counters /* [0] next row [1] generated [2] arena cursor [3] segments */,
+             int* overflow) {
   extern __shared__ __align__(16) unsigned char smem[];
   CtaTables T = dh_cta_stage(P, smem);
   WarpScratch* wsp = reinterpret_cast<WarpScratch*>(smem + ((dh_cta_table_bytes(P.n) + 15) & ~(size_t)15));
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   WarpScratch& ws = wsp[warp];
-  u64 gen = 0;
+  BuildSink sink{hkeys, hidx, hcap, acol, aval, arena_cap, counters, segs, seg_cap, overflow, 0, 0, 0, 0, 0, 0, 0ull, lane, -1};
   for (;;) {
     u64 row = 0;
     if (lane == 0) row = atomicAdd(counters, 1ull);
@@ -84,25 +117,32 @@ build_kernel(EnumParams P, const u64* __restrict__ dets, int64_t nd, double eps,
     if ((int64_t)row >= nd) break;
     const u64 da = dets[2 * row], db = dets[2 * row + 1];
     dh_fill_occ(P, ws, da, db, lane);
-    BuildSink sink{hkeys, hidx, hcap, nullptr, nullptr, 0, 0ull, lane, -1};
-    int64_t base = 0;
-    if (FILL) {
-      base = row_ptr[row];
-      double e0 = dh_fill_U(P, T, ws, lane);
-      if (lane == 0) { col[base] = (int)row; val[base] = e0; }
-      sink.col = col + base; sink.val = val + base; sink.count = 1;
-    }
+    const double e0 = dh_fill_U(P, T, ws, lane);
+    sink.begin_row((int)row);
+    sink.put(lane == 0, (int)row, e0);  // the diagonal is always kept (reading Q4)
     u64 zsrc = 0;
     if (lane == 0) zsrc = dh_zobrist(da, db, T.Z);
     zsrc = __shfl_sync(0xffffffffu, zsrc, 0);
     dh_enumerate(P, T, ws, da, db, eps, zsrc, 0u, sink, lane);
-    if (!FILL && lane == 0) row_cnt[row] = sink.count + 1;
-    gen += sink.generated;
+    sink.end_row();
+    if (lane == 0) row_cnt[row] = sink.count;
     __syncwarp();
   }
-  if (!FILL) {
-    for (int o = 16; o > 0; o >>= 1) gen += __shfl_xor_sync(0xffffffffu, gen, o);
-    if (lane == 0 && gen) atomicAdd(counters + 1, gen);
+  u64 gen = sink.generated;
+  for (int o = 16; o > 0; o >>= 1) gen += __shfl_xor_sync(0xffffffffu, gen, o);
+  if (lane == 0 && gen) atomicAdd(counters + 1, gen);
+}
+
+// arena segments -> CSR positions, one warp per segment
+__global__ void __launch_bounds__(256)
+copy_segs_kernel(const Seg* __restrict__ segs, int64_t nseg, const int64_t* __restrict__ row_ptr, const int* __restrict__ acol,
+                 const double* __restrict__ aval, int* __restrict__ col, double* __restrict__ val) {
+  const int lane = threadIdx.x & 31;
+  const int64_t nw = (int64_t)gridDim.x * (blockDim.x >> 5);
+  for (int64_t s = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); s < nseg; s += nw) {
+    const Seg g = segs[s];
+    const int64_t dst = row_ptr[g.row] + g.local;
+    for (int t = lane; t < g.cnt; t += 32) { col[dst + t] = acol[g.off + t]; val[dst + t] = aval[g.off + t]; }
   }
 }
 
@@ -245,26 +285,49 @@ dh_status dh_ham_build(detham_ctx* c, double eps) {
     c->row_cap = nd;
   }
   c->nnz = -1;
-  size_t smem = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + kWarpsPerCta * sizeof(WarpScratch);
-  st = set_smem(c, build_kernel<false>, smem); if (st != DH_OK) return st;
-  st = set_smem(c, build_kernel<true>, smem); if (st != DH_OK) return st;
+  const size_t smem = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + kWarpsPerCta * sizeof(WarpScratch);
+  st = set_smem(c, build_kernel, smem); if (st != DH_OK) return st;
   int64_t want = (nd + kWarpsPerCta - 1) / kWarpsPerCta;
-  int grid = (int)(want < (int64_t)c->sm_count * 4 ? want : (int64_t)c->sm_count * 4);
-  DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 8 * sizeof(u64), c->stream));
-  DH_TICK(c, 0);
-  build_kernel<false><<<grid, kWarpsPerCta * 32, smem, c->stream>>>(P, c->dets, nd, eps, c->shash_key, c->shash_idx,
-                                                                      (u64)c->shash_cap, c->row_cnt, nullptr, nullptr,
-                                                                      nullptr, c->dcount);
-  DH_CUDA(c, cudaGetLastError());
-  scan_rows_kernel<<<1, 1024, 0, c->stream>>>(c->row_cnt, nd, c->row_ptr);
-  DH_CUDA(c, cudaGetLastError());
-  DH_TICK(c, 1);
+  const int grid = (int)(want < (int64_t)c->sm_count * 4 ? want : (int64_t)c->sm_count * 4);
+  const int64_t slack = (int64_t)grid * kWarpsPerCta * kBlk;  // every warp may leave one block partly used
+  int* overflow = reinterpret_cast<int*>(c->dcount + 8);
   int64_t* h = reinterpret_cast<int64_t*>(c->pinned);
-  DH_CUDA(c, cudaMemcpyAsync(h, c->row_ptr + nd, sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
-  DH_CUDA(c, cudaMemcpyAsync(h + 1, c->dcount + 1, sizeof(u64), cudaMemcpyDeviceToHost, c->stream));
-  DH_CUDA(c, cudaStreamSynchronize(c->stream));
-  const int64_t nnz = h[0];
-  c->ctr.build_generated = h[1];
+  int64_t nnz = 0;
+  double ms_pass = 0.0;
+  int64_t want_arena = c->arena_cap > 0 ? c->arena_cap : nd * 64 + slack;  // first build: a guess; later: the last size
+  for (int attempt = 0;; ++attempt) {
+    if (c->arena_cap < want_arena) {
+      if (c->acol) cudaFree(c->acol);
+      if (c->aval) cudaFree(c->aval);
+      if (c->segs) cudaFree(c->segs);
+      c->acol = nullptr; c->aval = nullptr; c->segs = nullptr; c->arena_cap = 0;
+      c->seg_cap = nd + want_arena / kBlk + 4096;
+      DH_CUDA(c, cudaMalloc(&c->acol, want_arena * sizeof(int)));
+      DH_CUDA(c, cudaMalloc(&c->aval, want_arena * sizeof(double)));
+      DH_CUDA(c, cudaMalloc(&c->segs, c->seg_cap * sizeof(Seg)));
+      c->arena_cap = want_arena;
+    }
+    DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 16 * sizeof(u64), c->stream));
+    DH_TICK(c, 0);
+    build_kernel<<<grid, kWarpsPerCta * 32, smem, c->stream>>>(P, c->dets, nd, eps, c->shash_key, c->shash_idx, (u64)c->shash_cap,
+                                                               c->row_cnt, c->acol, c->aval, c->arena_cap,
+                                                               reinterpret_cast<Seg*>(c->segs), c->seg_cap, c->dcount, overflow);
+    DH_CUDA(c, cudaGetLastError());
+    scan_rows_kernel<<<1, 1024, 0, c->stream>>>(c->row_cnt, nd, c->row_ptr);
+    DH_CUDA(c, cudaGetLastError());
+    DH_TICK(c, 1);
+    DH_CUDA(c, cudaMemcpyAsync(h, c->row_ptr + nd, sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(c, cudaMemcpyAsync(h + 1, c->dcount, 4 * sizeof(u64), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(c, cudaMemcpyAsync(h + 5, overflow, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(c, cudaStreamSynchronize(c->stream));
+    ms_pass += dh_elapsed(c, 0, 1);
+    nnz = h[0];
+    c->ctr.build_generated = h[2];
+    if (!*reinterpret_cast<int*>(h + 5)) break;
+    if (attempt >= 1) return DH_ENOMEM;  // cannot happen: the second attempt is sized from the exact count
+    want_arena = nnz + slack;
+  }
+  const int64_t nseg = h[4];
   if (c->csr_cap < nnz) {
     if (c->col) cudaFree(c->col);
     if (c->val) cudaFree(c->val);
@@ -273,19 +336,20 @@ dh_status dh_ham_build(detham_ctx* c, double eps) {
     DH_CUDA(c, cudaMalloc(&c->val, nnz * sizeof(double)));
     c->csr_cap = nnz;
   }
-  DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 8 * sizeof(u64), c->stream));
   DH_TICK(c, 2);
-  build_kernel<true><<<grid, kWarpsPerCta * 32, smem, c->stream>>>(P, c->dets, nd, eps, c->shash_key, c->shash_idx,
-                                                                     (u64)c->shash_cap, c->row_cnt, c->row_ptr, c->col,
-                                                                     c->val, c->dcount);
-  DH_CUDA(c, cudaGetLastError());
+  {
+    int64_t blocks = (nseg + 7) / 8;
+    const int cgrid = (int)(blocks < (int64_t)c->sm_count * 8 ? (blocks > 0 ? blocks : 1) : (int64_t)c->sm_count * 8);
+    copy_segs_kernel<<<cgrid, 256, 0, c->stream>>>(reinterpret_cast<const Seg*>(c->segs), nseg, c->row_ptr, c->acol, c->aval, c->col, c->val);
+    DH_CUDA(c, cudaGetLastError());
+  }
   sort_rows_warp_kernel<<<(unsigned)((nd + kWarpsPerCta - 1) / kWarpsPerCta), kWarpsPerCta * 32, 0, c->stream>>>(c->row_ptr, nd, c->col, c->val);
   DH_CUDA(c, cudaGetLastError());
   sort_rows_cta_kernel<<<c->sm_count * 2, 1024, 0, c->stream>>>(c->row_ptr, nd, c->col, c->val);
   DH_CUDA(c, cudaGetLastError());
   DH_TICK(c, 3);
   DH_CUDA(c, cudaEventSynchronize(c->ev[3]));
-  c->ctr.ms_build_count = dh_elapsed(c, 0, 1);
+  c->ctr.ms_build_count = ms_pass;
   c->ctr.ms_build_fill = dh_elapsed(c, 2, 3);
   c->nnz = nnz;
   c->ctr.nnz = nnz;
