@@ -22,7 +22,7 @@ void free_all(detham_ctx* c) {
   auto f = [](void* p) { if (p) cudaFree(p); };
   f(c->h1); f(c->eri); f(c->J); f(c->JK); f(c->hd);
   for (auto& L : c->lists) { f(L.sub_off); f(L.val); f(L.ab); }
-  f(c->dets_owned); f(c->psi_owned); f(c->shash_key); f(c->shash_idx);
+  f(c->dets_owned); f(c->psi_owned); f(c->shash_key); f(c->shash_idx); f(c->sbits);
   f(c->row_ptr); f(c->col); f(c->val); f(c->row_cnt); f(c->acol); f(c->aval); f(c->segs); f(c->table); f(c->red); f(c->dcount); f(c->hist);
   if (c->pinned) cudaFreeHost(c->pinned);
   for (auto& e : c->ev) if (e) cudaEventDestroy(e);

@@ -58,6 +58,8 @@ struct detham_ctx {
   u64* shash_key = nullptr;   // device [shash_cap][2], open addressing, EMPTY = {0,0}
   int* shash_idx = nullptr;   // device [shash_cap]
   int64_t shash_cap = 0;
+  unsigned* sbits = nullptr;  // membership pre-filter: bit mulhi(z(D), sbits_n) set for every D in S
+  int64_t sbits_n = 0;
 
   // CSR H_SS (a6)
   int64_t* row_ptr = nullptr;
@@ -183,17 +185,10 @@ __device__ __forceinline__ int dh_shash_find(const u64* __restrict__ keys, const
   }
 }
 
-// 32-byte streaming store / load of one PT2 contribution record (evict-first: each is touched once)
-__device__ __forceinline__ void dh_st256_cs(void* p, u64 a, u64 b, u64 c, u64 d) {
-  asm volatile("st.global.cs.v4.u64 [%0], {%1,%2,%3,%4};" ::"l"(p), "l"(a), "l"(b), "l"(c), "l"(d) : "memory");
+// membership pre-filter of the determinant store: false = certainly not in S (one 4-byte L2 load)
+__device__ __forceinline__ bool dh_maybe_member(const unsigned* __restrict__ bits, u64 nbits, u64 z) {
+  const u64 h = __umul64hi(z, nbits);
+  return (__ldg(bits + (h >> 5)) >> (h & 31)) & 1u;
 }
-
-// hash of a 128-bit determinant key for the PT2 bins and tables (independent of the key-partition words)
-__device__ __forceinline__ u64 dh_keymix(u64 ka, u64 kb) {
-  u64 m = (ka * 0x9E3779B97F4A7C15ull) ^ (kb * 0xC2B2AE3D27D4EB4Full);
-  m ^= m >> 32; m *= 0xD6E8FEB86659FD93ull; m ^= m >> 32;
-  return m;
-}
-__device__ __forceinline__ u64 dh_keymix2(u64 m) { m = (m ^ (m >> 31)) * 0x94D049BB133111EBull; return m ^ (m >> 29); }
 
 #endif  // __CUDACC__

@@ -19,14 +19,18 @@ __global__ void validate_kernel(const u64* __restrict__ dets, int64_t nd, int n,
 }
 
 // L2-resident open-addressing index of S: slot = mulhi(z(D), cap), linear probing, EMPTY = {0,0}
-__global__ void shash_insert_kernel(const u64* __restrict__ dets, int64_t nd, u64* keys, int* idx, u64 cap) {
+__global__ void shash_insert_kernel(const u64* __restrict__ dets, int64_t nd, u64* keys, int* idx, u64 cap, unsigned* bits,
+                                    u64 nbits) {
   __shared__ u64 Z[128];
   for (int t = threadIdx.x; t < 128; t += blockDim.x) Z[t] = dh_zword(t);
   __syncthreads();
   int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= nd) return;
   u64 a = dets[2 * t], b = dets[2 * t + 1];
-  u64 slot = __umul64hi(dh_zobrist(a, b, Z), cap);
+  const u64 z = dh_zobrist(a, b, Z);
+  const u64 hb = __umul64hi(z, nbits);  // membership pre-filter: one bit per determinant (dh_member)
+  atomicOr(bits + (hb >> 5), 1u << (hb & 31));
+  u64 slot = __umul64hi(z, cap);
   for (;;) {
     Key128 old = dh_cas128(keys + 2 * slot, Key128{0ull, 0ull}, Key128{a, b});
     if (old.a == 0ull && old.b == 0ull) { idx[slot] = (int)t; return; }
@@ -45,6 +49,7 @@ struct Seg { int row, local, cnt, pad; int64_t off; };
 struct BuildSink {
   static constexpr bool kLookupFirst = true;
   const u64* keys; const int* idx; u64 cap;
+  const unsigned* bits; u64 nbits;
   int* acol; double* aval; int64_t arena_cap;
   u64* cursors;            // [2] arena cursor, [3] segment cursor
   Seg* segs; int64_t seg_cap; int* overflow;
@@ -86,14 +91,14 @@ struct BuildSink {
   }
   __device__ __forceinline__ bool pre(u64 ka, u64 kb, u64 z) {
     ++generated;
-    pre_tok = dh_shash_find(keys, idx, cap, ka, kb, z);
+    pre_tok = dh_maybe_member(bits, nbits, z) ? dh_shash_find(keys, idx, cap, ka, kb, z) : -1;
     return pre_tok >= 0;
   }
   __device__ __forceinline__ void emit(bool act, u64 ka, u64 kb, u64 z, double H, int kind, int, int, int, int, int) {
     int tok = -1;
     if (act) {
       if (kind == 0) tok = pre_tok;
-      else { ++generated; tok = dh_shash_find(keys, idx, cap, ka, kb, z); }
+      else { ++generated; if (dh_maybe_member(bits, nbits, z)) tok = dh_shash_find(keys, idx, cap, ka, kb, z); }
     }
     put(tok >= 0, tok, H);
   }
@@ -101,7 +106,7 @@ struct BuildSink {
 
 __global__ void __launch_bounds__(kWarpsPerCta * 32)
 build_kernel(EnumParams P, const u64* __restrict__ dets, int64_t nd, double eps, const u64* __restrict__ hkeys,
-             const int* __restrict__ hidx, u64 hcap, int* __restrict__ row_cnt, int* acol, double* aval, int64_t arena_cap,
+             const int* __restrict__ hidx, u64 hcap, const unsigned* __restrict__ hbits, u64 hnbits, int* __restrict__ row_cnt, int* acol, double* aval, int64_t arena_cap,
              Seg* segs, int64_t seg_cap, u64* counters /* [0] next row [1] generated [2] arena cursor [3] segments */,
              int* overflow) {
   extern __shared__ __align__(16) unsigned char smem[];
@@ -109,7 +114,7 @@ build_kernel(EnumParams P, const u64* __restrict__ dets, int64_t nd, double eps,
   WarpScratch* wsp = reinterpret_cast<WarpScratch*>(smem + ((dh_cta_table_bytes(P.n) + 15) & ~(size_t)15));
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   WarpScratch& ws = wsp[warp];
-  BuildSink sink{hkeys, hidx, hcap, acol, aval, arena_cap, counters, segs, seg_cap, overflow, 0, 0, 0, 0, 0, 0, 0ull, lane, -1};
+  BuildSink sink{hkeys, hidx, hcap, hbits, hnbits, acol, aval, arena_cap, counters, segs, seg_cap, overflow, 0, 0, 0, 0, 0, 0, 0ull, lane, -1};
   for (;;) {
     u64 row = 0;
     if (lane == 0) row = atomicAdd(counters, 1ull);
@@ -255,8 +260,18 @@ dh_status dh_build_shash(detham_ctx* c) {
     DH_CUDA(c, cudaMalloc(&c->shash_idx, cap * sizeof(int)));
     c->shash_cap = cap;
   }
+  int64_t nbits = 1 << 16;  // >= 64 bits per determinant: < 1.6 % of non-members pass the filter
+  while (nbits < 64 * c->nd && nbits < (1ll << 28)) nbits <<= 1;
+  if (nbits != c->sbits_n) {
+    if (c->sbits) cudaFree(c->sbits);
+    c->sbits = nullptr; c->sbits_n = 0;
+    DH_CUDA(c, cudaMalloc(&c->sbits, nbits / 8));
+    c->sbits_n = nbits;
+  }
+  DH_CUDA(c, cudaMemsetAsync(c->sbits, 0, nbits / 8, c->stream));
   DH_CUDA(c, cudaMemsetAsync(c->shash_key, 0, cap * 2 * sizeof(u64), c->stream));
-  shash_insert_kernel<<<(unsigned)((c->nd + 255) / 256), 256, 0, c->stream>>>(c->dets, c->nd, c->shash_key, c->shash_idx, (u64)cap);
+  shash_insert_kernel<<<(unsigned)((c->nd + 255) / 256), 256, 0, c->stream>>>(c->dets, c->nd, c->shash_key, c->shash_idx, (u64)cap,
+                                                                            c->sbits, (u64)nbits);
   DH_CUDA(c, cudaGetLastError());
   return DH_OK;
 }
@@ -310,7 +325,7 @@ dh_status dh_ham_build(detham_ctx* c, double eps) {
     DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 16 * sizeof(u64), c->stream));
     DH_TICK(c, 0);
     build_kernel<<<grid, kWarpsPerCta * 32, smem, c->stream>>>(P, c->dets, nd, eps, c->shash_key, c->shash_idx, (u64)c->shash_cap,
-                                                               c->row_cnt, c->acol, c->aval, c->arena_cap,
+                                                               c->sbits, (u64)c->sbits_n, c->row_cnt, c->acol, c->aval, c->arena_cap,
                                                                reinterpret_cast<Seg*>(c->segs), c->seg_cap, c->dcount, overflow);
     DH_CUDA(c, cudaGetLastError());
     scan_rows_kernel<<<1, 1024, 0, c->stream>>>(c->row_cnt, nd, c->row_ptr);

@@ -537,8 +537,10 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
   // launch shape: (warps per CTA, probes in flight per lane); DETHAM_PT2_VARIANT selects another one for tuning
   using AccKernel = void (*)(EnumParams, const u64*, const double*, int64_t, double, unsigned, Slot*, u64, u64*, int*);
   struct Variant { int warps, u; AccKernel k; };
+  // measured on B200 (profiles/r1_v2_summary.md): more probes in flight per lane do not help, the table is bound by the
+  // throughput of random sector read-modify-writes, not by their latency
   static const Variant variants[] = {{16, 1, pt2_accumulate_kernel<16, 1>}, {16, 2, pt2_accumulate_kernel<16, 2>},
-                                     {12, 4, pt2_accumulate_kernel<12, 4>}, {8, 4, pt2_accumulate_kernel<8, 4>}};
+                                     {12, 4, pt2_accumulate_kernel<12, 4>}, {12, 1, pt2_accumulate_kernel<12, 1>}};
   int vi = 0;
   if (const char* e = getenv("DETHAM_PT2_VARIANT")) { int v = atoi(e); if (v >= 0 && v < (int)(sizeof(variants) / sizeof(variants[0]))) vi = v; }
   const int warps = variants[vi].warps;
