@@ -51,6 +51,8 @@ def lib():
         L.orc_csr_free.argtypes = [C.c_void_p]
         L.orc_energy.restype = None
         L.orc_energy.argtypes = [C.c_int64, ip, C.POINTER(C.c_int32), dp, dp, dp, dp, dp]
+        L.orc_residual.restype = None
+        L.orc_residual.argtypes = [C.c_int64, ip, C.POINTER(C.c_int32), dp, dp, C.c_double, dp, dp]
         L.orc_pt2.restype = None
         L.orc_pt2.argtypes = [C.c_int, dp, dp, C.c_double, up, C.c_int64, dp, C.c_double, C.c_double, C.c_int,
                               C.c_int, C.c_int, dp, ip, ip, dp, dp, dp]
@@ -150,6 +152,19 @@ def energy(row_ptr, col, val, psi, want_y=False):
     lib().orc_energy(nd, _i(row_ptr), col.ctypes.data_as(C.POINTER(C.c_int32)), _d(val), _d(psi), C.byref(e),
                      C.byref(n2), _d(y))
     return (e.value, n2.value, y) if want_y else (e.value, n2.value)
+
+
+def residual(row_ptr, col, val, psi, e_s):
+    """(r = H_SS psi - e_s psi, internal term of Eq. 13 = sum_i r_i^2 / (e_s - H_ii) / psi^T psi)."""
+    row_ptr = np.ascontiguousarray(row_ptr, dtype=np.int64)
+    col = np.ascontiguousarray(col, dtype=np.int32)
+    val, psi = _f64(val), _f64(psi)
+    nd = psi.shape[0]
+    r = np.empty(nd, dtype=np.float64)
+    out = C.c_double(0)
+    lib().orc_residual(nd, _i(row_ptr), col.ctypes.data_as(C.POINTER(C.c_int32)), _d(val), _d(psi), float(e_s), _d(r),
+                       C.byref(out))
+    return r, out.value
 
 
 def pt2(n, h1, eri, e_core, dets, psi, e_s, eps2, n_parts=1, part_begin=0, part_end=None):

@@ -262,6 +262,26 @@ void orc_energy(int64_t nd, const int64_t* row_ptr, const int32_t* col, const do
   if (norm2_out) *norm2_out = (double)den;
 }
 
+// Internal term of Eq. 13 (first sum) and the residual vector that Eq. 12 contracts with
+// grad psi:  r_x = sum_{x' in V} H_xx' psi(x') - E psi(x),   dE_int = (1/psi^T psi) sum_{x in V} r_x^2 / (E - H_xx),
+// on the CSR H_VV (whose row x holds its diagonal H_xx).  A term with r_x == 0 contributes 0 whatever its denominator.
+void orc_residual(int64_t nd, const int64_t* row_ptr, const int32_t* col, const double* val, const double* psi, double e,
+                  double* r_out, double* internal_out) {
+  long double sum = 0, den = 0;
+  for (int64_t i = 0; i < nd; ++i) {
+    long double y = 0, hii = 0;
+    for (int64_t k = row_ptr[i]; k < row_ptr[i + 1]; ++k) {
+      y += (long double)val[k] * psi[col[k]];
+      if (col[k] == i) hii = val[k];
+    }
+    const long double r = y - (long double)e * psi[i];
+    if (r_out) r_out[i] = (double)r;
+    if (r != 0) sum += r * r / ((long double)e - hii);
+    den += (long double)psi[i] * psi[i];
+  }
+  *internal_out = (double)(sum / den);
+}
+
 // pt2, Eq. 13 second term with the screened sum of readings Q6, Q9, Q10:
 //   for each source i with psi_i != 0: tau_i = eps2/|psi_i| (0 when eps2 == 0); for (D_a, H) in conn(D_i, tau_i),
 //   D_a not in S: v_a += H psi_i.   dE = (1/psi^T psi) sum_a v_a^2 / (E_S - diag(D_a)).

@@ -232,3 +232,39 @@ def test_zobrist_is_xor_of_orbital_words(orc):
         x = ((x ^ (x >> 27)) * 0x94D049BB133111EB) & m
         return x ^ (x >> 31)
     assert z(1 << 5, 0) == sm(260121310 + 5) and z(0, 1 << 9) == sm(260121310 + 64 + 9)
+
+
+# ---------------------------------------------------------------- P11: internal term of Eq. 13 and the residual of Eq. 12
+def test_p11_residual_and_internal_term(orc):
+    """(a) eigenvector of the full-space matrix: r = 0 and the internal term vanishes; (b) two-level textbook second
+    order K^2 / (E_1 - E_2) for psi = (1, 0) on the closed-shell pair of two electrons in two orbitals (first
+    sum); (c) r and the term against numpy on the dense matrix built by the bitstring-difference path `element`."""
+    n, na, nb = 6, 3, 3
+    h1, eri = small_integrals(n, 31)
+    dets = full_space(n, na, nb)
+    H = orc.dense(n, h1, eri, 0.1, dets)
+    w, V = np.linalg.eigh(H)
+    rp, col, val = orc.ham_build(n, h1, eri, 0.1, dets, 0.0)
+    r, t = orc.residual(rp, col, val, V[:, 3], w[3])
+    assert np.max(np.abs(r)) < 1e-12 and abs(t) < 1e-20
+    # (b)
+    h2, e2 = small_integrals(2, 51)
+    g = dense_eri(2, e2)
+    two = np.array([[1, 1], [2, 2]], dtype=np.uint64)
+    rp2, col2, val2 = orc.ham_build(2, h2, e2, 0.0, two, 0.0)
+    e1, e22, k = 2 * h2[0, 0] + g[0, 0, 0, 0], 2 * h2[1, 1] + g[1, 1, 1, 1], g[0, 1, 1, 0]
+    r2, t2 = orc.residual(rp2, col2, val2, np.array([1.0, 0.0]), e1)
+    assert np.allclose(r2, [0.0, k], rtol=1e-14, atol=1e-15)
+    assert np.isclose(t2, k * k / (e1 - e22), rtol=1e-13)
+    # (c)
+    rng = np.random.default_rng(8)
+    idx = np.sort(rng.choice(400, size=90, replace=False))
+    psi = rng.standard_normal(90)
+    rp, col, val = orc.ham_build(n, h1, eri, 0.1, dets[idx], 0.0)
+    Hs = H[np.ix_(idx, idx)]
+    e = psi @ Hs @ psi / (psi @ psi)
+    r, t = orc.residual(rp, col, val, psi, e)
+    r_ref = Hs @ psi - e * psi
+    assert np.allclose(r, r_ref, rtol=1e-12, atol=1e-13)
+    assert np.isclose(t, np.sum(r_ref ** 2 / (e - np.diag(Hs))) / (psi @ psi), rtol=1e-11)
+    assert abs(psi @ r_ref) < 1e-10 * np.linalg.norm(psi) * np.linalg.norm(r_ref)  # the residual is orthogonal to psi
