@@ -27,7 +27,7 @@ if ROOT not in sys.path:
 
 METRIC = "hamiltonian_elements_per_sec"
 UNIT = "elements/s"
-DEFAULT_WORKLOAD = "h2o"
+DEFAULT_WORKLOAD = "cr2"  # the configuration BASELINE.json's roofline target is stated on; fits one B200
 
 
 def load_peaks():
@@ -102,9 +102,10 @@ def oracle_sample(p, m_sources, seed=1):
 
 
 def sample_size(p):
-    exc = {"tiny": 875, "h2o": 12635, "n2": 30723, "n2sweep": 30723, "cr2": 404712}[p["name"]]
-    # ~1.2e8 element visits (two enumerations per source) plus the serial sort + H_aa work is 10-30 s of oracle time
-    return int(max(16, min(len(p["psi"]), 6e7 / exc)))
+    # sources per sample, sized so that the oracle (no early exit: it visits every excitation of every sampled source and
+    # sorts the externals) runs 10-30 s on a 16-core host; measured 27.7 s / 4749 (h2o), 64 s / 1953 (n2), 56 s / 149 (cr2)
+    m = {"tiny": 2000, "h2o": 4000, "n2": 700, "n2sweep": 700, "cr2": 60}[p["name"]]
+    return int(min(len(p["psi"]), m))
 
 
 def run_reference(args, p):
@@ -135,7 +136,7 @@ def workload_config(p):
 def main():
     ap = argparse.ArgumentParser()
     ap.add_argument("--gpus", type=int, default=1)
-    ap.add_argument("--steps", type=int, default=5)
+    ap.add_argument("--steps", type=int, default=3)
     ap.add_argument("--warmup", type=int, default=3)
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD)
@@ -232,7 +233,11 @@ def main():
     roofline = {"bound": "hbm", "kernel": "pt2_accumulate_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
                 "bytes_per_launch": bytes_accum_launch, "launch_ms": acc_ms, "launches_per_step": parts,
-                "energy_plus_pt2_GBps": path_gbs, "energy_plus_pt2_frac": path_gbs / peak}
+                "energy_plus_pt2_GBps": path_gbs, "energy_plus_pt2_frac": path_gbs / peak,
+                # what random 32-byte read-modify-writes can reach on this GPU (profiles/r1_microbench.md): 15 G/s for
+                # duplicates, 10.8-12.5 G/s for first touches, x 32 algorithmic bytes each
+                "pattern_ceiling_GBps": [32 * 10.8, 32 * 15.0],
+                "contributions_per_sec": c["pt2_contrib"] / (statistics.mean(x["ms_pt2_accum"] for x in phases) * 1e-3)}
     traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(traffic_file):
         try:
@@ -251,7 +256,9 @@ def main():
                                           "pt2_parts", "pt2_max_probe", "pt2_table_slots", "pt2_sum_abs", "pt2_min_abs_den")},
            "results": {"E_S": e_s, "PT2": pt2}, "es_pt2_wall_ms": mean("ms_build_count") + mean("ms_build_fill") + t_energy + t_pt2,
            "stored_nnz_per_sec": c["nnz"] / ((mean("ms_build_count") + mean("ms_build_fill")) * 1e-3),
-           "gpu_launches": 7 + 2 + (1 if c["ms_pt2_plan"] > 0 else 0) + 2 + 4 * parts}
+           # kernels of libdetham.so per step: store 2 (validate, index insert), ham_build 5 (enumerate, row scan, segment copy,
+           # two row sorts), energy 2, pt2 3 (plan histogram, norm) + 3 per key partition (accumulate, scan, reduce)
+           "gpu_launches": 2 + 5 + 2 + 3 + 3 * parts}
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     if not args.no_e2e:
@@ -260,7 +267,7 @@ def main():
         dh, ph = dets_pin.numpy().view(np.uint64), psi_pin.numpy()
         ctx.solve_host(dh, ph, p["eps"], p["eps2"])
         e2e_ms = []
-        for _ in range(max(2, min(args.steps, 3))):
+        for _ in range(2):
             flush.fill_(1)
             torch.cuda.synchronize()
             t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)

@@ -96,6 +96,12 @@ dh_status detham_csr_copy(detham_ctx* ctx, int64_t* row_ptr, int32_t* col, doubl
  * psi: DEVICE fp64 [n_dets].  y_out: DEVICE fp64 [n_dets] or NULL.  e_out, norm2_out: HOST (norm2_out may be NULL). */
 dh_status detham_energy(detham_ctx* ctx, const double* psi, double* e_out, double* norm2_out, double* y_out);
 
+/* residual: r = H_SS psi - e_s psi, the vector that Eq. 12 contracts with grad psi,
+ * and the internal term of Eq. 13 (first sum) on the CSR built last (reading Q4: the screened
+ * operator): *internal_out = (1 / psi^T psi) sum_{i in S} r_i^2 / (e_s - H_ii); a row with r_i == 0 contributes 0.
+ * psi: DEVICE fp64 [n_dets]; r_out: DEVICE fp64 [n_dets] or NULL; internal_out: HOST.  No regularisation of the denominators. */
+dh_status detham_residual(detham_ctx* ctx, const double* psi, double e_s, double* r_out, double* internal_out);
+
 /* Configure pt2: table_slots = hash-table capacity in 32-byte slots (0 = choose from free device memory);
  * n_parts = number of key partitions / passes, a power of two <= 1024 (0 = choose so that every partition fits). */
 dh_status detham_pt2_config(detham_ctx* ctx, int64_t table_slots, int n_parts);

@@ -12,7 +12,7 @@ _lib = None
 STATUS = {0: "DH_OK", 1: "DH_EINVAL", 2: "DH_EUNSORTED", 3: "DH_EPOPCOUNT", 4: "DH_ENOMEM", 5: "DH_ETABLEFULL", 6: "DH_ECUDA"}
 
 # every symbol include/detham.h declares
-SYMBOLS = ["detham_create", "detham_set_subspace", "detham_ham_build", "detham_csr", "detham_csr_copy", "detham_energy",
+SYMBOLS = ["detham_create", "detham_set_subspace", "detham_ham_build", "detham_csr", "detham_csr_copy", "detham_energy", "detham_residual",
            "detham_pt2_config", "detham_pt2", "detham_pt2_partials", "detham_solve_host", "detham_connections",
            "detham_diagonals", "detham_get_counters", "detham_destroy", "detham_strerror", "detham_last_cuda_error"]
 
@@ -48,6 +48,7 @@ def load_library():
     L.detham_csr.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
     L.detham_csr_copy.argtypes = [vp, vp, vp, vp]
     L.detham_energy.argtypes = [vp, vp, dp, dp, vp]
+    L.detham_residual.argtypes = [vp, vp, C.c_double, vp, dp]
     L.detham_pt2_config.argtypes = [vp, C.c_int64, C.c_int]
     L.detham_pt2.argtypes = [vp, vp, C.c_double, C.c_double, dp, ip, ip]
     L.detham_pt2_partials.argtypes = [vp, dp, C.c_int, C.POINTER(C.c_int)]
@@ -139,6 +140,15 @@ class Detham:
         y = torch.empty_like(psi) if want_y else None
         self._check(self._L.detham_energy(self._h, psi.data_ptr(), C.byref(e), C.byref(n2), y.data_ptr() if want_y else None))
         return (e.value, n2.value, y) if want_y else (e.value, n2.value)
+
+    def residual(self, psi, e_s, want_r=True):
+        """(r = H_SS psi - e_s psi as a CUDA tensor or None, internal term of Eq. 13)."""
+        import torch
+        assert psi.is_cuda and psi.dtype == torch.float64 and psi.is_contiguous() and psi.numel() == self.n_dets
+        out = C.c_double(0)
+        r = torch.empty_like(psi) if want_r else None
+        self._check(self._L.detham_residual(self._h, psi.data_ptr(), float(e_s), r.data_ptr() if want_r else None, C.byref(out)))
+        return r, out.value
 
     def pt2_config(self, table_slots=0, n_parts=0):
         self._check(self._L.detham_pt2_config(self._h, int(table_slots), int(n_parts)))

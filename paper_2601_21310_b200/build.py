@@ -32,5 +32,22 @@ def build(force: bool = False, verbose: bool = False) -> str:
     return SO
 
 
+def build_probes(force: bool = False) -> list:
+    """Compile the stand-alone microbenchmarks under probes/ (random-slot traffic, appends, store variants) for sm_100a."""
+    nvcc = os.environ.get("NVCC", "/usr/local/cuda/bin/nvcc")
+    src_dir = os.path.join(PKG, "probes")
+    out_dir = os.path.join(src_dir, "bin")
+    os.makedirs(out_dir, exist_ok=True)
+    built = []
+    for f in sorted(os.listdir(src_dir)):
+        if not f.endswith(".cu"):
+            continue
+        src, exe = os.path.join(src_dir, f), os.path.join(out_dir, f[:-3])
+        if force or not os.path.exists(exe) or os.path.getmtime(src) > os.path.getmtime(exe):
+            subprocess.check_call([nvcc, "-gencode", "arch=compute_100a,code=sm_100a", "-O3", "-lineinfo", "-std=c++17", src, "-o", exe])
+        built.append(exe)
+    return built
+
+
 if __name__ == "__main__":
     print(build(force=True, verbose=True))

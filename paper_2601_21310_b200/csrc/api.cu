@@ -128,6 +128,11 @@ dh_status detham_energy(detham_ctx* c, const double* psi, double* e_out, double*
   return dh_energy(c, psi, e_out, norm2_out, y_out);
 }
 
+dh_status detham_residual(detham_ctx* c, const double* psi, double e_s, double* r_out, double* internal_out) {
+  if (!c || !psi || !internal_out || c->nnz < 0 || !std::isfinite(e_s)) return DH_EINVAL;
+  return dh_residual(c, psi, e_s, r_out, internal_out);
+}
+
 dh_status detham_pt2_config(detham_ctx* c, int64_t table_slots, int n_parts) {
   if (!c || table_slots < 0 || n_parts < 0 || n_parts > (1 << DH_MAX_PBITS) || (n_parts & (n_parts - 1))) return DH_EINVAL;
   if (table_slots > 0 && table_slots < 64) return DH_EINVAL;

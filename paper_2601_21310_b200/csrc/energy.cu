@@ -39,6 +39,51 @@ spmv_energy_kernel(const int64_t* __restrict__ row_ptr, const int* __restrict__ 
   }
 }
 
+// residual r = H_SS psi - e psi (the vector Eq. 12 contracts with grad psi) fused with the internal term of
+// Eq. 13 (first sum): sum_i r_i^2 / (e - H_ii); H_ii is the row's own diagonal entry.  8 threads per row.
+__global__ void __launch_bounds__(256)
+residual_kernel(const int64_t* __restrict__ row_ptr, const int* __restrict__ col, const double* __restrict__ val,
+                const double* __restrict__ psi, int64_t nd, double e, double* __restrict__ r_out, double* __restrict__ part) {
+  constexpr int TPR = 8;
+  const int sub = threadIdx.x % TPR;
+  const int64_t rows_per_cta = 256 / TPR;
+  double num = 0.0, den = 0.0;
+  for (int64_t rbase = (int64_t)blockIdx.x * rows_per_cta; rbase < nd; rbase += (int64_t)gridDim.x * rows_per_cta) {
+    const int64_t row = rbase + threadIdx.x / TPR;
+    const bool live = row < nd;
+    const int64_t b = live ? row_ptr[row] : 0, en = live ? row_ptr[row + 1] : 0;
+    double acc = 0.0, hii = 0.0;
+    for (int64_t k = b + sub; k < en; k += TPR) {
+      const int c = col[k];
+      const double v = val[k];
+      acc = fma(v, __ldg(psi + c), acc);
+      if (c == row) hii = v;
+    }
+#pragma unroll
+    for (int o = TPR / 2; o > 0; o >>= 1) {
+      acc += __shfl_xor_sync(0xffffffffu, acc, o, TPR);
+      hii += __shfl_xor_sync(0xffffffffu, hii, o, TPR);  // exactly one lane holds the diagonal, the others 0
+    }
+    if (sub == 0 && live) {
+      const double p = psi[row];
+      const double r = acc - e * p;
+      if (r_out) r_out[row] = r;
+      if (r != 0.0) num += r * r / (e - hii);
+      den = fma(p, p, den);
+    }
+  }
+  __shared__ double sn[8], sd[8];
+  for (int o = 16; o > 0; o >>= 1) { num += __shfl_xor_sync(0xffffffffu, num, o); den += __shfl_xor_sync(0xffffffffu, den, o); }
+  if ((threadIdx.x & 31) == 0) { sn[threadIdx.x >> 5] = num; sd[threadIdx.x >> 5] = den; }
+  __syncthreads();
+  if (threadIdx.x == 0) {
+    double a = 0.0, b2 = 0.0;
+    for (int w = 0; w < 8; ++w) { a += sn[w]; b2 += sd[w]; }
+    part[2 * blockIdx.x] = a;
+    part[2 * blockIdx.x + 1] = b2;
+  }
+}
+
 __global__ void final_reduce2_kernel(const double* __restrict__ part, int nblk, double* out) {
   __shared__ double sa[256], sb[256];
   double a = 0.0, b = 0.0;
@@ -86,5 +131,23 @@ dh_status dh_energy(detham_ctx* c, const double* psi, double* e_out, double* n2_
   c->ctr.ms_energy = dh_elapsed(c, 0, 1);
   *e_out = h[0] / h[1];
   if (n2_out) *n2_out = h[1];
+  return DH_OK;
+}
+
+dh_status dh_residual(detham_ctx* c, const double* psi, double e_s, double* r_out, double* internal_out) {
+  const int64_t nd = c->nd;
+  int64_t want = (nd + 31) / 32;
+  int grid = (int)(want < (int64_t)c->sm_count * 8 ? want : (int64_t)c->sm_count * 8);
+  dh_status st = dh_ensure_red(c, 2 * (int64_t)grid + 2);
+  if (st != DH_OK) return st;
+  double* part = c->red + 2;
+  residual_kernel<<<grid, 256, 0, c->stream>>>(c->row_ptr, c->col, c->val, psi, nd, e_s, r_out, part);
+  DH_CUDA(c, cudaGetLastError());
+  final_reduce2_kernel<<<1, 256, 0, c->stream>>>(part, grid, c->red);
+  DH_CUDA(c, cudaGetLastError());
+  double* h = reinterpret_cast<double*>(c->pinned);
+  DH_CUDA(c, cudaMemcpyAsync(h, c->red, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  DH_CUDA(c, cudaStreamSynchronize(c->stream));
+  *internal_out = h[0] / h[1];
   return DH_OK;
 }

@@ -537,7 +537,7 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
   // launch shape: (warps per CTA, probes in flight per lane); DETHAM_PT2_VARIANT selects another one for tuning
   using AccKernel = void (*)(EnumParams, const u64*, const double*, int64_t, double, unsigned, Slot*, u64, u64*, int*);
   struct Variant { int warps, u; AccKernel k; };
-  // measured on B200 (profiles/r1_v2_summary.md): more probes in flight per lane do not help, the table is bound by the
+  // measured on B200 (profiles/r1_microbench.md): more probes in flight per lane do not help, the table is bound by the
   // throughput of random sector read-modify-writes, not by their latency
   static const Variant variants[] = {{16, 1, pt2_accumulate_kernel<16, 1>}, {16, 2, pt2_accumulate_kernel<16, 2>},
                                      {12, 4, pt2_accumulate_kernel<12, 4>}, {12, 1, pt2_accumulate_kernel<12, 1>}};
@@ -624,7 +624,7 @@ dh_status dh_pt2(detham_ctx* c, const double* psi, double e_s, double eps2, doub
   // 36 G sectors/s up to 64 GB, 29 at 80 GB, 17 at 96 GB, 8.7 at 160 GB (profiles/r1_microbench.md).  More passes over a
   // smaller table beat fewer passes over a bigger one, so the table never exceeds this many bytes unless configured.
   double max_table_gb = 60.0;
-  if (const char* e = getenv("DETHAM_PT2_MAX_TABLE_GB")) { double v = atof(e); if (v >= 0.001 && v <= 4096.0) max_table_gb = v; }
+  if (const char* e = getenv("DETHAM_PT2_MAX_TABLE_GB")) { double v = atof(e); if (v >= 1e-6 && v <= 4096.0) max_table_gb = v; }
 
   // ---- plan: partition count and table capacity
   int pbits = 0;

@@ -304,3 +304,61 @@ def test_solve_host_end_to_end(pkg, orc):
     assert abs(e - e_ref) <= E_TOL * abs(e_ref)
     assert abs(pt2 - o["pt2"]) <= 10 * PT2_TOL * abs(o["pt2"])  # E_S differs by 1e-10 relative between the two sides
     ctx.close()
+
+
+def test_small_table_cap_forces_many_passes(pkg, orc, monkeypatch):
+    """The planner prefers more key partitions over a table beyond the TLB-safe size; with the cap forced down to
+    0.5 MB the Tiny case needs >= 64 passes (sampled/exact histogram, adaptive shrink after pass 0) and must still agree."""
+    monkeypatch.setenv("DETHAM_PT2_MAX_TABLE_GB", "0.0005")
+    p = make_problem("tiny")
+    ctx = _ctx(pkg, p)
+    psi = _psi(p)
+    e_s = -30.0
+    o = orc.pt2(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"], p["psi"], e_s, 1e-6)
+    ctx.pt2_config(0, 0)
+    g_pt2, g_ext, g_con = ctx.pt2(psi, e_s, 1e-6)
+    c = ctx.counters()
+    assert c["pt2_parts"] >= 64 and c["pt2_table_slots"] <= 16000
+    assert (g_ext, g_con) == (o["n_external"], o["n_contrib"])
+    assert abs(g_pt2 - o["pt2"]) <= PT2_TOL * abs(o["pt2"])
+    ctx.close()
+
+
+def test_ham_build_repeated_with_different_eps(pkg, orc):
+    """The build arena is sized from the previous build: growing, shrinking and growing again must all give the oracle's CSR."""
+    p = make_problem("tiny", n_dets=1200)
+    ctx = _ctx(pkg, p)
+    for eps in (5e-2, 0.0, 1e-3, 0.0):
+        nnz = ctx.ham_build(eps)
+        ref = orc.ham_build(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"], eps)
+        assert nnz == len(ref[1])
+        _check_csr(ctx, ref)
+    # a different (larger) subspace on the same context
+    q = make_problem("tiny")
+    ctx.set_subspace(q["dets"])
+    nnz = ctx.ham_build(1e-4)
+    ref = orc.ham_build(q["n"], q["h1"], q["eri"], q["e_core"], q["dets"], 1e-4)
+    assert nnz == len(ref[1])
+    _check_csr(ctx, ref)
+    ctx.close()
+
+
+@pytest.mark.parametrize("name,n_dets,eps", [("tiny", None, 0.0), ("tiny", 700, 1e-3), ("h2o", 6000, 1e-5)])
+def test_residual_and_internal_term(pkg, orc, name, n_dets, eps):
+    """r = H_SS psi - E psi (Eq. 12) and the internal term of Eq. 13 against the oracle."""
+    p = make_problem(name, n_dets=n_dets)
+    ctx = _ctx(pkg, p)
+    ctx.ham_build(eps)
+    psi = _psi(p)
+    ref = orc.ham_build(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"], eps)
+    e_ref, _ = orc.energy(*ref, p["psi"])
+    r_ref, t_ref = orc.residual(*ref, p["psi"], e_ref)
+    r, t = ctx.residual(psi, e_ref)
+    r = r.cpu().numpy()
+    scale = np.max(np.abs(r_ref))
+    assert np.allclose(r, r_ref, rtol=1e-11, atol=1e-13 * max(scale, 1.0))
+    den_min = np.min(np.abs(e_ref - ref[2][ref[1] == np.repeat(np.arange(len(p["psi"])), np.diff(ref[0]))]))
+    assert abs(t - t_ref) <= 1e-9 * max(abs(t_ref), np.sum(r_ref ** 2) / den_min * 1e-3), (t, t_ref)
+    _, t2 = ctx.residual(psi, e_ref, want_r=False)
+    assert t2 == t  # deterministic reduction order
+    ctx.close()
