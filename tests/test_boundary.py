@@ -64,3 +64,22 @@ def test_product_and_oracle_share_no_code():
                 assert "oracle" not in open(os.path.join(dirpath, f)).read().replace("oracle/", "").lower() or f in ("common.cuh",), f
     osrc = open(os.path.join(ROOT, "oracle", "oracle.cpp")).read() + open(os.path.join(ROOT, "oracle", "__init__.py")).read()
     assert "detham" not in osrc and "#include \"common" not in osrc and "paper_2601_21310_b200 import" not in osrc
+
+
+def test_reference_arm_under_torchrun_two_ranks():
+    """bench.py --impl reference under a 2-rank launch (the driver's N > 1 invocation, gloo-free: no collective is needed):
+    rank 0 alone runs the oracle and prints ONE JSON line with the contract's keys, the other rank exits 0 without work."""
+    import json
+    import subprocess
+    import sys
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", "29771", os.path.join(ROOT, "bench.py"), "--impl", "reference", "--gpus", "2", "--workload", "tiny",
+           "--steps", "1", "--warmup", "0"]
+    out = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert out.returncode == 0, out.stderr[-2000:]
+    lines = [l for l in out.stdout.splitlines() if l.startswith("{")]
+    assert len(lines) == 1
+    d = json.loads(lines[0])
+    assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["value"] > 0 and d["unit"] == "elements/s"
+    assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
+    assert d["config"]["workload"].startswith("tiny")
