@@ -141,6 +141,7 @@ def main():
     ap.add_argument("--impl", default="ours", choices=["ours", "reference"])
     ap.add_argument("--workload", default=DEFAULT_WORKLOAD)
     ap.add_argument("--n-dets", type=int, default=None)
+    ap.add_argument("--eps2", type=float, default=None, help="override the config's PT2 threshold (scaling sweep, configs[3])")
     ap.add_argument("--n-parts", type=int, default=0, help="pt2 key partitions (0 = planned by the library)")
     ap.add_argument("--table-slots", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
@@ -157,6 +158,8 @@ def main():
         if rank != 0:
             return 0
         p = make_problem(args.workload, n_dets=args.n_dets)
+        if args.eps2 is not None:
+            p["eps2"] = args.eps2
         print(json.dumps(run_reference(args, p)))
         return 0
 
@@ -171,6 +174,8 @@ def main():
         dist.init_process_group("nccl", device_id=torch.device("cuda", local_rank))
 
     p = make_problem(args.workload, n_dets=args.n_dets)
+    if args.eps2 is not None:
+        p["eps2"] = args.eps2
     nd = len(p["psi"])
     ctx = pkg.create(p["n"], p["na"], p["nb"], p["h1"], p["eri"], p["e_core"])
     ctx.pt2_config(args.table_slots, args.n_parts)

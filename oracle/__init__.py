@@ -154,6 +154,20 @@ def energy(row_ptr, col, val, psi, want_y=False):
     return (e.value, n2.value, y) if want_y else (e.value, n2.value)
 
 
+def ediag(row_ptr, col, val):
+    """E_diag = lambda_min(H_VV) ("diagnostic post-hoc diagonalization energy").  The plain definition through
+    a library eigensolver: LAPACK on the dense matrix up to 4000 rows, ARPACK (scipy eigsh, smallest algebraic) beyond."""
+    import scipy.sparse as sp
+    nd = len(row_ptr) - 1
+    A = sp.csr_matrix((_f64(val), np.ascontiguousarray(col, dtype=np.int32), np.ascontiguousarray(row_ptr, dtype=np.int64)),
+                      shape=(nd, nd))
+    if nd <= 4000:
+        return float(np.linalg.eigvalsh(A.toarray())[0])
+    from scipy.sparse.linalg import eigsh
+    w = eigsh(A, k=1, which="SA", tol=1e-13, maxiter=20000, return_eigenvectors=False)
+    return float(w[0])
+
+
 def residual(row_ptr, col, val, psi, e_s):
     """(r = H_SS psi - e_s psi, internal term of Eq. 13 = sum_i r_i^2 / (e_s - H_ii) / psi^T psi)."""
     row_ptr = np.ascontiguousarray(row_ptr, dtype=np.int64)

@@ -268,3 +268,31 @@ def test_p11_residual_and_internal_term(orc):
     assert np.allclose(r, r_ref, rtol=1e-12, atol=1e-13)
     assert np.isclose(t, np.sum(r_ref ** 2 / (e - np.diag(Hs))) / (psi @ psi), rtol=1e-11)
     assert abs(psi @ r_ref) < 1e-10 * np.linalg.norm(psi) * np.linalg.norm(r_ref)  # the residual is orthogonal to psi
+
+
+# ---------------------------------------------------------------- P12: E_diag = lambda_min(H_VV)
+def test_p12_ediag(orc):
+    """(a) two-level closed form (a+b)/2 - sqrt(((a-b)/2)^2 + k^2); (b) both solver branches (dense LAPACK / ARPACK) agree with
+    LAPACK on the dense matrix built by `element`; (c) E_diag <= E_var for any psi (Delta_opt >= 0)."""
+    h2, e2 = small_integrals(2, 51)
+    g = dense_eri(2, e2)
+    two = np.array([[1, 1], [2, 2]], dtype=np.uint64)
+    rp, col, val = orc.ham_build(2, h2, e2, 0.0, two, 0.0)
+    a, b, k = 2 * h2[0, 0] + g[0, 0, 0, 0], 2 * h2[1, 1] + g[1, 1, 1, 1], g[0, 1, 1, 0]
+    assert np.isclose(orc.ediag(rp, col, val), 0.5 * (a + b) - np.sqrt(0.25 * (a - b) ** 2 + k * k), rtol=1e-13)
+    n, na, nb = 6, 3, 3
+    h1, eri = small_integrals(n, 31)
+    dets = full_space(n, na, nb)
+    rng = np.random.default_rng(3)
+    idx = np.sort(rng.choice(400, size=150, replace=False))
+    H = orc.dense(n, h1, eri, 0.1, dets[idx])
+    rp, col, val = orc.ham_build(n, h1, eri, 0.1, dets[idx], 0.0)
+    lam = np.linalg.eigvalsh(H)[0]
+    assert np.isclose(orc.ediag(rp, col, val), lam, rtol=1e-12)
+    import scipy.sparse as sp
+    from scipy.sparse.linalg import eigsh
+    A = sp.csr_matrix((val, col, rp), shape=(150, 150))
+    assert np.isclose(eigsh(A, k=1, which="SA", tol=1e-13, return_eigenvectors=False)[0], lam, rtol=1e-11)
+    psi = rng.standard_normal(150)
+    e, _ = orc.energy(rp, col, val, psi)
+    assert e >= lam - 1e-12
