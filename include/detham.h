@@ -102,6 +102,12 @@ dh_status detham_energy(detham_ctx* ctx, const double* psi, double* e_out, doubl
  * psi: DEVICE fp64 [n_dets]; r_out: DEVICE fp64 [n_dets] or NULL; internal_out: HOST.  No regularisation of the denominators. */
 dh_status detham_residual(detham_ctx* ctx, const double* psi, double e_s, double* r_out, double* internal_out);
 
+/* ediag: E_diag = lambda_min(H_SS) of the CSR built last, by Lanczos on the device
+ * (SpMV = the energy kernel).  v0: DEVICE fp64 [n_dets] start vector (psi is a good one) or NULL (all ones); stops when the
+ * smallest Ritz value moves by less than tol * |value| between two steps, when the Krylov space closes, or after max_iter
+ * steps.  e_out, iters_out (may be NULL): HOST.  Delta_opt of the paper = E_S - *e_out >= 0. */
+dh_status detham_ediag(detham_ctx* ctx, const double* v0, double tol, int max_iter, double* e_out, int* iters_out);
+
 /* Configure pt2: table_slots = hash-table capacity in 32-byte slots (0 = choose from free device memory);
  * n_parts = number of key partitions / passes, a power of two <= 1024 (0 = choose so that every partition fits). */
 dh_status detham_pt2_config(detham_ctx* ctx, int64_t table_slots, int n_parts);

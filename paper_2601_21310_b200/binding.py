@@ -12,7 +12,7 @@ _lib = None
 STATUS = {0: "DH_OK", 1: "DH_EINVAL", 2: "DH_EUNSORTED", 3: "DH_EPOPCOUNT", 4: "DH_ENOMEM", 5: "DH_ETABLEFULL", 6: "DH_ECUDA"}
 
 # every symbol include/detham.h declares
-SYMBOLS = ["detham_create", "detham_set_subspace", "detham_ham_build", "detham_csr", "detham_csr_copy", "detham_energy", "detham_residual",
+SYMBOLS = ["detham_create", "detham_set_subspace", "detham_ham_build", "detham_csr", "detham_csr_copy", "detham_energy", "detham_residual", "detham_ediag",
            "detham_pt2_config", "detham_pt2", "detham_pt2_partials", "detham_solve_host", "detham_connections",
            "detham_diagonals", "detham_get_counters", "detham_destroy", "detham_strerror", "detham_last_cuda_error"]
 
@@ -49,6 +49,7 @@ def load_library():
     L.detham_csr_copy.argtypes = [vp, vp, vp, vp]
     L.detham_energy.argtypes = [vp, vp, dp, dp, vp]
     L.detham_residual.argtypes = [vp, vp, C.c_double, vp, dp]
+    L.detham_ediag.argtypes = [vp, vp, C.c_double, C.c_int, dp, C.POINTER(C.c_int)]
     L.detham_pt2_config.argtypes = [vp, C.c_int64, C.c_int]
     L.detham_pt2.argtypes = [vp, vp, C.c_double, C.c_double, dp, ip, ip]
     L.detham_pt2_partials.argtypes = [vp, dp, C.c_int, C.POINTER(C.c_int)]
@@ -149,6 +150,16 @@ class Detham:
         r = torch.empty_like(psi) if want_r else None
         self._check(self._L.detham_residual(self._h, psi.data_ptr(), float(e_s), r.data_ptr() if want_r else None, C.byref(out)))
         return r, out.value
+
+    def ediag(self, v0=None, tol=1e-12, max_iter=500):
+        """(E_diag = lambda_min(H_SS), Lanczos steps taken)."""
+        import torch
+        if v0 is not None:
+            assert v0.is_cuda and v0.dtype == torch.float64 and v0.is_contiguous() and v0.numel() == self.n_dets
+        e, it = C.c_double(0), C.c_int(0)
+        self._check(self._L.detham_ediag(self._h, v0.data_ptr() if v0 is not None else None, float(tol), int(max_iter),
+                                         C.byref(e), C.byref(it)))
+        return e.value, it.value
 
     def pt2_config(self, table_slots=0, n_parts=0):
         self._check(self._L.detham_pt2_config(self._h, int(table_slots), int(n_parts)))

@@ -133,6 +133,11 @@ dh_status detham_residual(detham_ctx* c, const double* psi, double e_s, double* 
   return dh_residual(c, psi, e_s, r_out, internal_out);
 }
 
+dh_status detham_ediag(detham_ctx* c, const double* v0, double tol, int max_iter, double* e_out, int* iters_out) {
+  if (!c || !e_out || c->nnz < 0 || !(tol > 0.0) || max_iter < 1) return DH_EINVAL;
+  return dh_ediag(c, v0, tol, max_iter, e_out, iters_out);
+}
+
 dh_status detham_pt2_config(detham_ctx* c, int64_t table_slots, int n_parts) {
   if (!c || table_slots < 0 || n_parts < 0 || n_parts > (1 << DH_MAX_PBITS) || (n_parts & (n_parts - 1))) return DH_EINVAL;
   if (table_slots > 0 && table_slots < 64) return DH_EINVAL;

@@ -1,0 +1,136 @@
+// E_diag = lambda_min(H_SS) ("diagnostic post-hoc diagonalization energy
+// E_diag = lambda_min(H_VV), evaluated on the final selected configurations"; Delta_opt = E_var - E_diag).
+// Plain Lanczos on the device CSR: the SpMV is the energy kernel's (a second workload for it), the three-term recurrence
+// runs in two small fused kernels, the tridiagonal eigenvalue is found on the host by Sturm bisection.  No
+// re-orthogonalisation: ghost copies of converged Ritz values do not move the smallest one.
+#include <math.h>
+
+#include <vector>
+
+#include "common.cuh"
+
+dh_status dh_spmv(detham_ctx* c, const double* x, double* y, double* xy_out, double* xx_out);  // energy.cu
+
+namespace {
+
+// w = y - alpha v - beta v_prev, partial sums of w^T w
+__global__ void __launch_bounds__(256)
+lanczos_update_kernel(const double* __restrict__ y, const double* __restrict__ v, const double* __restrict__ vprev, double alpha,
+                      double beta, int64_t nd, double* __restrict__ w, double* __restrict__ part) {
+  double s = 0.0;
+  for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < nd; t += (int64_t)gridDim.x * blockDim.x) {
+    double x = y[t] - alpha * v[t];
+    if (vprev) x -= beta * vprev[t];
+    w[t] = x;
+    s = fma(x, x, s);
+  }
+  __shared__ double sh[8];
+  for (int o = 16; o > 0; o >>= 1) s += __shfl_xor_sync(0xffffffffu, s, o);
+  if ((threadIdx.x & 31) == 0) sh[threadIdx.x >> 5] = s;
+  __syncthreads();
+  if (threadIdx.x == 0) { double a = 0; for (int k = 0; k < 8; ++k) a += sh[k]; part[2 * blockIdx.x] = a; part[2 * blockIdx.x + 1] = 0.0; }
+}
+
+__global__ void __launch_bounds__(256)
+scale_kernel(const double* __restrict__ x, double s, int64_t nd, double* __restrict__ out) {
+  for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < nd; t += (int64_t)gridDim.x * blockDim.x) out[t] = x[t] * s;
+}
+
+__global__ void fill_kernel(double* x, double value, int64_t nd) {
+  for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < nd; t += (int64_t)gridDim.x * blockDim.x) x[t] = value;
+}
+
+__global__ void sum2_kernel(const double* __restrict__ part, int nblk, double* out) {
+  __shared__ double sa[256];
+  double a = 0.0;
+  for (int t = threadIdx.x; t < nblk; t += 256) a += part[2 * t];
+  sa[threadIdx.x] = a;
+  __syncthreads();
+  for (int s = 128; s > 0; s >>= 1) { if (threadIdx.x < s) sa[threadIdx.x] += sa[threadIdx.x + s]; __syncthreads(); }
+  if (threadIdx.x == 0) out[0] = sa[0];
+}
+
+// number of eigenvalues of the symmetric tridiagonal (a, b) below x (Sturm sequence)
+int sturm_count(const std::vector<double>& a, const std::vector<double>& b, double x) {
+  int cnt = 0;
+  double d = 1.0;
+  for (size_t k = 0; k < a.size(); ++k) {
+    const double off = k == 0 ? 0.0 : b[k - 1] * b[k - 1];
+    d = a[k] - x - (k == 0 ? 0.0 : off / d);
+    if (d == 0.0) d = -1e-300;
+    if (d < 0.0) ++cnt;
+  }
+  return cnt;
+}
+
+double tridiag_min(const std::vector<double>& a, const std::vector<double>& b) {
+  double lo = INFINITY, hi = -INFINITY;
+  for (size_t k = 0; k < a.size(); ++k) {  // Gershgorin
+    const double r = (k > 0 ? fabs(b[k - 1]) : 0.0) + (k + 1 < a.size() ? fabs(b[k]) : 0.0);
+    lo = fmin(lo, a[k] - r); hi = fmax(hi, a[k] + r);
+  }
+  for (int it = 0; it < 200 && hi - lo > 4e-16 * fmax(fabs(lo), fabs(hi)); ++it) {
+    const double mid = 0.5 * (lo + hi);
+    if (sturm_count(a, b, mid) >= 1) hi = mid; else lo = mid;
+  }
+  return 0.5 * (lo + hi);
+}
+
+}  // namespace
+
+dh_status dh_ediag(detham_ctx* c, const double* v0, double tol, int max_iter, double* e_out, int* iters_out) {
+  const int64_t nd = c->nd;
+  const int grid = (int)((nd + 255) / 256 < (int64_t)c->sm_count * 8 ? (nd + 255) / 256 : (int64_t)c->sm_count * 8);
+  double* buf = nullptr;  // v_prev, v, w, y
+  DH_CUDA(c, cudaMalloc(&buf, (size_t)4 * nd * sizeof(double)));
+  double* part = nullptr;
+  DH_CUDA(c, cudaMalloc(&part, (size_t)(2 * grid + 2) * sizeof(double)));
+  double *vprev = buf, *v = buf + nd, *w = buf + 2 * nd, *y = buf + 3 * nd;
+  double* h = reinterpret_cast<double*>(c->pinned);
+  auto cleanup = [&]() { cudaFree(buf); cudaFree(part); };
+  auto norm2_of = [&](const double* x, double* out) -> dh_status {  // x^T x through the update kernel's reduction (alpha = beta = 0)
+    lanczos_update_kernel<<<grid, 256, 0, c->stream>>>(x, x, nullptr, 0.0, 0.0, nd, w, part);
+    sum2_kernel<<<1, 256, 0, c->stream>>>(part, grid, part + 2 * grid);
+    DH_CUDA(c, cudaGetLastError());
+    DH_CUDA(c, cudaMemcpyAsync(h, part + 2 * grid, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(c, cudaStreamSynchronize(c->stream));
+    *out = h[0];
+    return DH_OK;
+  };
+  dh_status st;
+  // start vector: the caller's (e.g. psi: already close to the ground vector of H_SS), else all ones
+  if (v0) DH_CUDA(c, cudaMemcpyAsync(y, v0, nd * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
+  else fill_kernel<<<grid, 256, 0, c->stream>>>(y, 1.0, nd);
+  double n2 = 0.0;
+  st = norm2_of(y, &n2); if (st != DH_OK) { cleanup(); return st; }
+  if (!(n2 > 0.0) || !isfinite(n2)) { cleanup(); return DH_EINVAL; }
+  scale_kernel<<<grid, 256, 0, c->stream>>>(y, 1.0 / sqrt(n2), nd, v);
+  std::vector<double> a, b;
+  double beta = 0.0, theta = 0.0, theta_prev = INFINITY;
+  int it = 0;
+  for (; it < max_iter; ++it) {
+    double alpha = 0.0, vv = 0.0;
+    st = dh_spmv(c, v, y, &alpha, &vv); if (st != DH_OK) { cleanup(); return st; }  // alpha = v^T H v (v is normalised)
+    alpha /= vv;
+    a.push_back(alpha);
+    theta = tridiag_min(a, b);
+    if (it > 0 && fabs(theta - theta_prev) <= tol * fmax(fabs(theta), 1e-300)) { ++it; break; }
+    theta_prev = theta;
+    lanczos_update_kernel<<<grid, 256, 0, c->stream>>>(y, v, it > 0 ? vprev : nullptr, alpha, beta, nd, w, part);
+    sum2_kernel<<<1, 256, 0, c->stream>>>(part, grid, part + 2 * grid);
+    DH_CUDA(c, cudaGetLastError());
+    DH_CUDA(c, cudaMemcpyAsync(h, part + 2 * grid, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(c, cudaStreamSynchronize(c->stream));
+    beta = sqrt(h[0]);
+    if (!(beta > 1e-14 * fmax(fabs(alpha), 1.0))) { ++it; break; }  // invariant subspace reached: theta is exact
+    b.push_back(beta);
+    double* t = vprev; vprev = v; v = t;           // v_prev <- v
+    scale_kernel<<<grid, 256, 0, c->stream>>>(w, 1.0 / beta, nd, v);  // v <- w / beta
+    DH_CUDA(c, cudaGetLastError());
+  }
+  DH_CUDA(c, cudaStreamSynchronize(c->stream));
+  cleanup();
+  *e_out = theta;
+  if (iters_out) *iters_out = it;
+  return DH_OK;
+}

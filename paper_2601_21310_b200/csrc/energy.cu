@@ -151,3 +151,27 @@ dh_status dh_residual(detham_ctx* c, const double* psi, double e_s, double* r_ou
   *internal_out = h[0] / h[1];
   return DH_OK;
 }
+
+// y = H_SS x with x^T y and x^T x (the Lanczos step of ediag.cu); same kernels as dh_energy, no timers
+dh_status dh_spmv(detham_ctx* c, const double* x, double* y, double* xy_out, double* xx_out) {
+  const int64_t nd = c->nd;
+  const double avg = (double)c->nnz / (double)nd;
+  const int tpr = avg <= 6 ? 4 : (avg <= 24 ? 8 : 32);
+  int64_t want = (nd + (256 / tpr) - 1) / (256 / tpr);
+  int grid = (int)(want < (int64_t)c->sm_count * 8 ? want : (int64_t)c->sm_count * 8);
+  dh_status st = dh_ensure_red(c, 2 * (int64_t)grid + 2);
+  if (st != DH_OK) return st;
+  double* part = c->red + 2;
+  if (tpr == 4) spmv_energy_kernel<4><<<grid, 256, 0, c->stream>>>(c->row_ptr, c->col, c->val, x, nd, y, part);
+  else if (tpr == 8) spmv_energy_kernel<8><<<grid, 256, 0, c->stream>>>(c->row_ptr, c->col, c->val, x, nd, y, part);
+  else spmv_energy_kernel<32><<<grid, 256, 0, c->stream>>>(c->row_ptr, c->col, c->val, x, nd, y, part);
+  DH_CUDA(c, cudaGetLastError());
+  final_reduce2_kernel<<<1, 256, 0, c->stream>>>(part, grid, c->red);
+  DH_CUDA(c, cudaGetLastError());
+  double* h = reinterpret_cast<double*>(c->pinned) + 8;
+  DH_CUDA(c, cudaMemcpyAsync(h, c->red, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
+  DH_CUDA(c, cudaStreamSynchronize(c->stream));
+  *xy_out = h[0];
+  *xx_out = h[1];
+  return DH_OK;
+}

@@ -340,7 +340,7 @@ dh_status dh_ham_build(detham_ctx* c, double eps) {
     c->ctr.build_generated = h[2];
     if (!*reinterpret_cast<int*>(h + 5)) break;
     if (attempt >= 1) return DH_ENOMEM;  // cannot happen: the second attempt is sized from the exact count
-    want_arena = nnz + slack;
+    want_arena = nnz + nnz / 32 + slack;  // a block is closed when the next batch of <= 32 hits does not fit: < 32 of 1024 entries lost
   }
   const int64_t nseg = h[4];
   if (c->csr_cap < nnz) {

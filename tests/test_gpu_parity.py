@@ -362,3 +362,20 @@ def test_residual_and_internal_term(pkg, orc, name, n_dets, eps):
     _, t2 = ctx.residual(psi, e_ref, want_r=False)
     assert t2 == t  # deterministic reduction order
     ctx.close()
+
+
+@pytest.mark.parametrize("name,n_dets,eps", [("tiny", None, 0.0), ("tiny", 1, 0.0), ("h2o", 6000, 1e-5), ("n2", 20000, 1e-5)])
+def test_ediag_lanczos(pkg, orc, name, n_dets, eps):
+    """E_diag = lambda_min(H_SS) by device Lanczos against LAPACK / ARPACK on the oracle's CSR."""
+    p = make_problem(name, n_dets=n_dets)
+    ctx = _ctx(pkg, p)
+    ctx.ham_build(eps)
+    ref = orc.ham_build(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"], eps)
+    lam = orc.ediag(*ref)
+    e1, it1 = ctx.ediag(_psi(p))
+    e2, it2 = ctx.ediag(None)
+    assert abs(e1 - lam) <= 1e-9 * abs(lam), (e1, lam, it1)
+    assert abs(e2 - lam) <= 1e-9 * abs(lam), (e2, lam, it2)
+    e_var, _ = ctx.energy(_psi(p))
+    assert e_var >= e1 - 1e-9 * abs(e1)  # Delta_opt >= 0
+    ctx.close()
