@@ -96,8 +96,25 @@ __device__ __forceinline__ double dh_excited_diag(const CtaTables& T, const Warp
 __device__ __forceinline__ double dh_single_value(const EnumParams& P, const WarpScratch& ws, u64 wsame, int s, int i, int a) {
   double v = __ldg(P.h1 + i * P.n + a);
   const int ns = s == 0 ? P.na : P.nb, no = s == 0 ? P.nb : P.na;
-  for (int k = 0; k < ns; ++k) { int q = ws.occ[s][k]; v = v + (dh_eri(P.eri, i, a, q, q) - dh_eri(P.eri, i, q, q, a)); }
-  for (int k = 0; k < no; ++k) { int q = ws.occ[s ^ 1][k]; v = v + dh_eri(P.eri, i, a, q, q); }
+  // the loads of four terms are issued before the first is added (the additions keep the order of reading Q7)
+  int k = 0;
+  for (; k + 4 <= ns; k += 4) {
+    double t[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { const int q = ws.occ[s][k + u]; t[u] = dh_eri(P.eri, i, a, q, q) - dh_eri(P.eri, i, q, q, a); }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) v = v + t[u];
+  }
+  for (; k < ns; ++k) { const int q = ws.occ[s][k]; v = v + (dh_eri(P.eri, i, a, q, q) - dh_eri(P.eri, i, q, q, a)); }
+  k = 0;
+  for (; k + 4 <= no; k += 4) {
+    double t[4];
+#pragma unroll
+    for (int u = 0; u < 4; ++u) { const int q = ws.occ[s ^ 1][k + u]; t[u] = dh_eri(P.eri, i, a, q, q); }
+#pragma unroll
+    for (int u = 0; u < 4; ++u) v = v + t[u];
+  }
+  for (; k < no; ++k) { const int q = ws.occ[s ^ 1][k]; v = v + dh_eri(P.eri, i, a, q, q); }
   return dh_parity_between(wsame, i, a) ? -v : v;
 }
 

@@ -526,8 +526,10 @@ static dh_status ensure_table(detham_ctx* c, int64_t slots) {
 // One attempt at the whole PT2 with 2^pbits key partitions and a table of `slots` slots.  `adapt`: after pass 0 the
 // capacity used by the later passes is shrunk to (distinct keys of pass 0) / load, which cuts the scan traffic when the
 // table was sized from the contribution count (an upper bound of the distinct keys).
+// `pilot` (may be NULL): run pass 0 only and return {distinct externals, milliseconds} - the planner's probe of how many
+// contributions share an external.
 static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, double eps2, int pbits, int64_t slots, bool adapt,
-                             double load, double* out) {
+                             double load, double* out, double* pilot = nullptr) {
   const int64_t nd = c->nd;
   dh_status st = ensure_table(c, slots); if (st != DH_OK) return st;
   Slot* table = reinterpret_cast<Slot*>(c->table);
@@ -585,6 +587,7 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
     ms_accum += dh_elapsed(c, 2, 3); ms_scan += dh_elapsed(c, 3, 4);
     gen += hp[1]; contrib += hp[2]; if (hp[3] > max_probe) max_probe = hp[3];
     if (*reinterpret_cast<int*>(hp + 4)) return DH_ETABLEFULL;  // the scan above already cleared the table
+    if (pilot) { pilot[0] = reinterpret_cast<double*>(hp + 8)[3]; pilot[1] = ms_accum + ms_scan; return DH_OK; }
     if (adapt && pass == 0 && nparts > 1) {
       const double u0 = reinterpret_cast<double*>(hp + 8)[3] + (double)nd / nparts;  // distinct externals + members of one class
       const double need = (u0 + 8.0 * sqrt(u0) + 1024.0) / load;
@@ -677,6 +680,27 @@ dh_status dh_pt2(detham_ctx* c, const double* psi, double e_s, double eps2, doub
     if (auto_slots) {
       int64_t need = (int64_t)(max_class(pbits) / load) + 1024;
       slots = need < max_slots ? need : max_slots;
+    }
+  }
+  if (auto_parts && auto_slots && pbits >= 3) {  // worth it from 8 planned passes on: the probe costs 1/8 of one
+    // The contribution count bounds the distinct externals from above, often by a wide margin (9 contributions per
+    // external on N2-shaped |S| = 1e6), and every pass costs a list start-up per source.  Probe one slice of the key space
+    // 8x finer than a planned pass, count its distinct keys, and re-plan the passes from that.
+    const int pp = pbits + 3 < DH_MAX_PBITS ? pbits + 3 : DH_MAX_PBITS;
+    double pilot[2] = {0.0, 0.0};
+    const int64_t pilot_slots = (pp - pbits == 3 && slots / 4 > 1024) ? slots / 4 : slots;  // 1/8 of the keys in 1/4 of the slots
+    st = pt2_attempt(c, psi, e_s, eps2, pp, pilot_slots, false, load, out, pilot);
+    if (st == DH_OK && pilot[0] > 0.0) {
+      c->ctr.ms_pt2_plan += pilot[1];
+      auto uniq_class = [&](int pb) { const double u = pilot[0] * (double)(1 << (pp - pb)); return 1.2 * u + 8.0 * sqrt(u) + 4096.0; };
+      int pb2 = 0;
+      while (pb2 < pbits && uniq_class(pb2) > load * (double)max_slots) ++pb2;
+      pbits = pb2;
+      int64_t need = (int64_t)(uniq_class(pbits) / load);
+      slots = need < max_slots ? need : max_slots;
+      if (slots < 1024) slots = 1024;
+    } else if (st != DH_OK && st != DH_ETABLEFULL) {
+      return st;
     }
   }
   for (;;) {

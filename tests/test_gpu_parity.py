@@ -308,7 +308,8 @@ def test_solve_host_end_to_end(pkg, orc):
 
 def test_small_table_cap_forces_many_passes(pkg, orc, monkeypatch):
     """The planner prefers more key partitions over a table beyond the TLB-safe size; with the cap forced down to
-    0.5 MB the Tiny case needs >= 64 passes (sampled/exact histogram, adaptive shrink after pass 0) and must still agree."""
+    0.5 MB the Tiny case is planned at >= 64 passes from the contribution count, probed (27 contributions per external),
+    re-planned at fewer, larger-key passes, and must still agree."""
     monkeypatch.setenv("DETHAM_PT2_MAX_TABLE_GB", "0.0005")
     p = make_problem("tiny")
     ctx = _ctx(pkg, p)
@@ -318,7 +319,7 @@ def test_small_table_cap_forces_many_passes(pkg, orc, monkeypatch):
     ctx.pt2_config(0, 0)
     g_pt2, g_ext, g_con = ctx.pt2(psi, e_s, 1e-6)
     c = ctx.counters()
-    assert c["pt2_parts"] >= 64 and c["pt2_table_slots"] <= 16000
+    assert 4 <= c["pt2_parts"] <= 64 and c["pt2_table_slots"] <= 16000
     assert (g_ext, g_con) == (o["n_external"], o["n_contrib"])
     assert abs(g_pt2 - o["pt2"]) <= PT2_TOL * abs(o["pt2"])
     ctx.close()
