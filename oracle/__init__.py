@@ -56,6 +56,8 @@ def lib():
         L.orc_pt2.restype = None
         L.orc_pt2.argtypes = [C.c_int, dp, dp, C.c_double, up, C.c_int64, dp, C.c_double, C.c_double, C.c_int,
                               C.c_int, C.c_int, dp, ip, ip, dp, dp, dp]
+        L.orc_expand.restype = C.c_int64
+        L.orc_expand.argtypes = [C.c_int, dp, dp, C.c_double, up, C.c_int64, dp, C.c_double, up, dp, dp, dp, C.c_int64]
         L.orc_num_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -166,6 +168,17 @@ def ediag(row_ptr, col, val):
     from scipy.sparse.linalg import eigsh
     w = eigsh(A, k=1, which="SA", tol=1e-13, maxiter=20000, return_eigenvectors=False)
     return float(w[0])
+
+
+def expand(n, h1, eri, e_core, dets, psi, eps2):
+    """Perturbative set P of Eq. 14: (keys [|P|, 2] sorted ascending, score = max_i |H_ai psi_i|, v = sum_i H_ai psi_i, H_aa)."""
+    h1, eri, dets, psi = _f64(h1), _f64(eri), _u64(dets), _f64(psi)
+    m = lib().orc_expand(n, _d(h1), _d(eri), e_core, _u(dets), dets.shape[0], _d(psi), eps2, None, None, None, None, 0)
+    keys = np.zeros((m, 2), dtype=np.uint64)
+    score, v, haa = np.zeros(m), np.zeros(m), np.zeros(m)
+    if m:
+        lib().orc_expand(n, _d(h1), _d(eri), e_core, _u(dets), dets.shape[0], _d(psi), eps2, _u(keys), _d(score), _d(v), _d(haa), m)
+    return keys, score, v, haa
 
 
 def residual(row_ptr, col, val, psi, e_s):

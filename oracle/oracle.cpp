@@ -26,6 +26,7 @@
 #include <cmath>
 #include <cstdint>
 #include <cstring>
+#include <map>
 #include <vector>
 #ifdef _OPENMP
 #include <omp.h>
@@ -356,6 +357,43 @@ void orc_pt2(int n, const double* h1, const double* eri_, double e_core, const u
   if (n_contrib_out) *n_contrib_out = n_contrib;
   if (sum_abs_out) *sum_abs_out = (double)(total_abs / norm2);
   if (min_abs_den_out) *min_abs_den_out = min_den;
+}
+
+// Subspace expansion, Alg. 1 "Subspace Expansion" with the screen of Eq. 14:
+// the perturbative set P = { x' not in V : max_{x in V} |H_x'x psi(x)| >= eps } generated exactly as in orc_pt2 (the tau
+// rule produces precisely the couplings with |H psi| >= eps, so an external belongs to P iff it is generated at least once),
+// returned sorted ascending and deduplicated, with for each a in P: score_a = max_i |H_ai psi_i| over the generated
+// couplings, v_a = their sum (reading Q9) and H_aa.  Returns |P|; writes min(|P|, cap) entries.
+int64_t orc_expand(int n, const double* h1, const double* eri_, double e_core, const u64* dets, int64_t nd, const double* psi,
+                   double eps2, u64* keys_out, double* score_out, double* v_out, double* haa_out, int64_t cap) {
+  Integrals I{n, h1, eri_, e_core};
+  const Det* S = reinterpret_cast<const Det*>(dets);
+  struct Acc { double score; long double v; };
+  std::map<Det, Acc> P;
+  for (int64_t i = 0; i < nd; ++i) {
+    if (psi[i] == 0.0) continue;  // reading Q6
+    const double tau = eps2 == 0.0 ? 0.0 : eps2 / std::fabs(psi[i]);
+    std::vector<Conn> c;
+    connections(I, S[i], tau, &c);
+    for (const Conn& x : c) {
+      if (std::binary_search(S, S + nd, x.d)) continue;  // P = C \ V
+      const double hp = x.h * psi[i];
+      auto it = P.find(x.d);
+      if (it == P.end()) P.emplace(x.d, Acc{std::fabs(hp), (long double)hp});
+      else { it->second.score = std::max(it->second.score, std::fabs(hp)); it->second.v += hp; }
+    }
+  }
+  int64_t k = 0;
+  for (const auto& kv : P) {  // std::map iterates in ascending key order
+    if (k < cap) {
+      keys_out[2 * k] = kv.first.a; keys_out[2 * k + 1] = kv.first.b;
+      if (score_out) score_out[k] = kv.second.score;
+      if (v_out) v_out[k] = (double)kv.second.v;
+      if (haa_out) haa_out[k] = diagonal(I, kv.first);
+    }
+    ++k;
+  }
+  return k;
 }
 
 int orc_num_threads(void) {

@@ -296,3 +296,40 @@ def test_p12_ediag(orc):
     psi = rng.standard_normal(150)
     e, _ = orc.energy(rp, col, val, psi)
     assert e >= lam - 1e-12
+
+
+# ---------------------------------------------------------------- P13: the perturbative set of Eq. 14 (subspace expansion)
+@pytest.mark.parametrize("eps2", [0.0, 1e-3, 2e-2])
+def test_p13_expand_dense_brute_force(orc, eps2):
+    """P = {a not in S : max_i |H_ai psi_i| >= eps} (Eq. 14) against element-wise masks on the dense matrix:
+    the key set (sorted, unique), the score max_i |H_ai psi_i|, the screened sum v_a and H_aa."""
+    n, na, nb = 7, 3, 3
+    h1, eri = small_integrals(n, 61)
+    dets = full_space(n, na, nb)  # 1225, sorted ascending
+    H = orc.dense(n, h1, eri, 0.0, dets)
+    rng = np.random.default_rng(8)
+    idx = np.sort(rng.choice(len(dets), size=150, replace=False))
+    psi = rng.standard_normal(150) * np.exp(-rng.random(150) * 4)
+    psi[7] = 0.0
+    ext = np.setdiff1d(np.arange(len(dets)), idx)
+    Hx = H[np.ix_(ext, idx)]
+    C = Hx * psi[None, :]
+    if eps2 > 0:
+        tau = np.where(psi != 0, eps2 / np.abs(np.where(psi != 0, psi, 1.0)), np.inf)
+    else:
+        tau = np.zeros(150)
+    keep = (np.abs(Hx) >= tau[None, :]) & (Hx != 0) & (psi != 0)[None, :]
+    touched = keep.any(axis=1)
+    keys, score, v, haa = orc.expand(n, h1, eri, 0.0, dets[idx], psi, eps2)
+    assert np.array_equal(keys, dets[ext][touched])                       # full_space is sorted, so this is the sorted set
+    assert np.allclose(score, np.max(np.abs(C) * keep, axis=1)[touched], rtol=1e-13)
+    assert np.allclose(v, (C * keep).sum(axis=1)[touched], rtol=1e-12, atol=1e-15)
+    assert np.allclose(haa, np.diag(H)[ext][touched], rtol=1e-13)
+    if eps2 > 0:
+        # Eq. 14 literally: membership by the max rule equals "generated at least once" (|H psi| >= eps <=> |H| >= eps/|psi|
+        # up to the last ulp of the division, reading Q6; the random data keep clear of that edge)
+        assert np.array_equal(touched, (np.max(np.abs(C) * (Hx != 0), axis=1) >= eps2))
+        assert np.all(score >= eps2 * (1 - 1e-12))
+    r = orc.pt2(n, h1, eri, 0.0, dets[idx], psi, -3.0, eps2)
+    assert r["n_external"] == len(keys)
+    assert np.isclose(r["pt2"], np.sum(v ** 2 / (-3.0 - haa)) / (psi @ psi), rtol=1e-12)
