@@ -119,6 +119,16 @@ dh_status detham_pt2_config(detham_ctx* ctx, int64_t table_slots, int n_parts);
 dh_status detham_pt2(detham_ctx* ctx, const double* psi, double e_s, double eps2, double* pt2_out,
                      int64_t* n_external_out, int64_t* n_contrib_out);
 
+/* expand (Alg. 1 "Subspace Expansion"): the perturbative set of Eq. 14
+ *   P = { a not in S : max_i |H_ai psi_i| >= eps2 },
+ * generated by the same screened enumeration as pt2 (an external belongs to P iff it is generated at least once), written
+ * deduplicated and sorted ascending by (alpha, beta) with, per external: score = max_i |H_ai psi_i|, v = sum_i H_ai psi_i over the
+ * generated couplings (reading Q9) and H_aa (from scratch).  All buffers DEVICE: keys_out uint64 [cap][2]; score_out, v_out,
+ * haa_out fp64 [cap], each may be NULL.  *n_out (HOST) = |P|; if |P| > cap nothing is written and the call returns DH_EINVAL
+ * with *n_out set, so a first call with cap = 0 sizes the buffers.  |P| < 2^32. */
+dh_status detham_expand(detham_ctx* ctx, const double* psi, double eps2, uint64_t* keys_out, double* score_out, double* v_out,
+                        double* haa_out, int64_t cap, int64_t* n_out);
+
 /* Per-partition partial sums (already divided by psi^T psi) of the last detham_pt2; writes min(cap, n_parts) values to
  * `out` (HOST) and the partition count to *n_parts_out. */
 dh_status detham_pt2_partials(detham_ctx* ctx, double* out, int cap, int* n_parts_out);

@@ -13,7 +13,7 @@ STATUS = {0: "DH_OK", 1: "DH_EINVAL", 2: "DH_EUNSORTED", 3: "DH_EPOPCOUNT", 4: "
 
 # every symbol include/detham.h declares
 SYMBOLS = ["detham_create", "detham_set_subspace", "detham_ham_build", "detham_csr", "detham_csr_copy", "detham_energy", "detham_residual", "detham_ediag",
-           "detham_pt2_config", "detham_pt2", "detham_pt2_partials", "detham_solve_host", "detham_connections",
+           "detham_pt2_config", "detham_pt2", "detham_expand", "detham_pt2_partials", "detham_solve_host", "detham_connections",
            "detham_diagonals", "detham_get_counters", "detham_destroy", "detham_strerror", "detham_last_cuda_error"]
 
 
@@ -52,6 +52,7 @@ def load_library():
     L.detham_ediag.argtypes = [vp, vp, C.c_double, C.c_int, dp, C.POINTER(C.c_int)]
     L.detham_pt2_config.argtypes = [vp, C.c_int64, C.c_int]
     L.detham_pt2.argtypes = [vp, vp, C.c_double, C.c_double, dp, ip, ip]
+    L.detham_expand.argtypes = [vp, vp, C.c_double, vp, vp, vp, vp, C.c_int64, ip]
     L.detham_pt2_partials.argtypes = [vp, dp, C.c_int, C.POINTER(C.c_int)]
     L.detham_solve_host.argtypes = [vp, vp, vp, C.c_int64, C.c_double, C.c_double, dp, dp, ip, ip]
     L.detham_connections.argtypes = [vp, C.c_int64, C.c_double, vp, vp, C.c_int64, ip]
@@ -160,6 +161,22 @@ class Detham:
         self._check(self._L.detham_ediag(self._h, v0.data_ptr() if v0 is not None else None, float(tol), int(max_iter),
                                          C.byref(e), C.byref(it)))
         return e.value, it.value
+
+    def expand(self, psi, eps2):
+        """Perturbative set P of Eq. 14 as CUDA tensors: (keys int64 [|P|, 2] sorted, score, v, H_aa)."""
+        import torch
+        assert psi.is_cuda and psi.dtype == torch.float64 and psi.is_contiguous() and psi.numel() == self.n_dets
+        m = C.c_int64(0)
+        st = self._L.detham_expand(self._h, psi.data_ptr(), float(eps2), None, None, None, None, 0, C.byref(m))
+        if st != 0 and not (st == 1 and m.value > 0):
+            self._check(st)
+        n = m.value
+        keys = torch.empty((n, 2), dtype=torch.int64, device=psi.device)
+        score, v, haa = (torch.empty(n, dtype=torch.float64, device=psi.device) for _ in range(3))
+        if n:
+            self._check(self._L.detham_expand(self._h, psi.data_ptr(), float(eps2), keys.data_ptr(), score.data_ptr(), v.data_ptr(),
+                                              haa.data_ptr(), n, C.byref(m)))
+        return keys, score, v, haa
 
     def pt2_config(self, table_slots=0, n_parts=0):
         self._check(self._L.detham_pt2_config(self._h, int(table_slots), int(n_parts)))

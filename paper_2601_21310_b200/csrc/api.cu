@@ -156,6 +156,12 @@ dh_status detham_pt2(detham_ctx* c, const double* psi, double e_s, double eps2, 
   return DH_OK;
 }
 
+dh_status detham_expand(detham_ctx* c, const double* psi, double eps2, uint64_t* keys_out, double* score_out, double* v_out,
+                        double* haa_out, int64_t cap, int64_t* n_out) {
+  if (!c || !c->dets || !psi || !(eps2 >= 0.0) || !n_out || cap < 0 || (cap > 0 && !keys_out)) return DH_EINVAL;
+  return dh_expand(c, psi, eps2, reinterpret_cast<u64*>(keys_out), score_out, v_out, haa_out, cap, n_out);
+}
+
 dh_status detham_pt2_partials(detham_ctx* c, double* out, int cap, int* n_parts_out) {
   if (!c || !out || cap < 0) return DH_EINVAL;
   int m = (int)c->partials.size();

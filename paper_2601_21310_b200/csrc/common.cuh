@@ -111,6 +111,8 @@ dh_status dh_build_jk(detham_ctx* c);
 dh_status dh_get_lists(detham_ctx* c, int pbits, const HbLists** out);
 dh_status dh_ham_build(detham_ctx* c, double eps);
 dh_status dh_energy(detham_ctx* c, const double* psi, double* e_out, double* n2_out, double* y_out);
+dh_status dh_expand(detham_ctx* c, const double* psi, double eps2, u64* keys_out, double* score_out, double* v_out, double* haa_out,
+                    int64_t cap, int64_t* n_out);
 dh_status dh_ediag(detham_ctx* c, const double* v0, double tol, int max_iter, double* e_out, int* iters_out);
 dh_status dh_residual(detham_ctx* c, const double* psi, double e_s, double* r_out, double* internal_out);
 dh_status dh_pt2(detham_ctx* c, const double* psi, double e_s, double eps2, double* out);

@@ -122,9 +122,17 @@ __device__ __forceinline__ double meta_diag(const ProbeCtx& pc, unsigned m) {
                          (int)((m >> 12) & 63u), (int)((m >> 6) & 63u), (int)(m & 63u));
 }
 
+// v_a += H_ai psi_i; in expand mode (row f2) the slot's second payload word holds max_i |H_ai psi_i| (Eq. 14's score)
+// instead of H_aa: the bit patterns of non-negative doubles order like the values, so an unsigned RED.MAX does it.
+template <bool kExpand>
+__device__ __forceinline__ void slot_add(Slot* sp, double cv) {
+  atomicAdd(&sp->v, cv);
+  if (kExpand) atomicMax(reinterpret_cast<u64*>(&sp->haa), (u64)__double_as_longlong(fabs(cv)));
+}
+
 // Resolve up to U candidates per lane: all pending slots are loaded before any is examined, all needed CAS are issued
 // before any result is used.  A slot is {key, v, H_aa}; members of S carry the NaN flag in v and absorb nothing.
-template <int U>
+template <int U, bool kExpand>
 __device__ __forceinline__ void probe_batch(ProbeCtx& pc, const u64 (&ka)[U], const u64 (&kb)[U], const double (&cv)[U],
                                             u64 (&slot)[U], const unsigned (&meta)[U], unsigned pend) {
   if (!pend) return;
@@ -139,7 +147,7 @@ __device__ __forceinline__ void probe_batch(ProbeCtx& pc, const u64 (&ka)[U], co
     for (int u = 0; u < U; ++u)
       if ((pend >> u) & 1u) {
         if (k0[u] == ka[u] && k1[u] == kb[u]) {
-          if (vb[u] != (u64)0x7ff8000000000001ull) { atomicAdd(&pc.table[slot[u]].v, cv[u]); ++pc.contrib; }
+          if (vb[u] != (u64)0x7ff8000000000001ull) { slot_add<kExpand>(pc.table + slot[u], cv[u]); ++pc.contrib; }
           pend &= ~(1u << u);
         } else if ((k0[u] | k1[u]) == 0ull) {
           cas |= 1u << u;
@@ -158,11 +166,11 @@ __device__ __forceinline__ void probe_batch(ProbeCtx& pc, const u64 (&ka)[U], co
       for (int u = 0; u < U; ++u)
         if ((cas >> u) & 1u) {
           if ((k0[u] | k1[u]) == 0ull) {  // claimed: this thread also records H_aa
-            pc.table[slot[u]].haa = meta_diag(pc, meta[u]);
-            atomicAdd(&pc.table[slot[u]].v, cv[u]); ++pc.contrib;
+            if (!kExpand) pc.table[slot[u]].haa = meta_diag(pc, meta[u]);
+            slot_add<kExpand>(pc.table + slot[u], cv[u]); ++pc.contrib;
             pend &= ~(1u << u);
           } else if (k0[u] == ka[u] && k1[u] == kb[u]) {  // lost the race to the same key (never a member: those are pre-inserted)
-            atomicAdd(&pc.table[slot[u]].v, cv[u]); ++pc.contrib;
+            slot_add<kExpand>(pc.table + slot[u], cv[u]); ++pc.contrib;
             pend &= ~(1u << u);
           } else if (++slot[u] == pc.cap) {
             slot[u] = 0;
@@ -183,7 +191,7 @@ __device__ __forceinline__ void tri_decode(int t, int& x, int& y) {
   x = t - y * (y - 1) / 2;
 }
 
-template <int kAccWarps, int kU>
+template <int kAccWarps, int kU, bool kExpand>
 __global__ void __launch_bounds__(kAccWarps * 32, 1)
 pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* __restrict__ psi, int64_t nd, double eps2,
                       unsigned pass, Slot* table, u64 cap, u64* counters /* [0] next row [1] gen [2] contrib [3] max probe */,
@@ -267,7 +275,7 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
           __syncwarp();
           qn -= take;
           gen += pend;
-          probe_batch<1>(pc, ka, kb, cv, slot, meta, pend);
+          probe_batch<1, kExpand>(pc, ka, kb, cv, slot, meta, pend);
         }
       }
     }
@@ -377,7 +385,7 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
           }
         }
         gen += __popc(pend);
-        probe_batch<kU>(pc, ka, kb, cv, slot, meta, pend);
+        probe_batch<kU, kExpand>(pc, ka, kb, cv, slot, meta, pend);
       }
       __syncwarp();
     }
@@ -436,6 +444,35 @@ pt2_scan_kernel(Slot* table, u64 cap, double e_s, double* __restrict__ part /* [
     for (int w = 0; w < 8; ++w) { a += sh[0][w]; b += sh[1][w]; m = fmin(m, sh[2][w]); n += sh[3][w]; }
     double* o = part + 4 * (size_t)blockIdx.x;
     o[0] = a; o[1] = b; o[2] = m; o[3] = n;
+  }
+}
+
+// expand mode (row f2): move every external of this pass {key, v_a, score_a} to the output arrays (order arbitrary: the
+// caller sorts by key afterwards) and clear the table.  Warp-aggregated: one atomic per warp and step.
+__global__ void __launch_bounds__(256)
+pt2_compact_kernel(Slot* table, u64 cap, u64* __restrict__ keys_out, double* __restrict__ v_out, double* __restrict__ score_out,
+                   u64 out_cap, u64* cursor) {
+  const u64 stride = (u64)gridDim.x * blockDim.x;
+  const int lane = threadIdx.x & 31;
+  const u64 cap_pad = (cap + 31) & ~(u64)31;
+  for (u64 t = (u64)blockIdx.x * blockDim.x + threadIdx.x; t < cap_pad; t += stride) {
+    u64 x = 0, y = 0, z = 0, w = 0;
+    if (t < cap) dh_ld256_cs(table + t, x, y, z, w);
+    const bool occ = (x | y) != 0ull;
+    const bool ext = occ && z != (u64)0x7ff8000000000001ull;
+    const unsigned m = __ballot_sync(0xffffffffu, ext);
+    u64 base = 0;
+    if (lane == 0 && m) base = atomicAdd(cursor, (u64)__popc(m));
+    base = __shfl_sync(0xffffffffu, base, 0);
+    if (ext) {
+      const u64 pos = base + __popc(m & ((1u << lane) - 1u));
+      if (pos < out_cap) {
+        keys_out[2 * pos] = x; keys_out[2 * pos + 1] = y;
+        if (v_out) v_out[pos] = __longlong_as_double((long long)z);
+        if (score_out) score_out[pos] = __longlong_as_double((long long)w);
+      }
+    }
+    if (occ) dh_st256_zero(table + t);
   }
 }
 
@@ -528,8 +565,10 @@ static dh_status ensure_table(detham_ctx* c, int64_t slots) {
 // table was sized from the contribution count (an upper bound of the distinct keys).
 // `pilot` (may be NULL): run pass 0 only and return {distinct externals, milliseconds} - the planner's probe of how many
 // contributions share an external.
+struct ExpandOut { u64* keys; double* v; double* score; u64 cap; u64* cursor; };  // device buffers of expand mode
+
 static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, double eps2, int pbits, int64_t slots, bool adapt,
-                             double load, double* out, double* pilot = nullptr) {
+                             double load, double* out, double* pilot = nullptr, const ExpandOut* ex = nullptr) {
   const int64_t nd = c->nd;
   dh_status st = ensure_table(c, slots); if (st != DH_OK) return st;
   Slot* table = reinterpret_cast<Slot*>(c->table);
@@ -541,12 +580,12 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
   struct Variant { int warps, u; AccKernel k; };
   // measured on B200 (profiles/r1_microbench.md): more probes in flight per lane do not help, the table is bound by the
   // throughput of random sector read-modify-writes, not by their latency
-  static const Variant variants[] = {{16, 1, pt2_accumulate_kernel<16, 1>}, {16, 2, pt2_accumulate_kernel<16, 2>},
-                                     {12, 4, pt2_accumulate_kernel<12, 4>}, {12, 1, pt2_accumulate_kernel<12, 1>}};
+  static const Variant variants[] = {{16, 1, pt2_accumulate_kernel<16, 1, false>}, {16, 2, pt2_accumulate_kernel<16, 2, false>},
+                                     {12, 4, pt2_accumulate_kernel<12, 4, false>}, {12, 1, pt2_accumulate_kernel<12, 1, false>}};
   int vi = 0;
   if (const char* e = getenv("DETHAM_PT2_VARIANT")) { int v = atoi(e); if (v >= 0 && v < (int)(sizeof(variants) / sizeof(variants[0]))) vi = v; }
-  const int warps = variants[vi].warps;
-  AccKernel acc_kernel = variants[vi].k;
+  const int warps = ex ? 16 : variants[vi].warps;
+  AccKernel acc_kernel = ex ? pt2_accumulate_kernel<16, 1, true> : variants[vi].k;
   const size_t smem = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + warps * (sizeof(WarpScratch) + sizeof(FlatScratch));
   DH_CUDA(c, cudaFuncSetAttribute(acc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int64_t want = (nd + warps - 1) / warps;
@@ -576,8 +615,13 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
     member_insert_kernel<<<(unsigned)((nd + 255) / 256), 256, 0, c->stream>>>(c->dets, nd, (unsigned)(nparts - 1), (unsigned)pass, table, (u64)cap, overflow);
     acc_kernel<<<grid, warps * 32, smem, c->stream>>>(P, c->dets, psi, nd, eps2, (unsigned)pass, table, (u64)cap, c->dcount, overflow);
     DH_TICK(c, 3);
-    pt2_scan_kernel<<<sgrid, 256, 0, c->stream>>>(table, (u64)cap, e_s, part);
-    final_reduce4_kernel<<<1, 256, 0, c->stream>>>(part, sgrid, results + 4 * pass);
+    if (ex && !pilot) {
+      pt2_compact_kernel<<<sgrid, 256, 0, c->stream>>>(table, (u64)cap, ex->keys, ex->v, ex->score, ex->cap, ex->cursor);
+      DH_CUDA(c, cudaMemsetAsync(results + 4 * pass, 0, 4 * sizeof(double), c->stream));
+    } else {
+      pt2_scan_kernel<<<sgrid, 256, 0, c->stream>>>(table, (u64)cap, e_s, part);
+      final_reduce4_kernel<<<1, 256, 0, c->stream>>>(part, sgrid, results + 4 * pass);
+    }
     DH_CUDA(c, cudaGetLastError());
     DH_TICK(c, 4);
     DH_CUDA(c, cudaMemcpyAsync(hp, c->dcount, 4 * sizeof(u64), cudaMemcpyDeviceToHost, c->stream));
@@ -618,7 +662,7 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
   return DH_OK;
 }
 
-dh_status dh_pt2(detham_ctx* c, const double* psi, double e_s, double eps2, double* out) {
+static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double eps2, double* out, const ExpandOut* ex) {
   const int64_t nd = c->nd;
   dh_status st;
   double load = 0.5;  // target load factor of the table (DETHAM_PT2_LOAD overrides; tuning knob)
@@ -689,7 +733,7 @@ dh_status dh_pt2(detham_ctx* c, const double* psi, double e_s, double eps2, doub
     const int pp = pbits + 3 < DH_MAX_PBITS ? pbits + 3 : DH_MAX_PBITS;
     double pilot[2] = {0.0, 0.0};
     const int64_t pilot_slots = (pp - pbits == 3 && slots / 4 > 1024) ? slots / 4 : slots;  // 1/8 of the keys in 1/4 of the slots
-    st = pt2_attempt(c, psi, e_s, eps2, pp, pilot_slots, false, load, out, pilot);
+    st = pt2_attempt(c, psi, e_s, eps2, pp, pilot_slots, false, load, out, pilot, ex);
     if (st == DH_OK && pilot[0] > 0.0) {
       c->ctr.ms_pt2_plan += pilot[1];
       auto uniq_class = [&](int pb) { const double u = pilot[0] * (double)(1 << (pp - pb)); return 1.2 * u + 8.0 * sqrt(u) + 4096.0; };
@@ -704,11 +748,50 @@ dh_status dh_pt2(detham_ctx* c, const double* psi, double e_s, double eps2, doub
     }
   }
   for (;;) {
-    st = pt2_attempt(c, psi, e_s, eps2, pbits, slots, auto_slots, load, out);
+    if (ex) DH_CUDA(c, cudaMemsetAsync(ex->cursor, 0, sizeof(u64), c->stream));
+    st = pt2_attempt(c, psi, e_s, eps2, pbits, slots, auto_slots && !ex, load, out, nullptr, ex);
     if (st != DH_ETABLEFULL || !auto_parts || pbits >= DH_MAX_PBITS) return st;
     ++pbits;  // the plan was too optimistic: halve the keys per pass and start over
     if (auto_slots) slots = max_slots;
   }
+}
+
+dh_status dh_pt2(detham_ctx* c, const double* psi, double e_s, double eps2, double* out) {
+  return pt2_run(c, psi, e_s, eps2, out, nullptr);
+}
+
+dh_status dh_sort_externals(detham_ctx* c, u64* keys_tmp, double* v_tmp, double* score_tmp, int64_t m, u64* keys_out, double* v_out,
+                            double* score_out);  // expand.cu
+
+// Subspace expansion (row f2): the perturbative set P of Eq. 14 (Alg. 1 "Subspace Expansion"),
+// sorted ascending and deduplicated, with score_a = max_i |H_ai psi_i|, v_a = sum_i H_ai psi_i and H_aa.
+dh_status dh_expand(detham_ctx* c, const double* psi, double eps2, u64* keys_out, double* score_out, double* v_out, double* haa_out,
+                    int64_t cap, int64_t* n_out) {
+  u64* cursor = c->dcount + 16;
+  u64* keys_tmp = nullptr; double* v_tmp = nullptr; double* score_tmp = nullptr;
+  const int64_t tcap = cap > 0 ? cap : 1;
+  DH_CUDA(c, cudaMalloc(&keys_tmp, (size_t)tcap * 2 * sizeof(u64)));
+  auto cleanup = [&]() { cudaFree(keys_tmp); if (v_tmp) cudaFree(v_tmp); if (score_tmp) cudaFree(score_tmp); };
+  if (v_out && cudaMalloc(&v_tmp, (size_t)tcap * sizeof(double)) != cudaSuccess) { cleanup(); cudaGetLastError(); return DH_ENOMEM; }
+  if (score_out && cudaMalloc(&score_tmp, (size_t)tcap * sizeof(double)) != cudaSuccess) { cleanup(); cudaGetLastError(); return DH_ENOMEM; }
+  ExpandOut ex{keys_tmp, v_tmp, score_tmp, (u64)cap, cursor};
+  double dummy = 0.0;
+  dh_status st = pt2_run(c, psi, 0.0, eps2, &dummy, &ex);
+  if (st != DH_OK) { cleanup(); return st; }
+  u64* hp = reinterpret_cast<u64*>(c->pinned);
+  DH_CUDA(c, cudaMemcpyAsync(hp, cursor, sizeof(u64), cudaMemcpyDeviceToHost, c->stream));
+  DH_CUDA(c, cudaStreamSynchronize(c->stream));
+  const int64_t m = (int64_t)hp[0];
+  *n_out = m;
+  c->ctr.pt2_external = m;
+  if (m > cap) { cleanup(); return DH_EINVAL; }  // *n_out tells the caller how much room it takes
+  if (m > 0) {
+    st = dh_sort_externals(c, keys_tmp, v_tmp, score_tmp, m, keys_out, v_out, score_out);
+    if (st == DH_OK && haa_out) st = dh_diagonals(c, keys_out, m, haa_out);
+  }
+  if (st == DH_OK) DH_CUDA(c, cudaStreamSynchronize(c->stream));
+  cleanup();
+  return st;
 }
 
 dh_status dh_connections(detham_ctx* c, int64_t row, double tau, std::vector<u64>& keys, std::vector<double>& h) {

@@ -380,3 +380,26 @@ def test_ediag_lanczos(pkg, orc, name, n_dets, eps):
     e_var, _ = ctx.energy(_psi(p))
     assert e_var >= e1 - 1e-9 * abs(e1)  # Delta_opt >= 0
     ctx.close()
+
+
+@pytest.mark.parametrize("name,n_dets,eps2,parts", [("tiny", None, 0.0, 0), ("tiny", 600, 1e-4, 4), ("h2o", 1500, 1e-6, 0), ("tiny", 1, 0.0, 0)])
+def test_expand_perturbative_set(pkg, orc, name, n_dets, eps2, parts):
+    """the perturbative set P of Eq. 14 (sorted, deduplicated) with score, screened sum and H_aa."""
+    p = make_problem(name, n_dets=n_dets)
+    if n_dets == 1:
+        p["psi"] = np.array([1.0])
+    ctx = _ctx(pkg, p)
+    ctx.pt2_config(0, parts)
+    keys, score, v, haa = (t.cpu().numpy() for t in ctx.expand(_psi(p), eps2))
+    okeys, oscore, ov, ohaa = orc.expand(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"], p["psi"], eps2)
+    assert np.array_equal(keys.view(np.uint64), okeys)          # the set, bit-exact and in sorted order
+    assert np.array_equal(score, oscore)                        # max of identical products: identical bits
+    assert np.allclose(v, ov, rtol=1e-11, atol=1e-14 * np.max(np.abs(ov)))
+    assert np.allclose(haa, ohaa, rtol=1e-13)
+    # the table is left clean: a PT2 on the same context still agrees
+    e_s = float(np.min(ohaa)) - 1.0
+    o = orc.pt2(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"], p["psi"], e_s, eps2)
+    g_pt2, g_ext, g_con = ctx.pt2(_psi(p), e_s, eps2)
+    assert (g_ext, g_con) == (o["n_external"], o["n_contrib"]) and g_ext == len(okeys)
+    assert abs(g_pt2 - o["pt2"]) <= PT2_TOL * abs(o["pt2"])
+    ctx.close()
