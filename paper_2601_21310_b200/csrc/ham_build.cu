@@ -3,7 +3,8 @@
 
 namespace {
 
-constexpr int kWarpsPerCta = 8;
+constexpr int kWarpsPerCta = 8;    // row-sort kernels
+constexpr int kBuildWarps = 16;    // build_kernel: 2 CTAs per SM share the staged tables; 64 registers -> 32 warps per SM
 
 // ---------------------------------------------------------------- determinant store
 __global__ void validate_kernel(const u64* __restrict__ dets, int64_t nd, int n, int na, int nb, int* flags) {
@@ -104,7 +105,7 @@ struct BuildSink {
   }
 };
 
-__global__ void __launch_bounds__(kWarpsPerCta * 32)
+__global__ void __launch_bounds__(kBuildWarps * 32, 2)
 build_kernel(EnumParams P, const u64* __restrict__ dets, int64_t nd, double eps, const u64* __restrict__ hkeys,
              const int* __restrict__ hidx, u64 hcap, const unsigned* __restrict__ hbits, u64 hnbits, int* __restrict__ row_cnt, int* acol, double* aval, int64_t arena_cap,
              Seg* segs, int64_t seg_cap, u64* counters /* [0] next row [1] generated [2] arena cursor [3] segments */,
@@ -300,11 +301,11 @@ dh_status dh_ham_build(detham_ctx* c, double eps) {
     c->row_cap = nd;
   }
   c->nnz = -1;
-  const size_t smem = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + kWarpsPerCta * sizeof(WarpScratch);
+  const size_t smem = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + kBuildWarps * sizeof(WarpScratch);
   st = set_smem(c, build_kernel, smem); if (st != DH_OK) return st;
-  int64_t want = (nd + kWarpsPerCta - 1) / kWarpsPerCta;
-  const int grid = (int)(want < (int64_t)c->sm_count * 4 ? want : (int64_t)c->sm_count * 4);
-  const int64_t slack = (int64_t)grid * kWarpsPerCta * kBlk;  // every warp may leave one block partly used
+  int64_t want = (nd + kBuildWarps - 1) / kBuildWarps;
+  const int grid = (int)(want < (int64_t)c->sm_count * 2 ? want : (int64_t)c->sm_count * 2);
+  const int64_t slack = (int64_t)grid * kBuildWarps * kBlk;  // every warp may leave one block partly used
   int* overflow = reinterpret_cast<int*>(c->dcount + 8);
   int64_t* h = reinterpret_cast<int64_t*>(c->pinned);
   int64_t nnz = 0;
@@ -324,7 +325,7 @@ dh_status dh_ham_build(detham_ctx* c, double eps) {
     }
     DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 16 * sizeof(u64), c->stream));
     DH_TICK(c, 0);
-    build_kernel<<<grid, kWarpsPerCta * 32, smem, c->stream>>>(P, c->dets, nd, eps, c->shash_key, c->shash_idx, (u64)c->shash_cap,
+    build_kernel<<<grid, kBuildWarps * 32, smem, c->stream>>>(P, c->dets, nd, eps, c->shash_key, c->shash_idx, (u64)c->shash_cap,
                                                                c->sbits, (u64)c->sbits_n, c->row_cnt, c->acol, c->aval, c->arena_cap,
                                                                reinterpret_cast<Seg*>(c->segs), c->seg_cap, c->dcount, overflow);
     DH_CUDA(c, cudaGetLastError());
