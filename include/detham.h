@@ -53,6 +53,7 @@ typedef struct {
   int32_t pt2_parts;        /* key partitions (passes) used by the last pt2 */
   int32_t pt2_max_probe;    /* longest probe sequence seen */
   int64_t pt2_table_slots;  /* slots of the hash table used by each pass */
+  int64_t pt2_probe_parts;  /* 0, or the partition count of the one-slice probe the planner ran to measure duplication */
   double pt2_sum_abs;       /* sum_a |v_a^2 / (E_S - H_aa)| / psi^T psi  (conditioning report, reading Q11) */
   double pt2_min_abs_den;   /* min_a |E_S - H_aa| */
   /* device times (CUDA events on the context's stream) of the kernels of the last calls, milliseconds */

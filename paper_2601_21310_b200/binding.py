@@ -20,7 +20,7 @@ SYMBOLS = ["detham_create", "detham_set_subspace", "detham_ham_build", "detham_c
 class Counters(C.Structure):
     _fields_ = [("nnz", C.c_int64), ("build_generated", C.c_int64), ("pt2_generated", C.c_int64),
                 ("pt2_contrib", C.c_int64), ("pt2_external", C.c_int64), ("pt2_parts", C.c_int32),
-                ("pt2_max_probe", C.c_int32), ("pt2_table_slots", C.c_int64), ("pt2_sum_abs", C.c_double),
+                ("pt2_max_probe", C.c_int32), ("pt2_table_slots", C.c_int64), ("pt2_probe_parts", C.c_int64), ("pt2_sum_abs", C.c_double),
                 ("pt2_min_abs_den", C.c_double), ("ms_store", C.c_double), ("ms_build_count", C.c_double),
                 ("ms_build_fill", C.c_double), ("ms_energy", C.c_double), ("ms_pt2_plan", C.c_double),
                 ("ms_pt2_accum", C.c_double), ("ms_pt2_scan", C.c_double)]

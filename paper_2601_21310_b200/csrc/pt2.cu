@@ -93,7 +93,7 @@ __global__ void member_insert_kernel(const u64* __restrict__ dets, int64_t nd, u
 //              phase B: the concatenation of all prefixes is walked 32*kU entries at a time, so every lane holds an
 //              entry whatever the individual prefix lengths are, and each lane issues kU independent table probes
 //              before it waits on any of them.
-constexpr int kChunk = 256;     // occupied pairs per phase-A chunk
+constexpr int kChunk = 128;     // occupied pairs per phase-A chunk
 // kAccWarps warps per CTA and kU table probes in flight per lane are template parameters of the kernel
 
 struct FlatScratch {
@@ -578,14 +578,14 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
   // launch shape: (warps per CTA, probes in flight per lane); DETHAM_PT2_VARIANT selects another one for tuning
   using AccKernel = void (*)(EnumParams, const u64*, const double*, int64_t, double, unsigned, Slot*, u64, u64*, int*);
   struct Variant { int warps, u; AccKernel k; };
-  // measured on B200 (profiles/r1_microbench.md): more probes in flight per lane do not help, the table is bound by the
-  // throughput of random sector read-modify-writes, not by their latency
-  static const Variant variants[] = {{16, 1, pt2_accumulate_kernel<16, 1, false>}, {16, 2, pt2_accumulate_kernel<16, 2, false>},
-                                     {12, 4, pt2_accumulate_kernel<12, 4, false>}, {12, 1, pt2_accumulate_kernel<12, 1, false>}};
+  // measured on B200 (profiles/r1_v2_summary.md): more warps per SM help (Cr2-shaped accumulate 1419 / 1084 / 1025 / 994 ms at
+  // 16 / 24 / 28 / 32 warps), more probes in flight per lane do not (16 warps x 2 probes: slower than x 1)
+  static const Variant variants[] = {{32, 1, pt2_accumulate_kernel<32, 1, false>}, {24, 1, pt2_accumulate_kernel<24, 1, false>},
+                                     {16, 1, pt2_accumulate_kernel<16, 1, false>}, {16, 2, pt2_accumulate_kernel<16, 2, false>}};
   int vi = 0;
   if (const char* e = getenv("DETHAM_PT2_VARIANT")) { int v = atoi(e); if (v >= 0 && v < (int)(sizeof(variants) / sizeof(variants[0]))) vi = v; }
-  const int warps = ex ? 16 : variants[vi].warps;
-  AccKernel acc_kernel = ex ? pt2_accumulate_kernel<16, 1, true> : variants[vi].k;
+  const int warps = ex ? 32 : variants[vi].warps;
+  AccKernel acc_kernel = ex ? pt2_accumulate_kernel<32, 1, true> : variants[vi].k;
   const size_t smem = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + warps * (sizeof(WarpScratch) + sizeof(FlatScratch));
   DH_CUDA(c, cudaFuncSetAttribute(acc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int64_t want = (nd + warps - 1) / warps;
@@ -726,6 +726,7 @@ static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double ep
       slots = need < max_slots ? need : max_slots;
     }
   }
+  int64_t probe_parts = 0;
   if (auto_parts && auto_slots && pbits >= 3) {  // worth it from 8 planned passes on: the probe costs 1/8 of one
     // The contribution count bounds the distinct externals from above, often by a wide margin (9 contributions per
     // external on N2-shaped |S| = 1e6), and every pass costs a list start-up per source.  Probe one slice of the key space
@@ -734,6 +735,7 @@ static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double ep
     double pilot[2] = {0.0, 0.0};
     const int64_t pilot_slots = (pp - pbits == 3 && slots / 4 > 1024) ? slots / 4 : slots;  // 1/8 of the keys in 1/4 of the slots
     st = pt2_attempt(c, psi, e_s, eps2, pp, pilot_slots, false, load, out, pilot, ex);
+    if (st == DH_OK) probe_parts = 1ll << pp;
     if (st == DH_OK && pilot[0] > 0.0) {
       c->ctr.ms_pt2_plan += pilot[1];
       auto uniq_class = [&](int pb) { const double u = pilot[0] * (double)(1 << (pp - pb)); return 1.2 * u + 8.0 * sqrt(u) + 4096.0; };
@@ -750,6 +752,7 @@ static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double ep
   for (;;) {
     if (ex) DH_CUDA(c, cudaMemsetAsync(ex->cursor, 0, sizeof(u64), c->stream));
     st = pt2_attempt(c, psi, e_s, eps2, pbits, slots, auto_slots && !ex, load, out, nullptr, ex);
+    if (st == DH_OK) c->ctr.pt2_probe_parts = probe_parts;
     if (st != DH_ETABLEFULL || !auto_parts || pbits >= DH_MAX_PBITS) return st;
     ++pbits;  // the plan was too optimistic: halve the keys per pass and start over
     if (auto_slots) slots = max_slots;
