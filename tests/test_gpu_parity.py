@@ -403,3 +403,35 @@ def test_expand_perturbative_set(pkg, orc, name, n_dets, eps2, parts):
     assert (g_ext, g_con) == (o["n_external"], o["n_contrib"]) and g_ext == len(okeys)
     assert abs(g_pt2 - o["pt2"]) <= PT2_TOL * abs(o["pt2"])
     ctx.close()
+
+
+def test_against_stored_oracle_values(pkg):
+    """The CUDA path against tests/golden/tiny_oracle.json (written by the oracle alone, tests/golden/make_golden.py)."""
+    import json
+    import os
+    ref = json.load(open(os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden", "tiny_oracle.json")))
+    for tag, n_dets in (("tiny_full", None), ("tiny_600_screened", 600)):
+        g = ref[tag]
+        p = make_problem("tiny", n_dets=n_dets)
+        ctx = _ctx(pkg, p)
+        psi = _psi(p)
+        assert ctx.ham_build(g["eps"]) == g["nnz"]
+        e, n2 = ctx.energy(psi)
+        assert abs(e - g["e_s"]) <= E_TOL * abs(g["e_s"])
+        _, t_int = ctx.residual(psi, g["e_s"], want_r=False)
+        assert abs(t_int - g["internal"]) <= 1e-9 * abs(g["internal"])
+        ed, _ = ctx.ediag(psi)
+        assert abs(ed - g["e_diag"]) <= 1e-9 * abs(g["e_diag"])
+        ctx.pt2_config(0, 4)
+        pt2, n_ext, n_con = ctx.pt2(psi, g["e_s"], g["eps2"])
+        assert (n_ext, n_con) == (g["n_external"], g["n_contrib"])
+        assert abs(pt2 - g["pt2"]) <= PT2_TOL * abs(g["pt2"])
+        assert np.allclose(ctx.pt2_partials(), g["part_sums"], rtol=1e-8, atol=1e-12 * g["sum_abs"])
+        keys, score, _, _ = ctx.expand(psi, g["eps2"])
+        assert keys.shape[0] == g["expand_size"]
+        k = keys.cpu().numpy().view(np.uint64)
+        assert [int(k[0, 0]), int(k[0, 1])] == g["first_key"] and [int(k[-1, 0]), int(k[-1, 1])] == g["last_key"]
+        assert abs(float(score.sum()) - g["expand_score_sum"]) <= 1e-11 * g["expand_score_sum"]
+        ck, ch = ctx.connections(0, g["eps"])
+        assert len(ch) == g["row0_connections"] and abs(float(np.sum(np.abs(ch))) - g["row0_abs_sum"]) <= 1e-12 * g["row0_abs_sum"]
+        ctx.close()

@@ -333,3 +333,27 @@ def test_p13_expand_dense_brute_force(orc, eps2):
     r = orc.pt2(n, h1, eri, 0.0, dets[idx], psi, -3.0, eps2)
     assert r["n_external"] == len(keys)
     assert np.isclose(r["pt2"], np.sum(v ** 2 / (-3.0 - haa)) / (psi @ psi), rtol=1e-12)
+
+
+def test_golden_regression_values():
+    """tests/golden/tiny_oracle.json (written by tests/golden/make_golden.py from the oracle alone: the paper prints no value
+    for this path) still describes the oracle: integers exactly, floating point to 1e-11."""
+    import importlib.util
+    import json
+    import os
+    here = os.path.join(os.path.dirname(os.path.abspath(__file__)), "golden")
+    spec = importlib.util.spec_from_file_location("make_golden", os.path.join(here, "make_golden.py"))
+    mod = importlib.util.module_from_spec(spec)
+    spec.loader.exec_module(mod)
+    now = mod.compute()
+    ref = json.load(open(os.path.join(here, "tiny_oracle.json")))
+    assert sorted(now) == sorted(ref)
+    for tag in ref:
+        for k, v in ref[tag].items():
+            w = now[tag][k]
+            if isinstance(v, float):
+                assert abs(w - v) <= 1e-11 * max(abs(v), 1e-30), (tag, k, v, w)
+            elif isinstance(v, list) and v and isinstance(v[0], float):
+                assert np.allclose(w, v, rtol=1e-11, atol=1e-15), (tag, k)
+            else:
+                assert w == v, (tag, k, v, w)
