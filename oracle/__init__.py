@@ -58,6 +58,8 @@ def lib():
                               C.c_int, C.c_int, dp, ip, ip, dp, dp, dp]
         L.orc_expand.restype = C.c_int64
         L.orc_expand.argtypes = [C.c_int, dp, dp, C.c_double, up, C.c_int64, dp, C.c_double, up, dp, dp, dp, C.c_int64]
+        L.orc_hsp_build.restype = C.c_void_p
+        L.orc_hsp_build.argtypes = [C.c_int, dp, dp, C.c_double, up, C.c_int64, dp, C.c_double, up, C.c_int64]
         L.orc_num_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -179,6 +181,21 @@ def expand(n, h1, eri, e_core, dets, psi, eps2):
     if m:
         lib().orc_expand(n, _d(h1), _d(eri), e_core, _u(dets), dets.shape[0], _d(psi), eps2, _u(keys), _d(score), _d(v), _d(haa), m)
     return keys, score, v, haa
+
+
+def hsp_build(n, h1, eri, e_core, dets, psi, eps2, pkeys):
+    """CSR H_VP (rows = determinants of V, columns = indices into the sorted key list `pkeys`), couplings screened by
+    tau_i = eps2 / |psi_i| as in expand(); (row_ptr int64 [nd+1], col int32 [nnz], val fp64 [nnz])."""
+    h1, eri, dets, psi, pkeys = _f64(h1), _f64(eri), _u64(dets), _f64(psi), _u64(pkeys)
+    nd = dets.shape[0]
+    hnd = lib().orc_hsp_build(n, _d(h1), _d(eri), e_core, _u(dets), nd, _d(psi), eps2, _u(pkeys), pkeys.shape[0])
+    nnz = lib().orc_csr_nnz(hnd)
+    row_ptr = np.empty(nd + 1, dtype=np.int64)
+    col = np.empty(nnz, dtype=np.int32)
+    val = np.empty(nnz, dtype=np.float64)
+    lib().orc_csr_copy(hnd, _i(row_ptr), col.ctypes.data_as(C.POINTER(C.c_int32)), _d(val))
+    lib().orc_csr_free(hnd)
+    return row_ptr, col, val
 
 
 def residual(row_ptr, col, val, psi, e_s):

@@ -19,7 +19,8 @@
 // Parity pins (tests/test_oracle_pins.py): P1 explicit second-quantised operator application, P2 dense FCI
 // eigenvalue bound, P3 bitwise symmetry, P4 eps=0 == unscreened, P5 closed-form counts, P6 PT2 = 0 on the
 // full space, P7 two-electron closed forms, P8 dense brute-force PT2, P9 sum rule, P10 spin-swap symmetry and
-// the textbook Epstein-Nesbet energy of a single reference.  Every function below is pinned by at least one.
+// the textbook Epstein-Nesbet energy of a single reference; P11-P13 the widened rows f1, f2, f4; P14 H_VP / the Proxy
+// Hamiltonian of Eq. 8 against the dense matrix.  Every function below is pinned by at least one.
 //
 // Build: g++ -O2 -std=c++17 -fopenmp -ffp-contract=off -shared -fPIC oracle.cpp -o liboracle.so
 #include <algorithm>
@@ -394,6 +395,39 @@ int64_t orc_expand(int n, const double* h1, const double* eri_, double e_core, c
     ++k;
   }
   return k;
+}
+
+// H_VP in CSR (Eq. 8 PAPER.md:126 "exact off-diagonal elements involving V_k", Eq. S3
+// "H_VP denotes the Hamiltonian block with rows in V and columns in P"; "constructs the sparse Hamiltonian blocks
+// H_VV and H_VP in CSR format").  P is GIVEN as a sorted key list (the output of orc_expand, or any sorted subset a selector
+// kept).  Row i = { (k, H_{P_k, i}) : (P_k, H) in conn(D_i, tau_i) }, tau_i = eps2 / |psi_i| (the same screen that generated P:
+// reading Q9 - only the generated couplings), rows with psi_i == 0 are empty (reading Q6), columns ascending.  No diagonal.
+// Same handle type as orc_ham_build.  The P-P block of Eq. 8 is diagonal: H_aa = orc_diagonal, returned by orc_expand.
+void* orc_hsp_build(int n, const double* h1, const double* eri_, double e_core, const u64* dets, int64_t nd, const double* psi,
+                    double eps2, const u64* pkeys, int64_t m) {
+  Integrals I{n, h1, eri_, e_core};
+  const Det* S = reinterpret_cast<const Det*>(dets);
+  const Det* Pk = reinterpret_cast<const Det*>(pkeys);
+  std::vector<std::vector<std::pair<int32_t, double>>> rows(nd);
+#pragma omp parallel for schedule(dynamic, 16)
+  for (int64_t i = 0; i < nd; ++i) {
+    if (psi[i] == 0.0) continue;
+    const double tau = eps2 == 0.0 ? 0.0 : eps2 / std::fabs(psi[i]);
+    std::vector<Conn> c;
+    connections(I, S[i], tau, &c);
+    auto& r = rows[i];
+    for (const Conn& x : c) {
+      const Det* it = std::lower_bound(Pk, Pk + m, x.d);
+      if (it != Pk + m && *it == x.d) r.push_back({(int32_t)(it - Pk), x.h});
+    }
+    std::sort(r.begin(), r.end(), [](auto& x, auto& y) { return x.first < y.first; });
+  }
+  Csr* out = new Csr;
+  out->row_ptr.assign(nd + 1, 0);
+  for (int64_t i = 0; i < nd; ++i) out->row_ptr[i + 1] = out->row_ptr[i] + (int64_t)rows[i].size();
+  out->col.reserve(out->row_ptr[nd]); out->val.reserve(out->row_ptr[nd]);
+  for (int64_t i = 0; i < nd; ++i) for (auto& e : rows[i]) { out->col.push_back(e.first); out->val.push_back(e.second); }
+  return out;
 }
 
 int orc_num_threads(void) {

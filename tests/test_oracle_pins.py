@@ -335,6 +335,63 @@ def test_p13_expand_dense_brute_force(orc, eps2):
     assert np.isclose(r["pt2"], np.sum(v ** 2 / (-3.0 - haa)) / (psi @ psi), rtol=1e-12)
 
 
+# ---------------------------------------------------------------- P14: H_VP in CSR and the Proxy Hamiltonian of Eq. 8
+@pytest.mark.parametrize("eps2", [0.0, 1e-3, 2e-2])
+def test_p14_hsp_dense_brute_force(orc, eps2):
+    """H_VP against element-wise masks on the dense matrix: entry (i, k) = H[P_k, V_i] where the coupling is
+    generated (|H| >= eps2/|psi_i|, != 0, psi_i != 0), nothing else; columns ascending; a subset of P keeps only its columns;
+    psi_V^T H_VP psi_P of Eq. S3; and at eps2 = 0 the Rayleigh quotient of the Proxy Hamiltonian of Eq. 8-9
+    built from {H_VV, H_VP, diag H_PP} equals the one of the dense matrix with its P-P block replaced by its diagonal."""
+    import scipy.sparse as sp
+    n, na, nb = 7, 3, 3
+    h1, eri = small_integrals(n, 62)
+    dets = full_space(n, na, nb)
+    H = orc.dense(n, h1, eri, 0.0, dets)
+    rng = np.random.default_rng(9)
+    idx = np.sort(rng.choice(len(dets), size=120, replace=False))
+    psi = rng.standard_normal(120) * np.exp(-rng.random(120) * 4)
+    psi[11] = 0.0
+    S = dets[idx]
+    keys, score, v, haa = orc.expand(n, h1, eri, 0.0, S, psi, eps2)
+    pidx = np.array([np.flatnonzero((dets[:, 0] == k[0]) & (dets[:, 1] == k[1]))[0] for k in keys])
+    rp, col, val = orc.hsp_build(n, h1, eri, 0.0, S, psi, eps2, keys)
+    A = sp.csr_matrix((val, col, rp), shape=(120, len(keys))).toarray()
+    Hvp = H[np.ix_(idx, pidx)]
+    tau = np.where(psi != 0, eps2 / np.abs(np.where(psi != 0, psi, 1.0)), np.inf) if eps2 > 0 else np.zeros(120)
+    keep = (np.abs(Hvp) >= tau[:, None]) & (Hvp != 0) & (psi != 0)[:, None]
+    assert np.array_equal(A != 0, keep)
+    assert np.array_equal(A, np.where(keep, Hvp, 0.0))          # same integrals, same operand order: bit for bit
+    for i in range(120):
+        assert np.all(np.diff(col[rp[i]:rp[i + 1]]) > 0)
+    assert np.allclose(A.T @ psi, v, rtol=1e-12, atol=1e-15)    # v_a = sum_i H_ai psi_i over the generated couplings
+    # a selector keeps a subset of P: only those columns survive, renumbered
+    sub = np.sort(rng.choice(len(keys), size=len(keys) // 3, replace=False))
+    rp2, col2, val2 = orc.hsp_build(n, h1, eri, 0.0, S, psi, eps2, keys[sub])
+    A2 = sp.csr_matrix((val2, col2, rp2), shape=(120, len(sub))).toarray()
+    assert np.array_equal(A2, A[:, sub])
+    # Eq. S3: N = psi_V^T H_VV psi_V + psi_V^T H_VP psi_P
+    rps, cols, vals = orc.ham_build(n, h1, eri, 0.0, S, 0.0)
+    Hvv = sp.csr_matrix((vals, cols, rps), shape=(120, 120)).toarray()
+    assert np.array_equal(Hvv, H[np.ix_(idx, idx)])
+    if eps2 == 0.0:
+        psi2 = psi.copy(); psi2[11] = 0.3                      # all rows generate: H_VP is the complete block
+        keys0, _, _, haa0 = orc.expand(n, h1, eri, 0.0, S, psi2, 0.0)
+        p0 = np.array([np.flatnonzero((dets[:, 0] == k[0]) & (dets[:, 1] == k[1]))[0] for k in keys0])
+        rp0, col0, val0 = orc.hsp_build(n, h1, eri, 0.0, S, psi2, 0.0, keys0)
+        B = sp.csr_matrix((val0, col0, rp0), shape=(120, len(keys0))).toarray()
+        T = np.concatenate([idx, p0])
+        Ht = H[np.ix_(T, T)].copy()                             # Eq. 8: exact where a row or column is in V ...
+        pp = Ht[120:, 120:]
+        Ht[120:, 120:] = np.diag(np.diag(pp))                   # ... diagonal on the P-P block
+        proxy = np.block([[Hvv, B], [B.T, np.diag(haa0)]])
+        assert np.allclose(proxy, Ht, rtol=0, atol=1e-13)
+        psi_t = np.concatenate([psi2, rng.standard_normal(len(keys0)) * 0.1])
+        e_proxy = psi_t @ (proxy @ psi_t) / (psi_t @ psi_t)
+        assert np.isclose(e_proxy, psi_t @ (Ht @ psi_t) / (psi_t @ psi_t), rtol=1e-13)
+        n_s3 = psi2 @ (Hvv @ psi2) + psi2 @ (B @ psi_t[120:])
+        assert np.isclose(n_s3, psi2 @ (H[np.ix_(idx, T)] @ psi_t), rtol=1e-12)
+
+
 def test_golden_regression_values():
     """tests/golden/tiny_oracle.json (written by tests/golden/make_golden.py from the oracle alone: the paper prints no value
     for this path) still describes the oracle: integers exactly, floating point to 1e-11."""
