@@ -65,6 +65,9 @@ typedef struct {
   double ms_pt2_plan;       /* pt2 class histogram (pass planning), 0 when both table_slots and n_parts are configured */
   double ms_pt2_accum;      /* pt2 member insert + enumerate/accumulate kernels, summed over passes */
   double ms_pt2_scan;       /* pt2 table scan/clear + reductions, summed over passes */
+  int64_t hsp_nnz;          /* stored entries of H_SP (last detham_hsp_build) */
+  int64_t hsp_generated;    /* excitations that passed the screen in hsp_build (looked up in P) */
+  double ms_hsp_build;      /* hsp_build enumeration pass + arena -> CSR copy + per-row column sort */
 } detham_counters;
 
 /* Create a context: uploads the integrals, derives J_pq = (pp|qq), K_pq = (pq|qp), and builds the heat-bath lists
@@ -129,6 +132,21 @@ dh_status detham_pt2(detham_ctx* ctx, const double* psi, double e_s, double eps2
  * with *n_out set, so a first call with cap = 0 sizes the buffers.  |P| < 2^32. */
 dh_status detham_expand(detham_ctx* ctx, const double* psi, double eps2, uint64_t* keys_out, double* score_out, double* v_out,
                         double* haa_out, int64_t cap, int64_t* n_out);
+
+/* hsp_build ("constructs the sparse Hamiltonian blocks H_VV and H_VP in CSR format"; H_VP
+ * of Eq. S3; the V-P block of the Proxy Hamiltonian, Eq. 8): CSR with one row per determinant of S
+ * and one column per entry of `pkeys` - DEVICE uint64 [m][2], strictly ascending by (alpha, beta), same electron counts as S
+ * (DH_EUNSORTED / DH_EPOPCOUNT otherwise): the output of detham_expand or any sorted subset a selector kept; borrowed for the
+ * duration of the call only.  Row i holds H_{P_k, i} for every coupling the screen of Eq. 14 generates from source i
+ * (|H| >= eps2 / |psi_i|, H != 0; rows with psi_i == 0 are empty: readings Q6, Q9) whose target is in `pkeys`; columns ascending.
+ * The P-P block of Eq. 8 is diagonal: it is detham_expand's haa_out (or detham_diagonals).  psi: DEVICE fp64 [n_dets].
+ * m < 2^31, may be 0.  *nnz_out (HOST, may be NULL).  The CSR is owned by the context (detham_hsp_csr / detham_hsp_csr_copy),
+ * valid until the next detham_hsp_build / detham_set_subspace / detham_destroy. */
+dh_status detham_hsp_build(detham_ctx* ctx, const double* psi, double eps2, const uint64_t* pkeys, int64_t m, int64_t* nnz_out);
+/* Device pointers of H_SP: row_ptr int64 [n_dets+1], col int32 [nnz], val fp64 [nnz].  DH_EINVAL if none exists. */
+dh_status detham_hsp_csr(detham_ctx* ctx, const int64_t** row_ptr, const int32_t** col, const double** val);
+/* Copy H_SP into caller buffers (each HOST or DEVICE, detected; any may be NULL to skip).  Synchronises the stream. */
+dh_status detham_hsp_csr_copy(detham_ctx* ctx, int64_t* row_ptr, int32_t* col, double* val);
 
 /* Per-partition partial sums (already divided by psi^T psi) of the last detham_pt2; writes min(cap, n_parts) values to
  * `out` (HOST) and the partition count to *n_parts_out. */

@@ -13,7 +13,7 @@ STATUS = {0: "DH_OK", 1: "DH_EINVAL", 2: "DH_EUNSORTED", 3: "DH_EPOPCOUNT", 4: "
 
 # every symbol include/detham.h declares
 SYMBOLS = ["detham_create", "detham_set_subspace", "detham_ham_build", "detham_csr", "detham_csr_copy", "detham_energy", "detham_residual", "detham_ediag",
-           "detham_pt2_config", "detham_pt2", "detham_expand", "detham_pt2_partials", "detham_solve_host", "detham_connections",
+           "detham_pt2_config", "detham_pt2", "detham_expand", "detham_hsp_build", "detham_hsp_csr", "detham_hsp_csr_copy", "detham_pt2_partials", "detham_solve_host", "detham_connections",
            "detham_diagonals", "detham_get_counters", "detham_destroy", "detham_strerror", "detham_last_cuda_error"]
 
 
@@ -23,7 +23,8 @@ class Counters(C.Structure):
                 ("pt2_max_probe", C.c_int32), ("pt2_table_slots", C.c_int64), ("pt2_probe_parts", C.c_int64), ("pt2_sum_abs", C.c_double),
                 ("pt2_min_abs_den", C.c_double), ("ms_store", C.c_double), ("ms_build_count", C.c_double),
                 ("ms_build_fill", C.c_double), ("ms_energy", C.c_double), ("ms_pt2_plan", C.c_double),
-                ("ms_pt2_accum", C.c_double), ("ms_pt2_scan", C.c_double)]
+                ("ms_pt2_accum", C.c_double), ("ms_pt2_scan", C.c_double),
+                ("hsp_nnz", C.c_int64), ("hsp_generated", C.c_int64), ("ms_hsp_build", C.c_double)]
 
 
 class DethamError(RuntimeError):
@@ -53,6 +54,9 @@ def load_library():
     L.detham_pt2_config.argtypes = [vp, C.c_int64, C.c_int]
     L.detham_pt2.argtypes = [vp, vp, C.c_double, C.c_double, dp, ip, ip]
     L.detham_expand.argtypes = [vp, vp, C.c_double, vp, vp, vp, vp, C.c_int64, ip]
+    L.detham_hsp_build.argtypes = [vp, vp, C.c_double, vp, C.c_int64, ip]
+    L.detham_hsp_csr.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
+    L.detham_hsp_csr_copy.argtypes = [vp, vp, vp, vp]
     L.detham_pt2_partials.argtypes = [vp, dp, C.c_int, C.POINTER(C.c_int)]
     L.detham_solve_host.argtypes = [vp, vp, vp, C.c_int64, C.c_double, C.c_double, dp, dp, ip, ip]
     L.detham_connections.argtypes = [vp, C.c_int64, C.c_double, vp, vp, C.c_int64, ip]
@@ -177,6 +181,25 @@ class Detham:
             self._check(self._L.detham_expand(self._h, psi.data_ptr(), float(eps2), keys.data_ptr(), score.data_ptr(), v.data_ptr(),
                                               haa.data_ptr(), n, C.byref(m)))
         return keys, score, v, haa
+
+    def hsp_build(self, psi, eps2, pkeys):
+        """H_SP in CSR against the sorted key list `pkeys` (CUDA [m, 2] int64/uint64, e.g. expand()'s keys); returns nnz."""
+        import torch
+        assert psi.is_cuda and psi.dtype == torch.float64 and psi.is_contiguous() and psi.numel() == self.n_dets
+        ptr, m = _dev_u64(pkeys)
+        nnz = C.c_int64(0)
+        self._check(self._L.detham_hsp_build(self._h, psi.data_ptr(), float(eps2), ptr if m else None, m, C.byref(nnz)))
+        self.hsp_nnz = nnz.value
+        return nnz.value
+
+    def hsp_csr(self):
+        """(row_ptr int64 [|S|+1], col int32 [nnz], val fp64 [nnz]) of H_SP as new torch CUDA tensors."""
+        import torch
+        rp = torch.empty(self.n_dets + 1, dtype=torch.int64, device="cuda")
+        col = torch.empty(self.hsp_nnz, dtype=torch.int32, device="cuda")
+        val = torch.empty(self.hsp_nnz, dtype=torch.float64, device="cuda")
+        self._check(self._L.detham_hsp_csr_copy(self._h, rp.data_ptr(), col.data_ptr(), val.data_ptr()))
+        return rp, col, val
 
     def pt2_config(self, table_slots=0, n_parts=0):
         self._check(self._L.detham_pt2_config(self._h, int(table_slots), int(n_parts)))

@@ -23,7 +23,7 @@ void free_all(detham_ctx* c) {
   f(c->h1); f(c->eri); f(c->J); f(c->JK); f(c->hd);
   for (auto& L : c->lists) { f(L.sub_off); f(L.val); f(L.ab); }
   f(c->dets_owned); f(c->psi_owned); f(c->shash_key); f(c->shash_idx); f(c->sbits);
-  f(c->row_ptr); f(c->col); f(c->val); f(c->row_cnt); f(c->acol); f(c->aval); f(c->segs); f(c->table); f(c->red); f(c->dcount); f(c->hist);
+  f(c->row_ptr); f(c->col); f(c->val); f(c->row_cnt); f(c->sp_row_ptr); f(c->sp_col); f(c->sp_val); f(c->phash_key); f(c->phash_idx); f(c->acol); f(c->aval); f(c->segs); f(c->table); f(c->red); f(c->dcount); f(c->hist);
   if (c->pinned) cudaFreeHost(c->pinned);
   for (auto& e : c->ev) if (e) cudaEventDestroy(e);
 }
@@ -86,7 +86,7 @@ dh_status detham_create(detham_ctx** out, int n_orb, int n_alpha, int n_beta, co
 dh_status detham_set_subspace(detham_ctx* c, const uint64_t* dets, int64_t n_dets) {
   if (!c || !dets || n_dets < 1 || n_dets >= (1ll << 31)) return DH_EINVAL;
   if (!is_device_ptr(dets)) return DH_EINVAL;
-  c->dets = nullptr; c->nd = 0; c->nnz = -1;
+  c->dets = nullptr; c->nd = 0; c->nnz = -1; c->sp_nnz = -1;
   DH_TICK(c, 0);
   dh_status st = dh_validate_subspace(c, reinterpret_cast<const u64*>(dets), n_dets);
   if (st != DH_OK) return st;
@@ -160,6 +160,30 @@ dh_status detham_expand(detham_ctx* c, const double* psi, double eps2, uint64_t*
                         double* haa_out, int64_t cap, int64_t* n_out) {
   if (!c || !c->dets || !psi || !(eps2 >= 0.0) || !n_out || cap < 0 || (cap > 0 && !keys_out)) return DH_EINVAL;
   return dh_expand(c, psi, eps2, reinterpret_cast<u64*>(keys_out), score_out, v_out, haa_out, cap, n_out);
+}
+
+dh_status detham_hsp_build(detham_ctx* c, const double* psi, double eps2, const uint64_t* pkeys, int64_t m, int64_t* nnz_out) {
+  if (!c || !c->dets || !psi || !(eps2 >= 0.0) || m < 0 || m >= (1ll << 31) || (m > 0 && (!pkeys || !is_device_ptr(pkeys)))) return DH_EINVAL;
+  c->sp_nnz = -1;
+  dh_status st = dh_hsp_build(c, psi, eps2, reinterpret_cast<const u64*>(pkeys), m);
+  if (st == DH_OK && nnz_out) *nnz_out = c->sp_nnz;
+  return st;
+}
+
+dh_status detham_hsp_csr(detham_ctx* c, const int64_t** row_ptr, const int32_t** col, const double** val) {
+  if (!c || c->sp_nnz < 0 || !row_ptr || !col || !val) return DH_EINVAL;
+  *row_ptr = c->sp_row_ptr; *col = c->sp_col; *val = c->sp_val;
+  return DH_OK;
+}
+
+dh_status detham_hsp_csr_copy(detham_ctx* c, int64_t* row_ptr, int32_t* col, double* val) {
+  if (!c || c->sp_nnz < 0) return DH_EINVAL;
+  auto kind = [](const void* p) { return is_device_ptr(p) ? cudaMemcpyDeviceToDevice : cudaMemcpyDeviceToHost; };
+  if (row_ptr) DH_CUDA(c, cudaMemcpyAsync(row_ptr, c->sp_row_ptr, (c->nd + 1) * sizeof(int64_t), kind(row_ptr), c->stream));
+  if (col && c->sp_nnz) DH_CUDA(c, cudaMemcpyAsync(col, c->sp_col, c->sp_nnz * sizeof(int), kind(col), c->stream));
+  if (val && c->sp_nnz) DH_CUDA(c, cudaMemcpyAsync(val, c->sp_val, c->sp_nnz * sizeof(double), kind(val), c->stream));
+  DH_CUDA(c, cudaStreamSynchronize(c->stream));
+  return DH_OK;
 }
 
 dh_status detham_pt2_partials(detham_ctx* c, double* out, int cap, int* n_parts_out) {

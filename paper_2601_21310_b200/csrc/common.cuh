@@ -67,13 +67,26 @@ struct detham_ctx {
   double* val = nullptr;
   int64_t nnz = -1;
   int64_t csr_cap = 0;
-  int* row_cnt = nullptr;  // device int32 [nd]
-  int64_t row_cap = 0;
+  int64_t row_cap = 0;     // rows row_ptr has room for
+  int* row_cnt = nullptr;  // device int32 [nd], shared by the H_SS and H_SP builds
+  int64_t row_cnt_cap = 0;
   int* acol = nullptr;     // build arena: hits in warp order, copied to col/val once the row offsets are known
   double* aval = nullptr;
   int64_t arena_cap = 0;   // entries
   void* segs = nullptr;    // arena segments
   int64_t seg_cap = 0;
+
+  // CSR H_SP (row f3) and the lookup index of the caller's P it was built against
+  int64_t* sp_row_ptr = nullptr;
+  int* sp_col = nullptr;
+  double* sp_val = nullptr;
+  int64_t sp_nnz = -1;
+  int64_t sp_csr_cap = 0;
+  int64_t sp_row_cap = 0;
+  int64_t sp_cols = 0;
+  u64* phash_key = nullptr;
+  int* phash_idx = nullptr;
+  int64_t phash_cap = 0;
 
   // pt2
   int64_t cfg_table_slots = 0;
@@ -110,6 +123,7 @@ inline double dh_elapsed(detham_ctx* c, int a, int b) { float ms = 0.f; cudaEven
 dh_status dh_build_jk(detham_ctx* c);
 dh_status dh_get_lists(detham_ctx* c, int pbits, const HbLists** out);
 dh_status dh_ham_build(detham_ctx* c, double eps);
+dh_status dh_hsp_build(detham_ctx* c, const double* psi, double eps2, const u64* pkeys, int64_t m);
 dh_status dh_energy(detham_ctx* c, const double* psi, double* e_out, double* n2_out, double* y_out);
 dh_status dh_expand(detham_ctx* c, const double* psi, double eps2, u64* keys_out, double* score_out, double* v_out, double* haa_out,
                     int64_t cap, int64_t* n_out);

@@ -168,16 +168,22 @@ __device__ __forceinline__ void dh_enumerate(const EnumParams& P, const CtaTable
         const int64_t so = (int64_t)(s * P.nss + j * (j - 1) / 2 + i) * NP + cls;
         const int beg = __ldg(P.sub_off + so), end = __ldg(P.sub_off + so + 1);
         const u64 wij = w ^ (1ull << i) ^ (1ull << j);
+        // the next 32 entries (value and orbital pair) are loaded before this batch is looked up, so the list latency hides
+        // behind the sink's; the batch past the early exit is loaded in vain (one per pair)
+        double vn = beg + lane < end ? __ldg(P.lval + beg + lane) : 0.0;
+        unsigned mn = beg + lane < end ? __ldg(P.lab + beg + lane) : 0u;
         for (int k0 = beg; k0 < end; k0 += 32) {
-          int k = k0 + lane;
-          bool inb = k < end;
-          double v = inb ? __ldg(P.lval + k) : 0.0;
+          const bool inb = k0 + lane < end;
+          double v = vn;
+          const unsigned m = mn;
+          const int kn = k0 + 32 + lane;
+          vn = kn < end ? __ldg(P.lval + kn) : 0.0;
+          mn = kn < end ? __ldg(P.lab + kn) : 0u;
           bool big = inb && fabs(v) >= tau;
           bool act = big && v != 0.0;
           int a = 0, b = 0;
           u64 ka = da, kb = db, z = zij;
           if (act) {
-            unsigned m = __ldg(P.lab + k);
             a = m & 0xFF; b = m >> 8;
             act = !((w >> a) & 1ull) && !((w >> b) & 1ull);
             if (act) {
@@ -204,16 +210,20 @@ __device__ __forceinline__ void dh_enumerate(const EnumParams& P, const CtaTable
       const unsigned cls = ((unsigned)zij ^ pass) & pmask;
       const int64_t so = (int64_t)(2 * P.nss + i * n + j) * NP + cls;
       const int beg = __ldg(P.sub_off + so), end = __ldg(P.sub_off + so + 1);
+      double vn = beg + lane < end ? __ldg(P.lval + beg + lane) : 0.0;
+      unsigned mn = beg + lane < end ? __ldg(P.lab + beg + lane) : 0u;
       for (int k0 = beg; k0 < end; k0 += 32) {
-        int k = k0 + lane;
-        bool inb = k < end;
-        double v = inb ? __ldg(P.lval + k) : 0.0;
+        const bool inb = k0 + lane < end;
+        double v = vn;
+        const unsigned m = mn;
+        const int kn = k0 + 32 + lane;
+        vn = kn < end ? __ldg(P.lval + kn) : 0.0;
+        mn = kn < end ? __ldg(P.lab + kn) : 0u;
         bool big = inb && fabs(v) >= tau;
         bool act = big && v != 0.0;
         int a = 0, b = 0;
         u64 ka = da, kb = db, z = zij;
         if (act) {
-          unsigned m = __ldg(P.lab + k);
           a = m & 0xFF; b = m >> 8;
           act = !((da >> a) & 1ull) && !((db >> b) & 1ull);
           if (act) {

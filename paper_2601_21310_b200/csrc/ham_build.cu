@@ -29,8 +29,10 @@ __global__ void shash_insert_kernel(const u64* __restrict__ dets, int64_t nd, u6
   if (t >= nd) return;
   u64 a = dets[2 * t], b = dets[2 * t + 1];
   const u64 z = dh_zobrist(a, b, Z);
-  const u64 hb = __umul64hi(z, nbits);  // membership pre-filter: one bit per determinant (dh_member)
-  atomicOr(bits + (hb >> 5), 1u << (hb & 31));
+  if (bits) {  // membership pre-filter: one bit per determinant (dh_maybe_member); the index of P has none
+    const u64 hb = __umul64hi(z, nbits);
+    atomicOr(bits + (hb >> 5), 1u << (hb & 31));
+  }
   u64 slot = __umul64hi(z, cap);
   for (;;) {
     Key128 old = dh_cas128(keys + 2 * slot, Key128{0ull, 0ull}, Key128{a, b});
@@ -92,21 +94,24 @@ struct BuildSink {
   }
   __device__ __forceinline__ bool pre(u64 ka, u64 kb, u64 z) {
     ++generated;
-    pre_tok = dh_maybe_member(bits, nbits, z) ? dh_shash_find(keys, idx, cap, ka, kb, z) : -1;
+    pre_tok = (!bits || dh_maybe_member(bits, nbits, z)) ? dh_shash_find(keys, idx, cap, ka, kb, z) : -1;
     return pre_tok >= 0;
   }
   __device__ __forceinline__ void emit(bool act, u64 ka, u64 kb, u64 z, double H, int kind, int, int, int, int, int) {
     int tok = -1;
     if (act) {
       if (kind == 0) tok = pre_tok;
-      else { ++generated; if (dh_maybe_member(bits, nbits, z)) tok = dh_shash_find(keys, idx, cap, ka, kb, z); }
+      else { ++generated; if (!bits || dh_maybe_member(bits, nbits, z)) tok = dh_shash_find(keys, idx, cap, ka, kb, z); }
     }
     put(tok >= 0, tok, H);
   }
 };
 
+// kSP = false: H_SS (a6): tau = eps for every row, diagonal first.  kSP = true: H_SP (row f3): the index is that of the caller's
+// sorted P, tau_i = eps / |psi_i| as in pt2 / expand (reading Q6, Q9), rows with psi_i == 0 stay empty, no diagonal.
+template <bool kSP>
 __global__ void __launch_bounds__(kBuildWarps * 32, 2)
-build_kernel(EnumParams P, const u64* __restrict__ dets, int64_t nd, double eps, const u64* __restrict__ hkeys,
+build_kernel(EnumParams P, const u64* __restrict__ dets, const double* __restrict__ psi, int64_t nd, double eps, const u64* __restrict__ hkeys,
              const int* __restrict__ hidx, u64 hcap, const unsigned* __restrict__ hbits, u64 hnbits, int* __restrict__ row_cnt, int* acol, double* aval, int64_t arena_cap,
              Seg* segs, int64_t seg_cap, u64* counters /* [0] next row [1] generated [2] arena cursor [3] segments */,
              int* overflow) {
@@ -122,14 +127,20 @@ build_kernel(EnumParams P, const u64* __restrict__ dets, int64_t nd, double eps,
     row = __shfl_sync(0xffffffffu, row, 0);
     if ((int64_t)row >= nd) break;
     const u64 da = dets[2 * row], db = dets[2 * row + 1];
+    double tau = eps;
+    if (kSP) {
+      const double p = psi[row];
+      if (p == 0.0) { if (lane == 0) row_cnt[row] = 0; continue; }
+      tau = eps == 0.0 ? 0.0 : __ddiv_rn(eps, fabs(p));
+    }
     dh_fill_occ(P, ws, da, db, lane);
     const double e0 = dh_fill_U(P, T, ws, lane);
     sink.begin_row((int)row);
-    sink.put(lane == 0, (int)row, e0);  // the diagonal is always kept (reading Q4)
+    if (!kSP) sink.put(lane == 0, (int)row, e0);  // the diagonal is always kept (reading Q4)
     u64 zsrc = 0;
     if (lane == 0) zsrc = dh_zobrist(da, db, T.Z);
     zsrc = __shfl_sync(0xffffffffu, zsrc, 0);
-    dh_enumerate(P, T, ws, da, db, eps, zsrc, 0u, sink, lane);
+    dh_enumerate(P, T, ws, da, db, tau, zsrc, 0u, sink, lane);
     sink.end_row();
     if (lane == 0) row_cnt[row] = sink.count;
     __syncwarp();
@@ -286,23 +297,36 @@ static EnumParams make_params(detham_ctx* c, const HbLists* L) {
 }
 EnumParams dh_make_params(detham_ctx* c, const HbLists* L) { return make_params(c, L); }
 
-dh_status dh_ham_build(detham_ctx* c, double eps) {
+// The CSR a build writes and the index its candidates are looked up in: H_SS (columns = positions in S) or H_SP (row f3:
+// columns = positions in the caller's sorted P).  Both share the arena and the row-count buffer.
+struct CsrTarget {
+  int64_t** row_ptr; int** col; double** val; int64_t* nnz; int64_t* csr_cap; int64_t* row_cap;
+  const u64* hkeys; const int* hidx; int64_t hcap; const unsigned* hbits; int64_t hnbits;
+};
+
+static dh_status build_csr(detham_ctx* c, const CsrTarget& T, const double* psi /* NULL: H_SS */, double eps) {
+  const bool sp = psi != nullptr;
   const HbLists* L = nullptr;
   dh_status st = dh_get_lists(c, 0, &L);
   if (st != DH_OK) return st;
   EnumParams P = make_params(c, L);
   const int64_t nd = c->nd;
-  if (c->row_cap < nd) {
+  if (c->row_cnt_cap < nd) {
     if (c->row_cnt) cudaFree(c->row_cnt);
-    if (c->row_ptr) cudaFree(c->row_ptr);
-    c->row_cnt = nullptr; c->row_ptr = nullptr; c->row_cap = 0;
+    c->row_cnt = nullptr; c->row_cnt_cap = 0;
     DH_CUDA(c, cudaMalloc(&c->row_cnt, nd * sizeof(int)));
-    DH_CUDA(c, cudaMalloc(&c->row_ptr, (nd + 1) * sizeof(int64_t)));
-    c->row_cap = nd;
+    c->row_cnt_cap = nd;
   }
-  c->nnz = -1;
+  if (*T.row_cap < nd) {
+    if (*T.row_ptr) cudaFree(*T.row_ptr);
+    *T.row_ptr = nullptr; *T.row_cap = 0;
+    DH_CUDA(c, cudaMalloc(T.row_ptr, (nd + 1) * sizeof(int64_t)));
+    *T.row_cap = nd;
+  }
+  *T.nnz = -1;
   const size_t smem = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + kBuildWarps * sizeof(WarpScratch);
-  st = set_smem(c, build_kernel, smem); if (st != DH_OK) return st;
+  st = sp ? set_smem(c, build_kernel<true>, smem) : set_smem(c, build_kernel<false>, smem);
+  if (st != DH_OK) return st;
   int64_t want = (nd + kBuildWarps - 1) / kBuildWarps;
   const int grid = (int)(want < (int64_t)c->sm_count * 2 ? want : (int64_t)c->sm_count * 2);
   const int64_t slack = (int64_t)grid * kBuildWarps * kBlk;  // every warp may leave one block partly used
@@ -325,49 +349,89 @@ dh_status dh_ham_build(detham_ctx* c, double eps) {
     }
     DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 16 * sizeof(u64), c->stream));
     DH_TICK(c, 0);
-    build_kernel<<<grid, kBuildWarps * 32, smem, c->stream>>>(P, c->dets, nd, eps, c->shash_key, c->shash_idx, (u64)c->shash_cap,
-                                                               c->sbits, (u64)c->sbits_n, c->row_cnt, c->acol, c->aval, c->arena_cap,
-                                                               reinterpret_cast<Seg*>(c->segs), c->seg_cap, c->dcount, overflow);
+    auto kernel = sp ? build_kernel<true> : build_kernel<false>;
+    kernel<<<grid, kBuildWarps * 32, smem, c->stream>>>(P, c->dets, psi, nd, eps, T.hkeys, T.hidx, (u64)T.hcap, T.hbits, (u64)T.hnbits,
+                                                        c->row_cnt, c->acol, c->aval, c->arena_cap,
+                                                        reinterpret_cast<Seg*>(c->segs), c->seg_cap, c->dcount, overflow);
     DH_CUDA(c, cudaGetLastError());
-    scan_rows_kernel<<<1, 1024, 0, c->stream>>>(c->row_cnt, nd, c->row_ptr);
+    scan_rows_kernel<<<1, 1024, 0, c->stream>>>(c->row_cnt, nd, *T.row_ptr);
     DH_CUDA(c, cudaGetLastError());
     DH_TICK(c, 1);
-    DH_CUDA(c, cudaMemcpyAsync(h, c->row_ptr + nd, sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(c, cudaMemcpyAsync(h, *T.row_ptr + nd, sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
     DH_CUDA(c, cudaMemcpyAsync(h + 1, c->dcount, 4 * sizeof(u64), cudaMemcpyDeviceToHost, c->stream));
     DH_CUDA(c, cudaMemcpyAsync(h + 5, overflow, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
     DH_CUDA(c, cudaStreamSynchronize(c->stream));
     ms_pass += dh_elapsed(c, 0, 1);
     nnz = h[0];
-    c->ctr.build_generated = h[2];
+    if (sp) c->ctr.hsp_generated = h[2]; else c->ctr.build_generated = h[2];
     if (!*reinterpret_cast<int*>(h + 5)) break;
     if (attempt >= 1) return DH_ENOMEM;  // cannot happen: the second attempt is sized from the exact count
     want_arena = nnz + nnz / 32 + slack;  // a block is closed when the next batch of <= 32 hits does not fit: < 32 of 1024 entries lost
   }
   const int64_t nseg = h[4];
-  if (c->csr_cap < nnz) {
-    if (c->col) cudaFree(c->col);
-    if (c->val) cudaFree(c->val);
-    c->col = nullptr; c->val = nullptr; c->csr_cap = 0;
-    DH_CUDA(c, cudaMalloc(&c->col, nnz * sizeof(int)));
-    DH_CUDA(c, cudaMalloc(&c->val, nnz * sizeof(double)));
-    c->csr_cap = nnz;
+  if (*T.csr_cap < nnz) {
+    if (*T.col) cudaFree(*T.col);
+    if (*T.val) cudaFree(*T.val);
+    *T.col = nullptr; *T.val = nullptr; *T.csr_cap = 0;
+    const int64_t cap = nnz > 0 ? nnz : 1;
+    DH_CUDA(c, cudaMalloc(T.col, cap * sizeof(int)));
+    DH_CUDA(c, cudaMalloc(T.val, cap * sizeof(double)));
+    *T.csr_cap = cap;
   }
   DH_TICK(c, 2);
   {
     int64_t blocks = (nseg + 7) / 8;
     const int cgrid = (int)(blocks < (int64_t)c->sm_count * 8 ? (blocks > 0 ? blocks : 1) : (int64_t)c->sm_count * 8);
-    copy_segs_kernel<<<cgrid, 256, 0, c->stream>>>(reinterpret_cast<const Seg*>(c->segs), nseg, c->row_ptr, c->acol, c->aval, c->col, c->val);
+    copy_segs_kernel<<<cgrid, 256, 0, c->stream>>>(reinterpret_cast<const Seg*>(c->segs), nseg, *T.row_ptr, c->acol, c->aval, *T.col, *T.val);
     DH_CUDA(c, cudaGetLastError());
   }
-  sort_rows_warp_kernel<<<(unsigned)((nd + kWarpsPerCta - 1) / kWarpsPerCta), kWarpsPerCta * 32, 0, c->stream>>>(c->row_ptr, nd, c->col, c->val);
+  sort_rows_warp_kernel<<<(unsigned)((nd + kWarpsPerCta - 1) / kWarpsPerCta), kWarpsPerCta * 32, 0, c->stream>>>(*T.row_ptr, nd, *T.col, *T.val);
   DH_CUDA(c, cudaGetLastError());
-  sort_rows_cta_kernel<<<c->sm_count * 2, 1024, 0, c->stream>>>(c->row_ptr, nd, c->col, c->val);
+  sort_rows_cta_kernel<<<c->sm_count * 2, 1024, 0, c->stream>>>(*T.row_ptr, nd, *T.col, *T.val);
   DH_CUDA(c, cudaGetLastError());
   DH_TICK(c, 3);
   DH_CUDA(c, cudaEventSynchronize(c->ev[3]));
-  c->ctr.ms_build_count = ms_pass;
-  c->ctr.ms_build_fill = dh_elapsed(c, 2, 3);
-  c->nnz = nnz;
-  c->ctr.nnz = nnz;
+  if (sp) {
+    c->ctr.ms_hsp_build = ms_pass + dh_elapsed(c, 2, 3);
+    c->ctr.hsp_nnz = nnz;
+  } else {
+    c->ctr.ms_build_count = ms_pass;
+    c->ctr.ms_build_fill = dh_elapsed(c, 2, 3);
+    c->ctr.nnz = nnz;
+  }
+  *T.nnz = nnz;
   return DH_OK;
+}
+
+dh_status dh_ham_build(detham_ctx* c, double eps) {
+  CsrTarget T{&c->row_ptr, &c->col, &c->val, &c->nnz, &c->csr_cap, &c->row_cap,
+              c->shash_key, c->shash_idx, c->shash_cap, c->sbits, c->sbits_n};
+  return build_csr(c, T, nullptr, eps);
+}
+
+// H_SP (row f3; "constructs the sparse Hamiltonian blocks H_VV and H_VP in CSR format", Eq. 8 PAPER.md:126,
+// Eq. S3): rows = determinants of S, columns = positions in the caller's sorted, deduplicated key list P
+// (detham_expand's output or any sorted subset of it), values H_{P_k, i} of the couplings the screen of Eq. 14 generates.
+dh_status dh_hsp_build(detham_ctx* c, const double* psi, double eps2, const u64* pkeys, int64_t m) {
+  dh_status st = m > 0 ? dh_validate_subspace(c, pkeys, m) : DH_OK;  // strictly ascending, electron counts, high bits clear
+  if (st != DH_OK) return st;
+  int64_t cap = 1024;
+  while (cap < 2 * m) cap <<= 1;
+  if (cap != c->phash_cap) {
+    if (c->phash_key) cudaFree(c->phash_key);
+    if (c->phash_idx) cudaFree(c->phash_idx);
+    c->phash_key = nullptr; c->phash_idx = nullptr; c->phash_cap = 0;
+    DH_CUDA(c, cudaMalloc(&c->phash_key, cap * 2 * sizeof(u64)));
+    DH_CUDA(c, cudaMalloc(&c->phash_idx, cap * sizeof(int)));
+    c->phash_cap = cap;
+  }
+  DH_CUDA(c, cudaMemsetAsync(c->phash_key, 0, cap * 2 * sizeof(u64), c->stream));
+  if (m > 0) {
+    shash_insert_kernel<<<(unsigned)((m + 255) / 256), 256, 0, c->stream>>>(pkeys, m, c->phash_key, c->phash_idx, (u64)cap, nullptr, 0ull);
+    DH_CUDA(c, cudaGetLastError());
+  }
+  c->sp_cols = m;
+  CsrTarget T{&c->sp_row_ptr, &c->sp_col, &c->sp_val, &c->sp_nnz, &c->sp_csr_cap, &c->sp_row_cap,
+              c->phash_key, c->phash_idx, c->phash_cap, nullptr, 0};
+  return build_csr(c, T, psi, eps2);
 }

@@ -405,6 +405,47 @@ def test_expand_perturbative_set(pkg, orc, name, n_dets, eps2, parts):
     ctx.close()
 
 
+@pytest.mark.parametrize("name,n_dets,eps2,zero", [("tiny", None, 0.0, False), ("tiny", 600, 1e-4, True), ("h2o", 1500, 1e-6, True),
+                                                   ("tiny", 1, 0.0, False), ("n2", 300, 1e-6, False)])
+def test_hsp_build(pkg, orc, name, n_dets, eps2, zero):
+    """H_SP in CSR against the sorted P (columns and values bit for bit), on a subset of P, with an empty P,
+    and with H_SS left intact on the same context; unsorted P is an error."""
+    import torch
+    p = make_problem(name, n_dets=n_dets)
+    if n_dets == 1:
+        p["psi"] = np.array([1.0])
+    if zero:
+        p["psi"] = p["psi"].copy(); p["psi"][::7] = 0.0         # reading Q6: those rows stay empty
+    ctx = _ctx(pkg, p)
+    psi = _psi(p)
+    nnz_ss = ctx.ham_build(1e-5)
+    ss = [t.cpu().numpy() for t in ctx.csr()]
+    keys = ctx.expand(psi, eps2)[0]
+    okeys = orc.expand(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"], p["psi"], eps2)[0]
+    assert np.array_equal(keys.cpu().numpy().view(np.uint64), okeys)
+    for sel in (None, slice(1, None, 3), slice(0, 0)):
+        pk = keys if sel is None else keys[sel].contiguous()
+        ok = okeys if sel is None else np.ascontiguousarray(okeys[sel])
+        nnz = ctx.hsp_build(psi, eps2, pk)
+        rp, col, val = (t.cpu().numpy() for t in ctx.hsp_csr())
+        orp, ocol, oval = orc.hsp_build(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"], p["psi"], eps2, ok)
+        assert nnz == len(ocol) == ctx.counters()["hsp_nnz"]
+        assert np.array_equal(rp, orp) and np.array_equal(col, ocol)
+        assert np.array_equal(val, oval)                        # same integrals in the same operand order (reading Q7)
+        if sel is None:                                         # every generated external is a column of the full P
+            o = orc.pt2(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"], p["psi"], -1e3, eps2)
+            assert nnz == o["n_contrib"]
+    if len(okeys) > 1:
+        bad = keys.flip(0).contiguous()
+        with pytest.raises(pkg.DethamError) as ei:
+            ctx.hsp_build(psi, eps2, bad)
+        assert ei.value.status == "DH_EUNSORTED"
+    assert ctx.ham_build(1e-5) == nnz_ss                        # the two CSRs share the arena, not the result
+    for a, b in zip(ss, ctx.csr()):
+        assert np.array_equal(a, b.cpu().numpy())
+    ctx.close()
+
+
 def test_against_stored_oracle_values(pkg):
     """The CUDA path against tests/golden/tiny_oracle.json (written by the oracle alone, tests/golden/make_golden.py)."""
     import json
