@@ -66,6 +66,80 @@ part_kernel(Rec* pool, u64* gcur, int B, u64 cap_lines, int iters, u64 seed, u64
   }
   if (drop) atomicAdd(dropped, drop);
 }
+// A2: the same staging, but every CTA owns a private segment of each bin, so a line's position comes from a shared-memory
+// counter and no global atomic sits between two uses of a staging line; NL lines per bin (ring).
+template <int K, int NL>
+__global__ void __launch_bounds__(1024, 1)
+part_private_kernel(Rec* pool, int B, u64 cap_lines /* per (bin, CTA) */, int iters, u64 seed, u64* dropped, unsigned* used /* [B][grid] */) {
+  extern __shared__ __align__(32) unsigned char sm[];
+  Rec* stage = reinterpret_cast<Rec*>(sm);                       // [B][NL][K]
+  unsigned* tick = reinterpret_cast<unsigned*>(stage + (size_t)B * NL * K);
+  unsigned* nline = tick + B;                                    // [B] lines flushed by this CTA
+  unsigned* done = nline + B;                                    // [B][NL]
+  volatile unsigned* lgen = done + NL * B;                       // [B][NL]
+  for (int t = threadIdx.x; t < (2 + 2 * NL) * B; t += blockDim.x) tick[t] = 0;
+  __syncthreads();
+  const u64 tid = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+  u64 drop = 0;
+  for (int it = 0; it < iters; ++it) {
+    const u64 r = mix(seed + tid * 1315423911ull + (u64)it * 0x100000001B3ull);
+    const int b = (int)(((r >> 32) * (u64)B) >> 32);
+    const unsigned t = atomicAdd(&tick[b], 1u);
+    const unsigned g = t / K, pos = t % K, line = g % NL, use = g / NL;
+    Rec* ln = stage + ((size_t)b * NL + line) * K;
+    bool pending = true;
+    while (pending) {
+      if (lgen[NL * b + line] == use) {
+        ln[pos] = Rec{r | 1ull, r * 3ull, 1.0, 2.0};
+        __threadfence_block();
+        const unsigned d = atomicAdd(&done[NL * b + line], 1u);
+        if (d == K - 1) {
+          __threadfence_block();
+          done[NL * b + line] = 0;
+          const unsigned gl = atomicAdd(&nline[b], 1u);
+          if (gl < cap_lines) {
+            Rec* dst = pool + (((u64)b * gridDim.x + blockIdx.x) * cap_lines + gl) * K;
+#pragma unroll
+            for (int k = 0; k < K; ++k) { const Rec x = ln[k]; st256(dst + k, x.ka, x.kb, __double_as_longlong(x.v), __double_as_longlong(x.h)); }
+          } else drop += K;
+          __threadfence_block();
+          lgen[NL * b + line] = use + 1;
+        }
+        pending = false;
+      }
+    }
+  }
+  __syncthreads();
+  for (int b = threadIdx.x; b < B; b += blockDim.x) used[(size_t)b * gridDim.x + blockIdx.x] = nline[b];
+  if (drop) atomicAdd(dropped, drop);
+}
+// A3: no staging: every CTA owns a private segment of each bin and appends with a shared-memory counter (no global atomic);
+// consecutive records of a (bin, CTA) fill consecutive sectors, so L2 gets to combine them into full lines before write-back.
+template <int U>
+__global__ void __launch_bounds__(1024, 1)
+append_private_kernel(Rec* pool, int B, unsigned cap_recs /* per (bin, CTA) */, int iters, u64 seed, u64* dropped, unsigned* used) {
+  extern __shared__ __align__(32) unsigned char sm[];
+  unsigned* cnt = reinterpret_cast<unsigned*>(sm);
+  for (int t = threadIdx.x; t < B; t += blockDim.x) cnt[t] = 0;
+  __syncthreads();
+  const u64 tid = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+  u64 drop = 0;
+  for (int it = 0; it < iters; it += U) {
+    u64 r[U]; int b[U]; unsigned p[U];
+#pragma unroll
+    for (int u = 0; u < U; ++u) { r[u] = mix(seed + tid * 1315423911ull + (u64)(it + u) * 0x100000001B3ull); b[u] = (int)(((r[u] >> 32) * (u64)B) >> 32); }
+#pragma unroll
+    for (int u = 0; u < U; ++u) p[u] = atomicAdd(&cnt[b[u]], 1u);
+#pragma unroll
+    for (int u = 0; u < U; ++u) {
+      if (p[u] < cap_recs) st256(pool + ((u64)b[u] * gridDim.x + blockIdx.x) * cap_recs + p[u], r[u] | 1ull, r[u] * 3ull, __double_as_longlong(1.0), __double_as_longlong(2.0));
+      else ++drop;
+    }
+  }
+  __syncthreads();
+  for (int b = threadIdx.x; b < B; b += blockDim.x) used[(size_t)b * gridDim.x + blockIdx.x] = cnt[b];
+  if (drop) atomicAdd(dropped, drop);
+}
 // baseline: one global atomic + one scattered 32-byte store per record
 __global__ void __launch_bounds__(1024, 1)
 append_kernel(Rec* pool, u64* gcur, int B, u64 cap_recs, int iters, u64 seed, u64* dropped) {
@@ -189,6 +263,32 @@ template <int K> void run_part(int B, Rec* pool, u64 pool_recs, u64* gcur, u64* 
     if (rep) printf("A staged  B=%5d K=%d (line %3d B, smem %3zu KB): %7.2f G rec/s  %6.2f TB/s  dropped %llu\n", B, K, K * 32, smem >> 10, total / (ms * 1e6), total * 32 / (ms * 1e9), d);
   }
 }
+template <int K, int NL> void run_part_private(int B, Rec* pool, u64 pool_recs, unsigned* used, u64* dropped, int sms) {
+  const int iters = 2048;
+  const u64 total = (u64)sms * 1024 * iters;
+  const u64 cap_lines = pool_recs / B / sms / K;
+  const size_t smem = (size_t)B * NL * K * sizeof(Rec) + (2 + 2 * NL) * (size_t)B * sizeof(unsigned);
+  CK(cudaFuncSetAttribute(part_private_kernel<K, NL>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  for (int rep = 0; rep < 2; ++rep) {
+    CK(cudaMemset(dropped, 0, 8));
+    float ms = timed([&] { part_private_kernel<K, NL><<<sms, 1024, smem>>>(pool, B, cap_lines, iters, 77 + rep, dropped, used); });
+    u64 d = 0; CK(cudaMemcpy(&d, dropped, 8, cudaMemcpyDeviceToHost));
+    if (rep) printf("A2 private B=%5d K=%d NL=%d (line %3d B, smem %3zu KB): %7.2f G rec/s  %6.2f TB/s  dropped %llu\n", B, K, NL, K * 32, smem >> 10, total / (ms * 1e6), total * 32 / (ms * 1e9), d);
+  }
+}
+template <int U> void run_append_private(int B, Rec* pool, u64 pool_recs, unsigned* used, u64* dropped, int sms) {
+  const int iters = 2048;
+  const u64 total = (u64)sms * 1024 * iters;
+  const unsigned cap = (unsigned)(pool_recs / B / sms);
+  const size_t smem = (size_t)B * sizeof(unsigned);
+  CK(cudaFuncSetAttribute(append_private_kernel<U>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  for (int rep = 0; rep < 2; ++rep) {
+    CK(cudaMemset(dropped, 0, 8));
+    float ms = timed([&] { append_private_kernel<U><<<sms, 1024, smem>>>(pool, B, cap, iters, 77 + rep, dropped, used); });
+    u64 d = 0; CK(cudaMemcpy(&d, dropped, 8, cudaMemcpyDeviceToHost));
+    if (rep) printf("A3 private append B=%5d U=%d (open lines %.1f MB): %7.2f G rec/s  %6.2f TB/s  dropped %llu\n", B, U, (double)B * sms * 128 / 1048576.0, total / (ms * 1e6), total * 32 / (ms * 1e9), d);
+  }
+}
 void run_append(int B, Rec* pool, u64 pool_recs, u64* gcur, u64* dropped, int sms) {
   const int iters = 2048;
   const u64 total = (u64)sms * 1024 * iters;
@@ -232,6 +332,13 @@ int main() {
   CK(cudaMalloc(&gcur, 65536 * 8)); CK(cudaMalloc(&dropped, 8)); CK(cudaMalloc(&cursor, 8)); CK(cudaMalloc(&overflow, 4)); CK(cudaMalloc(&out, 8));
   for (int B : {256, 512, 768}) run_part<4>(B, pool, pool_recs, gcur, dropped, sms);
   for (int B : {512, 1024, 1536}) run_part<2>(B, pool, pool_recs, gcur, dropped, sms);
+  unsigned* used; CK(cudaMalloc(&used, 16384 * 256 * 4));
+  for (int B : {256, 512, 768}) run_part_private<4, 2>(B, pool, pool_recs, used, dropped, sms);
+  for (int B : {128, 256, 384}) run_part_private<4, 4>(B, pool, pool_recs, used, dropped, sms);
+  for (int B : {512, 1024, 1536}) run_part_private<2, 2>(B, pool, pool_recs, used, dropped, sms);
+  for (int B : {256, 512, 768}) run_part_private<2, 4>(B, pool, pool_recs, used, dropped, sms);
+  for (int B : {256, 1024, 2048, 4096, 16384}) run_append_private<1>(B, pool, pool_recs, used, dropped, sms);
+  for (int B : {256, 1024, 2048, 4096, 16384}) run_append_private<4>(B, pool, pool_recs, used, dropped, sms);
   for (int B : {512, 2048, 16384}) run_append(B, pool, pool_recs, gcur, dropped, sms);
   for (int dup : {1, 2, 4}) { run_dedupe<1024>(pool, 1ull << 27, dup, out, sms); run_dedupe<2048>(pool, 1ull << 27, dup, out, sms); run_dedupe<4096>(pool, 1ull << 27, dup, out, sms); }
   const u64 table_slots = 1ull << 30;                            // 32 GB table
