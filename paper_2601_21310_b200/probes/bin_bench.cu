@@ -322,7 +322,9 @@ void run_merge(Rec* recs, u64 n, Rec* table, u64 table_slots, u64 region_bytes, 
          (double)per_region / dup / region_slots, dup, (double)per_region * nreg / (ms * 1e6), ov ? "  OVERFLOW" : "");
 }
 
-int main() {
+int main(int argc, char** argv) {
+  const char* sel = argc > 1 ? argv[1] : "abcdef";  // a staged, b private staged, c private append, d append, e dedupe, f merge
+  auto on = [&](char c) { for (const char* q = sel; *q; ++q) if (*q == c) return true; return false; };
   cudaDeviceProp prop; CK(cudaGetDeviceProperties(&prop, 0));
   const int sms = prop.multiProcessorCount;
   printf("%s, %d SMs, L2 %d MB\n", prop.name, sms, prop.l2CacheSize >> 20);
@@ -330,17 +332,24 @@ int main() {
   Rec* pool; CK(cudaMalloc(&pool, pool_recs * 32));
   u64 *gcur, *dropped, *cursor; int* overflow; double* out;
   CK(cudaMalloc(&gcur, 65536 * 8)); CK(cudaMalloc(&dropped, 8)); CK(cudaMalloc(&cursor, 8)); CK(cudaMalloc(&overflow, 4)); CK(cudaMalloc(&out, 8));
-  for (int B : {256, 512, 768}) run_part<4>(B, pool, pool_recs, gcur, dropped, sms);
-  for (int B : {512, 1024, 1536}) run_part<2>(B, pool, pool_recs, gcur, dropped, sms);
+  if (on('a')) {
+    for (int B : {256, 512, 768}) run_part<4>(B, pool, pool_recs, gcur, dropped, sms);
+    for (int B : {512, 1024, 1536}) run_part<2>(B, pool, pool_recs, gcur, dropped, sms);
+  }
   unsigned* used; CK(cudaMalloc(&used, 16384 * 256 * 4));
+  if (on('b')) {
   for (int B : {256, 512, 768}) run_part_private<4, 2>(B, pool, pool_recs, used, dropped, sms);
   for (int B : {128, 256, 384}) run_part_private<4, 4>(B, pool, pool_recs, used, dropped, sms);
-  for (int B : {512, 1024, 1536}) run_part_private<2, 2>(B, pool, pool_recs, used, dropped, sms);
-  for (int B : {256, 512, 768}) run_part_private<2, 4>(B, pool, pool_recs, used, dropped, sms);
+  for (int B : {512, 1024, 1408}) run_part_private<2, 2>(B, pool, pool_recs, used, dropped, sms);
+  for (int B : {256, 512, 704}) run_part_private<2, 4>(B, pool, pool_recs, used, dropped, sms);
+  }
+  if (on('c')) {
   for (int B : {256, 1024, 2048, 4096, 16384}) run_append_private<1>(B, pool, pool_recs, used, dropped, sms);
   for (int B : {256, 1024, 2048, 4096, 16384}) run_append_private<4>(B, pool, pool_recs, used, dropped, sms);
-  for (int B : {512, 2048, 16384}) run_append(B, pool, pool_recs, gcur, dropped, sms);
-  for (int dup : {1, 2, 4}) { run_dedupe<1024>(pool, 1ull << 27, dup, out, sms); run_dedupe<2048>(pool, 1ull << 27, dup, out, sms); run_dedupe<4096>(pool, 1ull << 27, dup, out, sms); }
+  }
+  if (on('d')) for (int B : {512, 2048, 16384}) run_append(B, pool, pool_recs, gcur, dropped, sms);
+  if (on('e')) for (int dup : {1, 2, 4}) { run_dedupe<1024>(pool, 1ull << 27, dup, out, sms); run_dedupe<2048>(pool, 1ull << 27, dup, out, sms); run_dedupe<4096>(pool, 1ull << 27, dup, out, sms); }
+  if (!on('f')) return 0;
   const u64 table_slots = 1ull << 30;                            // 32 GB table
   Rec* table; CK(cudaMalloc(&table, table_slots * 32));
   for (int dup : {2, 4})
