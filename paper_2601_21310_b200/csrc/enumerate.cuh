@@ -118,10 +118,23 @@ __device__ __forceinline__ double dh_single_value(const EnumParams& P, const War
   return dh_parity_between(wsame, i, a) ? -v : v;
 }
 
+// parity (0 even, 1 odd) of the phase of a double excitation of (da, db), reading Q1.  kind 1: same spin s, i<j -> a<b:
+// a+_a a+_b a_j a_i = (a+_b a_j)(a+_a a_i): phase(i->a on w) * phase(j->b on w with i->a applied).  kind 2: i alpha -> a,
+// j beta -> b: the product of the two single phases.
+__device__ __forceinline__ int dh_double_parity(u64 da, u64 db, int kind, int s, int i, int j, int a, int b) {
+  if (kind == 1) {
+    const u64 w = s ? db : da;
+    return dh_parity_between(w, i, a) ^ dh_parity_between((w ^ (1ull << i)) | (1ull << a), j, b);
+  }
+  return dh_parity_between(da, i, a) ^ dh_parity_between(db, j, b);
+}
+
 // Enumerate every excitation D' of (da, db) with |H| >= tau, H != 0 whose key class (low pbits of its partition word)
 // equals `pass`, and hand it to the sink.  Requires dh_fill_occ done.  All 32 lanes call sink.emit convergently:
 //   sink.emit(active, ka, kb, z, H, kind, s, i, j, a, b)
 // If Sink::kLookupFirst, singles are offered to sink.pre(ka, kb, z) before their O(N_e) evaluation.
+// If Sink::kLazySign, doubles arrive with the list's value, WITHOUT the fermionic phase: a sink that drops most candidates
+// (ham_build: 98 % are not in S) applies dh_double_parity itself to the few it keeps.
 template <class Sink>
 __device__ __forceinline__ void dh_enumerate(const EnumParams& P, const CtaTables& T, const WarpScratch& ws, u64 da, u64 db,
                                              double tau, u64 zsrc, unsigned pass, Sink& sink, int lane) {
@@ -190,9 +203,7 @@ __device__ __forceinline__ void dh_enumerate(const EnumParams& P, const CtaTable
               u64 nw = wij | (1ull << a) | (1ull << b);
               if (s == 0) ka = nw; else kb = nw;
               z = zij ^ T.Z[64 * s + a] ^ T.Z[64 * s + b];
-              // a+_a a+_b a_j a_i = (a+_b a_j)(a+_a a_i): phase(i->a on w) * phase(j->b on w with i->a applied)
-              int par = dh_parity_between(w, i, a) ^ dh_parity_between((w ^ (1ull << i)) | (1ull << a), j, b);
-              if (par) v = -v;
+              if (!Sink::kLazySign && dh_double_parity(da, db, 1, s, i, j, a, b)) v = -v;
             }
           }
           sink.emit(act, ka, kb, z, v, 1, s, i, j, a, b);
@@ -230,7 +241,7 @@ __device__ __forceinline__ void dh_enumerate(const EnumParams& P, const CtaTable
             ka = (da ^ (1ull << i)) | (1ull << a);
             kb = (db ^ (1ull << j)) | (1ull << b);
             z = zij ^ T.Z[a] ^ T.Z[64 + b];
-            if (dh_parity_between(da, i, a) ^ dh_parity_between(db, j, b)) v = -v;
+            if (!Sink::kLazySign && dh_double_parity(da, db, 2, 0, i, j, a, b)) v = -v;
           }
         }
         sink.emit(act, ka, kb, z, v, 2, 0, i, j, a, b);

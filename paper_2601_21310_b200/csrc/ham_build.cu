@@ -51,6 +51,8 @@ struct Seg { int row, local, cnt, pad; int64_t off; };
 
 struct BuildSink {
   static constexpr bool kLookupFirst = true;
+  static constexpr bool kLazySign = true;   // the phase of a double is worked out for the hits only
+  u64 da, db;              // the row's determinant (for the lazy phase)
   const u64* keys; const int* idx; u64 cap;
   const unsigned* bits; u64 nbits;
   int* acol; double* aval; int64_t arena_cap;
@@ -71,7 +73,7 @@ struct BuildSink {
       else *overflow = 1;
     }
   }
-  __device__ __forceinline__ void begin_row(int r) { row = r; count = 0; seg_start = wpos; seg_local = 0; }
+  __device__ __forceinline__ void begin_row(int r, u64 a, u64 b) { row = r; da = a; db = b; count = 0; seg_start = wpos; seg_local = 0; }
   __device__ __forceinline__ void end_row() { close_seg(); }
   __device__ __forceinline__ void put(bool has, int tok, double H) {
     const unsigned hit = __ballot_sync(0xffffffffu, has);
@@ -97,11 +99,15 @@ struct BuildSink {
     pre_tok = (!bits || dh_maybe_member(bits, nbits, z)) ? dh_shash_find(keys, idx, cap, ka, kb, z) : -1;
     return pre_tok >= 0;
   }
-  __device__ __forceinline__ void emit(bool act, u64 ka, u64 kb, u64 z, double H, int kind, int, int, int, int, int) {
+  __device__ __forceinline__ void emit(bool act, u64 ka, u64 kb, u64 z, double H, int kind, int s, int i, int j, int a, int b) {
     int tok = -1;
     if (act) {
       if (kind == 0) tok = pre_tok;
-      else { ++generated; if (!bits || dh_maybe_member(bits, nbits, z)) tok = dh_shash_find(keys, idx, cap, ka, kb, z); }
+      else {
+        ++generated;
+        if (!bits || dh_maybe_member(bits, nbits, z)) tok = dh_shash_find(keys, idx, cap, ka, kb, z);
+        if (tok >= 0 && dh_double_parity(da, db, kind, s, i, j, a, b)) H = -H;
+      }
     }
     put(tok >= 0, tok, H);
   }
@@ -120,7 +126,7 @@ build_kernel(EnumParams P, const u64* __restrict__ dets, const double* __restric
   WarpScratch* wsp = reinterpret_cast<WarpScratch*>(smem + ((dh_cta_table_bytes(P.n) + 15) & ~(size_t)15));
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   WarpScratch& ws = wsp[warp];
-  BuildSink sink{hkeys, hidx, hcap, hbits, hnbits, acol, aval, arena_cap, counters, segs, seg_cap, overflow, 0, 0, 0, 0, 0, 0, 0ull, lane, -1};
+  BuildSink sink{0ull, 0ull, hkeys, hidx, hcap, hbits, hnbits, acol, aval, arena_cap, counters, segs, seg_cap, overflow, 0, 0, 0, 0, 0, 0, 0ull, lane, -1};
   for (;;) {
     u64 row = 0;
     if (lane == 0) row = atomicAdd(counters, 1ull);
@@ -135,7 +141,7 @@ build_kernel(EnumParams P, const u64* __restrict__ dets, const double* __restric
     }
     dh_fill_occ(P, ws, da, db, lane);
     const double e0 = dh_fill_U(P, T, ws, lane);
-    sink.begin_row((int)row);
+    sink.begin_row((int)row, da, db);
     if (!kSP) sink.put(lane == 0, (int)row, e0);  // the diagonal is always kept (reading Q4)
     u64 zsrc = 0;
     if (lane == 0) zsrc = dh_zobrist(da, db, T.Z);

@@ -22,6 +22,7 @@ __device__ __forceinline__ double member_flag() { return __longlong_as_double(0x
 // ---------------------------------------------------------------- class histogram (pass planning)
 struct CountSink {
   static constexpr bool kLookupFirst = true;  // singles are counted (upper bound) without being evaluated
+  static constexpr bool kLazySign = true;     // only counts
   unsigned* hist;
   __device__ __forceinline__ bool pre(u64, u64, u64 z) { atomicAdd(hist + ((unsigned)z & (kFine - 1)), 1u); return false; }
   __device__ __forceinline__ void emit(bool act, u64, u64, u64 z, double, int, int, int, int, int, int) {
@@ -505,6 +506,7 @@ __global__ void norm2_kernel(const double* __restrict__ psi, int64_t nd, double*
 // ---------------------------------------------------------------- test hooks
 struct ConnSink {
   static constexpr bool kLookupFirst = false;
+  static constexpr bool kLazySign = false;
   u64* keys; double* h; int count; int lane;
   __device__ __forceinline__ bool pre(u64, u64, u64) { return true; }
   __device__ __forceinline__ void emit(bool act, u64 ka, u64 kb, u64, double H, int, int, int, int, int, int) {
