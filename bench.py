@@ -146,6 +146,8 @@ def main():
     ap.add_argument("--table-slots", type=int, default=0)
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
+    ap.add_argument("--widened", action="store_true",
+                    help="also time the SURVEY.md 8(f) rows (residual, E_diag, expand, H_SP) on this workload; adds a 'widened' object")
     args = ap.parse_args()
     args.warmup = max(args.warmup, 0)
 
@@ -265,6 +267,42 @@ def main():
            # two row sorts), energy 2, pt2 3 (plan histogram, norm + reduce) + 4 per key partition (member insert, accumulate,
            # scan, reduce) + 4 when the planner probed one slice
            "gpu_launches": 2 + 5 + 2 + 3 + 4 * parts + (4 if c["pt2_probe_parts"] else 0)}
+
+    # ---- the widened rows, timed on the same workload after the hot path: median of 3, CUDA events
+    if args.widened and rank == 0:
+        def timed(fn, reps=3):
+            ms, res = [], None
+            for _ in range(reps):
+                flush.fill_(1)
+                torch.cuda.synchronize()
+                t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
+                t0.record()
+                res = fn()
+                t1.record()
+                torch.cuda.synchronize()
+                ms.append(t0.elapsed_time(t1))
+            return statistics.median(ms), res
+        w = {}
+        ms, (_, t_int) = timed(lambda: ctx.residual(psi_dev, e_s, want_r=True))
+        w["f1_residual"] = {"ms": ms, "internal_term": t_int, "GBps": (b_energy + 8.0 * nd) / (ms * 1e-3) / 1e9,
+                            "frac_of_hbm_peak": (b_energy + 8.0 * nd) / (ms * 1e-3) / 1e9 / peak}
+        ms, (e_diag, iters) = timed(lambda: ctx.ediag(psi_dev, tol=1e-10, max_iter=300), reps=3)
+        w["f4_ediag"] = {"ms": ms, "E_diag": e_diag, "lanczos_steps": iters, "ms_per_step": ms / max(1, iters),
+                         "GBps_per_step": (b_energy + 48.0 * nd) / (ms / max(1, iters) * 1e-3) / 1e9}
+        if c["pt2_external"] <= 250_000_000:  # the set has to fit: 40 bytes per external plus the sort's buffers
+            ms, (keys, score, v, haa) = timed(lambda: ctx.expand(psi_dev, p["eps2"]), reps=2)
+            w["f2_expand"] = {"ms": ms, "n_P": int(keys.shape[0]), "externals_per_sec": keys.shape[0] / (ms * 1e-3),
+                              "contributions_per_sec": c["pt2_contrib"] / (ms * 1e-3)}
+            del score, v, haa
+            ms, nnz_sp = timed(lambda: ctx.hsp_build(psi_dev, p["eps2"], keys), reps=2)
+            cw = ctx.counters()
+            w["f3_hsp_build"] = {"ms": ms, "nnz": nnz_sp, "looked_up": cw["hsp_generated"],
+                                 "lookups_per_sec": cw["hsp_generated"] / (ms * 1e-3), "stored_nnz_per_sec": nnz_sp / (ms * 1e-3),
+                                 "csr_write_GBps": 12.0 * nnz_sp / (ms * 1e-3) / 1e9}
+            del keys
+        else:
+            w["f2_expand"] = w["f3_hsp_build"] = {"skipped": f"|P| = {c['pt2_external']} does not fit the device as a materialised set"}
+        out["widened"] = w
 
     # ---- end to end through the C ABI with HOST buffers (pinned), copies inside the timed region
     if not args.no_e2e:

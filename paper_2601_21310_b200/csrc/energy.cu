@@ -40,11 +40,12 @@ spmv_energy_kernel(const int64_t* __restrict__ row_ptr, const int* __restrict__ 
 }
 
 // residual r = H_SS psi - e psi (the vector Eq. 12 contracts with grad psi) fused with the internal term of
-// Eq. 13 (first sum): sum_i r_i^2 / (e - H_ii); H_ii is the row's own diagonal entry.  8 threads per row.
+// Eq. 13 (first sum): sum_i r_i^2 / (e - H_ii); H_ii is the row's own diagonal entry.  TPR threads per row,
+// chosen like the energy kernel's.
+template <int TPR>
 __global__ void __launch_bounds__(256)
 residual_kernel(const int64_t* __restrict__ row_ptr, const int* __restrict__ col, const double* __restrict__ val,
                 const double* __restrict__ psi, int64_t nd, double e, double* __restrict__ r_out, double* __restrict__ part) {
-  constexpr int TPR = 8;
   const int sub = threadIdx.x % TPR;
   const int64_t rows_per_cta = 256 / TPR;
   double num = 0.0, den = 0.0;
@@ -136,12 +137,16 @@ dh_status dh_energy(detham_ctx* c, const double* psi, double* e_out, double* n2_
 
 dh_status dh_residual(detham_ctx* c, const double* psi, double e_s, double* r_out, double* internal_out) {
   const int64_t nd = c->nd;
-  int64_t want = (nd + 31) / 32;
+  const double avg = (double)c->nnz / (double)nd;
+  const int tpr = avg <= 6 ? 4 : (avg <= 24 ? 8 : 32);
+  int64_t want = (nd + (256 / tpr) - 1) / (256 / tpr);
   int grid = (int)(want < (int64_t)c->sm_count * 8 ? want : (int64_t)c->sm_count * 8);
   dh_status st = dh_ensure_red(c, 2 * (int64_t)grid + 2);
   if (st != DH_OK) return st;
   double* part = c->red + 2;
-  residual_kernel<<<grid, 256, 0, c->stream>>>(c->row_ptr, c->col, c->val, psi, nd, e_s, r_out, part);
+  if (tpr == 4) residual_kernel<4><<<grid, 256, 0, c->stream>>>(c->row_ptr, c->col, c->val, psi, nd, e_s, r_out, part);
+  else if (tpr == 8) residual_kernel<8><<<grid, 256, 0, c->stream>>>(c->row_ptr, c->col, c->val, psi, nd, e_s, r_out, part);
+  else residual_kernel<32><<<grid, 256, 0, c->stream>>>(c->row_ptr, c->col, c->val, psi, nd, e_s, r_out, part);
   DH_CUDA(c, cudaGetLastError());
   final_reduce2_kernel<<<1, 256, 0, c->stream>>>(part, grid, c->red);
   DH_CUDA(c, cudaGetLastError());

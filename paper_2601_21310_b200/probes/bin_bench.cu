@@ -140,6 +140,86 @@ append_private_kernel(Rec* pool, int B, unsigned cap_recs /* per (bin, CTA) */, 
   for (int b = threadIdx.x; b < B; b += blockDim.x) used[(size_t)b * gridDim.x + blockIdx.x] = cnt[b];
   if (drop) atomicAdd(dropped, drop);
 }
+// A4: CTA-synchronous counting sort.  Warps append their records to a shared buffer (one shared atomic per warp, coalesced
+// stores); when the buffer holds N records the CTA histograms them by bin, scans, scatters them into bin order in a second
+// buffer and writes that out with consecutive threads on consecutive records, so every bin's run leaves as one or two
+// line-sized requests into the CTA's private segment of the bin.
+template <int N>
+__global__ void __launch_bounds__(1024, 1)
+part_sort_kernel(Rec* pool, int B, unsigned cap_recs /* per (bin, CTA) */, int rounds, u64 seed, u64* dropped, unsigned* used) {
+  extern __shared__ __align__(32) unsigned char sm[];
+  Rec* buf = reinterpret_cast<Rec*>(sm);                          // [N] arrival order
+  Rec* srt = buf + N;                                            // [N] bin order
+  unsigned* hist = reinterpret_cast<unsigned*>(srt + N);         // [B]
+  unsigned* base = hist + B;                                     // [B] exclusive scan of hist
+  unsigned* segu = base + B;                                     // [B] records this CTA has flushed per bin
+  unsigned short* sbin = reinterpret_cast<unsigned short*>(segu + B);  // [N] bin of sorted position
+  __shared__ unsigned fill, wtot[32];
+  for (int t = threadIdx.x; t < B; t += blockDim.x) { hist[t] = 0; segu[t] = 0; }
+  if (threadIdx.x == 0) fill = 0;
+  __syncthreads();
+  const u64 tid = (u64)blockIdx.x * blockDim.x + threadIdx.x;
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  constexpr int PER = N / 1024;                                  // records per thread and round
+  u64 drop = 0;
+  for (int rd = 0; rd < rounds; ++rd) {
+    // produce: every warp appends PER batches of 32 records
+#pragma unroll
+    for (int q = 0; q < PER; ++q) {
+      const u64 r = mix(seed + tid * 1315423911ull + (u64)(rd * PER + q) * 0x100000001B3ull);
+      unsigned pos = 0;
+      if (lane == 0) pos = atomicAdd(&fill, 32u);
+      pos = __shfl_sync(0xffffffffu, pos, 0) + lane;
+      buf[pos] = Rec{r | 1ull, r * 3ull, 1.0, 2.0};
+    }
+    __syncthreads();
+    // histogram + rank
+    unsigned rk[PER]; int bn[PER];
+#pragma unroll
+    for (int q = 0; q < PER; ++q) {
+      const u64 ka = buf[threadIdx.x + q * 1024].ka;
+      bn[q] = (int)(((ka >> 32) * (u64)B) >> 32);
+      rk[q] = atomicAdd(&hist[bn[q]], 1u);
+    }
+    __syncthreads();
+    // exclusive scan of hist over B <= 1024 bins: one bin per thread
+    {
+      unsigned v = threadIdx.x < B ? hist[threadIdx.x] : 0u, x = v;
+#pragma unroll
+      for (int o = 1; o < 32; o <<= 1) { unsigned y = __shfl_up_sync(0xffffffffu, x, o); if (lane >= o) x += y; }
+      if (lane == 31) wtot[warp] = x;
+      __syncthreads();
+      if (warp == 0) { unsigned w = wtot[lane], sx = w; for (int o = 1; o < 32; o <<= 1) { unsigned y = __shfl_up_sync(0xffffffffu, sx, o); if (lane >= o) sx += y; } wtot[lane] = sx - w; }
+      __syncthreads();
+      if (threadIdx.x < B) base[threadIdx.x] = wtot[warp] + x - v;
+    }
+    __syncthreads();
+    // scatter into bin order
+#pragma unroll
+    for (int q = 0; q < PER; ++q) {
+      const unsigned d = base[bn[q]] + rk[q];
+      srt[d] = buf[threadIdx.x + q * 1024];
+      sbin[d] = (unsigned short)bn[q];
+    }
+    __syncthreads();
+    // write out: consecutive threads, consecutive records of a bin's run
+#pragma unroll
+    for (int q = 0; q < PER; ++q) {
+      const int t = threadIdx.x + q * 1024;
+      const int b = sbin[t];
+      const unsigned p = segu[b] + ((unsigned)t - base[b]);
+      const Rec x = srt[t];
+      if (p < cap_recs) st256(pool + ((u64)b * gridDim.x + blockIdx.x) * cap_recs + p, x.ka, x.kb, __double_as_longlong(x.v), __double_as_longlong(x.h));
+      else ++drop;
+    }
+    __syncthreads();
+    if (threadIdx.x < B) { segu[threadIdx.x] += hist[threadIdx.x]; hist[threadIdx.x] = 0; }
+    if (threadIdx.x == 0) fill = 0;
+    __syncthreads();
+  }
+  for (int b = threadIdx.x; b < B; b += blockDim.x) used[(size_t)b * gridDim.x + blockIdx.x] = segu[b];
+  if (drop) atomicAdd(dropped, drop);
+}
 // baseline: one global atomic + one scattered 32-byte store per record
 __global__ void __launch_bounds__(1024, 1)
 append_kernel(Rec* pool, u64* gcur, int B, u64 cap_recs, int iters, u64 seed, u64* dropped) {
@@ -156,8 +236,8 @@ append_kernel(Rec* pool, u64* gcur, int B, u64 cap_recs, int iters, u64 seed, u6
 
 // ------------------------------------------------------------------ B: one bin per CTA pass, deduplicated in shared memory
 // bins: [nbins][M] records; keys inside a bin repeat `dup` times on average.  Table of record indices (short), 2M slots.
-template <int M>
-__global__ void __launch_bounds__(1024, 1)
+template <int M, int T>
+__global__ void __launch_bounds__(T)
 dedupe_kernel(const Rec* __restrict__ bins, int nbins, double e_s, double* out) {
   extern __shared__ __align__(32) unsigned char sm[];
   Rec* rec = reinterpret_cast<Rec*>(sm);                         // [M]
@@ -189,7 +269,7 @@ dedupe_kernel(const Rec* __restrict__ bins, int nbins, double e_s, double* out) 
   for (int o = 16; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o);
   if ((threadIdx.x & 31) == 0) wsum[threadIdx.x >> 5] = acc;
   __syncthreads();
-  if (threadIdx.x == 0) { double s = 0; for (int w = 0; w < 32; ++w) s += wsum[w]; atomicAdd(out, s); }
+  if (threadIdx.x == 0) { double s = 0; for (int w = 0; w < T / 32; ++w) s += wsum[w]; atomicAdd(out, s); }
 }
 __global__ void fill_bins_kernel(Rec* bins, u64 n, int M, int dup, u64 seed) {
   for (u64 t = (u64)blockIdx.x * blockDim.x + threadIdx.x; t < n; t += (u64)gridDim.x * blockDim.x) {
@@ -289,6 +369,19 @@ template <int U> void run_append_private(int B, Rec* pool, u64 pool_recs, unsign
     if (rep) printf("A3 private append B=%5d U=%d (open lines %.1f MB): %7.2f G rec/s  %6.2f TB/s  dropped %llu\n", B, U, (double)B * sms * 128 / 1048576.0, total / (ms * 1e6), total * 32 / (ms * 1e9), d);
   }
 }
+template <int N> void run_part_sort(int B, Rec* pool, u64 pool_recs, unsigned* used, u64* dropped, int sms) {
+  const int rounds = 2048 * 1024 / N;
+  const u64 total = (u64)sms * N * rounds;
+  const unsigned cap = (unsigned)(pool_recs / B / sms);
+  const size_t smem = 2 * (size_t)N * sizeof(Rec) + 3 * (size_t)B * sizeof(unsigned) + (size_t)N * sizeof(unsigned short);
+  CK(cudaFuncSetAttribute(part_sort_kernel<N>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  for (int rep = 0; rep < 2; ++rep) {
+    CK(cudaMemset(dropped, 0, 8));
+    float ms = timed([&] { part_sort_kernel<N><<<sms, 1024, smem>>>(pool, B, cap, rounds, 77 + rep, dropped, used); });
+    u64 d = 0; CK(cudaMemcpy(&d, dropped, 8, cudaMemcpyDeviceToHost));
+    if (rep) printf("A4 counting sort B=%5d N=%d (avg run %5.1f rec, smem %3zu KB): %7.2f G rec/s  %6.2f TB/s  dropped %llu\n", B, N, (double)N / B, smem >> 10, total / (ms * 1e6), total * 32 / (ms * 1e9), d);
+  }
+}
 void run_append(int B, Rec* pool, u64 pool_recs, u64* gcur, u64* dropped, int sms) {
   const int iters = 2048;
   const u64 total = (u64)sms * 1024 * iters;
@@ -298,16 +391,17 @@ void run_append(int B, Rec* pool, u64 pool_recs, u64* gcur, u64* dropped, int sm
     if (rep) printf("A append  B=%5d                          : %7.2f G rec/s  %6.2f TB/s\n", B, total / (ms * 1e6), total * 32 / (ms * 1e9));
   }
 }
-template <int M> void run_dedupe(Rec* buf, u64 buf_recs, int dup, double* out, int sms) {
+template <int M, int T> void run_dedupe(Rec* buf, u64 buf_recs, int dup, double* out, int sms) {
   const int nbins = (int)(buf_recs / M);
   fill_bins_kernel<<<sms * 8, 256>>>(buf, (u64)nbins * M, M, dup, 5); CK(cudaDeviceSynchronize());
   const size_t smem = (size_t)M * sizeof(Rec) + 2 * (size_t)M * sizeof(int);
-  CK(cudaFuncSetAttribute(dedupe_kernel<M>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  CK(cudaFuncSetAttribute(dedupe_kernel<M, T>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  int per_sm = 0; CK(cudaOccupancyMaxActiveBlocksPerMultiprocessor(&per_sm, dedupe_kernel<M, T>, T, smem));
   for (int rep = 0; rep < 2; ++rep) {
     CK(cudaMemset(out, 0, 8));
-    float ms = timed([&] { dedupe_kernel<M><<<sms, 1024, smem>>>(buf, nbins, 1.0, out); });
+    float ms = timed([&] { dedupe_kernel<M, T><<<sms * per_sm, T, smem>>>(buf, nbins, 1.0, out); });
     double s = 0; CK(cudaMemcpy(&s, out, 8, cudaMemcpyDeviceToHost));
-    if (rep) printf("B dedupe  M=%5d dup=%d (smem %3zu KB, %d bins): %7.2f G rec/s  %6.2f TB/s  sum %.6e\n", M, dup, smem >> 10, nbins, (double)nbins * M / (ms * 1e6), (double)nbins * M * 32 / (ms * 1e9), s);
+    if (rep) printf("B dedupe  M=%5d T=%4d x %d CTAs/SM dup=%d (smem %3zu KB, %d bins): %7.2f G rec/s  %6.2f TB/s  sum %.6e\n", M, T, per_sm, dup, smem >> 10, nbins, (double)nbins * M / (ms * 1e6), (double)nbins * M * 32 / (ms * 1e9), s);
   }
 }
 void run_merge(Rec* recs, u64 n, Rec* table, u64 table_slots, u64 region_bytes, int dup, u64* cursor, int* overflow, int sms) {
@@ -323,7 +417,7 @@ void run_merge(Rec* recs, u64 n, Rec* table, u64 table_slots, u64 region_bytes, 
 }
 
 int main(int argc, char** argv) {
-  const char* sel = argc > 1 ? argv[1] : "abcdef";  // a staged, b private staged, c private append, d append, e dedupe, f merge
+  const char* sel = argc > 1 ? argv[1] : "abcsdef";  // a staged, b private staged, c private append, s counting sort, d append, e dedupe, f merge
   auto on = [&](char c) { for (const char* q = sel; *q; ++q) if (*q == c) return true; return false; };
   cudaDeviceProp prop; CK(cudaGetDeviceProperties(&prop, 0));
   const int sms = prop.multiProcessorCount;
@@ -347,8 +441,16 @@ int main(int argc, char** argv) {
   for (int B : {256, 1024, 2048, 4096, 16384}) run_append_private<1>(B, pool, pool_recs, used, dropped, sms);
   for (int B : {256, 1024, 2048, 4096, 16384}) run_append_private<4>(B, pool, pool_recs, used, dropped, sms);
   }
+  if (on('s')) {
+    for (int B : {128, 256, 512, 1024}) run_part_sort<2048>(B, pool, pool_recs, used, dropped, sms);
+    for (int B : {128, 256, 512, 1024}) run_part_sort<3072>(B, pool, pool_recs, used, dropped, sms);
+    for (int B : {128, 256, 512}) run_part_sort<1024>(B, pool, pool_recs, used, dropped, sms);
+  }
   if (on('d')) for (int B : {512, 2048, 16384}) run_append(B, pool, pool_recs, gcur, dropped, sms);
-  if (on('e')) for (int dup : {1, 2, 4}) { run_dedupe<1024>(pool, 1ull << 27, dup, out, sms); run_dedupe<2048>(pool, 1ull << 27, dup, out, sms); run_dedupe<4096>(pool, 1ull << 27, dup, out, sms); }
+  if (on('e')) for (int dup : {1, 2, 4}) {
+    run_dedupe<1024, 1024>(pool, 1ull << 27, dup, out, sms); run_dedupe<2048, 1024>(pool, 1ull << 27, dup, out, sms); run_dedupe<4096, 1024>(pool, 1ull << 27, dup, out, sms);
+    run_dedupe<1024, 512>(pool, 1ull << 27, dup, out, sms); run_dedupe<2048, 512>(pool, 1ull << 27, dup, out, sms); run_dedupe<1024, 256>(pool, 1ull << 27, dup, out, sms);
+  }
   if (!on('f')) return 0;
   const u64 table_slots = 1ull << 30;                            // 32 GB table
   Rec* table; CK(cudaMalloc(&table, table_slots * 32));

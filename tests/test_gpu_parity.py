@@ -181,6 +181,48 @@ def test_cr2_shaped_masked(pkg, orc):
     assert nnz >= len(p["psi"])
 
 
+def test_cr2_shaped_full_size_bench_configuration(pkg):
+    """The Cr2-shaped config at FULL size in the launch configuration bench.py times (auto-planned passes, 60 GB table cap).
+    The oracle cannot run it (SURVEY.md 8(d) tier 3), so this checks what holds at any size: E_S against a library CSR
+    product of the same matrix, structural invariants of the counters, and PT2 / counts invariant under a different key
+    partitioning (forced 128 passes on a smaller table), whose per-class sums must add up to the same total."""
+    import torch
+    p = make_problem("cr2")
+    ctx = _ctx(pkg, p)
+    psi = _psi(p)
+    nnz = ctx.ham_build(p["eps"])
+    e_s, n2 = ctx.energy(psi)
+    rp, col, val = ctx.csr()
+    assert int(rp[-1]) == nnz and bool((rp[1:] > rp[:-1]).all())              # every row holds at least its diagonal
+    A = torch.sparse_csr_tensor(rp, col.to(torch.int64), val, size=(len(psi), len(psi)))
+    y = A @ psi
+    e_lib = float(psi @ y) / float(psi @ psi)
+    assert abs(e_s - e_lib) <= E_TOL * abs(e_lib)
+    x = torch.sin(torch.arange(len(psi), dtype=torch.float64, device="cuda"))
+    assert abs(float(x @ y) - float(psi @ (A @ x))) <= 1e-11 * float(x.abs() @ y.abs())           # x^T H psi = psi^T H x
+    del A, y, x, rp, col, val
+    torch.cuda.empty_cache()
+    ctx.pt2_config(0, 0)
+    a_pt2, a_ext, a_con = ctx.pt2(psi, e_s, p["eps2"])
+    ca = ctx.counters()
+    a_parts = np.array(ctx.pt2_partials())
+    assert ca["pt2_parts"] >= 32 and a_ext <= a_con <= ca["pt2_generated"]
+    assert abs(a_parts.sum() - a_pt2) <= 1e-12 * ca["pt2_sum_abs"]
+    ctx.pt2_config(900_000_000, 128)
+    b_pt2, b_ext, b_con = ctx.pt2(psi, e_s, p["eps2"])
+    cb = ctx.counters()
+    assert cb["pt2_parts"] == 128 and (b_ext, b_con, cb["pt2_generated"]) == (a_ext, a_con, ca["pt2_generated"])
+    assert abs(a_pt2 - b_pt2) <= PT2_TOL * max(abs(a_pt2), 1e-3 * ca["pt2_sum_abs"])
+    b_parts = np.array(ctx.pt2_partials())
+    # class c of 64 partitions = classes c and c + 64 of 128 (low bits of the same partition word, reading Q14)
+    if ca["pt2_parts"] == 64:
+        # per class the two runs differ by which source's O(1) update wrote H_aa first (rounding, amplified by the smallest
+        # |E_S - H_aa| ~ 2e-9 of this synthetic psi: DESIGN.md section 6, floating-point note)
+        diff = np.abs(a_parts - (b_parts[:64] + b_parts[64:]))
+        assert diff.max() <= 1e-9 * ca["pt2_sum_abs"], diff.max()
+    ctx.close()
+
+
 # ---------------------------------------------------------------- edge cases
 def test_single_determinant_hf(pkg, orc):
     p = make_problem("tiny", n_dets=1)
