@@ -67,7 +67,8 @@ typedef struct {
   double ms_pt2_scan;       /* pt2 table scan/clear + reductions, summed over passes */
   int64_t hsp_nnz;          /* stored entries of H_SP (last detham_hsp_build) */
   int64_t hsp_generated;    /* excitations that passed the screen in hsp_build (looked up in P) */
-  double ms_hsp_build;      /* hsp_build enumeration pass + arena -> CSR copy + per-row column sort */
+  double ms_hsp_build;      /* hsp_build enumeration pass (enumerate + lookup in P, hits appended to the arena) + row scan */
+  double ms_hsp_fill;       /* hsp_build arena -> CSR copy + per-row column sort */
 } detham_counters;
 
 /* Create a context: uploads the integrals, derives J_pq = (pp|qq), K_pq = (pq|qp), and builds the heat-bath lists

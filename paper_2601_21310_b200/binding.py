@@ -24,7 +24,8 @@ class Counters(C.Structure):
                 ("pt2_min_abs_den", C.c_double), ("ms_store", C.c_double), ("ms_build_count", C.c_double),
                 ("ms_build_fill", C.c_double), ("ms_energy", C.c_double), ("ms_pt2_plan", C.c_double),
                 ("ms_pt2_accum", C.c_double), ("ms_pt2_scan", C.c_double),
-                ("hsp_nnz", C.c_int64), ("hsp_generated", C.c_int64), ("ms_hsp_build", C.c_double)]
+                ("hsp_nnz", C.c_int64), ("hsp_generated", C.c_int64), ("ms_hsp_build", C.c_double),
+                ("ms_hsp_fill", C.c_double)]
 
 
 class DethamError(RuntimeError):

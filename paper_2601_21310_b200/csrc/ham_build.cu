@@ -235,14 +235,50 @@ sort_rows_warp_kernel(const int64_t* __restrict__ row_ptr, int64_t nd, int* __re
   for (int t = lane; t < len; t += 32) { col[b + t] = sc[warp][t]; val[b + t] = sv[warp][t]; }
 }
 
-// rows longer than kSortWarpCap: one CTA per row, sorted in place in global memory (L2)
+// rows longer than kSortWarpCap: one CTA per row.  Chunks of up to kSortCtaCap entries are sorted in shared memory (12 bytes
+// per entry; the network's virtual +inf tail pads to a power of two); a longer row is then merged pairwise, run width
+// doubling per round: every entry finds its rank in the partner run by a binary search (columns are unique within a row),
+// ping-ponging between the CSR and the build arena, which is free once the segments have been copied.
+constexpr int kSortCtaCap = 16384;
 __global__ void __launch_bounds__(1024)
-sort_rows_cta_kernel(const int64_t* __restrict__ row_ptr, int64_t nd, int* __restrict__ col, double* __restrict__ val) {
+sort_rows_cta_kernel(const int64_t* __restrict__ row_ptr, int64_t nd, int* __restrict__ col, double* __restrict__ val,
+                     int* __restrict__ tcol, double* __restrict__ tval) {
+  extern __shared__ __align__(16) unsigned char sort_smem[];
+  double* sv = reinterpret_cast<double*>(sort_smem);             // [kSortCtaCap]
+  int* sc = reinterpret_cast<int*>(sv + kSortCtaCap);            // [kSortCtaCap]
   for (int64_t row = blockIdx.x; row < nd; row += gridDim.x) {
-    int64_t b = row_ptr[row];
-    int len = (int)(row_ptr[row + 1] - b);
+    const int64_t b = row_ptr[row];
+    const int len = (int)(row_ptr[row + 1] - b);
     if (len <= kSortWarpCap) continue;
-    bitonic_rows(col + b, val + b, len, threadIdx.x, blockDim.x, [] { __syncthreads(); });
+    for (int c0 = 0; c0 < len; c0 += kSortCtaCap) {
+      const int m = min(kSortCtaCap, len - c0);
+      for (int t = threadIdx.x; t < m; t += blockDim.x) { sc[t] = col[b + c0 + t]; sv[t] = val[b + c0 + t]; }
+      __syncthreads();
+      bitonic_rows(sc, sv, m, threadIdx.x, blockDim.x, [] { __syncthreads(); });
+      for (int t = threadIdx.x; t < m; t += blockDim.x) { col[b + c0 + t] = sc[t]; val[b + c0 + t] = sv[t]; }
+      __syncthreads();
+    }
+    int* scol = col + b; double* sval = val + b;                 // source of the current merge round
+    int* dcol = tcol + b; double* dval = tval + b;
+    for (int width = kSortCtaCap; width < len; width <<= 1) {
+      for (int t = threadIdx.x; t < len; t += blockDim.x) {
+        const int pair0 = (t / (2 * width)) * (2 * width);       // start of this entry's pair of runs
+        const int mid = min(pair0 + width, len), end = min(pair0 + 2 * width, len);
+        const bool left = t < mid;
+        const int key = scol[t];
+        int lo = left ? mid : pair0, hi = left ? end : mid;      // the partner run
+        while (lo < hi) { const int md = (lo + hi) >> 1; if (scol[md] < key) lo = md + 1; else hi = md; }
+        const int pos = left ? t + (lo - mid) : (t - mid) + lo;  // own rank + entries of the partner run below the key
+        dcol[pos] = key; dval[pos] = sval[t];
+      }
+      __syncthreads();
+      int* xc = scol; scol = dcol; dcol = xc;
+      double* xv = sval; sval = dval; dval = xv;
+    }
+    if (scol != col + b) {
+      for (int t = threadIdx.x; t < len; t += blockDim.x) { col[b + t] = scol[t]; val[b + t] = sval[t]; }
+      __syncthreads();
+    }
   }
 }
 
@@ -393,12 +429,17 @@ static dh_status build_csr(detham_ctx* c, const CsrTarget& T, const double* psi 
   }
   sort_rows_warp_kernel<<<(unsigned)((nd + kWarpsPerCta - 1) / kWarpsPerCta), kWarpsPerCta * 32, 0, c->stream>>>(*T.row_ptr, nd, *T.col, *T.val);
   DH_CUDA(c, cudaGetLastError());
-  sort_rows_cta_kernel<<<c->sm_count * 2, 1024, 0, c->stream>>>(*T.row_ptr, nd, *T.col, *T.val);
+  {
+    const size_t sort_smem = (size_t)kSortCtaCap * (sizeof(double) + sizeof(int));
+    st = set_smem(c, sort_rows_cta_kernel, sort_smem); if (st != DH_OK) return st;
+    sort_rows_cta_kernel<<<c->sm_count, 1024, sort_smem, c->stream>>>(*T.row_ptr, nd, *T.col, *T.val, c->acol, c->aval);
+  }
   DH_CUDA(c, cudaGetLastError());
   DH_TICK(c, 3);
   DH_CUDA(c, cudaEventSynchronize(c->ev[3]));
   if (sp) {
-    c->ctr.ms_hsp_build = ms_pass + dh_elapsed(c, 2, 3);
+    c->ctr.ms_hsp_build = ms_pass;
+    c->ctr.ms_hsp_fill = dh_elapsed(c, 2, 3);
     c->ctr.hsp_nnz = nnz;
   } else {
     c->ctr.ms_build_count = ms_pass;

@@ -12,6 +12,7 @@ namespace {
 constexpr int kWarpsPerCta = 8;
 constexpr int kFine = 1 << DH_MAX_PBITS;  // finest class histogram
 constexpr int kProbeLimit = 1 << 16;
+constexpr double kSmallDen = 1e-3;  // |E_S - H_aa| below which the scan recomputes H_aa from scratch
 
 // one 32-byte sector per external: key, v_a = sum_i H_ai psi_i, H_aa.  Members of S are pre-inserted with v = NaN.
 struct __align__(32) Slot { u64 ka, kb; double v, haa; };
@@ -407,9 +408,30 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
   }
 }
 
+// H_DD from the determinant alone (no source, no update): E_core + sum_p h_pp + 1/2 sum_{p,q} [J or J-K], one thread
+__device__ __forceinline__ double diag_from_scratch(int n, const double* __restrict__ J, const double* __restrict__ JK,
+                                                    const double* __restrict__ hd, double e_core, u64 a, u64 b) {
+  double one = 0.0, two = 0.0;
+  for (int p = 0; p < n; ++p) {
+    bool pa = (a >> p) & 1ull, pb = (b >> p) & 1ull;
+    if (pa) one += hd[p];
+    if (pb) one += hd[p];
+    if (!pa && !pb) continue;
+    for (int q = 0; q < n; ++q) {
+      bool qa = (a >> q) & 1ull, qb = (b >> q) & 1ull;
+      if (pa && qa) two += JK[p * n + q];
+      if (pb && qb) two += JK[p * n + q];
+      if (pa && qb) two += J[p * n + q];
+      if (pb && qa) two += J[p * n + q];
+    }
+  }
+  return e_core + one + 0.5 * two;
+}
+
 // ---------------------------------------------------------------- reduce: sum_a v_a^2 / (E_S - H_aa), and clear the table
 __global__ void __launch_bounds__(256)
-pt2_scan_kernel(Slot* table, u64 cap, double e_s, double* __restrict__ part /* [grid][4]: sum, sum_abs, min_den, count */) {
+pt2_scan_kernel(Slot* table, u64 cap, double e_s, int n, const double* __restrict__ J, const double* __restrict__ JK,
+                const double* __restrict__ hd, double e_core, double* __restrict__ part /* [grid][4]: sum, sum_abs, min_den, count */) {
   double sum = 0.0, sabs = 0.0, mden = INFINITY, cnt = 0.0;
   constexpr int V = 4;  // independent 32-byte loads in flight per thread
   const u64 stride = (u64)gridDim.x * blockDim.x;
@@ -426,6 +448,10 @@ pt2_scan_kernel(Slot* table, u64 cap, double e_s, double* __restrict__ part /* [
       if (x[k] | y[k]) {
         if (z[k] != (u64)0x7ff8000000000001ull) {
           double v = __longlong_as_double((long long)z[k]), den = e_s - __longlong_as_double((long long)w[k]);
+          // The slot's H_aa came from the O(1) update of whichever source claimed it first, so it carries that source's
+          // rounding (~1e-13).  Where the denominator is small enough to amplify that, take H_aa from the key alone:
+          // the same value in every run and for every partitioning (a few externals in a million).
+          if (fabs(den) < kSmallDen) den = e_s - diag_from_scratch(n, J, JK, hd, e_core, x[k], y[k]);
           double term = v * v / den;
           sum += term; sabs += fabs(term); mden = fmin(mden, fabs(den)); cnt += 1.0;
         }
@@ -533,21 +559,7 @@ __global__ void diagonals_kernel(int n, const double* __restrict__ J, const doub
                                  double e_core, const u64* __restrict__ dets, int64_t m, double* __restrict__ out) {
   int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= m) return;
-  u64 a = dets[2 * t], b = dets[2 * t + 1];
-  double one = 0.0, two = 0.0;
-  for (int p = 0; p < n; ++p) {
-    bool pa = (a >> p) & 1ull, pb = (b >> p) & 1ull;
-    if (pa) one += hd[p];
-    if (pb) one += hd[p];
-    for (int q = 0; q < n; ++q) {
-      bool qa = (a >> q) & 1ull, qb = (b >> q) & 1ull;
-      if (pa && qa) two += JK[p * n + q];
-      if (pb && qb) two += JK[p * n + q];
-      if (pa && qb) two += J[p * n + q];
-      if (pb && qa) two += J[p * n + q];
-    }
-  }
-  out[t] = e_core + one + 0.5 * two;
+  out[t] = diag_from_scratch(n, J, JK, hd, e_core, dets[2 * t], dets[2 * t + 1]);
 }
 
 }  // namespace
@@ -621,7 +633,7 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
       pt2_compact_kernel<<<sgrid, 256, 0, c->stream>>>(table, (u64)cap, ex->keys, ex->v, ex->score, ex->cap, ex->cursor);
       DH_CUDA(c, cudaMemsetAsync(results + 4 * pass, 0, 4 * sizeof(double), c->stream));
     } else {
-      pt2_scan_kernel<<<sgrid, 256, 0, c->stream>>>(table, (u64)cap, e_s, part);
+      pt2_scan_kernel<<<sgrid, 256, 0, c->stream>>>(table, (u64)cap, e_s, c->n, c->J, c->JK, c->hd, c->e_core, part);
       final_reduce4_kernel<<<1, 256, 0, c->stream>>>(part, sgrid, results + 4 * pass);
     }
     DH_CUDA(c, cudaGetLastError());

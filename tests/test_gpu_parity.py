@@ -448,10 +448,11 @@ def test_expand_perturbative_set(pkg, orc, name, n_dets, eps2, parts):
 
 
 @pytest.mark.parametrize("name,n_dets,eps2,zero", [("tiny", None, 0.0, False), ("tiny", 600, 1e-4, True), ("h2o", 1500, 1e-6, True),
-                                                   ("tiny", 1, 0.0, False), ("n2", 300, 1e-6, False)])
+                                                   ("tiny", 1, 0.0, False), ("n2", 300, 1e-6, False), ("cr2", 24, 1e-6, False)])
 def test_hsp_build(pkg, orc, name, n_dets, eps2, zero):
     """H_SP in CSR against the sorted P (columns and values bit for bit), on a subset of P, with an empty P,
-    and with H_SS left intact on the same context; unsorted P is an error."""
+    and with H_SS left intact on the same context; unsorted P is an error.  The N2- and Cr2-shaped cases have rows of 2e4-3e5
+    entries: the chunked shared-memory sort with one and with several merge rounds."""
     import torch
     p = make_problem(name, n_dets=n_dets)
     if n_dets == 1:
