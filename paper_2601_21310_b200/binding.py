@@ -119,6 +119,7 @@ class Detham:
         self._dets = dets  # keep the borrowed buffer alive
         self._check(self._L.detham_set_subspace(self._h, ptr, m))
         self.n_dets = m
+        self._last_external = 0
 
     def ham_build(self, eps):
         nnz = C.c_int64(0)
@@ -168,20 +169,29 @@ class Detham:
         return e.value, it.value
 
     def expand(self, psi, eps2):
-        """Perturbative set P of Eq. 14 as CUDA tensors: (keys int64 [|P|, 2] sorted, score, v, H_aa)."""
+        """Perturbative set P of Eq. 14 as CUDA tensors: (keys int64 [|P|, 2] sorted, score, v, H_aa).
+
+        The buffers are sized from the external count of the last pt2() on this context when there is one (same S: the usual
+        case, one enumeration); otherwise, or if that was too small, a sizing call (cap = 0) runs first."""
         import torch
         assert psi.is_cuda and psi.dtype == torch.float64 and psi.is_contiguous() and psi.numel() == self.n_dets
         m = C.c_int64(0)
-        st = self._L.detham_expand(self._h, psi.data_ptr(), float(eps2), None, None, None, None, 0, C.byref(m))
-        if st != 0 and not (st == 1 and m.value > 0):
+        cap = int(getattr(self, "_last_external", 0))
+        for _ in range(3):
+            keys = torch.empty((cap, 2), dtype=torch.int64, device=psi.device)
+            score, v, haa = (torch.empty(cap, dtype=torch.float64, device=psi.device) for _ in range(3))
+            st = self._L.detham_expand(self._h, psi.data_ptr(), float(eps2), keys.data_ptr() if cap else None,
+                                       score.data_ptr() if cap else None, v.data_ptr() if cap else None,
+                                       haa.data_ptr() if cap else None, cap, C.byref(m))
+            if st == 0:
+                n = m.value
+                return keys[:n], score[:n], v[:n], haa[:n]
+            if st == 1 and m.value > cap:      # DH_EINVAL with *n_out set: the set needs m.value entries
+                cap = m.value
+                del keys, score, v, haa
+                continue
             self._check(st)
-        n = m.value
-        keys = torch.empty((n, 2), dtype=torch.int64, device=psi.device)
-        score, v, haa = (torch.empty(n, dtype=torch.float64, device=psi.device) for _ in range(3))
-        if n:
-            self._check(self._L.detham_expand(self._h, psi.data_ptr(), float(eps2), keys.data_ptr(), score.data_ptr(), v.data_ptr(),
-                                              haa.data_ptr(), n, C.byref(m)))
-        return keys, score, v, haa
+        raise DethamError(1, "detham_expand did not settle on a buffer size")
 
     def hsp_build(self, psi, eps2, pkeys):
         """H_SP in CSR against the sorted key list `pkeys` (CUDA [m, 2] int64/uint64, e.g. expand()'s keys); returns nnz."""
@@ -211,6 +221,7 @@ class Detham:
         out = C.c_double(0)
         ne, nc = C.c_int64(0), C.c_int64(0)
         self._check(self._L.detham_pt2(self._h, psi.data_ptr(), float(e_s), float(eps2), C.byref(out), C.byref(ne), C.byref(nc)))
+        self._last_external = ne.value
         return out.value, ne.value, nc.value
 
     def pt2_partials(self):
