@@ -260,13 +260,14 @@ def main():
            "phases_ms": {k: mean(k) for k in ("ms_store", "ms_build_count", "ms_build_fill", "ms_energy", "ms_pt2_plan",
                                               "ms_pt2_accum", "ms_pt2_scan")},
            "counters": {k: c[k] for k in ("nnz", "build_generated", "pt2_generated", "pt2_contrib", "pt2_external",
-                                          "pt2_parts", "pt2_probe_parts", "pt2_max_probe", "pt2_table_slots", "pt2_sum_abs", "pt2_min_abs_den")},
+                                          "pt2_parts", "pt2_probe_parts", "pt2_max_probe", "pt2_table_slots", "pt2_sum_abs", "pt2_min_abs_den",
+                                          "pt2_binned")},
            "results": {"E_S": e_s, "PT2": pt2}, "es_pt2_wall_ms": mean("ms_build_count") + mean("ms_build_fill") + t_energy + t_pt2,
            "stored_nnz_per_sec": c["nnz"] / ((mean("ms_build_count") + mean("ms_build_fill")) * 1e-3),
            # kernels of libdetham.so per step: store 2 (validate, index insert), ham_build 5 (enumerate, row scan, segment copy,
            # two row sorts), energy 2, pt2 3 (plan histogram, norm + reduce) + 4 per key partition (member insert, accumulate,
            # scan, reduce) + 4 when the planner probed one slice
-           "gpu_launches": 2 + 5 + 2 + 3 + 4 * parts + (4 if c["pt2_probe_parts"] else 0)}
+           "gpu_launches": 2 + 5 + 2 + 3 + (5 if c["pt2_binned"] else 4) * parts + (4 if c["pt2_probe_parts"] else 0)}
 
     # ---- the widened rows, timed on the same workload after the hot path: median of 3, CUDA events
     if args.widened and rank == 0:

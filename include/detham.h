@@ -69,6 +69,7 @@ typedef struct {
   int64_t hsp_generated;    /* excitations that passed the screen in hsp_build (looked up in P) */
   double ms_hsp_build;      /* hsp_build enumeration pass (enumerate + lookup in P, hits appended to the arena) + row scan */
   double ms_hsp_fill;       /* hsp_build arena -> CSR copy + per-row column sort */
+  int64_t pt2_binned;       /* 1 if the last pt2 ran binned (records appended per table region, then merged region by region) */
 } detham_counters;
 
 /* Create a context: uploads the integrals, derives J_pq = (pp|qq), K_pq = (pq|qp), and builds the heat-bath lists

@@ -25,7 +25,7 @@ class Counters(C.Structure):
                 ("ms_build_fill", C.c_double), ("ms_energy", C.c_double), ("ms_pt2_plan", C.c_double),
                 ("ms_pt2_accum", C.c_double), ("ms_pt2_scan", C.c_double),
                 ("hsp_nnz", C.c_int64), ("hsp_generated", C.c_int64), ("ms_hsp_build", C.c_double),
-                ("ms_hsp_fill", C.c_double)]
+                ("ms_hsp_fill", C.c_double), ("pt2_binned", C.c_int64)]
 
 
 class DethamError(RuntimeError):

@@ -94,6 +94,9 @@ struct detham_ctx {
   void* table = nullptr;      // zero between calls (the scan clears what it reads)
   int64_t table_slots = 0;
   std::vector<double> partials;
+  void* pool = nullptr;       // binned PT2: contribution records {key, H psi, H_aa}, [bin][CTA][seg_cap]
+  int64_t pool_bytes = 0;
+  unsigned* pool_used = nullptr;  // records per (bin, CTA) segment, [1024][grid]
 
   // scratch
   double* red = nullptr;      // device reduction buffer
@@ -180,6 +183,9 @@ __device__ __forceinline__ void dh_ld256(const void* p, u64& a, u64& b, u64& c, 
 // streaming variants for the table scan (evict-first: the scan touches every slot exactly once)
 __device__ __forceinline__ void dh_ld256_cs(const void* p, u64& a, u64& b, u64& c, u64& d) {
   asm volatile("ld.global.cs.v4.u64 {%0,%1,%2,%3}, [%4];" : "=l"(a), "=l"(b), "=l"(c), "=l"(d) : "l"(p) : "memory");
+}
+__device__ __forceinline__ void dh_st256(void* p, u64 a, u64 b, u64 c, u64 d) {
+  asm volatile("st.global.v4.u64 [%0], {%1,%2,%3,%4};" ::"l"(p), "l"(a), "l"(b), "l"(c), "l"(d) : "memory");
 }
 __device__ __forceinline__ void dh_st256_zero(void* p) {
   asm volatile("st.global.cs.v4.u64 [%0], {%1,%1,%1,%1};" ::"l"(p), "l"(0ull) : "memory");

@@ -185,6 +185,32 @@ __device__ __forceinline__ void probe_batch(ProbeCtx& pc, const u64 (&ka)[U], co
   pc.max_probe = max(pc.max_probe, probes);
 }
 
+// Binned mode (tables far beyond L2): instead of probing the table, a contribution is appended as a 32-byte record
+// {key, H_ai psi_i, H_aa} to this CTA's private segment of the bin its slot falls in (bin = slot >> shift: a contiguous
+// region of the table).  pt2_merge_kernel then walks the bins in order, so the probes of the whole GPU stay inside a window
+// of the table that fits L2 (profiles/r1_microbench.md, block C: 36-41 G/s against 15 G/s for random probes).  The position
+// in the segment comes from a shared-memory counter: no global atomic.  A record that does not fit its segment is probed
+// directly, as in the unbinned kernel.
+struct BinCtx { Slot* pool; unsigned* cnt; unsigned seg_cap; int shift; };
+
+template <int U>
+__device__ __forceinline__ unsigned bin_batch(ProbeCtx& pc, const BinCtx& bc, const u64 (&ka)[U], const u64 (&kb)[U],
+                                              const double (&cv)[U], const u64 (&slot)[U], const unsigned (&meta)[U], unsigned pend) {
+#pragma unroll
+  for (int u = 0; u < U; ++u)
+    if ((pend >> u) & 1u) {
+      const double haa = meta_diag(pc, meta[u]);
+      const unsigned bin = (unsigned)(slot[u] >> bc.shift);
+      const unsigned p = atomicAdd(&bc.cnt[bin], 1u);
+      if (p < bc.seg_cap) {
+        dh_st256(bc.pool + ((u64)bin * gridDim.x + blockIdx.x) * bc.seg_cap + p, ka[u], kb[u], (u64)__double_as_longlong(cv[u]),
+                 (u64)__double_as_longlong(haa));
+        pend &= ~(1u << u);
+      }
+    }
+  return pend;
+}
+
 // decode the triangular index t = y(y-1)/2 + x, x < y
 __device__ __forceinline__ void tri_decode(int t, int& x, int& y) {
   y = (int)((1.0f + sqrtf(1.0f + 8.0f * (float)t)) * 0.5f);
@@ -193,16 +219,22 @@ __device__ __forceinline__ void tri_decode(int t, int& x, int& y) {
   x = t - y * (y - 1) / 2;
 }
 
-template <int kAccWarps, int kU, bool kExpand>
+template <int kAccWarps, int kU, bool kExpand, bool kBinned = false>
 __global__ void __launch_bounds__(kAccWarps * 32, 1)
 pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* __restrict__ psi, int64_t nd, double eps2,
                       unsigned pass, Slot* table, u64 cap, u64* counters /* [0] next row [1] gen [2] contrib [3] max probe */,
-                      int* overflow) {
+                      int* overflow, Slot* pool, unsigned* used, unsigned seg_cap, int bin_shift, int nbins) {
   extern __shared__ __align__(16) unsigned char smem[];
   CtaTables T = dh_cta_stage(P, smem);
   size_t off = (dh_cta_table_bytes(P.n) + 15) & ~(size_t)15;
   WarpScratch* wsp = reinterpret_cast<WarpScratch*>(smem + off);
   FlatScratch* fsp = reinterpret_cast<FlatScratch*>(smem + off + kAccWarps * sizeof(WarpScratch));
+  unsigned* bcnt = reinterpret_cast<unsigned*>(fsp + kAccWarps);  // [nbins] records this CTA appended per bin (binned mode)
+  if (kBinned) {
+    for (int t = threadIdx.x; t < nbins; t += blockDim.x) bcnt[t] = 0;
+    __syncthreads();
+  }
+  const BinCtx bc{pool, bcnt, seg_cap, bin_shift};
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const unsigned lt = (1u << lane) - 1u;
   WarpScratch& ws = wsp[warp];
@@ -277,6 +309,7 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
           __syncwarp();
           qn -= take;
           gen += pend;
+          if (kBinned) pend = bin_batch<1>(pc, bc, ka, kb, cv, slot, meta, pend);
           probe_batch<1, kExpand>(pc, ka, kb, cv, slot, meta, pend);
         }
       }
@@ -387,6 +420,7 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
           }
         }
         gen += __popc(pend);
+        if (kBinned) pend = bin_batch<kU>(pc, bc, ka, kb, cv, slot, meta, pend);
         probe_batch<kU, kExpand>(pc, ka, kb, cv, slot, meta, pend);
       }
       __syncwarp();
@@ -406,6 +440,69 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
     if (ct) atomicAdd(counters + 2, ct);
     atomicMax(counters + 3, (u64)mp);
   }
+  if (kBinned) {
+    __syncthreads();
+    for (int t = threadIdx.x; t < nbins; t += blockDim.x) used[(size_t)t * gridDim.x + blockIdx.x] = min(bcnt[t], seg_cap);
+  }
+}
+
+// Binned mode, second half: the records of bin b (one segment per accumulate CTA) are merged into the table region the bin
+// covers.  The CTAs take (bin, segment) chunks from one global cursor in bin-major order, so at any time all probes of the
+// GPU fall into one or two neighbouring regions (16 MB each at 4096 bins of a 60 GB table).  The probe itself is the
+// unbinned kernel's; H_aa comes with the record.
+__global__ void __launch_bounds__(1024, 2)
+pt2_merge_kernel(const Slot* __restrict__ pool, const unsigned* __restrict__ used, unsigned seg_cap, int nbins, int nseg,
+                 Slot* table, u64 cap, u64* counters /* [2] contrib [3] max probe [5] chunk cursor */, int* overflow) {
+  // partition word of a key from byte-indexed tables: ZB[k][v] = XOR of the words of the orbitals set in byte v of byte k
+  // (16 lookups instead of one per electron)
+  __shared__ u64 ZB[16][256];
+  __shared__ u64 q_sh;
+  for (int t = threadIdx.x; t < 16 * 256; t += blockDim.x) {
+    const int k = t >> 8, v = t & 255;
+    u64 z = 0;
+    for (int bit = 0; bit < 8; ++bit) if ((v >> bit) & 1) z ^= dh_zword((k >= 8 ? 64 : 0) + 8 * (k & 7) + bit);
+    ZB[k][v] = z;
+  }
+  const u64 nchunks = (u64)nbins * nseg;
+  unsigned contrib = 0; int max_probe = 0;
+  for (;;) {
+    __syncthreads();
+    if (threadIdx.x == 0) q_sh = atomicAdd(counters + 5, 1ull);
+    __syncthreads();
+    const u64 q = q_sh;
+    if (q >= nchunks) break;
+    const unsigned n = used[q];                                   // chunk q = segment (q % nseg) of bin (q / nseg)
+    const Slot* src = pool + q * seg_cap;
+    for (unsigned t = threadIdx.x; t < n; t += blockDim.x) {
+      u64 ka, kb, vv, hh;
+      dh_ld256_cs(src + t, ka, kb, vv, hh);
+      u64 z = 0;
+#pragma unroll
+      for (int k = 0; k < 8; ++k) z ^= ZB[k][(ka >> (8 * k)) & 255u] ^ ZB[8 + k][(kb >> (8 * k)) & 255u];
+      u64 slot = __umul64hi(z, cap);
+      const double cv = __longlong_as_double((long long)vv);
+      int probes = 0;
+      for (;;) {
+        u64 k0, k1, vb, hb;
+        dh_ld256(table + slot, k0, k1, vb, hb);
+        if (k0 == ka && k1 == kb) {
+          if (vb != (u64)0x7ff8000000000001ull) { atomicAdd(&table[slot].v, cv); ++contrib; }
+          break;
+        }
+        if ((k0 | k1) == 0ull) {
+          Key128 old = dh_cas128(table + slot, Key128{0ull, 0ull}, Key128{ka, kb});
+          if ((old.a | old.b) == 0ull) { table[slot].haa = __longlong_as_double((long long)hh); atomicAdd(&table[slot].v, cv); ++contrib; break; }
+          if (old.a == ka && old.b == kb) { atomicAdd(&table[slot].v, cv); ++contrib; break; }
+        }
+        if (++slot == cap) slot = 0;
+        if (++probes > kProbeLimit) { *overflow = 1; break; }
+      }
+      max_probe = max(max_probe, probes);
+    }
+  }
+  u64 ct = contrib;
+  for (int o = 16; o > 0; o >>= 1) { ct += __shfl_xor_sync(0xffffffffu, ct, o); max_probe = max(max_probe, __shfl_xor_sync(0xffffffffu, max_probe, o)); }
+  if ((threadIdx.x & 31) == 0) { if (ct) atomicAdd(counters + 2, ct); atomicMax(counters + 3, (u64)max_probe); }
 }
 
 // H_DD from the determinant alone (no source, no update): E_core + sum_p h_pp + 1/2 sum_{p,q} [J or J-K], one thread
@@ -581,8 +678,10 @@ static dh_status ensure_table(detham_ctx* c, int64_t slots) {
 // contributions share an external.
 struct ExpandOut { u64* keys; double* v; double* score; u64 cap; u64* cursor; };  // device buffers of expand mode
 
+// `est_pass` (0 = unknown): upper estimate of the contributions of one pass; with it, and a table far beyond L2, the passes run
+// binned (bin_batch / pt2_merge_kernel).
 static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, double eps2, int pbits, int64_t slots, bool adapt,
-                             double load, double* out, double* pilot = nullptr, const ExpandOut* ex = nullptr) {
+                             double load, double* out, double* pilot = nullptr, const ExpandOut* ex = nullptr, double est_pass = 0.0) {
   const int64_t nd = c->nd;
   dh_status st = ensure_table(c, slots); if (st != DH_OK) return st;
   Slot* table = reinterpret_cast<Slot*>(c->table);
@@ -590,7 +689,8 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
   st = dh_get_lists(c, pbits, &L); if (st != DH_OK) return st;
   EnumParams P = dh_make_params(c, L);
   // launch shape: (warps per CTA, probes in flight per lane); DETHAM_PT2_VARIANT selects another one for tuning
-  using AccKernel = void (*)(EnumParams, const u64*, const double*, int64_t, double, unsigned, Slot*, u64, u64*, int*);
+  using AccKernel = void (*)(EnumParams, const u64*, const double*, int64_t, double, unsigned, Slot*, u64, u64*, int*, Slot*, unsigned*,
+                             unsigned, int, int);
   struct Variant { int warps, u; AccKernel k; };
   // measured on B200 (profiles/r1_v2_summary.md): more warps per SM help (Cr2-shaped accumulate 1419 / 1084 / 1025 / 994 ms at
   // 16 / 24 / 28 / 32 warps), more probes in flight per lane do not (16 warps x 2 probes: slower than x 1)
@@ -598,9 +698,34 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
                                      {16, 1, pt2_accumulate_kernel<16, 1, false>}, {16, 2, pt2_accumulate_kernel<16, 2, false>}};
   int vi = 0;
   if (const char* e = getenv("DETHAM_PT2_VARIANT")) { int v = atoi(e); if (v >= 0 && v < (int)(sizeof(variants) / sizeof(variants[0]))) vi = v; }
-  const int warps = ex ? 32 : variants[vi].warps;
-  AccKernel acc_kernel = ex ? pt2_accumulate_kernel<32, 1, true> : variants[vi].k;
-  const size_t smem = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + warps * (sizeof(WarpScratch) + sizeof(FlatScratch));
+  int64_t want0 = (nd + 31) / 32;
+  const int grid32 = (int)(want0 < (int64_t)c->sm_count ? want0 : (int64_t)c->sm_count);
+  // binned mode: DETHAM_PT2_BINNED = 0 | 1 overrides the rule "table beyond 32 GB, estimate available, not expand / pilot"
+  // (measured: H2O-shaped, 15 GB table, 5 contributions per external: 17.5 ms binned against 12.8 ms direct; N2-shaped, 60 GB: 143 against 152 ms)
+  constexpr int kMaxBins = 4096;
+  bool binned = !ex && !pilot && est_pass > 0.0 && slots * (int64_t)sizeof(Slot) > (32ll << 30) && grid32 == c->sm_count;
+  if (const char* e = getenv("DETHAM_PT2_BINNED")) { if (atoi(e) == 0) binned = false; else if (!ex && !pilot && est_pass > 0.0 && grid32 == c->sm_count) binned = true; }
+  if (binned) {
+    // the pool holds the records of one pass: 20 % head room over the estimate (an upper bound already) plus 64 records per
+    // segment; it is divided evenly over the pass's (bin, CTA) segments, and what does not fit a segment is probed directly
+    const int64_t bytes = (int64_t)((est_pass * 1.2 + 64.0 * kMaxBins * grid32) * sizeof(Slot));
+    size_t free_b = 0, total_b = 0;
+    DH_CUDA(c, cudaMemGetInfo(&free_b, &total_b));
+    if (c->pool_bytes < bytes) {
+      if ((double)bytes > 0.95 * ((double)free_b + (double)c->pool_bytes)) binned = false;
+      else {
+        if (c->pool) cudaFree(c->pool);
+        c->pool = nullptr; c->pool_bytes = 0;
+        if (cudaMalloc(&c->pool, (size_t)bytes) != cudaSuccess) { cudaGetLastError(); binned = false; }
+        else c->pool_bytes = bytes;
+      }
+    }
+    if (binned && !c->pool_used) DH_CUDA(c, cudaMalloc(&c->pool_used, (size_t)kMaxBins * c->sm_count * sizeof(unsigned)));
+  }
+  const int warps = (ex || binned) ? 32 : variants[vi].warps;
+  AccKernel acc_kernel = ex ? pt2_accumulate_kernel<32, 1, true> : (binned ? pt2_accumulate_kernel<32, 1, false, true> : variants[vi].k);
+  const size_t smem = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + warps * (sizeof(WarpScratch) + sizeof(FlatScratch)) +
+                      (binned ? kMaxBins * sizeof(unsigned) : 0);
   DH_CUDA(c, cudaFuncSetAttribute(acc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int64_t want = (nd + warps - 1) / warps;
   const int grid = (int)(want < (int64_t)c->sm_count ? want : (int64_t)c->sm_count);
@@ -624,10 +749,23 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
   for (int pass = 0; pass < nparts; ++pass) {
     const int64_t sblocks = (cap + 1023) / 1024;
     const int sgrid = (int)(sblocks < sgrid_max ? sblocks : sgrid_max);
-    DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 4 * sizeof(u64), c->stream));
+    DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 8 * sizeof(u64), c->stream));
     DH_TICK(c, 2);
     member_insert_kernel<<<(unsigned)((nd + 255) / 256), 256, 0, c->stream>>>(c->dets, nd, (unsigned)(nparts - 1), (unsigned)pass, table, (u64)cap, overflow);
-    acc_kernel<<<grid, warps * 32, smem, c->stream>>>(P, c->dets, psi, nd, eps2, (unsigned)pass, table, (u64)cap, c->dcount, overflow);
+    int bin_shift = 0, nbins = 1;
+    unsigned seg_cap = 0;
+    if (binned) {  // bins = contiguous table regions of 2^shift slots, at most kMaxBins of them
+      while ((((cap - 1) >> bin_shift) + 1) > kMaxBins) ++bin_shift;
+      nbins = (int)(((cap - 1) >> bin_shift) + 1);
+      seg_cap = (unsigned)(c->pool_bytes / ((int64_t)nbins * grid * (int64_t)sizeof(Slot)));
+    }
+    acc_kernel<<<grid, warps * 32, smem, c->stream>>>(P, c->dets, psi, nd, eps2, (unsigned)pass, table, (u64)cap, c->dcount, overflow,
+                                                      reinterpret_cast<Slot*>(c->pool), c->pool_used, seg_cap, bin_shift, nbins);
+    if (binned) {
+      DH_CUDA(c, cudaGetLastError());
+      pt2_merge_kernel<<<c->sm_count * 2, 1024, 0, c->stream>>>(reinterpret_cast<const Slot*>(c->pool), c->pool_used, seg_cap, nbins, grid, table,
+                                                               (u64)cap, c->dcount, overflow);
+    }
     DH_TICK(c, 3);
     if (ex && !pilot) {
       pt2_compact_kernel<<<sgrid, 256, 0, c->stream>>>(table, (u64)cap, ex->keys, ex->v, ex->score, ex->cap, ex->cursor);
@@ -669,6 +807,7 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
   c->ctr.pt2_parts = nparts;
   c->ctr.pt2_max_probe = (int32_t)max_probe;
   c->ctr.pt2_table_slots = slots;
+  c->ctr.pt2_binned = binned ? 1 : 0;
   c->ctr.pt2_sum_abs = sabs / norm2;
   c->ctr.pt2_min_abs_den = mden;
   c->ctr.ms_pt2_accum = ms_accum;
@@ -694,6 +833,8 @@ static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double ep
   c->ctr.ms_pt2_plan = 0.0;
   if (!auto_parts) { while ((1 << pbits) < c->cfg_parts) ++pbits; }
   int64_t max_slots = slots;
+  std::vector<u64> hist;      // class histogram of the contributions (finest partition), empty when nothing was planned
+  double hist_scale = 1.0;
   if (auto_parts || auto_slots) {
     // class histogram of the contributions: exact for small inputs, else from every stride-th source (scaled, +10 %);
     // it only sizes the table - an underestimate is caught by the overflow flag and retried with more partitions
@@ -712,11 +853,12 @@ static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double ep
     count_kernel<<<grid, kWarpsPerCta * 32, smem, c->stream>>>(P0, c->dets, psi, nd, stride, eps2, c->dcount, reinterpret_cast<u64*>(c->hist));
     DH_CUDA(c, cudaGetLastError());
     DH_TICK(c, 1);
-    std::vector<u64> hist(kFine);
+    hist.assign(kFine, 0);
     DH_CUDA(c, cudaMemcpyAsync(hist.data(), c->hist, kFine * sizeof(u64), cudaMemcpyDeviceToHost, c->stream));
     DH_CUDA(c, cudaStreamSynchronize(c->stream));
     c->ctr.ms_pt2_plan = dh_elapsed(c, 0, 1);
     const double scale = stride == 1 ? 1.0 : 1.1 * (double)stride;
+    hist_scale = scale;
     size_t free_b = 0, total_b = 0;
     DH_CUDA(c, cudaMemGetInfo(&free_b, &total_b));
     max_slots = (int64_t)(((double)free_b + (double)c->table_slots * sizeof(Slot)) * 0.92 / sizeof(Slot));
@@ -765,7 +907,13 @@ static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double ep
   }
   for (;;) {
     if (ex) DH_CUDA(c, cudaMemsetAsync(ex->cursor, 0, sizeof(u64), c->stream));
-    st = pt2_attempt(c, psi, e_s, eps2, pbits, slots, auto_slots && !ex, load, out, nullptr, ex);
+    double est_pass = 0.0;  // contributions of the fullest class at this partition count (sizes the record pool of binned mode)
+    if (!hist.empty()) {
+      u64 m = 0;
+      for (int cl = 0; cl < (1 << pbits); ++cl) { u64 t = 0; for (int f = cl; f < kFine; f += (1 << pbits)) t += hist[f]; if (t > m) m = t; }
+      est_pass = (double)m * hist_scale + 64.0;
+    }
+    st = pt2_attempt(c, psi, e_s, eps2, pbits, slots, auto_slots && !ex, load, out, nullptr, ex, est_pass);
     if (st == DH_OK) c->ctr.pt2_probe_parts = probe_parts;
     if (st != DH_ETABLEFULL || !auto_parts || pbits >= DH_MAX_PBITS) return st;
     ++pbits;  // the plan was too optimistic: halve the keys per pass and start over
