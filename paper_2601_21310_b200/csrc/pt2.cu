@@ -456,24 +456,32 @@ pt2_merge_kernel(const Slot* __restrict__ pool, const unsigned* __restrict__ use
   // partition word of a key from byte-indexed tables: ZB[k][v] = XOR of the words of the orbitals set in byte v of byte k
   // (16 lookups instead of one per electron)
   __shared__ u64 ZB[16][256];
-  __shared__ u64 q_sh;
   for (int t = threadIdx.x; t < 16 * 256; t += blockDim.x) {
     const int k = t >> 8, v = t & 255;
     u64 z = 0;
     for (int bit = 0; bit < 8; ++bit) if ((v >> bit) & 1) z ^= dh_zword((k >= 8 ? 64 : 0) + 8 * (k & 7) + bit);
     ZB[k][v] = z;
   }
-  const u64 nchunks = (u64)nbins * nseg;
+  __syncthreads();
+  // work unit = kUnit consecutive records of one (bin, segment), taken per WARP from the global cursor in bin-major order: no
+  // CTA barrier in the loop, and the ~9500 resident warps span three or four bins (128-record units were slower than the
+  // CTA-wide chunks: 1e7 atomics per pass on the one cursor cost 18 ms)
+  const int lane = threadIdx.x & 31;
+  constexpr unsigned kUnit = 512;
+  const unsigned nsub = (seg_cap + kUnit - 1u) / kUnit;
+  const u64 nunits = (u64)nbins * nseg * nsub;
   unsigned contrib = 0; int max_probe = 0;
   for (;;) {
-    __syncthreads();
-    if (threadIdx.x == 0) q_sh = atomicAdd(counters + 5, 1ull);
-    __syncthreads();
-    const u64 q = q_sh;
-    if (q >= nchunks) break;
-    const unsigned n = used[q];                                   // chunk q = segment (q % nseg) of bin (q / nseg)
+    u64 u = 0;
+    if (lane == 0) u = atomicAdd(counters + 5, 1ull);
+    u = __shfl_sync(0xffffffffu, u, 0);
+    if (u >= nunits) break;
+    const u64 q = u / nsub;                                       // segment (q % nseg) of bin (q / nseg)
+    const unsigned lo = (unsigned)(u % nsub) * kUnit, n = used[q];
+    if (lo >= n) continue;
+    const unsigned hi = min(n, lo + kUnit);
     const Slot* src = pool + q * seg_cap;
-    for (unsigned t = threadIdx.x; t < n; t += blockDim.x) {
+    for (unsigned t = lo + lane; t < hi; t += 32) {
       u64 ka, kb, vv, hh;
       dh_ld256_cs(src + t, ka, kb, vv, hh);
       u64 z = 0;
