@@ -716,7 +716,10 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
   if (binned) {
     // the pool holds the records of one pass: 20 % head room over the estimate (an upper bound already) plus 64 records per
     // segment; it is divided evenly over the pass's (bin, CTA) segments, and what does not fit a segment is probed directly
-    const int64_t bytes = (int64_t)((est_pass * 1.2 + 64.0 * kMaxBins * grid32) * sizeof(Slot));
+    // (DETHAM_PT2_POOL_FRAC replaces the 1.2: a tuning knob, and the tests' way to make segments overflow)
+    double pool_frac = 1.2;
+    if (const char* e = getenv("DETHAM_PT2_POOL_FRAC")) { double v = atof(e); if (v >= 0.0 && v <= 8.0) pool_frac = v; }
+    const int64_t bytes = (int64_t)((est_pass * pool_frac + 64.0 * kMaxBins * grid32) * sizeof(Slot));
     size_t free_b = 0, total_b = 0;
     DH_CUDA(c, cudaMemGetInfo(&free_b, &total_b));
     if (c->pool_bytes < bytes) {

@@ -367,6 +367,44 @@ def test_small_table_cap_forces_many_passes(pkg, orc, monkeypatch):
     ctx.close()
 
 
+def test_pt2_binned_mode(pkg, orc, monkeypatch):
+    """Binned mode of pt2 (records appended per table region, then merged region by region) is chosen
+    by the library only for tables beyond 32 GB; DETHAM_PT2_BINNED=1 forces it here on a case the oracle finishes.  Covered:
+    the default record pool, a pool too small for most records (DETHAM_PT2_POOL_FRAC: the overflow goes straight to the
+    table, the rest through the merge), a pool of 64 records per segment, forced multi-pass, a mostly empty pool
+    (masked psi: 300 of 6000 sources), and DETHAM_PT2_BINNED=0."""
+    import torch
+    p = make_problem("h2o", n_dets=6000)
+    ctx = _ctx(pkg, p)
+    psi = _psi(p)
+    e_s = -0.7 + float(orc.diagonal(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"][0]))
+    o = orc.pt2(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"], p["psi"], e_s, p["eps2"], n_parts=16)
+    assert o["n_contrib"] > 20_000_000
+
+    def check(o, psi, n_parts, binned):
+        ctx.pt2_config(0, n_parts)
+        g_pt2, g_ext, g_con = ctx.pt2(psi, e_s, p["eps2"])
+        c = ctx.counters()
+        assert c["pt2_binned"] == binned
+        assert (g_ext, g_con) == (o["n_external"], o["n_contrib"]), (g_ext, g_con, o["n_external"], o["n_contrib"])
+        assert abs(g_pt2 - o["pt2"]) <= PT2_TOL * max(abs(o["pt2"]), 1e-3 * o["sum_abs"]), (g_pt2, o["pt2"])
+        assert abs(c["pt2_sum_abs"] - o["sum_abs"]) <= 1e-8 * o["sum_abs"]
+        if n_parts == 16:
+            assert np.allclose(ctx.pt2_partials(), o["part_sums"], rtol=1e-8, atol=1e-12 * o["sum_abs"])
+
+    monkeypatch.setenv("DETHAM_PT2_BINNED", "1")
+    for frac in ("0.05", "0", "1.2"):  # ascending pool size: the pool only grows within a context
+        monkeypatch.setenv("DETHAM_PT2_POOL_FRAC", frac)
+        check(o, psi, 0, 1)
+    check(o, psi, 16, 1)
+    q, _ = _masked(p, 300, 3)
+    om = orc.pt2(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"], q["psi"], e_s, p["eps2"], n_parts=16)
+    check(om, torch.from_numpy(q["psi"]).cuda(), 0, 1)
+    monkeypatch.setenv("DETHAM_PT2_BINNED", "0")
+    check(o, psi, 0, 0)
+    ctx.close()
+
+
 def test_ham_build_repeated_with_different_eps(pkg, orc):
     """The build arena is sized from the previous build: growing, shrinking and growing again must all give the oracle's CSR."""
     p = make_problem("tiny", n_dets=1200)
