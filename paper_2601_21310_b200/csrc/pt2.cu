@@ -710,7 +710,9 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
   const int grid32 = (int)(want0 < (int64_t)c->sm_count ? want0 : (int64_t)c->sm_count);
   // binned mode: DETHAM_PT2_BINNED = 0 | 1 overrides the rule "table beyond 32 GB, estimate available, not expand / pilot"
   // (measured: H2O-shaped, 15 GB table, 5 contributions per external: 17.5 ms binned against 12.8 ms direct; N2-shaped, 60 GB: 143 against 152 ms)
-  constexpr int kMaxBins = 4096;
+  // regions of the table (DETHAM_PT2_BINS: tuning knob, 64..8192; each costs 4 bytes of the accumulate CTA's shared memory)
+  int max_bins = 4096;
+  if (const char* e = getenv("DETHAM_PT2_BINS")) { int v = atoi(e); if (v >= 64 && v <= 8192) max_bins = v; }
   bool binned = !ex && !pilot && est_pass > 0.0 && slots * (int64_t)sizeof(Slot) > (32ll << 30) && grid32 == c->sm_count;
   if (const char* e = getenv("DETHAM_PT2_BINNED")) { if (atoi(e) == 0) binned = false; else if (!ex && !pilot && est_pass > 0.0 && grid32 == c->sm_count) binned = true; }
   if (binned) {
@@ -719,7 +721,7 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
     // (DETHAM_PT2_POOL_FRAC replaces the 1.2: a tuning knob, and the tests' way to make segments overflow)
     double pool_frac = 1.2;
     if (const char* e = getenv("DETHAM_PT2_POOL_FRAC")) { double v = atof(e); if (v >= 0.0 && v <= 8.0) pool_frac = v; }
-    const int64_t bytes = (int64_t)((est_pass * pool_frac + 64.0 * kMaxBins * grid32) * sizeof(Slot));
+    const int64_t bytes = (int64_t)((est_pass * pool_frac + 64.0 * max_bins * grid32) * sizeof(Slot));
     size_t free_b = 0, total_b = 0;
     DH_CUDA(c, cudaMemGetInfo(&free_b, &total_b));
     if (c->pool_bytes < bytes) {
@@ -731,12 +733,12 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
         else c->pool_bytes = bytes;
       }
     }
-    if (binned && !c->pool_used) DH_CUDA(c, cudaMalloc(&c->pool_used, (size_t)kMaxBins * c->sm_count * sizeof(unsigned)));
+    if (binned && !c->pool_used) DH_CUDA(c, cudaMalloc(&c->pool_used, (size_t)8192 * c->sm_count * sizeof(unsigned)));
   }
   const int warps = (ex || binned) ? 32 : variants[vi].warps;
   AccKernel acc_kernel = ex ? pt2_accumulate_kernel<32, 1, true> : (binned ? pt2_accumulate_kernel<32, 1, false, true> : variants[vi].k);
   const size_t smem = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + warps * (sizeof(WarpScratch) + sizeof(FlatScratch)) +
-                      (binned ? kMaxBins * sizeof(unsigned) : 0);
+                      (binned ? max_bins * sizeof(unsigned) : 0);
   DH_CUDA(c, cudaFuncSetAttribute(acc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int64_t want = (nd + warps - 1) / warps;
   const int grid = (int)(want < (int64_t)c->sm_count ? want : (int64_t)c->sm_count);
@@ -765,8 +767,8 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
     member_insert_kernel<<<(unsigned)((nd + 255) / 256), 256, 0, c->stream>>>(c->dets, nd, (unsigned)(nparts - 1), (unsigned)pass, table, (u64)cap, overflow);
     int bin_shift = 0, nbins = 1;
     unsigned seg_cap = 0;
-    if (binned) {  // bins = contiguous table regions of 2^shift slots, at most kMaxBins of them
-      while ((((cap - 1) >> bin_shift) + 1) > kMaxBins) ++bin_shift;
+    if (binned) {  // bins = contiguous table regions of 2^shift slots, at most max_bins of them
+      while ((((cap - 1) >> bin_shift) + 1) > max_bins) ++bin_shift;
       nbins = (int)(((cap - 1) >> bin_shift) + 1);
       seg_cap = (unsigned)(c->pool_bytes / ((int64_t)nbins * grid * (int64_t)sizeof(Slot)));
     }
