@@ -237,7 +237,9 @@ def main():
     b_energy = 12.0 * c["nnz"] + 8.0 * (nd + 1) + 16.0 * nd
     b_pt2 = 32.0 * c["pt2_contrib"] + 32.0 * c["pt2_external"] + 24.0 * nd
     path_gbs = (b_energy + b_pt2) / ((t_energy + t_pt2) * 1e-3) / 1e9
-    roofline = {"bound": "hbm", "kernel": "pt2_accumulate_kernel", "achieved": achieved, "peak": peak, "unit": "GB/s",
+    # binned mode: one key partition's accumulate step is the append + merge pair, timed together (ms_pt2_accum)
+    acc_name = "pt2_accumulate_kernel<binned> + pt2_merge_kernel" if c["pt2_binned"] else "pt2_accumulate_kernel"
+    roofline = {"bound": "hbm", "kernel": acc_name, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
                 "bytes_per_launch": bytes_accum_launch, "launch_ms": acc_ms, "launches_per_step": parts,
                 "energy_plus_pt2_GBps": path_gbs, "energy_plus_pt2_frac": path_gbs / peak,
