@@ -452,7 +452,7 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
 // unbinned kernel's; H_aa comes with the record.
 __global__ void __launch_bounds__(1024, 2)
 pt2_merge_kernel(const Slot* __restrict__ pool, const unsigned* __restrict__ used, unsigned seg_cap, int nbins, int nseg,
-                 Slot* table, u64 cap, u64* counters /* [2] contrib [3] max probe [5] chunk cursor */, int* overflow) {
+                 Slot* table, u64 cap, u64* counters /* [2] contrib [3] max probe [5] chunk cursor */, int* overflow, int nbytes) {
   // partition word of a key from byte-indexed tables: ZB[k][v] = XOR of the words of the orbitals set in byte v of byte k
   // (16 lookups instead of one per electron)
   __shared__ u64 ZB[16][256];
@@ -486,7 +486,8 @@ pt2_merge_kernel(const Slot* __restrict__ pool, const unsigned* __restrict__ use
       dh_ld256_cs(src + t, ka, kb, vv, hh);
       u64 z = 0;
 #pragma unroll
-      for (int k = 0; k < 8; ++k) z ^= ZB[k][(ka >> (8 * k)) & 255u] ^ ZB[8 + k][(kb >> (8 * k)) & 255u];
+      for (int k = 0; k < 8; ++k)  // bytes beyond the n orbitals of a spin word are zero and contribute nothing
+        if (k < nbytes) z ^= ZB[k][(ka >> (8 * k)) & 255u] ^ ZB[8 + k][(kb >> (8 * k)) & 255u];
       u64 slot = __umul64hi(z, cap);
       const double cv = __longlong_as_double((long long)vv);
       int probes = 0;
@@ -777,7 +778,7 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
     if (binned) {
       DH_CUDA(c, cudaGetLastError());
       pt2_merge_kernel<<<c->sm_count * 2, 1024, 0, c->stream>>>(reinterpret_cast<const Slot*>(c->pool), c->pool_used, seg_cap, nbins, grid, table,
-                                                               (u64)cap, c->dcount, overflow);
+                                                               (u64)cap, c->dcount, overflow, (c->n + 7) / 8);
     }
     DH_TICK(c, 3);
     if (ex && !pilot) {
