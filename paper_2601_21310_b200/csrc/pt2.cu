@@ -711,8 +711,8 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
   const int grid32 = (int)(want0 < (int64_t)c->sm_count ? want0 : (int64_t)c->sm_count);
   // binned mode: DETHAM_PT2_BINNED = 0 | 1 overrides the rule "table beyond 32 GB, estimate available, not expand / pilot"
   // (measured: H2O-shaped, 15 GB table, 5 contributions per external: 17.5 ms binned against 12.8 ms direct; N2-shaped, 60 GB: 143 against 152 ms)
-  // regions of the table (DETHAM_PT2_BINS: tuning knob, 64..8192; each costs 4 bytes of the accumulate CTA's shared memory)
-  int max_bins = 4096;
+  // regions of the table (DETHAM_PT2_BINS: tuning knob, 64..8192, a cap: the region size is a power of two of slots; each costs 4 bytes of the accumulate CTA's shared memory)
+  int max_bins = 2048;  // measured on Cr2-shaped (profiles/r1_v5_summary.md): accumulate 6174 / 5968 / 5941 / 6099 / 6947 ms at 512 / 1024 / 2048 / 4096 / 8192
   if (const char* e = getenv("DETHAM_PT2_BINS")) { int v = atoi(e); if (v >= 64 && v <= 8192) max_bins = v; }
   bool binned = !ex && !pilot && est_pass > 0.0 && slots * (int64_t)sizeof(Slot) > (32ll << 30) && grid32 == c->sm_count;
   if (const char* e = getenv("DETHAM_PT2_BINNED")) { if (atoi(e) == 0) binned = false; else if (!ex && !pilot && est_pass > 0.0 && grid32 == c->sm_count) binned = true; }
