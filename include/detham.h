@@ -69,8 +69,30 @@ typedef struct {
   int64_t hsp_generated;    /* excitations that passed the screen in hsp_build (looked up in P) */
   double ms_hsp_build;      /* hsp_build enumeration pass (enumerate + lookup in P, hits appended to the arena) + row scan */
   double ms_hsp_fill;       /* hsp_build arena -> CSR copy + per-row column sort */
-  int64_t pt2_binned;       /* 1 if the last pt2 ran binned (records appended per table region, then merged region by region) */
+  int64_t pt2_binned;       /* organisation of the last pt2: 0 = hash table in HBM, 2 = streamed (records partitioned by key
+                               region, deduplicated in L2-resident region tables; no table in HBM) */
+  int64_t pt2_stream_bins;  /* streamed organisation: key regions per pass (0 otherwise); pt2_table_slots = slots of one region table */
 } detham_counters;
+
+/* Options of pt2 (SURVEY.md section 5 "config / flag system").  Zero in every field = the defaults. */
+typedef struct {
+  int32_t mode;             /* 0 = choose: streamed when one pass of the table organisation would need a table beyond 24 GB;
+                               1 = hash table in HBM; 2 = streamed (DH_EINVAL if |S| < 16 x SM count) */
+  int32_t n_parts;          /* key partitions / passes, a power of two <= 1024 (streamed: <= 256); 0 = planned */
+  int64_t table_slots;      /* table organisation: capacity in 32-byte slots; 0 = planned from free device memory */
+  double table_load;        /* table organisation: target load factor, 0 = 0.5 */
+  double max_table_gb;      /* table organisation: the planner never sizes the table beyond this (random 32-byte accesses lose
+                               4x of their rate past ~70 GB on a B200: TLB reach); 0 = 60 */
+  double small_den;         /* externals with |E_S - H_aa| below this take H_aa from the key alone instead of the O(1) update from
+                               the source that claimed them (its rounding, ~1e-13, is amplified by 1 / denominator; DESIGN.md
+                               reading Q11); 0 = 1e-3, negative = never */
+  int32_t stream_bins;      /* streamed: key regions per pass (<= 4096); 0 = planned so that a region's distinct keys fit its table */
+  int32_t reserved;
+  double stream_ring_mb;    /* streamed: bytes of the three region tables together (they must stay in L2); 0 = 60 */
+  double stream_load;       /* streamed: target load factor of a region table; 0 = 0.6 */
+  double stream_pool_frac;  /* streamed: head room of the record pool over the planned estimate; 0 = 1.15 */
+  double stream_pool_gb;    /* streamed: budget of the record pool; 0 = 80 % of the free device memory */
+} detham_pt2_options;
 
 /* Create a context: uploads the integrals, derives J_pq = (pp|qq), K_pq = (pq|qp), and builds the heat-bath lists
  * ("we precompute a lookup table during initialization: for each pair of occupied spin-orbitals (i,j),
@@ -115,8 +137,16 @@ dh_status detham_residual(detham_ctx* ctx, const double* psi, double e_s, double
 dh_status detham_ediag(detham_ctx* ctx, const double* v0, double tol, int max_iter, double* e_out, int* iters_out);
 
 /* Configure pt2: table_slots = hash-table capacity in 32-byte slots (0 = choose from free device memory);
- * n_parts = number of key partitions / passes, a power of two <= 1024 (0 = choose so that every partition fits). */
+ * n_parts = number of key partitions / passes, a power of two <= 1024 (0 = choose so that every partition fits).
+ * Shorthand for the two fields of the same name of detham_pt2_options; the other options keep their values. */
 dh_status detham_pt2_config(detham_ctx* ctx, int64_t table_slots, int n_parts);
+
+/* Set every option of pt2 (opts == NULL: back to the defaults).  DH_EINVAL for values out of range; nothing is changed then. */
+dh_status detham_pt2_set_options(detham_ctx* ctx, const detham_pt2_options* opts);
+
+/* Release the large work buffers of pt2 (hash table, record pool, region tables, cached heat-bath list splits other than the
+ * unsplit one); they are re-created on demand.  For callers that share the device with other allocations. */
+dh_status detham_trim(detham_ctx* ctx);
 
 /* pt2 (Eq. 13 second term, screened per Eq. 14 / PAPER.md:227; readings Q6, Q9, Q10):
  * for every source i with psi_i != 0, tau_i = eps2 / |psi_i| (0 if eps2 == 0); for every single or double excitation a

@@ -13,7 +13,7 @@ STATUS = {0: "DH_OK", 1: "DH_EINVAL", 2: "DH_EUNSORTED", 3: "DH_EPOPCOUNT", 4: "
 
 # every symbol include/detham.h declares
 SYMBOLS = ["detham_create", "detham_set_subspace", "detham_ham_build", "detham_csr", "detham_csr_copy", "detham_energy", "detham_residual", "detham_ediag",
-           "detham_pt2_config", "detham_pt2", "detham_expand", "detham_hsp_build", "detham_hsp_csr", "detham_hsp_csr_copy", "detham_pt2_partials", "detham_solve_host", "detham_connections",
+           "detham_pt2_config", "detham_pt2_set_options", "detham_trim", "detham_pt2", "detham_expand", "detham_hsp_build", "detham_hsp_csr", "detham_hsp_csr_copy", "detham_pt2_partials", "detham_solve_host", "detham_connections",
            "detham_diagonals", "detham_get_counters", "detham_destroy", "detham_strerror", "detham_last_cuda_error"]
 
 
@@ -25,7 +25,17 @@ class Counters(C.Structure):
                 ("ms_build_fill", C.c_double), ("ms_energy", C.c_double), ("ms_pt2_plan", C.c_double),
                 ("ms_pt2_accum", C.c_double), ("ms_pt2_scan", C.c_double),
                 ("hsp_nnz", C.c_int64), ("hsp_generated", C.c_int64), ("ms_hsp_build", C.c_double),
-                ("ms_hsp_fill", C.c_double), ("pt2_binned", C.c_int64)]
+                ("ms_hsp_fill", C.c_double), ("pt2_binned", C.c_int64), ("pt2_stream_bins", C.c_int64)]
+
+
+class Pt2Options(C.Structure):
+    """detham_pt2_options (include/detham.h); zero in every field = the defaults."""
+    _fields_ = [("mode", C.c_int32), ("n_parts", C.c_int32), ("table_slots", C.c_int64), ("table_load", C.c_double),
+                ("max_table_gb", C.c_double), ("small_den", C.c_double), ("stream_bins", C.c_int32), ("reserved", C.c_int32),
+                ("stream_ring_mb", C.c_double), ("stream_load", C.c_double), ("stream_pool_frac", C.c_double),
+                ("stream_pool_gb", C.c_double)]
+
+MODES = {"auto": 0, "table": 1, "stream": 2}
 
 
 class DethamError(RuntimeError):
@@ -53,6 +63,8 @@ def load_library():
     L.detham_residual.argtypes = [vp, vp, C.c_double, vp, dp]
     L.detham_ediag.argtypes = [vp, vp, C.c_double, C.c_int, dp, C.POINTER(C.c_int)]
     L.detham_pt2_config.argtypes = [vp, C.c_int64, C.c_int]
+    L.detham_pt2_set_options.argtypes = [vp, C.POINTER(Pt2Options)]
+    L.detham_trim.argtypes = [vp]
     L.detham_pt2.argtypes = [vp, vp, C.c_double, C.c_double, dp, ip, ip]
     L.detham_expand.argtypes = [vp, vp, C.c_double, vp, vp, vp, vp, C.c_int64, ip]
     L.detham_hsp_build.argtypes = [vp, vp, C.c_double, vp, C.c_int64, ip]
@@ -214,6 +226,21 @@ class Detham:
 
     def pt2_config(self, table_slots=0, n_parts=0):
         self._check(self._L.detham_pt2_config(self._h, int(table_slots), int(n_parts)))
+
+    def pt2_set_options(self, **kw):
+        """Set every option of pt2 (detham_pt2_options); fields not named go back to their defaults.  mode: "auto" | "table" |
+        "stream" or 0 | 1 | 2.  No arguments = all defaults."""
+        o = Pt2Options()
+        for k, v in kw.items():
+            if k == "mode" and isinstance(v, str):
+                v = MODES[v]
+            if not hasattr(o, k):
+                raise DethamError(1, f"unknown pt2 option {k}")
+            setattr(o, k, v)
+        self._check(self._L.detham_pt2_set_options(self._h, C.byref(o)))
+
+    def trim(self):
+        self._check(self._L.detham_trim(self._h))
 
     def pt2(self, psi, e_s, eps2):
         import torch

@@ -1,7 +1,6 @@
 // C ABI entry points (include/detham.h): argument checks, context lifetime, host<->device plumbing.
 #include <algorithm>
 #include <cmath>
-#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <numeric>
@@ -23,9 +22,10 @@ void free_all(detham_ctx* c) {
   f(c->h1); f(c->eri); f(c->J); f(c->JK); f(c->hd);
   for (auto& L : c->lists) { f(L.sub_off); f(L.val); f(L.ab); }
   f(c->dets_owned); f(c->psi_owned); f(c->shash_key); f(c->shash_idx); f(c->sbits);
-  f(c->row_ptr); f(c->col); f(c->val); f(c->row_cnt); f(c->sp_row_ptr); f(c->sp_col); f(c->sp_val); f(c->phash_key); f(c->phash_idx); f(c->acol); f(c->aval); f(c->segs); f(c->table); f(c->pool); f(c->pool_used); f(c->red); f(c->dcount); f(c->hist);
+  f(c->row_ptr); f(c->col); f(c->val); f(c->row_cnt); f(c->sp_row_ptr); f(c->sp_col); f(c->sp_val); f(c->phash_key); f(c->phash_idx); f(c->acol); f(c->aval); f(c->segs); f(c->table); f(c->pool); f(c->ring); f(c->sflags); f(c->red); f(c->dcount); f(c->hist);
   if (c->pinned) cudaFreeHost(c->pinned);
   for (auto& e : c->ev) if (e) cudaEventDestroy(e);
+  for (auto& e : c->sev) cudaEventDestroy(e);
 }
 
 }  // namespace
@@ -48,13 +48,6 @@ dh_status detham_create(detham_ctx** out, int n_orb, int n_alpha, int n_beta, co
   auto fail = [&](dh_status s) { free_all(c); delete c; return s; };
   auto body = [&]() -> dh_status {
     DH_CUDA(c, cudaGetDevice(&c->device));
-    // The PT2 table is probed one 32-byte sector at a time at random addresses: ask L2 not to fetch neighbouring sectors.
-    // (A hint; DETHAM_L2_FETCH = 32 | 64 | 128 overrides it for tuning.)
-    {
-      size_t gran = 32;
-      if (const char* e = getenv("DETHAM_L2_FETCH")) { int v = atoi(e); if (v == 32 || v == 64 || v == 128) gran = (size_t)v; }
-      if (cudaDeviceSetLimit(cudaLimitMaxL2FetchGranularity, gran) != cudaSuccess) cudaGetLastError();
-    }
     DH_CUDA(c, cudaDeviceGetAttribute(&c->sm_count, cudaDevAttrMultiProcessorCount, c->device));
     const int64_t n = n_orb, npair = n * (n + 1) / 2;
     c->n_eri = npair * (npair + 1) / 2;
@@ -141,8 +134,38 @@ dh_status detham_ediag(detham_ctx* c, const double* v0, double tol, int max_iter
 dh_status detham_pt2_config(detham_ctx* c, int64_t table_slots, int n_parts) {
   if (!c || table_slots < 0 || n_parts < 0 || n_parts > (1 << DH_MAX_PBITS) || (n_parts & (n_parts - 1))) return DH_EINVAL;
   if (table_slots > 0 && table_slots < 64) return DH_EINVAL;
-  c->cfg_table_slots = table_slots;
-  c->cfg_parts = n_parts;
+  c->opt.table_slots = table_slots;
+  c->opt.n_parts = n_parts;
+  return DH_OK;
+}
+
+dh_status detham_pt2_set_options(detham_ctx* c, const detham_pt2_options* o) {
+  if (!c) return DH_EINVAL;
+  if (!o) { c->opt = detham_pt2_options{}; return DH_OK; }
+  auto fin = [](double x) { return std::isfinite(x); };
+  if (o->mode < 0 || o->mode > 2 || o->n_parts < 0 || o->n_parts > (1 << DH_MAX_PBITS) || (o->n_parts & (o->n_parts - 1)) ||
+      o->table_slots < 0 || (o->table_slots > 0 && o->table_slots < 64) || !fin(o->table_load) || o->table_load < 0.0 ||
+      o->table_load > 0.95 || !fin(o->max_table_gb) || o->max_table_gb < 0.0 || !fin(o->small_den) || o->stream_bins < 0 ||
+      o->stream_bins > 4096 || !fin(o->stream_ring_mb) || o->stream_ring_mb < 0.0 || !fin(o->stream_load) || o->stream_load < 0.0 ||
+      o->stream_load > 0.95 || !fin(o->stream_pool_frac) || o->stream_pool_frac < 0.0 || !fin(o->stream_pool_gb) || o->stream_pool_gb < 0.0)
+    return DH_EINVAL;
+  c->opt = *o;
+  return DH_OK;
+}
+
+dh_status detham_trim(detham_ctx* c) {
+  if (!c) return DH_EINVAL;
+  DH_CUDA(c, cudaStreamSynchronize(c->stream));
+  auto f = [](auto*& p) { if (p) cudaFree(p); p = nullptr; };
+  f(c->table); c->table_slots = 0;
+  f(c->pool); c->pool_bytes = 0;
+  f(c->ring); c->ring_bytes = 0;
+  f(c->sflags); c->sflags_bytes = 0;
+  for (int k = 1; k <= DH_MAX_PBITS; ++k) {
+    HbLists& L = c->lists[k];
+    f(L.sub_off); f(L.val); f(L.ab);
+    L.pbits = -1;
+  }
   return DH_OK;
 }
 

@@ -89,14 +89,17 @@ struct detham_ctx {
   int64_t phash_cap = 0;
 
   // pt2
-  int64_t cfg_table_slots = 0;
-  int cfg_parts = 0;
   void* table = nullptr;      // zero between calls (the scan clears what it reads)
   int64_t table_slots = 0;
   std::vector<double> partials;
-  void* pool = nullptr;       // binned PT2: contribution records {key, H psi, H_aa}, [bin][CTA][seg_cap]
+  void* pool = nullptr;       // streamed PT2: contribution records {key, H psi, H_aa} of one pass, [bin][CTA][seg_cap]
   int64_t pool_bytes = 0;
-  unsigned* pool_used = nullptr;  // records per (bin, CTA) segment, [1024][grid]
+  void* ring = nullptr;       // streamed PT2: the L2-resident region tables
+  size_t ring_bytes = 0;
+  void* sflags = nullptr;     // streamed PT2: records per (bin, CTA) segment + the hand-over counters of the merge
+  size_t sflags_bytes = 0;
+  std::vector<cudaEvent_t> sev;  // per-pass timers of the streamed PT2
+  detham_pt2_options opt{};   // detham_pt2_set_options (zero = defaults)
 
   // scratch
   double* red = nullptr;      // device reduction buffer

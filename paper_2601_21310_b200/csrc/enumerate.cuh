@@ -93,7 +93,7 @@ __device__ __forceinline__ double dh_excited_diag(const CtaTables& T, const Warp
 
 // Single-excitation element i -> a in spin s, evaluation order of DESIGN.md reading Q7 (adds only, no FMA possible):
 // h_ia, then ((ia|qq) - (iq|qa)) over same-spin occupied q ascending, then (ia|qq) over other-spin occupied q ascending.
-__device__ __forceinline__ double dh_single_value(const EnumParams& P, const WarpScratch& ws, u64 wsame, int s, int i, int a) {
+__device__ __forceinline__ double dh_single_value_occ(const EnumParams& P, const unsigned char (*occ)[DH_MAX_ORB], u64 wsame, int s, int i, int a) {
   double v = __ldg(P.h1 + i * P.n + a);
   const int ns = s == 0 ? P.na : P.nb, no = s == 0 ? P.nb : P.na;
   // the loads of four terms are issued before the first is added (the additions keep the order of reading Q7)
@@ -101,21 +101,24 @@ __device__ __forceinline__ double dh_single_value(const EnumParams& P, const War
   for (; k + 4 <= ns; k += 4) {
     double t[4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) { const int q = ws.occ[s][k + u]; t[u] = dh_eri(P.eri, i, a, q, q) - dh_eri(P.eri, i, q, q, a); }
+    for (int u = 0; u < 4; ++u) { const int q = occ[s][k + u]; t[u] = dh_eri(P.eri, i, a, q, q) - dh_eri(P.eri, i, q, q, a); }
 #pragma unroll
     for (int u = 0; u < 4; ++u) v = v + t[u];
   }
-  for (; k < ns; ++k) { const int q = ws.occ[s][k]; v = v + (dh_eri(P.eri, i, a, q, q) - dh_eri(P.eri, i, q, q, a)); }
+  for (; k < ns; ++k) { const int q = occ[s][k]; v = v + (dh_eri(P.eri, i, a, q, q) - dh_eri(P.eri, i, q, q, a)); }
   k = 0;
   for (; k + 4 <= no; k += 4) {
     double t[4];
 #pragma unroll
-    for (int u = 0; u < 4; ++u) { const int q = ws.occ[s ^ 1][k + u]; t[u] = dh_eri(P.eri, i, a, q, q); }
+    for (int u = 0; u < 4; ++u) { const int q = occ[s ^ 1][k + u]; t[u] = dh_eri(P.eri, i, a, q, q); }
 #pragma unroll
     for (int u = 0; u < 4; ++u) v = v + t[u];
   }
-  for (; k < no; ++k) { const int q = ws.occ[s ^ 1][k]; v = v + dh_eri(P.eri, i, a, q, q); }
+  for (; k < no; ++k) { const int q = occ[s ^ 1][k]; v = v + dh_eri(P.eri, i, a, q, q); }
   return dh_parity_between(wsame, i, a) ? -v : v;
+}
+__device__ __forceinline__ double dh_single_value(const EnumParams& P, const WarpScratch& ws, u64 wsame, int s, int i, int a) {
+  return dh_single_value_occ(P, ws.occ, wsame, s, i, a);
 }
 
 // parity (0 even, 1 odd) of the phase of a double excitation of (da, db), reading Q1.  kind 1: same spin s, i<j -> a<b:

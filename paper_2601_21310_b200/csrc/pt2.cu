@@ -3,7 +3,7 @@
 #include <math.h>
 #include <stdlib.h>
 
-#include "enumerate.cuh"
+#include "pt2_common.cuh"
 
 EnumParams dh_make_params(detham_ctx* c, const HbLists* L);
 
@@ -11,11 +11,8 @@ namespace {
 
 constexpr int kWarpsPerCta = 8;
 constexpr int kFine = 1 << DH_MAX_PBITS;  // finest class histogram
-constexpr int kProbeLimit = 1 << 16;
-constexpr double kSmallDen = 1e-3;  // |E_S - H_aa| below which the scan recomputes H_aa from scratch
 
-// one 32-byte sector per external: key, v_a = sum_i H_ai psi_i, H_aa.  Members of S are pre-inserted with v = NaN.
-struct __align__(32) Slot { u64 ka, kb; double v, haa; };
+// Slot (pt2_common.cuh): one 32-byte sector per external.  Members of S are pre-inserted with v = NaN.
 
 __device__ __forceinline__ double member_flag() { return __longlong_as_double(0x7ff8000000000001ll); }
 
@@ -185,32 +182,6 @@ __device__ __forceinline__ void probe_batch(ProbeCtx& pc, const u64 (&ka)[U], co
   pc.max_probe = max(pc.max_probe, probes);
 }
 
-// Binned mode (tables far beyond L2): instead of probing the table, a contribution is appended as a 32-byte record
-// {key, H_ai psi_i, H_aa} to this CTA's private segment of the bin its slot falls in (bin = slot >> shift: a contiguous
-// region of the table).  pt2_merge_kernel then walks the bins in order, so the probes of the whole GPU stay inside a window
-// of the table that fits L2 (profiles/r1_microbench.md, block C: 36-41 G/s against 15 G/s for random probes).  The position
-// in the segment comes from a shared-memory counter: no global atomic.  A record that does not fit its segment is probed
-// directly, as in the unbinned kernel.
-struct BinCtx { Slot* pool; unsigned* cnt; unsigned seg_cap; int shift; };
-
-template <int U>
-__device__ __forceinline__ unsigned bin_batch(ProbeCtx& pc, const BinCtx& bc, const u64 (&ka)[U], const u64 (&kb)[U],
-                                              const double (&cv)[U], const u64 (&slot)[U], const unsigned (&meta)[U], unsigned pend) {
-#pragma unroll
-  for (int u = 0; u < U; ++u)
-    if ((pend >> u) & 1u) {
-      const double haa = meta_diag(pc, meta[u]);
-      const unsigned bin = (unsigned)(slot[u] >> bc.shift);
-      const unsigned p = atomicAdd(&bc.cnt[bin], 1u);
-      if (p < bc.seg_cap) {
-        dh_st256(bc.pool + ((u64)bin * gridDim.x + blockIdx.x) * bc.seg_cap + p, ka[u], kb[u], (u64)__double_as_longlong(cv[u]),
-                 (u64)__double_as_longlong(haa));
-        pend &= ~(1u << u);
-      }
-    }
-  return pend;
-}
-
 // decode the triangular index t = y(y-1)/2 + x, x < y
 __device__ __forceinline__ void tri_decode(int t, int& x, int& y) {
   y = (int)((1.0f + sqrtf(1.0f + 8.0f * (float)t)) * 0.5f);
@@ -219,22 +190,16 @@ __device__ __forceinline__ void tri_decode(int t, int& x, int& y) {
   x = t - y * (y - 1) / 2;
 }
 
-template <int kAccWarps, int kU, bool kExpand, bool kBinned = false>
+template <int kAccWarps, int kU, bool kExpand>
 __global__ void __launch_bounds__(kAccWarps * 32, 1)
 pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* __restrict__ psi, int64_t nd, double eps2,
                       unsigned pass, Slot* table, u64 cap, u64* counters /* [0] next row [1] gen [2] contrib [3] max probe */,
-                      int* overflow, Slot* pool, unsigned* used, unsigned seg_cap, int bin_shift, int nbins) {
+                      int* overflow) {
   extern __shared__ __align__(16) unsigned char smem[];
   CtaTables T = dh_cta_stage(P, smem);
   size_t off = (dh_cta_table_bytes(P.n) + 15) & ~(size_t)15;
   WarpScratch* wsp = reinterpret_cast<WarpScratch*>(smem + off);
   FlatScratch* fsp = reinterpret_cast<FlatScratch*>(smem + off + kAccWarps * sizeof(WarpScratch));
-  unsigned* bcnt = reinterpret_cast<unsigned*>(fsp + kAccWarps);  // [nbins] records this CTA appended per bin (binned mode)
-  if (kBinned) {
-    for (int t = threadIdx.x; t < nbins; t += blockDim.x) bcnt[t] = 0;
-    __syncthreads();
-  }
-  const BinCtx bc{pool, bcnt, seg_cap, bin_shift};
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const unsigned lt = (1u << lane) - 1u;
   WarpScratch& ws = wsp[warp];
@@ -309,7 +274,6 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
           __syncwarp();
           qn -= take;
           gen += pend;
-          if (kBinned) pend = bin_batch<1>(pc, bc, ka, kb, cv, slot, meta, pend);
           probe_batch<1, kExpand>(pc, ka, kb, cv, slot, meta, pend);
         }
       }
@@ -420,7 +384,6 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
           }
         }
         gen += __popc(pend);
-        if (kBinned) pend = bin_batch<kU>(pc, bc, ka, kb, cv, slot, meta, pend);
         probe_batch<kU, kExpand>(pc, ka, kb, cv, slot, meta, pend);
       }
       __syncwarp();
@@ -440,104 +403,12 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
     if (ct) atomicAdd(counters + 2, ct);
     atomicMax(counters + 3, (u64)mp);
   }
-  if (kBinned) {
-    __syncthreads();
-    for (int t = threadIdx.x; t < nbins; t += blockDim.x) used[(size_t)t * gridDim.x + blockIdx.x] = min(bcnt[t], seg_cap);
-  }
-}
-
-// Binned mode, second half: the records of bin b (one segment per accumulate CTA) are merged into the table region the bin
-// covers.  The CTAs take (bin, segment) chunks from one global cursor in bin-major order, so at any time all probes of the
-// GPU fall into one or two neighbouring regions (16 MB each at 4096 bins of a 60 GB table).  The probe itself is the
-// unbinned kernel's; H_aa comes with the record.
-__global__ void __launch_bounds__(1024, 2)
-pt2_merge_kernel(const Slot* __restrict__ pool, const unsigned* __restrict__ used, unsigned seg_cap, int nbins, int nseg,
-                 Slot* table, u64 cap, u64* counters /* [2] contrib [3] max probe [5] chunk cursor */, int* overflow, int nbytes) {
-  // partition word of a key from byte-indexed tables: ZB[k][v] = XOR of the words of the orbitals set in byte v of byte k
-  // (16 lookups instead of one per electron)
-  __shared__ u64 ZB[16][256];
-  for (int t = threadIdx.x; t < 16 * 256; t += blockDim.x) {
-    const int k = t >> 8, v = t & 255;
-    u64 z = 0;
-    for (int bit = 0; bit < 8; ++bit) if ((v >> bit) & 1) z ^= dh_zword((k >= 8 ? 64 : 0) + 8 * (k & 7) + bit);
-    ZB[k][v] = z;
-  }
-  __syncthreads();
-  // work unit = kUnit consecutive records of one (bin, segment), taken per WARP from the global cursor in bin-major order: no
-  // CTA barrier in the loop, and the ~9500 resident warps span three or four bins (128-record units were slower than the
-  // CTA-wide chunks: 1e7 atomics per pass on the one cursor cost 18 ms)
-  const int lane = threadIdx.x & 31;
-  constexpr unsigned kUnit = 512;
-  const unsigned nsub = (seg_cap + kUnit - 1u) / kUnit;
-  const u64 nunits = (u64)nbins * nseg * nsub;
-  unsigned contrib = 0; int max_probe = 0;
-  for (;;) {
-    u64 u = 0;
-    if (lane == 0) u = atomicAdd(counters + 5, 1ull);
-    u = __shfl_sync(0xffffffffu, u, 0);
-    if (u >= nunits) break;
-    const u64 q = u / nsub;                                       // segment (q % nseg) of bin (q / nseg)
-    const unsigned lo = (unsigned)(u % nsub) * kUnit, n = used[q];
-    if (lo >= n) continue;
-    const unsigned hi = min(n, lo + kUnit);
-    const Slot* src = pool + q * seg_cap;
-    for (unsigned t = lo + lane; t < hi; t += 32) {
-      u64 ka, kb, vv, hh;
-      dh_ld256_cs(src + t, ka, kb, vv, hh);
-      u64 z = 0;
-#pragma unroll
-      for (int k = 0; k < 8; ++k)  // bytes beyond the n orbitals of a spin word are zero and contribute nothing
-        if (k < nbytes) z ^= ZB[k][(ka >> (8 * k)) & 255u] ^ ZB[8 + k][(kb >> (8 * k)) & 255u];
-      u64 slot = __umul64hi(z, cap);
-      const double cv = __longlong_as_double((long long)vv);
-      int probes = 0;
-      for (;;) {
-        u64 k0, k1, vb, hb;
-        dh_ld256(table + slot, k0, k1, vb, hb);
-        if (k0 == ka && k1 == kb) {
-          if (vb != (u64)0x7ff8000000000001ull) { atomicAdd(&table[slot].v, cv); ++contrib; }
-          break;
-        }
-        if ((k0 | k1) == 0ull) {
-          Key128 old = dh_cas128(table + slot, Key128{0ull, 0ull}, Key128{ka, kb});
-          if ((old.a | old.b) == 0ull) { table[slot].haa = __longlong_as_double((long long)hh); atomicAdd(&table[slot].v, cv); ++contrib; break; }
-          if (old.a == ka && old.b == kb) { atomicAdd(&table[slot].v, cv); ++contrib; break; }
-        }
-        if (++slot == cap) slot = 0;
-        if (++probes > kProbeLimit) { *overflow = 1; break; }
-      }
-      max_probe = max(max_probe, probes);
-    }
-  }
-  u64 ct = contrib;
-  for (int o = 16; o > 0; o >>= 1) { ct += __shfl_xor_sync(0xffffffffu, ct, o); max_probe = max(max_probe, __shfl_xor_sync(0xffffffffu, max_probe, o)); }
-  if ((threadIdx.x & 31) == 0) { if (ct) atomicAdd(counters + 2, ct); atomicMax(counters + 3, (u64)max_probe); }
-}
-
-// H_DD from the determinant alone (no source, no update): E_core + sum_p h_pp + 1/2 sum_{p,q} [J or J-K], one thread
-__device__ __forceinline__ double diag_from_scratch(int n, const double* __restrict__ J, const double* __restrict__ JK,
-                                                    const double* __restrict__ hd, double e_core, u64 a, u64 b) {
-  double one = 0.0, two = 0.0;
-  for (int p = 0; p < n; ++p) {
-    bool pa = (a >> p) & 1ull, pb = (b >> p) & 1ull;
-    if (pa) one += hd[p];
-    if (pb) one += hd[p];
-    if (!pa && !pb) continue;
-    for (int q = 0; q < n; ++q) {
-      bool qa = (a >> q) & 1ull, qb = (b >> q) & 1ull;
-      if (pa && qa) two += JK[p * n + q];
-      if (pb && qb) two += JK[p * n + q];
-      if (pa && qb) two += J[p * n + q];
-      if (pb && qa) two += J[p * n + q];
-    }
-  }
-  return e_core + one + 0.5 * two;
 }
 
 // ---------------------------------------------------------------- reduce: sum_a v_a^2 / (E_S - H_aa), and clear the table
 __global__ void __launch_bounds__(256)
 pt2_scan_kernel(Slot* table, u64 cap, double e_s, int n, const double* __restrict__ J, const double* __restrict__ JK,
-                const double* __restrict__ hd, double e_core, double* __restrict__ part /* [grid][4]: sum, sum_abs, min_den, count */) {
+                const double* __restrict__ hd, double e_core, double small_den, double* __restrict__ part /* [grid][4]: sum, sum_abs, min_den, count */) {
   double sum = 0.0, sabs = 0.0, mden = INFINITY, cnt = 0.0;
   constexpr int V = 4;  // independent 32-byte loads in flight per thread
   const u64 stride = (u64)gridDim.x * blockDim.x;
@@ -557,7 +428,7 @@ pt2_scan_kernel(Slot* table, u64 cap, double e_s, int n, const double* __restric
           // The slot's H_aa came from the O(1) update of whichever source claimed it first, so it carries that source's
           // rounding (~1e-13).  Where the denominator is small enough to amplify that, take H_aa from the key alone:
           // the same value in every run and for every partitioning (a few externals in a million).
-          if (fabs(den) < kSmallDen) den = e_s - diag_from_scratch(n, J, JK, hd, e_core, x[k], y[k]);
+          if (fabs(den) < small_den) den = e_s - dh_diag_from_scratch(n, J, JK, hd, e_core, x[k], y[k]);
           double term = v * v / den;
           sum += term; sabs += fabs(term); mden = fmin(mden, fabs(den)); cnt += 1.0;
         }
@@ -665,7 +536,7 @@ __global__ void diagonals_kernel(int n, const double* __restrict__ J, const doub
                                  double e_core, const u64* __restrict__ dets, int64_t m, double* __restrict__ out) {
   int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
   if (t >= m) return;
-  out[t] = diag_from_scratch(n, J, JK, hd, e_core, dets[2 * t], dets[2 * t + 1]);
+  out[t] = dh_diag_from_scratch(n, J, JK, hd, e_core, dets[2 * t], dets[2 * t + 1]);
 }
 
 }  // namespace
@@ -687,62 +558,23 @@ static dh_status ensure_table(detham_ctx* c, int64_t slots) {
 // contributions share an external.
 struct ExpandOut { u64* keys; double* v; double* score; u64 cap; u64* cursor; };  // device buffers of expand mode
 
-// `est_pass` (0 = unknown): upper estimate of the contributions of one pass; with it, and a table far beyond L2, the passes run
-// binned (bin_batch / pt2_merge_kernel).
 static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, double eps2, int pbits, int64_t slots, bool adapt,
-                             double load, double* out, double* pilot = nullptr, const ExpandOut* ex = nullptr, double est_pass = 0.0) {
+                             double load, double* out, double* pilot = nullptr, const ExpandOut* ex = nullptr) {
   const int64_t nd = c->nd;
   dh_status st = ensure_table(c, slots); if (st != DH_OK) return st;
   Slot* table = reinterpret_cast<Slot*>(c->table);
   const HbLists* L = nullptr;
   st = dh_get_lists(c, pbits, &L); if (st != DH_OK) return st;
   EnumParams P = dh_make_params(c, L);
-  // launch shape: (warps per CTA, probes in flight per lane); DETHAM_PT2_VARIANT selects another one for tuning
-  using AccKernel = void (*)(EnumParams, const u64*, const double*, int64_t, double, unsigned, Slot*, u64, u64*, int*, Slot*, unsigned*,
-                             unsigned, int, int);
-  struct Variant { int warps, u; AccKernel k; };
-  // measured on B200 (profiles/r1_v2_summary.md): more warps per SM help (Cr2-shaped accumulate 1419 / 1084 / 1025 / 994 ms at
-  // 16 / 24 / 28 / 32 warps), more probes in flight per lane do not (16 warps x 2 probes: slower than x 1)
-  static const Variant variants[] = {{32, 1, pt2_accumulate_kernel<32, 1, false>}, {24, 1, pt2_accumulate_kernel<24, 1, false>},
-                                     {16, 1, pt2_accumulate_kernel<16, 1, false>}, {16, 2, pt2_accumulate_kernel<16, 2, false>}};
-  int vi = 0;
-  if (const char* e = getenv("DETHAM_PT2_VARIANT")) { int v = atoi(e); if (v >= 0 && v < (int)(sizeof(variants) / sizeof(variants[0]))) vi = v; }
-  int64_t want0 = (nd + 31) / 32;
-  const int grid32 = (int)(want0 < (int64_t)c->sm_count ? want0 : (int64_t)c->sm_count);
-  // binned mode: DETHAM_PT2_BINNED = 0 | 1 overrides the rule "table beyond 32 GB, estimate available, not expand / pilot"
-  // (measured: H2O-shaped, 15 GB table, 5 contributions per external: 17.5 ms binned against 12.8 ms direct; N2-shaped, 60 GB: 143 against 152 ms)
-  // regions of the table (DETHAM_PT2_BINS: tuning knob, 64..8192, a cap: the region size is a power of two of slots; each costs 4 bytes of the accumulate CTA's shared memory)
-  int max_bins = 2048;  // measured on Cr2-shaped (profiles/r1_v5_summary.md): accumulate 6174 / 5968 / 5941 / 6099 / 6947 ms at 512 / 1024 / 2048 / 4096 / 8192
-  if (const char* e = getenv("DETHAM_PT2_BINS")) { int v = atoi(e); if (v >= 64 && v <= 8192) max_bins = v; }
-  bool binned = !ex && !pilot && est_pass > 0.0 && slots * (int64_t)sizeof(Slot) > (32ll << 30) && grid32 == c->sm_count;
-  if (const char* e = getenv("DETHAM_PT2_BINNED")) { if (atoi(e) == 0) binned = false; else if (!ex && !pilot && est_pass > 0.0 && grid32 == c->sm_count) binned = true; }
-  if (binned) {
-    // the pool holds the records of one pass: 20 % head room over the estimate (an upper bound already) plus 64 records per
-    // segment; it is divided evenly over the pass's (bin, CTA) segments, and what does not fit a segment is probed directly
-    // (DETHAM_PT2_POOL_FRAC replaces the 1.2: a tuning knob, and the tests' way to make segments overflow)
-    double pool_frac = 1.2;
-    if (const char* e = getenv("DETHAM_PT2_POOL_FRAC")) { double v = atof(e); if (v >= 0.0 && v <= 8.0) pool_frac = v; }
-    const int64_t bytes = (int64_t)((est_pass * pool_frac + 64.0 * max_bins * grid32) * sizeof(Slot));
-    size_t free_b = 0, total_b = 0;
-    DH_CUDA(c, cudaMemGetInfo(&free_b, &total_b));
-    if (c->pool_bytes < bytes) {
-      if ((double)bytes > 0.95 * ((double)free_b + (double)c->pool_bytes)) binned = false;
-      else {
-        if (c->pool) cudaFree(c->pool);
-        c->pool = nullptr; c->pool_bytes = 0;
-        if (cudaMalloc(&c->pool, (size_t)bytes) != cudaSuccess) { cudaGetLastError(); binned = false; }
-        else c->pool_bytes = bytes;
-      }
-    }
-    if (binned && !c->pool_used) DH_CUDA(c, cudaMalloc(&c->pool_used, (size_t)8192 * c->sm_count * sizeof(unsigned)));
-  }
-  const int warps = (ex || binned) ? 32 : variants[vi].warps;
-  AccKernel acc_kernel = ex ? pt2_accumulate_kernel<32, 1, true> : (binned ? pt2_accumulate_kernel<32, 1, false, true> : variants[vi].k);
-  const size_t smem = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + warps * (sizeof(WarpScratch) + sizeof(FlatScratch)) +
-                      (binned ? max_bins * sizeof(unsigned) : 0);
+  // launch shape: 32 warps per CTA, one probe in flight per lane.  Measured on B200 (round 1): more warps per SM help
+  // (Cr2-shaped accumulate 1419 / 1084 / 1025 / 994 ms at 16 / 24 / 28 / 32 warps), more probes in flight per lane do not.
+  const int warps = 32;
+  auto acc_kernel = ex ? pt2_accumulate_kernel<32, 1, true> : pt2_accumulate_kernel<32, 1, false>;
+  const size_t smem = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + warps * (sizeof(WarpScratch) + sizeof(FlatScratch));
   DH_CUDA(c, cudaFuncSetAttribute(acc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int64_t want = (nd + warps - 1) / warps;
   const int grid = (int)(want < (int64_t)c->sm_count ? want : (int64_t)c->sm_count);
+  const double small_den = c->opt.small_den == 0.0 ? 1e-3 : (c->opt.small_den < 0.0 ? 0.0 : c->opt.small_den);
 
   const int nparts = 1 << pbits;
   const int sgrid_max = c->sm_count * 16;
@@ -766,26 +598,13 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
     DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 8 * sizeof(u64), c->stream));
     DH_TICK(c, 2);
     member_insert_kernel<<<(unsigned)((nd + 255) / 256), 256, 0, c->stream>>>(c->dets, nd, (unsigned)(nparts - 1), (unsigned)pass, table, (u64)cap, overflow);
-    int bin_shift = 0, nbins = 1;
-    unsigned seg_cap = 0;
-    if (binned) {  // bins = contiguous table regions of 2^shift slots, at most max_bins of them
-      while ((((cap - 1) >> bin_shift) + 1) > max_bins) ++bin_shift;
-      nbins = (int)(((cap - 1) >> bin_shift) + 1);
-      seg_cap = (unsigned)(c->pool_bytes / ((int64_t)nbins * grid * (int64_t)sizeof(Slot)));
-    }
-    acc_kernel<<<grid, warps * 32, smem, c->stream>>>(P, c->dets, psi, nd, eps2, (unsigned)pass, table, (u64)cap, c->dcount, overflow,
-                                                      reinterpret_cast<Slot*>(c->pool), c->pool_used, seg_cap, bin_shift, nbins);
-    if (binned) {
-      DH_CUDA(c, cudaGetLastError());
-      pt2_merge_kernel<<<c->sm_count * 2, 1024, 0, c->stream>>>(reinterpret_cast<const Slot*>(c->pool), c->pool_used, seg_cap, nbins, grid, table,
-                                                               (u64)cap, c->dcount, overflow, (c->n + 7) / 8);
-    }
+    acc_kernel<<<grid, warps * 32, smem, c->stream>>>(P, c->dets, psi, nd, eps2, (unsigned)pass, table, (u64)cap, c->dcount, overflow);
     DH_TICK(c, 3);
     if (ex && !pilot) {
       pt2_compact_kernel<<<sgrid, 256, 0, c->stream>>>(table, (u64)cap, ex->keys, ex->v, ex->score, ex->cap, ex->cursor);
       DH_CUDA(c, cudaMemsetAsync(results + 4 * pass, 0, 4 * sizeof(double), c->stream));
     } else {
-      pt2_scan_kernel<<<sgrid, 256, 0, c->stream>>>(table, (u64)cap, e_s, c->n, c->J, c->JK, c->hd, c->e_core, part);
+      pt2_scan_kernel<<<sgrid, 256, 0, c->stream>>>(table, (u64)cap, e_s, c->n, c->J, c->JK, c->hd, c->e_core, small_den, part);
       final_reduce4_kernel<<<1, 256, 0, c->stream>>>(part, sgrid, results + 4 * pass);
     }
     DH_CUDA(c, cudaGetLastError());
@@ -821,7 +640,8 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
   c->ctr.pt2_parts = nparts;
   c->ctr.pt2_max_probe = (int32_t)max_probe;
   c->ctr.pt2_table_slots = slots;
-  c->ctr.pt2_binned = binned ? 1 : 0;
+  c->ctr.pt2_binned = 0;
+  c->ctr.pt2_stream_bins = 0;
   c->ctr.pt2_sum_abs = sabs / norm2;
   c->ctr.pt2_min_abs_den = mden;
   c->ctr.ms_pt2_accum = ms_accum;
@@ -829,27 +649,37 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
   return DH_OK;
 }
 
+void dh_launch_final_reduce4(const double* part, int nblk, double* out, cudaStream_t stream) {
+  final_reduce4_kernel<<<1, 256, 0, stream>>>(part, nblk, out);
+}
+
 static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double eps2, double* out, const ExpandOut* ex) {
   const int64_t nd = c->nd;
   dh_status st;
-  double load = 0.5;  // target load factor of the table (DETHAM_PT2_LOAD overrides; tuning knob)
-  if (const char* e = getenv("DETHAM_PT2_LOAD")) { double v = atof(e); if (v >= 0.05 && v <= 0.9) load = v; }
+  const detham_pt2_options& opt = c->opt;
+  const double load = opt.table_load > 0.0 ? fmin(fmax(opt.table_load, 0.05), 0.9) : 0.5;  // target load factor of the HBM table
   // Random 32-byte accesses fall off a cliff once their footprint exceeds what the GPU's TLBs cover: measured on B200,
   // 36 G sectors/s up to 64 GB, 29 at 80 GB, 17 at 96 GB, 8.7 at 160 GB (profiles/r1_microbench.md).  More passes over a
   // smaller table beat fewer passes over a bigger one, so the table never exceeds this many bytes unless configured.
-  double max_table_gb = 60.0;
-  if (const char* e = getenv("DETHAM_PT2_MAX_TABLE_GB")) { double v = atof(e); if (v >= 1e-6 && v <= 4096.0) max_table_gb = v; }
+  const double max_table_gb = opt.max_table_gb > 0.0 ? opt.max_table_gb : 60.0;
+  // streamed organisation (pt2_stream.cu): chosen when the table organisation would need a table far beyond L2
+  const bool stream_ok = !ex && opt.mode != 1 && nd >= (int64_t)c->sm_count * 16;
 
   // ---- plan: partition count and table capacity
   int pbits = 0;
-  int64_t slots = c->cfg_table_slots;
-  const bool auto_parts = c->cfg_parts == 0, auto_slots = slots == 0;
+  int64_t slots = opt.table_slots;
+  const bool auto_parts = opt.n_parts == 0, auto_slots = slots == 0;
   c->ctr.ms_pt2_plan = 0.0;
-  if (!auto_parts) { while ((1 << pbits) < c->cfg_parts) ++pbits; }
+  if (!auto_parts) { while ((1 << pbits) < opt.n_parts) ++pbits; }
   int64_t max_slots = slots;
   std::vector<u64> hist;      // class histogram of the contributions (finest partition), empty when nothing was planned
   double hist_scale = 1.0;
-  if (auto_parts || auto_slots) {
+  auto max_class = [&](int pb) {  // upper estimate of the contributions of the fullest of 2^pb key partitions
+    u64 m = 0;
+    for (int cl = 0; cl < (1 << pb); ++cl) { u64 t = 0; for (int f = cl; f < kFine; f += (1 << pb)) t += hist[f]; if (t > m) m = t; }
+    return (double)m * hist_scale + 64.0;
+  };
+  if (auto_parts || auto_slots || stream_ok) {
     // class histogram of the contributions: exact for small inputs, else from every stride-th source (scaled, +10 %);
     // it only sizes the table - an underestimate is caught by the overflow flag and retried with more partitions
     const HbLists* L0 = nullptr;
@@ -871,19 +701,15 @@ static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double ep
     DH_CUDA(c, cudaMemcpyAsync(hist.data(), c->hist, kFine * sizeof(u64), cudaMemcpyDeviceToHost, c->stream));
     DH_CUDA(c, cudaStreamSynchronize(c->stream));
     c->ctr.ms_pt2_plan = dh_elapsed(c, 0, 1);
-    const double scale = stride == 1 ? 1.0 : 1.1 * (double)stride;
-    hist_scale = scale;
+    hist_scale = stride == 1 ? 1.0 : 1.1 * (double)stride;
+  }
+  if (auto_parts || auto_slots) {
     size_t free_b = 0, total_b = 0;
     DH_CUDA(c, cudaMemGetInfo(&free_b, &total_b));
-    max_slots = (int64_t)(((double)free_b + (double)c->table_slots * sizeof(Slot)) * 0.92 / sizeof(Slot));
+    max_slots = (int64_t)(((double)free_b + (double)c->table_slots * sizeof(Slot) + (double)c->pool_bytes) * 0.92 / sizeof(Slot));
     const int64_t tlb_slots = (int64_t)(max_table_gb * 1e9 / sizeof(Slot));
     if (max_slots > tlb_slots) max_slots = tlb_slots;
     if (!auto_slots) max_slots = slots;
-    auto max_class = [&](int pb) {
-      u64 m = 0;
-      for (int cl = 0; cl < (1 << pb); ++cl) { u64 s = 0; for (int f = cl; f < kFine; f += (1 << pb)) s += hist[f]; if (s > m) m = s; }
-      return (double)m * scale + 64.0;
-    };
     if (auto_parts) {
       // contributions bound the distinct keys from above; 0.9 of the slots at worst (all distinct) still terminates,
       // and the typical duplication keeps the real load well below that
@@ -896,38 +722,69 @@ static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double ep
       slots = need < max_slots ? need : max_slots;
     }
   }
+  // the table organisation would need this many bytes for one pass over everything; beyond 24 GB (or when asked to) stream
+  const bool stream = stream_ok && !hist.empty() && (opt.mode == 2 || max_class(0) / load * (double)sizeof(Slot) > 24e9);
   int64_t probe_parts = 0;
-  if (auto_parts && auto_slots && pbits >= 3) {  // worth it from 8 planned passes on: the probe costs 1/8 of one
+  double pilot_distinct = 0.0;  // distinct externals of one of 2^pilot_pp key slices
+  int pilot_pp = 0;
+  if ((auto_parts && auto_slots && pbits >= 3) || stream) {
     // The contribution count bounds the distinct externals from above, often by a wide margin (9 contributions per
     // external on N2-shaped |S| = 1e6), and every pass costs a list start-up per source.  Probe one slice of the key space
-    // 8x finer than a planned pass, count its distinct keys, and re-plan the passes from that.
-    const int pp = pbits + 3 < DH_MAX_PBITS ? pbits + 3 : DH_MAX_PBITS;
+    // 8x finer than a planned pass (table organisation), count its distinct keys, and re-plan from that.
+    int pp = pbits + 3 < DH_MAX_PBITS ? pbits + 3 : DH_MAX_PBITS;
+    int64_t pilot_slots = (pp - pbits == 3 && slots / 4 > 1024) ? slots / 4 : slots;  // 1/8 of the keys in 1/4 of the slots
+    if (stream) {  // a slice of about 1e8 contributions: cheap, and still tens of millions of distinct keys
+      pp = 0;
+      while (pp < DH_MAX_PBITS && max_class(pp) > 1.5e8) ++pp;
+      pilot_slots = (int64_t)(max_class(pp) / load) + 1024;
+    }
     double pilot[2] = {0.0, 0.0};
-    const int64_t pilot_slots = (pp - pbits == 3 && slots / 4 > 1024) ? slots / 4 : slots;  // 1/8 of the keys in 1/4 of the slots
     st = pt2_attempt(c, psi, e_s, eps2, pp, pilot_slots, false, load, out, pilot, ex);
     if (st == DH_OK) probe_parts = 1ll << pp;
     if (st == DH_OK && pilot[0] > 0.0) {
       c->ctr.ms_pt2_plan += pilot[1];
-      auto uniq_class = [&](int pb) { const double u = pilot[0] * (double)(1 << (pp - pb)); return 1.2 * u + 8.0 * sqrt(u) + 4096.0; };
-      int pb2 = 0;
-      while (pb2 < pbits && uniq_class(pb2) > load * (double)max_slots) ++pb2;
-      pbits = pb2;
-      int64_t need = (int64_t)(uniq_class(pbits) / load);
-      slots = need < max_slots ? need : max_slots;
-      if (slots < 1024) slots = 1024;
+      pilot_distinct = pilot[0]; pilot_pp = pp;
+      if (auto_parts && auto_slots) {
+        auto uniq_class = [&](int pb) { const double u = pilot[0] * (double)(1 << (pp - pb)); return 1.2 * u + 8.0 * sqrt(u) + 4096.0; };
+        int pb2 = 0;
+        while (pb2 < pbits && uniq_class(pb2) > load * (double)max_slots) ++pb2;
+        pbits = pb2;
+        int64_t need = (int64_t)(uniq_class(pbits) / load);
+        slots = need < max_slots ? need : max_slots;
+        if (slots < 1024) slots = 1024;
+      }
     } else if (st != DH_OK && st != DH_ETABLEFULL) {
       return st;
     }
   }
+  if (stream) {
+    // passes: one pass's records (32 bytes each, with head room) must fit the pool budget
+    if (c->table) { cudaFree(c->table); c->table = nullptr; c->table_slots = 0; }  // the pilot's table
+    size_t free_b = 0, total_b = 0;
+    DH_CUDA(c, cudaMemGetInfo(&free_b, &total_b));
+    const double budget = opt.stream_pool_gb > 0.0 ? opt.stream_pool_gb * 1e9 : 0.80 * ((double)free_b + (double)c->pool_bytes);
+    int sp = 0;
+    if (!auto_parts) { while ((1 << sp) < opt.n_parts) ++sp; }
+    else while (sp < 8 && max_class(sp) * 1.25 * (double)sizeof(Slot) > budget) ++sp;
+    double dscale = 1.15;
+    for (int tries = 0; tries < 6; ++tries) {
+      const double recs = max_class(sp);
+      double distinct = pilot_distinct > 0.0 ? fmin(recs, dscale * pilot_distinct * ldexp(1.0, pilot_pp - sp)) : recs;
+      const StreamPlan plan{sp, recs, distinct};
+      st = dh_pt2_stream(c, psi, e_s, eps2, plan, out);
+      if (st == DH_OK) { c->ctr.pt2_probe_parts = probe_parts; return st; }
+      if (st != DH_ETABLEFULL) break;  // DH_EINVAL / DH_ENOMEM: not a case for this organisation
+      if (distinct < recs) dscale *= 2.0;   // a region table filled up: the slice probed was not representative
+      else if (auto_parts && sp < 8) ++sp;  // a pool segment filled up
+      else break;
+    }
+    if (st != DH_ETABLEFULL && st != DH_EINVAL && st != DH_ENOMEM) return st;
+    if (opt.mode == 2) return st;  // asked for explicitly: report instead of switching organisation
+    if (c->pool) { cudaFree(c->pool); c->pool = nullptr; c->pool_bytes = 0; }  // make room for the table
+  }
   for (;;) {
     if (ex) DH_CUDA(c, cudaMemsetAsync(ex->cursor, 0, sizeof(u64), c->stream));
-    double est_pass = 0.0;  // contributions of the fullest class at this partition count (sizes the record pool of binned mode)
-    if (!hist.empty()) {
-      u64 m = 0;
-      for (int cl = 0; cl < (1 << pbits); ++cl) { u64 t = 0; for (int f = cl; f < kFine; f += (1 << pbits)) t += hist[f]; if (t > m) m = t; }
-      est_pass = (double)m * hist_scale + 64.0;
-    }
-    st = pt2_attempt(c, psi, e_s, eps2, pbits, slots, auto_slots && !ex, load, out, nullptr, ex, est_pass);
+    st = pt2_attempt(c, psi, e_s, eps2, pbits, slots, auto_slots && !ex, load, out, nullptr, ex);
     if (st == DH_OK) c->ctr.pt2_probe_parts = probe_parts;
     if (st != DH_ETABLEFULL || !auto_parts || pbits >= DH_MAX_PBITS) return st;
     ++pbits;  // the plan was too optimistic: halve the keys per pass and start over

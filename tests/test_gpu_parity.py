@@ -182,10 +182,11 @@ def test_cr2_shaped_masked(pkg, orc):
 
 
 def test_cr2_shaped_full_size_bench_configuration(pkg):
-    """The Cr2-shaped config at FULL size in the launch configuration bench.py times (auto-planned passes, 60 GB table cap).
+    """The Cr2-shaped config at FULL size in the launch configuration bench.py times (planned passes, streamed organisation).
     The oracle cannot run it (SURVEY.md 8(d) tier 3), so this checks what holds at any size: E_S against a library CSR
-    product of the same matrix, structural invariants of the counters, and PT2 / counts invariant under a different key
-    partitioning (forced 128 passes on a smaller table), whose per-class sums must add up to the same total."""
+    product of the same matrix, structural invariants of the counters, and PT2 / counts invariant under the other
+    organisation and another key partitioning (hash table in HBM, forced 128 passes), whose per-class sums must add up to the
+    same total."""
     import torch
     p = make_problem("cr2")
     ctx = _ctx(pkg, p)
@@ -208,10 +209,12 @@ def test_cr2_shaped_full_size_bench_configuration(pkg):
     a_parts = np.array(ctx.pt2_partials())
     assert ca["pt2_parts"] >= 32 and a_ext <= a_con <= ca["pt2_generated"]
     assert abs(a_parts.sum() - a_pt2) <= 1e-12 * ca["pt2_sum_abs"]
-    ctx.pt2_config(900_000_000, 128)
+    assert ca["pt2_binned"] == 2                                               # the planner streams this configuration
+    ctx.trim()
+    ctx.pt2_set_options(mode="table", table_slots=900_000_000, n_parts=128)
     b_pt2, b_ext, b_con = ctx.pt2(psi, e_s, p["eps2"])
     cb = ctx.counters()
-    assert cb["pt2_parts"] == 128 and (b_ext, b_con, cb["pt2_generated"]) == (a_ext, a_con, ca["pt2_generated"])
+    assert cb["pt2_binned"] == 0 and cb["pt2_parts"] == 128 and (b_ext, b_con, cb["pt2_generated"]) == (a_ext, a_con, ca["pt2_generated"])
     assert abs(a_pt2 - b_pt2) <= PT2_TOL * max(abs(a_pt2), 1e-3 * ca["pt2_sum_abs"])
     b_parts = np.array(ctx.pt2_partials())
     # class c of 64 partitions = classes c and c + 64 of 128 (low bits of the same partition word, reading Q14)
@@ -348,17 +351,16 @@ def test_solve_host_end_to_end(pkg, orc):
     ctx.close()
 
 
-def test_small_table_cap_forces_many_passes(pkg, orc, monkeypatch):
+def test_small_table_cap_forces_many_passes(pkg, orc):
     """The planner prefers more key partitions over a table beyond the TLB-safe size; with the cap forced down to
     0.5 MB the Tiny case is planned at >= 64 passes from the contribution count, probed (27 contributions per external),
     re-planned at fewer, larger-key passes, and must still agree."""
-    monkeypatch.setenv("DETHAM_PT2_MAX_TABLE_GB", "0.0005")
     p = make_problem("tiny")
     ctx = _ctx(pkg, p)
     psi = _psi(p)
     e_s = -30.0
     o = orc.pt2(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"], p["psi"], e_s, 1e-6)
-    ctx.pt2_config(0, 0)
+    ctx.pt2_set_options(max_table_gb=0.0005)
     g_pt2, g_ext, g_con = ctx.pt2(psi, e_s, 1e-6)
     c = ctx.counters()
     assert 4 <= c["pt2_parts"] <= 64 and c["pt2_table_slots"] <= 16000
@@ -367,12 +369,13 @@ def test_small_table_cap_forces_many_passes(pkg, orc, monkeypatch):
     ctx.close()
 
 
-def test_pt2_binned_mode(pkg, orc, monkeypatch):
-    """Binned mode of pt2 (records appended per table region, then merged region by region) is chosen
-    by the library only for tables beyond 32 GB; DETHAM_PT2_BINNED=1 forces it here on a case the oracle finishes.  Covered:
-    the default record pool, a pool too small for most records (DETHAM_PT2_POOL_FRAC: the overflow goes straight to the
-    table, the rest through the merge), a pool of 64 records per segment, forced multi-pass, a mostly empty pool
-    (masked psi: 300 of 6000 sources), and DETHAM_PT2_BINNED=0."""
+def test_pt2_streamed_organisation(pkg, orc):
+    """Streamed organisation of pt2 (records partitioned by key region in shared memory, written to per-CTA
+    segments, deduplicated region by region in L2-resident tables) is chosen by the library only when the table organisation
+    would need a table beyond 24 GB; mode = "stream" forces it here on a case the oracle finishes.  Covered: the planned
+    layout, 16 key partitions (class-by-class partials), region tables of 16 K slots (hundreds of regions, many ring
+    turns), 4096 regions, a loaded region table (0.9), a mostly idle generator (masked psi: 300 of 6000 sources), a record
+    pool too small for its segments (reported, and the context recovers), and the table organisation on the same context."""
     import torch
     p = make_problem("h2o", n_dets=6000)
     ctx = _ctx(pkg, p)
@@ -381,27 +384,38 @@ def test_pt2_binned_mode(pkg, orc, monkeypatch):
     o = orc.pt2(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"], p["psi"], e_s, p["eps2"], n_parts=16)
     assert o["n_contrib"] > 20_000_000
 
-    def check(o, psi, n_parts, binned):
-        ctx.pt2_config(0, n_parts)
+    def check(o, psi, organisation, **opts):
+        ctx.pt2_set_options(**opts)
         g_pt2, g_ext, g_con = ctx.pt2(psi, e_s, p["eps2"])
         c = ctx.counters()
-        assert c["pt2_binned"] == binned
+        rel = abs(g_pt2 - o["pt2"]) / abs(o["pt2"])
+        print(f"pt2 {opts}: organisation {c['pt2_binned']}, {c['pt2_parts']} passes x {c['pt2_stream_bins']} regions of "
+              f"{c['pt2_table_slots']} slots, relative error {rel:.2e}, cond {o['sum_abs'] / abs(o['pt2']):.1f}")
+        assert c["pt2_binned"] == organisation
         assert (g_ext, g_con) == (o["n_external"], o["n_contrib"]), (g_ext, g_con, o["n_external"], o["n_contrib"])
         assert abs(g_pt2 - o["pt2"]) <= PT2_TOL * max(abs(o["pt2"]), 1e-3 * o["sum_abs"]), (g_pt2, o["pt2"])
         assert abs(c["pt2_sum_abs"] - o["sum_abs"]) <= 1e-8 * o["sum_abs"]
-        if n_parts == 16:
+        if opts.get("n_parts") == 16:
             assert np.allclose(ctx.pt2_partials(), o["part_sums"], rtol=1e-8, atol=1e-12 * o["sum_abs"])
+        return c
 
-    monkeypatch.setenv("DETHAM_PT2_BINNED", "1")
-    for frac in ("0.05", "0", "1.2"):  # ascending pool size: the pool only grows within a context
-        monkeypatch.setenv("DETHAM_PT2_POOL_FRAC", frac)
-        check(o, psi, 0, 1)
-    check(o, psi, 16, 1)
+    c = check(o, psi, 2, mode="stream")
+    assert c["pt2_generated"] >= o["n_contrib"]
+    check(o, psi, 2, mode="stream", n_parts=16)
+    c = check(o, psi, 2, mode="stream", stream_ring_mb=1.5)
+    assert c["pt2_stream_bins"] > 100
+    check(o, psi, 2, mode="stream", stream_bins=4096)
+    check(o, psi, 2, mode="stream", stream_load=0.9)
     q, _ = _masked(p, 300, 3)
     om = orc.pt2(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"], q["psi"], e_s, p["eps2"], n_parts=16)
-    check(om, torch.from_numpy(q["psi"]).cuda(), 0, 1)
-    monkeypatch.setenv("DETHAM_PT2_BINNED", "0")
-    check(o, psi, 0, 0)
+    check(om, torch.from_numpy(q["psi"]).cuda(), 2, mode="stream", stream_pool_frac=12.0)
+    ctx.pt2_set_options(mode="stream", stream_pool_frac=0.05)
+    with pytest.raises(pkg.DethamError) as e:
+        ctx.pt2(psi, e_s, p["eps2"])
+    assert e.value.status == "DH_ETABLEFULL"
+    check(o, psi, 2, mode="stream")
+    check(o, psi, 0, mode="table")
+    check(o, psi, 0)  # the planner keeps a 1 GB table in HBM
     ctx.close()
 
 
