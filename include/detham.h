@@ -89,7 +89,7 @@ typedef struct {
   int32_t stream_bins;      /* streamed: key regions per pass (<= 4096); 0 = planned so that a region's distinct keys fit its table */
   int32_t reserved;
   double stream_ring_mb;    /* streamed: bytes of the three region tables together (they must stay in L2); 0 = 60 */
-  double stream_load;       /* streamed: target load factor of a region table; 0 = 0.6 */
+  double stream_load;       /* streamed: target load factor of a region table; 0 = 0.45 */
   double stream_pool_frac;  /* streamed: head room of the record pool over the planned estimate; 0 = 1.15 */
   double stream_pool_gb;    /* streamed: budget of the record pool; 0 = 80 % of the free device memory */
 } detham_pt2_options;

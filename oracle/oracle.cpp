@@ -332,26 +332,40 @@ void orc_pt2(int n, const double* h1, const double* eri_, double e_core, const u
       }
     }
   }
+  // each partition is sorted and summed on its own (they share no key); the partitions' results are then added in class order
+  const int np_run = part_end - part_begin;
+  std::vector<long double> psums(np_run, 0), pabs(np_run, 0);
+  std::vector<double> pmin(np_run, INFINITY);
+  std::vector<int64_t> pext(np_run, 0), pcon(np_run, 0);
+#pragma omp parallel for schedule(dynamic, 1)
   for (int p = part_begin; p < part_end; ++p) {
     auto& v = parts[p];
     for (int t = 0; t < nthreads; ++t) { v.insert(v.end(), local[t][p].begin(), local[t][p].end()); std::vector<std::pair<Det, double>>().swap(local[t][p]); }
-    n_contrib += (int64_t)v.size();
+    pcon[p - part_begin] = (int64_t)v.size();
     std::sort(v.begin(), v.end(), [](auto& x, auto& y) { return x.first < y.first || (x.first == y.first && x.second < y.second); });
-    long double psum = 0;
+    long double psum = 0, pa = 0;
+    double md = INFINITY;
+    int64_t ne = 0;
     for (size_t k = 0; k < v.size();) {
       size_t e = k;
       long double va = 0;
       while (e < v.size() && v[e].first == v[k].first) va += v[e++].second;
       double den = e_s - diagonal(I, v[k].first);
       long double t = va * va / den;
-      psum += t; total_abs += fabsl(t);
-      min_den = std::min(min_den, std::fabs(den));
-      ++n_ext;
+      psum += t; pa += fabsl(t);
+      md = std::min(md, std::fabs(den));
+      ++ne;
       k = e;
     }
-    if (part_sums) part_sums[p] = (double)(psum / norm2);
-    total += psum;
+    psums[p - part_begin] = psum; pabs[p - part_begin] = pa; pmin[p - part_begin] = md; pext[p - part_begin] = ne;
     std::vector<std::pair<Det, double>>().swap(v);
+  }
+  for (int p = part_begin; p < part_end; ++p) {
+    const int q = p - part_begin;
+    if (part_sums) part_sums[p] = (double)(psums[q] / norm2);
+    total += psums[q]; total_abs += pabs[q];
+    min_den = std::min(min_den, pmin[q]);
+    n_ext += pext[q]; n_contrib += pcon[q];
   }
   *pt2_out = (double)(total / norm2);
   if (n_external_out) *n_external_out = n_ext;

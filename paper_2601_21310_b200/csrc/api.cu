@@ -1,6 +1,7 @@
 // C ABI entry points (include/detham.h): argument checks, context lifetime, host<->device plumbing.
 #include <algorithm>
 #include <cmath>
+#include <cstdlib>
 #include <cstring>
 #include <new>
 #include <numeric>
@@ -20,7 +21,7 @@ bool is_device_ptr(const void* p) {
 void free_all(detham_ctx* c) {
   auto f = [](void* p) { if (p) cudaFree(p); };
   f(c->h1); f(c->eri); f(c->J); f(c->JK); f(c->hd);
-  for (auto& L : c->lists) { f(L.sub_off); f(L.val); f(L.ab); }
+  for (auto& L : c->lists) { f(L.sub_off); f(L.val); f(L.ab); f(L.stat); }
   f(c->dets_owned); f(c->psi_owned); f(c->shash_key); f(c->shash_idx); f(c->sbits);
   f(c->row_ptr); f(c->col); f(c->val); f(c->row_cnt); f(c->sp_row_ptr); f(c->sp_col); f(c->sp_val); f(c->phash_key); f(c->phash_idx); f(c->acol); f(c->aval); f(c->segs); f(c->table); f(c->pool); f(c->ring); f(c->sflags); f(c->red); f(c->dcount); f(c->hist);
   if (c->pinned) cudaFreeHost(c->pinned);
@@ -45,6 +46,7 @@ dh_status detham_create(detham_ctx** out, int n_orb, int n_alpha, int n_beta, co
   if (!c) return DH_ENOMEM;
   c->n = n_orb; c->na = n_alpha; c->nb = n_beta; c->e_core = e_core;
   c->stream = reinterpret_cast<cudaStream_t>(cuda_stream);
+  if (const char* e = getenv("DETHAM_DEBUG")) c->debug = e[0] == '1';  // the library's one environment switch
   auto fail = [&](dh_status s) { free_all(c); delete c; return s; };
   auto body = [&]() -> dh_status {
     DH_CUDA(c, cudaGetDevice(&c->device));
@@ -163,7 +165,7 @@ dh_status detham_trim(detham_ctx* c) {
   f(c->sflags); c->sflags_bytes = 0;
   for (int k = 1; k <= DH_MAX_PBITS; ++k) {
     HbLists& L = c->lists[k];
-    f(L.sub_off); f(L.val); f(L.ab);
+    f(L.sub_off); f(L.val); f(L.ab); f(L.stat);
     L.pbits = -1;
   }
   return DH_OK;

@@ -29,6 +29,8 @@ struct HbLists {
   int* sub_off = nullptr;       // device int32 [nseg * P + 1]
   double* val = nullptr;        // device fp64 [total]
   unsigned short* ab = nullptr; // device u16 [total]: a | (b << 8)
+  double* stat = nullptr;       // device fp64 [total]: the source-independent part of H_aa - H_ii for the entry's double
+                                // excitation, X_ij + X_ab - (J-K)_ia - (J-K)_jb - X_ib - X_ja with X = J-K (same spin) or J
 };
 
 struct detham_ctx {
@@ -58,7 +60,7 @@ struct detham_ctx {
   u64* shash_key = nullptr;   // device [shash_cap][2], open addressing, EMPTY = {0,0}
   int* shash_idx = nullptr;   // device [shash_cap]
   int64_t shash_cap = 0;
-  unsigned* sbits = nullptr;  // membership pre-filter: bit mulhi(z(D), sbits_n) set for every D in S
+  unsigned* sbits = nullptr;  // membership pre-filter (dh_maybe_member): sbits_n bits, two set per D in S
   int64_t sbits_n = 0;
 
   // CSR H_SS (a6)
@@ -100,6 +102,7 @@ struct detham_ctx {
   size_t sflags_bytes = 0;
   std::vector<cudaEvent_t> sev;  // per-pass timers of the streamed PT2
   detham_pt2_options opt{};   // detham_pt2_set_options (zero = defaults)
+  bool debug = false;         // DETHAM_DEBUG=1 at detham_create: planning decisions go to stderr
 
   // scratch
   double* red = nullptr;      // device reduction buffer
@@ -212,10 +215,14 @@ __device__ __forceinline__ int dh_shash_find(const u64* __restrict__ keys, const
   }
 }
 
-// membership pre-filter of the determinant store: false = certainly not in S (one 4-byte L2 load)
+// membership pre-filter of the determinant store: false = certainly not in S (one 8-byte L2 load).  A blocked Bloom filter:
+// `nbits` (a power of two, >= 64 per determinant) bits seen as 64-bit words; a determinant sets two bits of the word its
+// partition word selects.  About 0.1-0.2 % of the non-members pass, so a warp of candidates rarely diverges into the index.
+__device__ __forceinline__ u64 dh_filter_mask(u64 z) { return (1ull << ((z >> 10) & 63ull)) | (1ull << ((z >> 16) & 63ull)); }
+__device__ __forceinline__ u64 dh_filter_word(u64 nbits, u64 z) { return z >> (__clzll((long long)nbits) + 7); }
 __device__ __forceinline__ bool dh_maybe_member(const unsigned* __restrict__ bits, u64 nbits, u64 z) {
-  const u64 h = __umul64hi(z, nbits);
-  return (__ldg(bits + (h >> 5)) >> (h & 31)) & 1u;
+  const u64 m = dh_filter_mask(z);
+  return (__ldg(reinterpret_cast<const u64*>(bits) + dh_filter_word(nbits, z)) & m) == m;
 }
 
 #endif  // __CUDACC__

@@ -13,6 +13,7 @@ struct EnumParams {
   const int* sub_off;        // heat-bath lists
   const double* lval;
   const unsigned short* lab;
+  const double* lstat;       // per list entry: source-independent part of the diagonal update (HbLists::stat)
   const double* J;           // global copies staged into shared memory by cta_stage
   const double* JK;
   const double* hd;

@@ -29,10 +29,8 @@ __global__ void shash_insert_kernel(const u64* __restrict__ dets, int64_t nd, u6
   if (t >= nd) return;
   u64 a = dets[2 * t], b = dets[2 * t + 1];
   const u64 z = dh_zobrist(a, b, Z);
-  if (bits) {  // membership pre-filter: one bit per determinant (dh_maybe_member); the index of P has none
-    const u64 hb = __umul64hi(z, nbits);
-    atomicOr(bits + (hb >> 5), 1u << (hb & 31));
-  }
+  if (bits)  // membership pre-filter (dh_maybe_member): two bits of one 64-bit word per determinant; the index of P has none
+    atomicOr(reinterpret_cast<u64*>(bits) + dh_filter_word(nbits, z), dh_filter_mask(z));
   u64 slot = __umul64hi(z, cap);
   for (;;) {
     Key128 old = dh_cas128(keys + 2 * slot, Key128{0ull, 0ull}, Key128{a, b});
@@ -314,7 +312,7 @@ dh_status dh_build_shash(detham_ctx* c) {
     DH_CUDA(c, cudaMalloc(&c->shash_idx, cap * sizeof(int)));
     c->shash_cap = cap;
   }
-  int64_t nbits = 1 << 16;  // >= 64 bits per determinant: < 1.6 % of non-members pass the filter
+  int64_t nbits = 1 << 16;  // >= 64 bits per determinant: 0.1-0.2 % of the non-members pass the filter
   while (nbits < 64 * c->nd && nbits < (1ll << 28)) nbits <<= 1;
   if (nbits != c->sbits_n) {
     if (c->sbits) cudaFree(c->sbits);
@@ -333,7 +331,7 @@ dh_status dh_build_shash(detham_ctx* c) {
 static EnumParams make_params(detham_ctx* c, const HbLists* L) {
   EnumParams P;
   P.n = c->n; P.na = c->na; P.nb = c->nb; P.pbits = L->pbits; P.nss = c->n * (c->n - 1) / 2;
-  P.h1 = c->h1; P.eri = c->eri; P.sub_off = L->sub_off; P.lval = L->val; P.lab = L->ab;
+  P.h1 = c->h1; P.eri = c->eri; P.sub_off = L->sub_off; P.lval = L->val; P.lab = L->ab; P.lstat = L->stat;
   P.J = c->J; P.JK = c->JK; P.hd = c->hd; P.e_core = c->e_core;
   return P;
 }
@@ -381,13 +379,19 @@ static dh_status build_csr(detham_ctx* c, const CsrTarget& T, const double* psi 
     if (c->arena_cap < want_arena) {
       if (c->acol) cudaFree(c->acol);
       if (c->aval) cudaFree(c->aval);
-      if (c->segs) cudaFree(c->segs);
-      c->acol = nullptr; c->aval = nullptr; c->segs = nullptr; c->arena_cap = 0;
-      c->seg_cap = nd + want_arena / kBlk + 4096;
+      c->acol = nullptr; c->aval = nullptr; c->arena_cap = 0;
       DH_CUDA(c, cudaMalloc(&c->acol, want_arena * sizeof(int)));
       DH_CUDA(c, cudaMalloc(&c->aval, want_arena * sizeof(double)));
-      DH_CUDA(c, cudaMalloc(&c->segs, c->seg_cap * sizeof(Seg)));
       c->arena_cap = want_arena;
+    }
+    // segments: at least one per non-empty row plus one per arena block; sized on its own, because a context reused for a
+    // larger subspace (the outer loop of Alg. 1) can need more rows than the arena of an earlier build implies
+    const int64_t need_seg = nd + c->arena_cap / kBlk + 4096;
+    if (c->seg_cap < need_seg) {
+      if (c->segs) cudaFree(c->segs);
+      c->segs = nullptr; c->seg_cap = 0;
+      DH_CUDA(c, cudaMalloc(&c->segs, need_seg * sizeof(Seg)));
+      c->seg_cap = need_seg;
     }
     DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 16 * sizeof(u64), c->stream));
     DH_TICK(c, 0);

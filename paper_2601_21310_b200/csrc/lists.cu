@@ -26,8 +26,9 @@ __device__ __forceinline__ bool hb_less(double vx, unsigned mx, double vy, unsig
 // One CTA per segment: evaluate the segment's integrals, sort them in shared memory (bitonic, ascending comparators
 // only so the virtual padding stays at the tail), write values / (a,b) / class offsets.
 __global__ void hb_build_kernel(int n, int pbits, int nss, int Lss, int Los, const double* __restrict__ eri,
+                                const double* __restrict__ J, const double* __restrict__ JK,
                                 int* __restrict__ sub_off, double* __restrict__ val, unsigned short* __restrict__ ab,
-                                int N /* padded power of two */) {
+                                double* __restrict__ stat, int N /* padded power of two */) {
   extern __shared__ unsigned char smem_raw[];
   double* sv = reinterpret_cast<double*>(smem_raw);
   unsigned* sm = reinterpret_cast<unsigned*>(sv + N);
@@ -99,6 +100,10 @@ __global__ void hb_build_kernel(int n, int pbits, int nss, int Lss, int Los, con
   for (int t = threadIdx.x; t < L; t += blockDim.x) {
     val[base + t] = sv[t];
     ab[base + t] = (unsigned short)(sm[t] & 0xFFFFu);
+    // H_aa of the excited determinant = H_ii - U(i) - U(j) + U(a) + U(b) + this (the U are the source's: enumerate.cuh)
+    const int a = (int)(sm[t] & 0xFFu), b = (int)((sm[t] >> 8) & 0xFFu);
+    const double* X = fam < 2 ? JK : J;
+    stat[base + t] = X[i * n + j] + X[a * n + b] - JK[i * n + a] - JK[j * n + b] - X[i * n + b] - X[j * n + a];
   }
   for (int c = threadIdx.x; c < P; c += blockDim.x) {  // first index whose class >= c
     int lo = 0, hi = L;
@@ -134,12 +139,13 @@ dh_status dh_get_lists(detham_ctx* c, int pbits, const HbLists** out) {
   DH_CUDA(c, cudaMalloc(&H.sub_off, ((int64_t)nseg * P + 1) * sizeof(int)));
   DH_CUDA(c, cudaMalloc(&H.val, (total > 0 ? total : 1) * sizeof(double)));
   DH_CUDA(c, cudaMalloc(&H.ab, (total > 0 ? total : 1) * sizeof(unsigned short)));
+  DH_CUDA(c, cudaMalloc(&H.stat, (total > 0 ? total : 1) * sizeof(double)));
   int Lmax = Lss > Los ? Lss : Los;
   int N = 2;
   while (N < Lmax) N <<= 1;
   size_t smem = (size_t)N * (sizeof(double) + sizeof(unsigned));
   DH_CUDA(c, cudaFuncSetAttribute(hb_build_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
-  hb_build_kernel<<<nseg, 256, smem, c->stream>>>(n, pbits, nss, Lss, Los, c->eri, H.sub_off, H.val, H.ab, N);
+  hb_build_kernel<<<nseg, 256, smem, c->stream>>>(n, pbits, nss, Lss, Los, c->eri, c->J, c->JK, H.sub_off, H.val, H.ab, H.stat, N);
   DH_CUDA(c, cudaGetLastError());
   H.pbits = pbits;
   H.nseg = nseg;

@@ -1,6 +1,7 @@
 // pt2 (a8, a9): external-determinant deduplication in an HBM open-addressing hash on 128-bit keys and the
 // Epstein-Nesbet reduction (Eq. 13 second term; screening Eq. 14 / PAPER.md:219-227).
 #include <math.h>
+#include <stdio.h>
 #include <stdlib.h>
 
 #include "pt2_common.cuh"
@@ -148,7 +149,9 @@ __device__ __forceinline__ void probe_batch(ProbeCtx& pc, const u64 (&ka)[U], co
         if (k0[u] == ka[u] && k1[u] == kb[u]) {
           if (vb[u] != (u64)0x7ff8000000000001ull) { slot_add<kExpand>(pc.table + slot[u], cv[u]); ++pc.contrib; }
           pend &= ~(1u << u);
-        } else if ((k0[u] | k1[u]) == 0ull) {
+        } else if ((k0[u] | k1[u]) == 0ull || (k0[u] == 0ull) != (k1[u] == 0ull)) {
+          // empty - or one word still zero: the 256-bit load is not single-copy atomic against another thread's 128-bit
+          // claim, so a half-written key is possible in principle; the CAS below returns the whole key atomically either way
           cas |= 1u << u;
         } else if (++slot[u] == pc.cap) {
           slot[u] = 0;
@@ -168,8 +171,9 @@ __device__ __forceinline__ void probe_batch(ProbeCtx& pc, const u64 (&ka)[U], co
             if (!kExpand) pc.table[slot[u]].haa = meta_diag(pc, meta[u]);
             slot_add<kExpand>(pc.table + slot[u], cv[u]); ++pc.contrib;
             pend &= ~(1u << u);
-          } else if (k0[u] == ka[u] && k1[u] == kb[u]) {  // lost the race to the same key (never a member: those are pre-inserted)
-            slot_add<kExpand>(pc.table + slot[u], cv[u]); ++pc.contrib;
+          } else if (k0[u] == ka[u] && k1[u] == kb[u]) {  // lost the race to the same key, or came here through the half-zero check
+            const u64 vb2 = *reinterpret_cast<volatile u64*>(&pc.table[slot[u]].v);  // members were flagged before this kernel started
+            if (vb2 != (u64)0x7ff8000000000001ull) { slot_add<kExpand>(pc.table + slot[u], cv[u]); ++pc.contrib; }
             pend &= ~(1u << u);
           } else if (++slot[u] == pc.cap) {
             slot[u] = 0;
@@ -216,7 +220,9 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
     if (lane == 0) row = atomicAdd(counters, 1ull);
     row = __shfl_sync(0xffffffffu, row, 0);
     if ((int64_t)row >= nd) break;
-    if (*reinterpret_cast<volatile int*>(overflow)) break;
+    int ovf = 0;
+    if (lane == 0) ovf = *reinterpret_cast<volatile int*>(overflow);
+    if (__shfl_sync(0xffffffffu, ovf, 0)) break;  // warp-uniform by construction
     const double p = psi[row];
     if (p == 0.0) continue;  // reading Q6: a source with zero amplitude generates nothing
     const double tau = eps2 == 0.0 ? 0.0 : __ddiv_rn(eps2, fabs(p));
@@ -740,6 +746,7 @@ static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double ep
     }
     double pilot[2] = {0.0, 0.0};
     st = pt2_attempt(c, psi, e_s, eps2, pp, pilot_slots, false, load, out, pilot, ex);
+    if (c->debug) fprintf(stderr, "[detham] pt2 probe: 1 of %d key slices, %lld slots -> status %d, %.0f distinct, %.1f ms\n", 1 << pp, (long long)pilot_slots, (int)st, pilot[0], pilot[1]);
     if (st == DH_OK) probe_parts = 1ll << pp;
     if (st == DH_OK && pilot[0] > 0.0) {
       c->ctr.ms_pt2_plan += pilot[1];
@@ -772,6 +779,7 @@ static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double ep
       double distinct = pilot_distinct > 0.0 ? fmin(recs, dscale * pilot_distinct * ldexp(1.0, pilot_pp - sp)) : recs;
       const StreamPlan plan{sp, recs, distinct};
       st = dh_pt2_stream(c, psi, e_s, eps2, plan, out);
+      if (c->debug) fprintf(stderr, "[detham] pt2 streamed: %d passes, %.3g records and %.3g distinct keys per pass planned (pool budget %.1f GB) -> status %d\n", 1 << sp, recs, distinct, budget / 1e9, (int)st);
       if (st == DH_OK) { c->ctr.pt2_probe_parts = probe_parts; return st; }
       if (st != DH_ETABLEFULL) break;  // DH_EINVAL / DH_ENOMEM: not a case for this organisation
       if (distinct < recs) dscale *= 2.0;   // a region table filled up: the slice probed was not representative

@@ -9,13 +9,14 @@
 //                     value + phase, a5; O(1) diagonal update) and writes each bin's run with consecutive threads into
 //                     the CTA's private segment of that bin: whole lines leave the SM, not scattered sectors.
 //   pt2_merge_kernel  cooperative launch, one CTA per SM.  Bin b = the externals whose partition word falls into region b.
-//                     All warps insert the records of bin b into region table b mod 3 (128-bit CAS claim + fp64 RED, both
-//                     served by L2: the three tables are the only memory the kernel addresses by key), then reduce
-//                     v_a^2 / (E_S - H_aa) over region b-1 and clear it (Eq. 13 second term).  Warps hand over
+//                     All warps insert the records of bin b into region table b mod 4 (128-bit CAS claim + fp64 RED, both
+//                     served by L2: the four tables are the only memory the kernel addresses by key), then reduce
+//                     v_a^2 / (E_S - H_aa) over region b-2 and clear it (Eq. 13 second term).  Warps hand over
 //                     through two counters per bin; nothing is written back to HBM but four doubles per CTA.
 //
 // Members of S are dropped by the generator (membership filter + index of the determinant store, a1), so a record is a
 // contribution to an external.  Singles (reading Q5) are evaluated by the walker and written straight into their segment.
+#include <stdio.h>
 #include <stdlib.h>
 
 #include <algorithm>
@@ -28,10 +29,18 @@ namespace {
 
 constexpr int kGenWarps = 16;
 constexpr int kPairChunk = 64;   // occupied pairs per phase-A chunk
+constexpr int kExpandU = 2;      // staged references a thread expands together
+constexpr int kWalkU = 2;        // batches of 32 list entries a warp has in flight (their L2 loads overlap)
 constexpr int kMaxSrcSlots = 4;  // sources a warp can have staged references of at one time
 constexpr int kMaxBins = 4096;
-constexpr int kRing = 3;         // region tables: merging b, reducing b-1, cleared for b+1
-constexpr int kMergeWarps = 16;
+constexpr int kRing = 4;         // region tables in flight
+constexpr int kLag = 2;          // a warp reduces region b - kLag after merging region b: two regions of slack on either side, so
+                                 // that no warp waits for the slowest one of the region it has just finished
+constexpr int kMergeWarps = 8;    // warps per merge CTA = units per block of the ordered work list
+constexpr int kMergeCtasPerSm = 4;
+constexpr int kUnitRec = 256;    // records of one merge unit (one warp)
+constexpr int kUnitSlots = 512;  // table slots of one reduce unit (one warp)
+constexpr int kMergeU = 2;       // records a lane has in flight (their CAS round trips overlap)
 
 // ---------------------------------------------------------------------------------------------- shared-memory layout
 struct GenLayout {
@@ -44,7 +53,7 @@ __host__ __device__ inline unsigned al16(unsigned x) { return (x + 15u) & ~15u; 
 __host__ __device__ inline GenLayout gen_layout(int n, int pbits, int npairs, int W, int K, int B, int N) {
   GenLayout L;
   unsigned o = 0;
-  L.tables = o; o = al16(o + (unsigned)dh_cta_table_bytes(n));
+  L.tables = o; o = al16(o + (unsigned)(n + 128) * 8u);  // h_pp and the key-partition words; J, J-K stay in L2 (read by rows)
   L.omask = o; o = al16(o + 2u * (1u << pbits) * 8u);
   L.ptab = o; o = al16(o + (unsigned)npairs * 2u);
   L.slot_stride = (unsigned)(2 * n + 6) * 8u;
@@ -60,7 +69,7 @@ __host__ __device__ inline GenLayout gen_layout(int n, int pbits, int npairs, in
   L.warp0 = o; o += (unsigned)W * w;
   L.cnt = o; o = al16(o + (unsigned)(B + 1) * 4u);
   L.used = o; o = al16(o + (unsigned)B * 4u);
-  const unsigned NS = (unsigned)(N + 32 * W);
+  const unsigned NS = (unsigned)(N + 32 * kWalkU * W);
   L.rec = o; o = al16(o + NS * 8u);
   L.rank = o; o = al16(o + NS * 2u);
   L.order = o; o = al16(o + NS * 2u);
@@ -69,10 +78,7 @@ __host__ __device__ inline GenLayout gen_layout(int n, int pbits, int npairs, in
   return L;
 }
 
-// staged reference: bin 12 | list entry 25 | i 6 | j 6 | fam 2 | source slot 3 | warp 5
-__device__ __forceinline__ u64 pack_ref(unsigned bin, unsigned k, unsigned i, unsigned j, unsigned fam, unsigned slot, unsigned warp) {
-  return (u64)bin | ((u64)k << 12) | ((u64)i << 37) | ((u64)j << 43) | ((u64)fam << 49) | ((u64)slot << 51) | ((u64)warp << 54);
-}
+// staged reference (8 bytes): bin 12 | list entry 25 | i 6 | j 6 | fam 2 | source slot 3 | warp 5
 
 // bit t of the result = parity of the electrons of w below orbital t
 __device__ __forceinline__ u64 prefix_parity(u64 w) {
@@ -101,6 +107,7 @@ struct GenParams {
   u64* counters;  // [0] next row [1] generated (members included) [2] contributions
   int* overflow;
   int stage_n, nslots, npairs;
+  u64* prof;  // debug: per-CTA cycles of the phases [walk (thread 0's own), walk barrier, sort, expand, advance, rounds], or NULL
 };
 
 __device__ __forceinline__ int ld_shared_volatile(const int* p) { return *reinterpret_cast<const volatile int*>(p); }
@@ -113,7 +120,12 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
   const unsigned pmask = (unsigned)NP - 1u;
   const int B = G.nbins, N = G.stage_n, K = G.nslots, npairs = G.npairs;
   const GenLayout L = gen_layout(n, P.pbits, npairs, kGenWarps, K, B, N);
-  CtaTables T = dh_cta_stage(P, smem + L.tables);
+  CtaTables T;
+  T.J = const_cast<double*>(P.J); T.JK = const_cast<double*>(P.JK);  // global (L2): only the per-source U vectors read them
+  T.hd = reinterpret_cast<double*>(smem + L.tables);
+  T.Z = reinterpret_cast<u64*>(T.hd + n);
+  for (int t = threadIdx.x; t < n; t += blockDim.x) T.hd[t] = P.hd[t];
+  for (int t = threadIdx.x; t < 128; t += blockDim.x) T.Z[t] = dh_zword(t);
   u64* omask = reinterpret_cast<u64*>(smem + L.omask);            // [2][NP]: orbitals of spin s whose class word is c
   unsigned short* ptab = reinterpret_cast<unsigned short*>(smem + L.ptab);  // pair q -> fam << 12 | x << 6 | y (positions in occ)
   unsigned* cnt = reinterpret_cast<unsigned*>(smem + L.cnt);
@@ -127,7 +139,7 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
   const unsigned lt = (1u << lane) - 1u;
   const unsigned full = 0xffffffffu;
   const int nAA = na * (na - 1) / 2, nBB = nb * (nb - 1) / 2;
-  const int NS = N + 32 * kGenWarps;
+  const int NS = N + 32 * kWalkU * kGenWarps;
 
   for (int t = tid; t < 2 * NP; t += nthr) omask[t] = 0ull;
   for (int t = tid; t <= B; t += nthr) cnt[t] = 0u;
@@ -173,7 +185,9 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
   double psi_v = 0.0, tau = 0.0, e0 = 0.0;
   u64 gen_total = 0, contrib_total = 0;
 
+  long long pc0 = 0, pacc[6] = {0, 0, 0, 0, 0, 0};
   for (;;) {
+    if (G.prof && tid == 0) pc0 = clock64();
     // =================================================================== walk: stage references until the buffer is full
     unsigned touched = phase != 0 ? (1u << cur_slot) : 0u;  // slots that staged references of this round point into
     while (ld_shared_volatile(&ctrl[0]) + ld_shared_volatile(&ctrl[3]) < N) {
@@ -213,8 +227,9 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
         double* U = reinterpret_cast<double*>(wb + (unsigned)cur_slot * L.slot_stride);
         for (int p = lane; p < n; p += 32) {
           double ua = T.hd[p], ub = T.hd[p];
-          for (int k = 0; k < na; ++k) { const int q = occ[0][k]; ua += T.JK[p * n + q]; ub += T.J[p * n + q]; }
-          for (int k = 0; k < nb; ++k) { const int q = occ[1][k]; ua += T.J[p * n + q]; ub += T.JK[p * n + q]; }
+          // J and J-K are symmetric (bit for bit: one packed integral each way): row q read by consecutive lanes
+          for (int k = 0; k < na; ++k) { const int q = occ[0][k]; ua += __ldg(T.JK + q * n + p); ub += __ldg(T.J + q * n + p); }
+          for (int k = 0; k < nb; ++k) { const int q = occ[1][k]; ua += __ldg(T.J + q * n + p); ub += __ldg(T.JK + q * n + p); }
           U[p] = ua; U[n + p] = ub;
         }
         __syncwarp();
@@ -271,7 +286,7 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
               const u64 z = zsrc ^ T.Z[64 * s + i] ^ T.Z[64 * s + a];
               ok = true;
               const double* U = reinterpret_cast<const double*>(wb + (unsigned)cur_slot * L.slot_stride);
-              haa = e0 - U[s * n + i] + U[s * n + a] - T.JK[i * n + a];
+              haa = e0 - U[s * n + i] + U[s * n + a] - __ldg(T.JK + i * n + a);
               cv = v * psi_v;
               bin = __umulhi((unsigned)(z >> 32), (unsigned)B);
               // member of S?  (filter first: one 4-byte load settles > 98 % of the non-members)
@@ -333,7 +348,7 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
               }
             }
             len = lo - beg;
-            pm = ((unsigned)fam << 12) | ((unsigned)i << 6) | (unsigned)j;
+            pm = ((unsigned)fam << 12) | ((unsigned)j << 6) | (unsigned)i;  // same field order as the staged reference
           }
           const unsigned m = __ballot_sync(full, len > 0);
           int x = len;
@@ -354,61 +369,91 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
         phase = 3;
         continue;
       }
-      // ---- phase B: 32 entries of the concatenated kept prefixes; stage the valid, non-member ones
+      // ---- phase B: kWalkU x 32 entries of the concatenated kept prefixes; stage the valid, non-member ones.  Three steps so
+      // that the list loads of all batches, then the filter loads of all batches, are in flight together.
       {
-        const int pe = (qcur + lane < pcnt) ? pref[qcur + lane + 1] - t0 : 0x7fffffff;  // end of pair qcur+lane, relative
-        const unsigned bm = __reduce_or_sync(full, pe < 32 ? (1u << pe) : 0u);
-        const int adv = __popc(__ballot_sync(full, pe <= 32));
-        const int myq = qcur + __popc(bm & ((2u << lane) - 1u));
-        qcur += adv;
-        const int t = t0 + lane;
-        bool ok = false;
-        u64 ref = 0;
-        unsigned bin = 0;
-        if (t < TT) {
-          const int k = pbeg[myq] + (t - pref[myq]);
-          const unsigned pm = pmeta[myq];
-          const unsigned ab = __ldg(P.lab + k);
-          const int a = (int)(ab & 0xFFu), b = (int)(ab >> 8);
-          const int fam = (int)(pm >> 12), i = (int)((pm >> 6) & 63u), j = (int)(pm & 63u);
-          u64 ka = da, kb = db, z;
-          if (fam < 2) {
-            const u64 w = fam ? db : da;
-            ok = !((w >> a) & 1ull) && !((w >> b) & 1ull);
-            const u64 nw = (w ^ (1ull << i) ^ (1ull << j)) | (1ull << a) | (1ull << b);
-            if (fam == 0) ka = nw; else kb = nw;
-            z = zq[myq] ^ T.Z[64 * fam + a] ^ T.Z[64 * fam + b];
-          } else {
-            ok = !((da >> a) & 1ull) && !((db >> b) & 1ull);
-            ka = (da ^ (1ull << i)) | (1ull << a);
-            kb = (db ^ (1ull << j)) | (1ull << b);
-            z = zq[myq] ^ T.Z[a] ^ T.Z[64 + b];
+        bool ok[kWalkU];
+        int kk[kWalkU], mq[kWalkU];
+        unsigned abv[kWalkU];
+#pragma unroll
+        for (int u = 0; u < kWalkU; ++u) {
+          ok[u] = false; kk[u] = 0; mq[u] = 0; abv[u] = 0u;
+          const int tt = t0 + 32 * u;
+          if (tt < TT) {  // warp-uniform
+            const int pe = (qcur + lane < pcnt) ? pref[qcur + lane + 1] - tt : 0x7fffffff;  // end of pair qcur+lane, relative
+            const unsigned bm = __reduce_or_sync(full, pe < 32 ? (1u << pe) : 0u);
+            const int adv = __popc(__ballot_sync(full, pe <= 32));
+            const int myq = qcur + __popc(bm & ((2u << lane) - 1u));
+            qcur += adv;
+            const int t = tt + lane;
+            if (t < TT) {
+              ok[u] = true; mq[u] = myq;
+              kk[u] = pbeg[myq] + (t - pref[myq]);
+              abv[u] = __ldg(P.lab + kk[u]);
+            }
           }
-          if (ok) {
+        }
+        u64 zv[kWalkU], fw[kWalkU];
+        unsigned pmv[kWalkU];
+#pragma unroll
+        for (int u = 0; u < kWalkU; ++u) {
+          zv[u] = 0ull; fw[u] = 0ull; pmv[u] = 0u;
+          if (ok[u]) {
+            const unsigned pm = pmeta[mq[u]];
+            const int a = (int)(abv[u] & 0xFFu), b = (int)(abv[u] >> 8);
+            const unsigned fam = pm >> 12;
+            const unsigned si = fam == 1u, sj = fam != 0u;  // spin of (i, a) and of (j, b)
+            const u64 wa = si ? db : da, wb2 = sj ? db : da;
+            ok[u] = !(((wa >> a) | (wb2 >> b)) & 1ull);
+            if (ok[u]) {
+              const u64 z = zq[mq[u]] ^ T.Z[64 * si + a] ^ T.Z[64 * sj + b];
+              zv[u] = z; pmv[u] = pm;
+              fw[u] = __ldg(reinterpret_cast<const u64*>(G.sbits) + dh_filter_word(G.sbits_n, z));
+            }
+          }
+        }
+        unsigned msk[kWalkU];
+        int nstage = 0;
+#pragma unroll
+        for (int u = 0; u < kWalkU; ++u) {
+          if (ok[u]) {
             gen_total += 1;
-            if (dh_maybe_member(G.sbits, G.sbits_n, z) && dh_shash_find(G.shash_key, G.shash_idx, G.shash_cap, ka, kb, z) >= 0) ok = false;
-            bin = __umulhi((unsigned)(z >> 32), (unsigned)B);
-            ref = pack_ref(bin, (unsigned)k, (unsigned)i, (unsigned)j, (unsigned)fam, (unsigned)cur_slot, (unsigned)warp);
+            const u64 fm = dh_filter_mask(zv[u]);
+            if ((fw[u] & fm) == fm) {  // rare: look the key up in the index of S
+              const unsigned pm = pmv[u], fam = pm >> 12;
+              const unsigned si = fam == 1u, sj = fam != 0u;
+              const u64 bia = (1ull << (pm & 63u)) | (1ull << (abv[u] & 0xFFu)), bjb = (1ull << ((pm >> 6) & 63u)) | (1ull << (abv[u] >> 8));
+              const u64 ka = da ^ ((si ? 0ull : bia) | (sj ? 0ull : bjb)), kb = db ^ ((si ? bia : 0ull) | (sj ? bjb : 0ull));
+              if (dh_shash_find(G.shash_key, G.shash_idx, G.shash_cap, ka, kb, zv[u]) >= 0) ok[u] = false;
+            }
           }
+          msk[u] = __ballot_sync(full, ok[u]);
+          nstage += __popc(msk[u]);
         }
-        const unsigned m = __ballot_sync(full, ok);
-        if (m) {
+        if (nstage) {
           int base = 0;
-          if (lane == 0) base = atomicAdd(&ctrl[0], __popc(m));
+          if (lane == 0) base = atomicAdd(&ctrl[0], nstage);
           base = __shfl_sync(full, base, 0);
-          if (ok) {
-            const int idx = base + __popc(m & lt);
-            rec[idx] = ref;
-            rnk[idx] = (unsigned short)atomicAdd(&cnt[bin], 1u);
-            contrib_total += 1;
+#pragma unroll
+          for (int u = 0; u < kWalkU; ++u) {
+            if (ok[u]) {
+              const int idx = base + __popc(msk[u] & lt);
+              const unsigned bin = __umulhi((unsigned)(zv[u] >> 32), (unsigned)B);
+              rec[idx] = (u64)bin | ((u64)(unsigned)kk[u] << 12) | ((u64)(pmv[u] & 0x3FFFu) << 37) | ((u64)cur_slot << 51) | ((u64)warp << 54);
+              rnk[idx] = (unsigned short)atomicAdd(&cnt[bin], 1u);
+              contrib_total += 1;
+            }
+            base += __popc(msk[u]);
           }
         }
-        t0 += 32;
+        t0 += 32 * kWalkU;
         if (t0 >= TT) { qb += kPairChunk; phase = 2; }
       }
     }
     if (out_of_rows && phase == 0 && !reported) { reported = true; if (lane == 0) atomicAdd(&ctrl[1], 1); }
+    if (G.prof && tid == 0) { const long long t = clock64(); pacc[0] += t - pc0; pc0 = t; }
     __syncthreads();
+    if (G.prof && tid == 0) { const long long t = clock64(); pacc[1] += t - pc0; pc0 = t; }
     const int staged = ctrl[0];
     const bool all_done = ctrl[1] == kGenWarps;
 
@@ -436,50 +481,65 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
     for (int idx = tid; idx < staged; idx += nthr) order[cnt[(unsigned)rec[idx] & 0xFFFu] + rnk[idx]] = (unsigned short)idx;
     __syncthreads();
 
+    if (G.prof && tid == 0) { const long long t = clock64(); pacc[2] += t - pc0; pc0 = t; }
     // =================================================================== expand in bin order and write the runs
-    for (int t = tid; t < total; t += nthr) {
-      const unsigned idx = order[t];
-      if (idx == 0xFFFFu) continue;  // a single: already written by the walker
-      order[t] = 0xFFFFu;
-      const u64 r = rec[idx];
-      const unsigned bin = (unsigned)r & 0xFFFu;
-      const unsigned k = (unsigned)(r >> 12) & 0x1FFFFFFu;
-      const int i = (int)(r >> 37) & 63, j = (int)(r >> 43) & 63, fam = (int)(r >> 49) & 3;
-      const unsigned slot = (unsigned)(r >> 51) & 7u, w = (unsigned)(r >> 54) & 31u;
-      const double* U = reinterpret_cast<const double*>(smem + L.warp0 + w * L.warp_stride + slot * L.slot_stride);
-      const u64* sw = reinterpret_cast<const u64*>(U + 2 * n);
-      const u64 sda = sw[0], sdb = sw[1];
-      const double spsi = reinterpret_cast<const double*>(sw)[4], se0 = reinterpret_cast<const double*>(sw)[5];
-      double v = __ldg(P.lval + k);
-      const unsigned ab = __ldg(P.lab + k);
-      const int a = (int)(ab & 0xFFu), b = (int)(ab >> 8);
-      u64 ka = sda, kb = sdb;
-      double haa;
-      unsigned par;
-      if (fam < 2) {
-        const u64 wq = fam ? sdb : sda;
-        const u64 pp = sw[2 + fam];
-        const u64 nw = (wq ^ (1ull << i) ^ (1ull << j)) | (1ull << a) | (1ull << b);
-        if (fam == 0) ka = nw; else kb = nw;
-        // a+_a a+_b a_j a_i = (a+_b a_j)(a+_a a_i): phase(i->a on w) * phase(j->b on w with i->a applied)   (reading Q1)
-        par = par_between(pp, i, a) ^ par_between(pp, j, b) ^ strictly_between(i, j, b) ^ strictly_between(a, j, b);
-        const double* Us = U + fam * n;
-        haa = se0 - Us[i] - Us[j] + Us[a] + Us[b] + T.JK[i * n + j] + T.JK[a * n + b] - T.JK[i * n + a] - T.JK[i * n + b] -
-              T.JK[j * n + a] - T.JK[j * n + b];
-      } else {
-        ka = (sda ^ (1ull << i)) | (1ull << a);
-        kb = (sdb ^ (1ull << j)) | (1ull << b);
-        par = par_between(sw[2], i, a) ^ par_between(sw[3], j, b);
-        haa = se0 - U[i] - U[n + j] + U[a] + U[n + b] + T.J[i * n + j] + T.J[a * n + b] - T.JK[i * n + a] - T.JK[j * n + b] -
-              T.J[i * n + b] - T.J[j * n + a];
+    for (int t0 = tid; t0 < total; t0 += nthr * kExpandU) {
+      // kExpandU references per thread: their list loads (value, orbital pair: L2) are issued before any is used
+      u64 rr[kExpandU];
+      double vv[kExpandU], sst[kExpandU];
+      unsigned abv[kExpandU];
+      bool live[kExpandU];
+#pragma unroll
+      for (int u = 0; u < kExpandU; ++u) {
+        const int t = t0 + u * nthr;
+        live[u] = false; rr[u] = 0ull; vv[u] = 0.0; sst[u] = 0.0; abv[u] = 0u;
+        if (t < total) {
+          const unsigned idx = order[t];
+          if (idx != 0xFFFFu) {  // 0xFFFF: a single, already written by the walker
+            order[t] = 0xFFFFu;
+            live[u] = true;
+            rr[u] = rec[idx];
+            const unsigned k = (unsigned)(rr[u] >> 12) & 0x1FFFFFFu;
+            vv[u] = __ldg(P.lval + k);
+            sst[u] = __ldg(P.lstat + k);
+            abv[u] = __ldg(P.lab + k);
+          }
+        }
       }
-      if (par) v = -v;
-      const double cv = v * spsi;
-      const unsigned pos = used[bin] + ((unsigned)t - cnt[bin]);
-      if (pos < G.seg_cap) dh_st256(my_pool + (size_t)bin * seg_stride + pos, ka, kb, (u64)__double_as_longlong(cv), (u64)__double_as_longlong(haa));
-      else *G.overflow = 1;
+#pragma unroll
+      for (int u = 0; u < kExpandU; ++u) {
+        if (!live[u]) continue;
+        const int t = t0 + u * nthr;
+        const u64 r = rr[u];
+        const unsigned bin = (unsigned)r & 0xFFFu;
+        const int i = (int)(r >> 37) & 63, j = (int)(r >> 43) & 63, fam = (int)(r >> 49) & 3;
+        const unsigned slot = (unsigned)(r >> 51) & 7u, w = (unsigned)(r >> 54) & 31u;
+        const double* U = reinterpret_cast<const double*>(smem + L.warp0 + w * L.warp_stride + slot * L.slot_stride);
+        const u64* sw = reinterpret_cast<const u64*>(U + 2 * n);
+        const u64 sda = sw[0], sdb = sw[1];
+        const double spsi = reinterpret_cast<const double*>(sw)[4], se0 = reinterpret_cast<const double*>(sw)[5];
+        double v = vv[u];
+        const int a = (int)(abv[u] & 0xFFu), b = (int)(abv[u] >> 8);
+        // one code path for the three families: fam 0 = alpha-alpha, 1 = beta-beta (i<j -> a<b in one spin), 2 = (i alpha -> a, j beta -> b)
+        const unsigned si = fam == 1, sj = fam != 0;  // spin of (i, a) and of (j, b)
+        const u64 bia = (1ull << i) | (1ull << a), bjb = (1ull << j) | (1ull << b);
+        const u64 ka = sda ^ ((si ? 0ull : bia) | (sj ? 0ull : bjb)), kb = sdb ^ ((si ? bia : 0ull) | (sj ? bjb : 0ull));
+        // reading Q1: a same-spin double is a+_a a+_b a_j a_i = (a+_b a_j)(a+_a a_i): phase(i->a on w) * phase(j->b on w with
+        // i->a applied); an alpha-beta double is the product of its two single phases
+        unsigned par = par_between(sw[2 + si], i, a) ^ par_between(sw[2 + sj], j, b);
+        if (fam < 2) par ^= strictly_between(i, j, b) ^ strictly_between(a, j, b);
+        const double* Ui = U + si * n;
+        const double* Uj = U + sj * n;
+        const double haa = se0 - Ui[i] - Uj[j] + Ui[a] + Uj[b] + sst[u];
+        if (par) v = -v;
+        const double cv = v * spsi;
+        const unsigned pos = used[bin] + ((unsigned)t - cnt[bin]);
+        if (pos < G.seg_cap) dh_st256(my_pool + (size_t)bin * seg_stride + pos, ka, kb, (u64)__double_as_longlong(cv), (u64)__double_as_longlong(haa));
+        else *G.overflow = 1;
+      }
     }
     __syncthreads();
+    if (G.prof && tid == 0) { const long long t = clock64(); pacc[3] += t - pc0; pc0 = t; }
     // =================================================================== advance the segment fill levels, reset the round
     {
       const int per = (B + nthr - 1) / nthr;
@@ -492,8 +552,10 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
       if (tid == 0) { cnt[B] = 0u; ctrl[0] = 0; ctrl[3] = 0; }
     }
     __syncthreads();
+    if (G.prof && tid == 0) { const long long t = clock64(); pacc[4] += t - pc0; pacc[5] += 1; }
     if (all_done && total == 0) break;
   }
+  if (G.prof && tid == 0) for (int k = 0; k < 6; ++k) G.prof[6 * blockIdx.x + k] = (u64)pacc[k];
   for (int b = tid; b < B; b += nthr) G.used_out[(size_t)b * gridDim.x + blockIdx.x] = min(used[b], G.seg_cap);
   u64 g = gen_total, ct = contrib_total;
   for (int o = 16; o > 0; o >>= 1) { g += __shfl_xor_sync(full, g, o); ct += __shfl_xor_sync(full, ct, o); }
@@ -511,15 +573,41 @@ struct MergeParams {
   double e_s; int n; const double* J; const double* JK; const double* hd; double e_core; double small_den;
   double* part;  // [gridDim.x][4]: sum, sum_abs, min_den, count
   int* overflow;
+  u64* ticket;  // next unit of the ordered work list
 };
+
+// L2 eviction policies (createpolicy): the region tables are the only reused lines of the merge - evict_last; the records are
+// read once - evict_first.  Measured without them (ncu, round 2): 48 % of the CAS and 40 % of the RED sectors missed L2.
+__device__ __forceinline__ u64 l2_policy_evict_last() {
+  u64 p;
+  asm volatile("createpolicy.fractional.L2::evict_last.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ u64 l2_policy_evict_first() {
+  u64 p;
+  asm volatile("createpolicy.fractional.L2::evict_first.b64 %0, 1.0;" : "=l"(p));
+  return p;
+}
+__device__ __forceinline__ void red_add_f64_hint(double* addr, double v, u64 pol) {
+  asm volatile("red.relaxed.gpu.global.add.L2::cache_hint.f64 [%0], %1, %2;" ::"l"(addr), "d"(v), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void st_f64_hint(double* addr, double v, u64 pol) {
+  asm volatile("st.relaxed.gpu.global.L2::cache_hint.f64 [%0], %1, %2;" ::"l"(addr), "d"(v), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void ld256_hint(const void* p, u64& a, u64& b, u64& c, u64& d, u64 pol) {
+  asm volatile("ld.relaxed.gpu.global.L2::cache_hint.v4.u64 {%0,%1,%2,%3}, [%4], %5;" : "=l"(a), "=l"(b), "=l"(c), "=l"(d) : "l"(p), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void ld256_stream(const void* p, u64& a, u64& b, u64& c, u64& d, u64 pol) {
+  asm volatile("ld.global.nc.L1::no_allocate.L2::cache_hint.v4.u64 {%0,%1,%2,%3}, [%4], %5;" : "=l"(a), "=l"(b), "=l"(c), "=l"(d) : "l"(p), "l"(pol) : "memory");
+}
+__device__ __forceinline__ void st256_zero_hint(void* p, u64 pol) {
+  asm volatile("st.relaxed.gpu.global.L2::cache_hint.v4.u64 [%0], {%1,%1,%1,%1}, %2;" ::"l"(p), "l"(0ull), "l"(pol) : "memory");
+}
 
 __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
   unsigned v;
   asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
-}
-__device__ __forceinline__ void wait_count(const unsigned* p, unsigned target) {
-  while (ld_acquire_u32(p) < target) __nanosleep(64);
 }
 // slot hash of a key inside its region: the bin already consumed the partition word, so this one is a multiplicative mix
 __device__ __forceinline__ unsigned key_hash(u64 ka, u64 kb) {
@@ -529,47 +617,99 @@ __device__ __forceinline__ unsigned key_hash(u64 ka, u64 kb) {
   return (unsigned)(h >> 32);
 }
 
-__global__ void __launch_bounds__(kMergeWarps * 32, 1) pt2_merge_kernel(MergeParams M) {
+__device__ __noinline__ double diag_cold(int n, const double* J, const double* JK, const double* hd, double e_core, u64 a, u64 b) {
+  return dh_diag_from_scratch(n, J, JK, hd, e_core, a, b);
+}
+
+// Work of one pass = an ORDERED list of units: for region g = 0, 1, ...: the merge units of region g (kUnitRec records of one
+// segment each), then the reduce units of region g - kLag (kUnitSlots slots each).  CTAs take blocks of kMergeWarps consecutive
+// units from one global counter (one unit per warp), so at any time the whole GPU works inside a window of about one region
+// - the three or four region tables it touches stay in L2 - and a slow warp delays only its own unit.  A merge unit of region g
+// needs region g - kRing reduced and cleared (same table), a reduce unit of region g needs region g merged: both depend on
+// units handed out earlier, to warps that are running (cooperative launch), so the waits cannot deadlock.
+__global__ void __launch_bounds__(kMergeWarps * 32, kMergeCtasPerSm) pt2_merge_kernel(MergeParams M) {
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const unsigned full = 0xffffffffu;
-  const unsigned TW = gridDim.x * kMergeWarps;            // warps of the kernel = arrivals per counter
-  const unsigned g = blockIdx.x * kMergeWarps + warp;     // this warp
-  const unsigned Q = (TW + M.nseg - 1) / M.nseg;          // sub-slices per segment, so that a bin has >= TW units
-  const unsigned nunits = (unsigned)M.nseg * Q;
+  const u64 keep = l2_policy_evict_last(), once = l2_policy_evict_first();
+  const unsigned QS = (M.seg_cap + kUnitRec - 1) / kUnitRec;                                   // merge units per segment (by capacity)
+  const unsigned UM = ((unsigned)M.nseg * QS + kMergeWarps - 1) / kMergeWarps * kMergeWarps;   // merge units per region, whole blocks
+  const unsigned US = ((M.cap + kUnitSlots - 1) / kUnitSlots + kMergeWarps - 1) / kMergeWarps * kMergeWarps;  // reduce units per region
+  const unsigned GS = UM + US;
+  const u64 total = (u64)(M.nbins + kLag) * GS;
   double sum = 0.0, sabs = 0.0, mden = INFINITY, cntd = 0.0;
-  const unsigned s_lo = (unsigned)(((u64)M.cap * g) / TW), s_hi = (unsigned)(((u64)M.cap * (g + 1)) / TW);  // reduce share
-  for (int b = 0; b <= M.nbins; ++b) {
-    if (b < M.nbins) {
-      Slot* tb = M.ring + (size_t)(b % kRing) * M.cap;
-      if (b >= kRing) wait_count(M.cleared + (b - kRing), TW);
-      for (unsigned u = g; u < nunits; u += TW) {
-        const unsigned s = u / Q, q = u % Q;
-        const unsigned nrec = M.used[(size_t)b * M.nseg + s];
-        const unsigned lo = (unsigned)(((u64)nrec * q) / Q), hi = (unsigned)(((u64)nrec * (q + 1)) / Q);
-        const Slot* src = M.pool + ((size_t)b * M.nseg + s) * M.seg_cap;
-        for (unsigned t = lo + lane; t < hi; t += 32) {
-          u64 ka, kb, vv, hh;
-          dh_ld256_cs(src + t, ka, kb, vv, hh);
-          unsigned slot = __umulhi(key_hash(ka, kb), M.cap);
-          const double cv = __longlong_as_double((long long)vv);
-          for (int probes = 0;; ++probes) {
-            Slot* sp = tb + slot;
-            const Key128 old = dh_cas128(sp, Key128{0ull, 0ull}, Key128{ka, kb});
-            if ((old.a | old.b) == 0ull) { sp->haa = __longlong_as_double((long long)hh); atomicAdd(&sp->v, cv); break; }
-            if (old.a == ka && old.b == kb) { atomicAdd(&sp->v, cv); break; }
-            if (++slot == M.cap) slot = 0;
+  __shared__ u64 s_base;
+  u64 next = 0;
+  if (threadIdx.x == 0) next = atomicAdd(M.ticket, (u64)kMergeWarps);
+  for (;;) {
+    __syncthreads();  // the previous block's units are done (every warp's atomics issued), s_base may be overwritten
+    if (threadIdx.x == 0) s_base = next;
+    __syncthreads();
+    const u64 base = s_base;
+    if (base >= total) break;
+    const unsigned g = (unsigned)(base / GS), r = (unsigned)(base % GS);
+    const bool is_merge = r < UM;
+    const int bin = is_merge ? (int)g : (int)g - kLag;
+    const bool valid = bin >= 0 && bin < M.nbins;
+    if (threadIdx.x == 0) {
+      next = atomicAdd(M.ticket, (u64)kMergeWarps);  // the next block's ticket travels while this one is worked on
+      if (valid) {
+        const unsigned* dep = nullptr;
+        unsigned target = 0;
+        if (is_merge) { if (bin >= kRing) { dep = M.cleared + (bin - kRing); target = US / kMergeWarps; } }
+        else { dep = M.merged + bin; target = UM / kMergeWarps; }
+        if (dep) { unsigned ns = 32; while (ld_acquire_u32(dep) < target) { __nanosleep(ns); if (ns < 1024) ns *= 2; } }
+      }
+    }
+    __syncthreads();
+    if (!valid) continue;
+    Slot* tb = M.ring + (size_t)(bin % kRing) * M.cap;
+    if (is_merge) {
+      const unsigned u = r + warp;
+      const unsigned s = u / QS, q = u % QS;
+      if (s < (unsigned)M.nseg) {
+        const unsigned nrec = M.used[(size_t)bin * M.nseg + s];
+        const unsigned lo = q * kUnitRec, hi = min(nrec, lo + kUnitRec);
+        const Slot* src = M.pool + ((size_t)bin * M.nseg + s) * M.seg_cap;
+        for (unsigned t0 = lo + lane; t0 < hi; t0 += 32 * kMergeU) {
+          u64 ka[kMergeU], kb[kMergeU], vv[kMergeU], hh[kMergeU];
+          unsigned slot[kMergeU];
+          unsigned pend = 0u;
+#pragma unroll
+          for (int k = 0; k < kMergeU; ++k) {
+            ka[k] = kb[k] = vv[k] = hh[k] = 0ull; slot[k] = 0u;
+            const unsigned t = t0 + 32 * k;
+            if (t < hi) { ld256_stream(src + t, ka[k], kb[k], vv[k], hh[k], once); pend |= 1u << k; }
+          }
+#pragma unroll
+          for (int k = 0; k < kMergeU; ++k) slot[k] = __umulhi(key_hash(ka[k], kb[k]), M.cap);
+          // every pending record's claim is issued before any result is looked at
+          for (int probes = 0; pend; ++probes) {
+            Key128 old[kMergeU];
+#pragma unroll
+            for (int k = 0; k < kMergeU; ++k)
+              if ((pend >> k) & 1u) old[k] = dh_cas128(tb + slot[k], Key128{0ull, 0ull}, Key128{ka[k], kb[k]});
+#pragma unroll
+            for (int k = 0; k < kMergeU; ++k)
+              if ((pend >> k) & 1u) {
+                Slot* sp = tb + slot[k];
+                if ((old[k].a | old[k].b) == 0ull) {  // claimed: this thread also records H_aa
+                  st_f64_hint(&sp->haa, __longlong_as_double((long long)hh[k]), keep);
+                  red_add_f64_hint(&sp->v, __longlong_as_double((long long)vv[k]), keep);
+                  pend &= ~(1u << k);
+                } else if (old[k].a == ka[k] && old[k].b == kb[k]) {
+                  red_add_f64_hint(&sp->v, __longlong_as_double((long long)vv[k]), keep);
+                  pend &= ~(1u << k);
+                } else if (++slot[k] == M.cap) {
+                  slot[k] = 0u;
+                }
+              }
             if (probes > kProbeLimit) { *M.overflow = 1; break; }
           }
         }
       }
-      __threadfence();
-      __syncwarp();
-      if (lane == 0) atomicAdd(M.merged + b, 1u);
-    }
-    if (b >= 1) {
-      const int bs = b - 1;
-      Slot* tb = M.ring + (size_t)(bs % kRing) * M.cap;
-      wait_count(M.merged + bs, TW);
+    } else {
+      const unsigned u = r - UM + warp;
+      const unsigned s_lo = min(M.cap, u * kUnitSlots), s_hi = min(M.cap, s_lo + kUnitSlots);
       constexpr int V = 4;
       for (unsigned t0 = s_lo + lane; t0 < s_hi; t0 += 32 * V) {
         u64 x[V], y[V], z[V], w[V];
@@ -577,7 +717,7 @@ __global__ void __launch_bounds__(kMergeWarps * 32, 1) pt2_merge_kernel(MergePar
         for (int k = 0; k < V; ++k) {
           x[k] = y[k] = z[k] = w[k] = 0ull;
           const unsigned t = t0 + 32 * k;
-          if (t < s_hi) dh_ld256(tb + t, x[k], y[k], z[k], w[k]);
+          if (t < s_hi) ld256_hint(tb + t, x[k], y[k], z[k], w[k], keep);
         }
 #pragma unroll
         for (int k = 0; k < V; ++k) {
@@ -586,17 +726,16 @@ __global__ void __launch_bounds__(kMergeWarps * 32, 1) pt2_merge_kernel(MergePar
             double den = M.e_s - __longlong_as_double((long long)w[k]);
             // H_aa came from the O(1) update of whichever source claimed the slot: where the denominator is small enough to
             // amplify that rounding, take H_aa from the key alone (the same value for every run and partitioning)
-            if (fabs(den) < M.small_den) den = M.e_s - dh_diag_from_scratch(M.n, M.J, M.JK, M.hd, M.e_core, x[k], y[k]);
+            if (fabs(den) < M.small_den) den = M.e_s - diag_cold(M.n, M.J, M.JK, M.hd, M.e_core, x[k], y[k]);
             const double term = v * v / den;
             sum += term; sabs += fabs(term); mden = fmin(mden, fabs(den)); cntd += 1.0;
-            dh_st256(tb + t0 + 32 * k, 0ull, 0ull, 0ull, 0ull);
+            st256_zero_hint(tb + t0 + 32 * k, keep);
           }
         }
       }
-      __threadfence();
-      __syncwarp();
-      if (lane == 0) atomicAdd(M.cleared + bs, 1u);
     }
+    __syncthreads();  // every warp of the block has issued its stores and atomics; one release for all of them
+    if (threadIdx.x == 0) { __threadfence(); atomicAdd(is_merge ? M.merged + bin : M.cleared + bin, 1u); }
   }
   __shared__ double sh[4][kMergeWarps];
   for (int o = 16; o > 0; o >>= 1) {
@@ -641,7 +780,7 @@ dh_status dh_pt2_stream(detham_ctx* c, const double* psi, double e_s, double eps
   if (nd < (int64_t)grid * kGenWarps || pbits > 8) return DH_EINVAL;  // the caller keeps small inputs on the table organisation
 
   // ---- region tables: kRing of them share the L2 budget; bins so that a region's distinct keys load it to <= `load`
-  const double load = c->opt.stream_load > 0.0 ? c->opt.stream_load : 0.6;
+  const double load = c->opt.stream_load > 0.0 ? c->opt.stream_load : 0.45;
   const double ring_mb = c->opt.stream_ring_mb > 0.0 ? c->opt.stream_ring_mb : 60.0;
   const double cap_max = ring_mb * 1048576.0 / (kRing * sizeof(Slot));
   const double distinct = plan.est_distinct > 0.0 ? plan.est_distinct : plan.est_records;
@@ -684,6 +823,7 @@ dh_status dh_pt2_stream(detham_ctx* c, const double* psi, double e_s, double eps
   unsigned* used = reinterpret_cast<unsigned*>(c->sflags);
   unsigned* flags = used + (size_t)nbins * grid;
 
+  if (c->debug) fprintf(stderr, "[detham] streamed layout: %d regions of %u slots (%.1f MB ring), segments of %u records, pool %.1f GB\n", nbins, cap, ring_bytes / 1048576.0, seg_cap, pool_bytes / 1e9);
   // ---- generator launch shape: staging takes what the tables and the per-warp scratch leave of the CTA's shared memory
   const int npairs = na * (na - 1) / 2 + nb * (nb - 1) / 2 + na * nb;
   int smem_max = 0;
@@ -697,12 +837,15 @@ dh_status dh_pt2_stream(detham_ctx* c, const double* psi, double e_s, double eps
   N = std::min(N, 60000) & ~31;
   if (N < 1024) return DH_EINVAL;
   const GenLayout GL = gen_layout(n, pbits, npairs, kGenWarps, K, nbins, N);
+  if (c->debug) fprintf(stderr, "[detham] generator: staging %d references, %d source slots per warp, %u bytes of shared memory\n", N, K, GL.total);
   DH_CUDA(c, cudaFuncSetAttribute(pt2_gen_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GL.total));
   G.dets = c->dets; G.psi = psi; G.nd = nd; G.eps2 = eps2;
   G.sbits = c->sbits; G.sbits_n = (u64)c->sbits_n; G.shash_key = c->shash_key; G.shash_idx = c->shash_idx; G.shash_cap = (u64)c->shash_cap;
   G.nbins = nbins; G.seg_cap = seg_cap; G.pool = reinterpret_cast<Slot*>(c->pool); G.used_out = used;
   G.counters = c->dcount; G.overflow = reinterpret_cast<int*>(c->dcount + 8);
   G.stage_n = N; G.nslots = K; G.npairs = npairs;
+  G.prof = nullptr;
+  if (c->debug) { DH_CUDA(c, cudaMalloc(&G.prof, 6 * sizeof(u64) * grid)); }
 
   MergeParams M{};
   M.pool = reinterpret_cast<const Slot*>(c->pool); M.used = used; M.seg_cap = seg_cap; M.nbins = nbins; M.nseg = grid;
@@ -710,10 +853,11 @@ dh_status dh_pt2_stream(detham_ctx* c, const double* psi, double e_s, double eps
   M.e_s = e_s; M.n = n; M.J = c->J; M.JK = c->JK; M.hd = c->hd; M.e_core = c->e_core;
   M.small_den = c->opt.small_den == 0.0 ? 1e-3 : (c->opt.small_den < 0.0 ? 0.0 : c->opt.small_den);
   M.overflow = G.overflow;
+  M.ticket = c->dcount + 16;
   int merge_occ = 0;
   DH_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&merge_occ, pt2_merge_kernel, kMergeWarps * 32, 0));
   if (merge_occ < 1) return DH_ECUDA;
-  const int mgrid = c->sm_count;  // one CTA per SM: every CTA is resident (cooperative launch), so the hand-over cannot stall
+  const int mgrid = c->sm_count * std::min(merge_occ, kMergeCtasPerSm);  // every CTA resident (cooperative launch): the waits cannot stall
 
   st = dh_ensure_red(c, 4 * ((int64_t)mgrid + 64) + 4 * (int64_t)(nparts + 1)); if (st != DH_OK) return st;
   double* results = c->red;  // [nparts + 1][4]; row nparts = psi^T psi
@@ -725,21 +869,70 @@ dh_status dh_pt2_stream(detham_ctx* c, const double* psi, double e_s, double eps
   dh_launch_final_reduce4(part, 64, results + 4 * nparts, c->stream);
   DH_CUDA(c, cudaGetLastError());
 
+  // The region tables are the merge's only reused lines.  Its loads, stores and reductions carry an evict_last policy; the
+  // 128-bit CAS takes no cache hint in PTX (ptxas: "Illegal modifier '.L2::cache_hint' for instruction 'atom'" for cas), so the
+  // tables are also declared a persisting access-policy window of the stream for the duration of the call.
+  size_t persist_bytes = 0, persist_before = 0;
+  cudaStreamAttrValue win_before{};
+  {
+    int max_persist = 0, max_window = 0;
+    DH_CUDA(c, cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, c->device));
+    DH_CUDA(c, cudaDeviceGetAttribute(&max_window, cudaDevAttrMaxAccessPolicyWindowSize, c->device));
+    DH_CUDA(c, cudaDeviceGetLimit(&persist_before, cudaLimitPersistingL2CacheSize));
+    const char* e = getenv("DETHAM_PERSIST");
+    if (!(e && e[0] == '0') && max_persist > 0 && max_window > 0) {
+      persist_bytes = std::min(ring_bytes, std::min((size_t)max_persist, (size_t)max_window));
+      if (cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, persist_bytes) != cudaSuccess) { cudaGetLastError(); persist_bytes = 0; }
+    }
+    if (persist_bytes) {
+      cudaStreamGetAttribute(c->stream, cudaStreamAttributeAccessPolicyWindow, &win_before);
+      cudaStreamAttrValue w{};
+      w.accessPolicyWindow.base_ptr = c->ring;
+      w.accessPolicyWindow.num_bytes = persist_bytes;
+      w.accessPolicyWindow.hitRatio = 1.0f;
+      w.accessPolicyWindow.hitProp = cudaAccessPropertyPersisting;
+      w.accessPolicyWindow.missProp = cudaAccessPropertyStreaming;
+      if (cudaStreamSetAttribute(c->stream, cudaStreamAttributeAccessPolicyWindow, &w) != cudaSuccess) { cudaGetLastError(); persist_bytes = 0; }
+    }
+    if (c->debug) fprintf(stderr, "[detham] L2 persistence: device allows %d bytes (window %d), region tables %zu, using %zu\n", max_persist, max_window, ring_bytes, persist_bytes);
+  }
   // events: [3 * pass + 0] before gen, +1 between, +2 after merge
   while ((int)c->sev.size() < 3 * nparts) { cudaEvent_t e; DH_CUDA(c, cudaEventCreate(&e)); c->sev.push_back(e); }
   for (int pass = 0; pass < nparts; ++pass) {
     DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, sizeof(u64), c->stream));  // the row cursor; [1], [2], [8] accumulate over the passes
+    DH_CUDA(c, cudaMemsetAsync(c->dcount + 16, 0, sizeof(u64), c->stream));  // the merge's unit counter
     DH_CUDA(c, cudaMemsetAsync(flags, 0, 2 * (size_t)nbins * sizeof(unsigned), c->stream));
     DH_CUDA(c, cudaEventRecord(c->sev[3 * pass], c->stream));
     G.pass = (unsigned)pass;
     pt2_gen_kernel<<<grid, kGenWarps * 32, GL.total, c->stream>>>(G);
     DH_CUDA(c, cudaGetLastError());
     DH_CUDA(c, cudaEventRecord(c->sev[3 * pass + 1], c->stream));
-    void* args[] = {&M};
-    DH_CUDA(c, cudaLaunchCooperativeKernel(reinterpret_cast<void*>(pt2_merge_kernel), dim3(mgrid), dim3(kMergeWarps * 32), args, 0, c->stream));
+    {
+      cudaLaunchConfig_t cfg{};
+      cfg.gridDim = dim3(mgrid); cfg.blockDim = dim3(kMergeWarps * 32); cfg.dynamicSmemBytes = 0; cfg.stream = c->stream;
+      cudaLaunchAttribute at[1];
+      at[0].id = cudaLaunchAttributeCooperative; at[0].val.cooperative = 1;
+      const unsigned nat = 1;
+      cfg.attrs = at; cfg.numAttrs = nat;
+      DH_CUDA(c, cudaLaunchKernelEx(&cfg, pt2_merge_kernel, M));
+    }
     dh_launch_final_reduce4(part, mgrid, results + 4 * pass, c->stream);
     DH_CUDA(c, cudaGetLastError());
     DH_CUDA(c, cudaEventRecord(c->sev[3 * pass + 2], c->stream));
+  }
+  if (persist_bytes) {
+    DH_CUDA(c, cudaStreamSynchronize(c->stream));
+    cudaStreamSetAttribute(c->stream, cudaStreamAttributeAccessPolicyWindow, &win_before);
+    cudaCtxResetPersistingL2Cache();
+    cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, persist_before);
+  }
+  if (G.prof) {  // phase cycles of the last pass, averaged over the CTAs
+    std::vector<u64> hpf(6 * (size_t)grid);
+    DH_CUDA(c, cudaMemcpy(hpf.data(), G.prof, hpf.size() * sizeof(u64), cudaMemcpyDeviceToHost));
+    double a[6] = {0, 0, 0, 0, 0, 0};
+    for (int b = 0; b < grid; ++b) for (int k = 0; k < 6; ++k) a[k] += (double)hpf[6 * b + k] / grid;
+    fprintf(stderr, "[detham] generator phases (cycles per CTA, last pass): walk %.3g, wait for the slowest walker %.3g, sort %.3g, expand %.3g, advance %.3g; %.0f rounds\n", a[0], a[1], a[2], a[3], a[4], a[5]);
+    cudaFree(G.prof);
   }
   std::vector<double> res(4 * (size_t)(nparts + 1));
   DH_CUDA(c, cudaMemcpyAsync(res.data(), results, res.size() * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
