@@ -69,14 +69,15 @@ typedef struct {
   int64_t hsp_generated;    /* excitations that passed the screen in hsp_build (looked up in P) */
   double ms_hsp_build;      /* hsp_build enumeration pass (enumerate + lookup in P, hits appended to the arena) + row scan */
   double ms_hsp_fill;       /* hsp_build arena -> CSR copy + per-row column sort */
-  int64_t pt2_binned;       /* organisation of the last pt2: 0 = hash table in HBM, 2 = streamed (records partitioned by key
-                               region, deduplicated in L2-resident region tables; no table in HBM) */
+  int64_t pt2_binned;       /* organisation of the last pt2: 0 = hash table in HBM probed directly, 1 = hash table in HBM with binned
+                               passes, 2 = streamed (records partitioned by key region, deduplicated in L2-resident region tables;
+                               no table in HBM) */
   int64_t pt2_stream_bins;  /* streamed organisation: key regions per pass (0 otherwise); pt2_table_slots = slots of one region table */
 } detham_counters;
 
 /* Options of pt2 (SURVEY.md section 5 "config / flag system").  Zero in every field = the defaults. */
 typedef struct {
-  int32_t mode;             /* 0 = choose: streamed when one pass of the table organisation would need a table beyond 24 GB;
+  int32_t mode;             /* 0 = choose (today: the hash table in HBM, with binned passes when it is far beyond L2);
                                1 = hash table in HBM; 2 = streamed (DH_EINVAL if |S| < 16 x SM count) */
   int32_t n_parts;          /* key partitions / passes, a power of two <= 1024 (streamed: <= 256); 0 = planned */
   int64_t table_slots;      /* table organisation: capacity in 32-byte slots; 0 = planned from free device memory */
@@ -87,10 +88,12 @@ typedef struct {
                                the source that claimed them (its rounding, ~1e-13, is amplified by 1 / denominator; DESIGN.md
                                reading Q11); 0 = 1e-3, negative = never */
   int32_t stream_bins;      /* streamed: key regions per pass (<= 4096); 0 = planned so that a region's distinct keys fit its table */
-  int32_t reserved;
+  int32_t table_regions;    /* table organisation, binned passes (contributions appended per table region, then merged region by
+                               region so that the probes stay in L2): 0 = when the table exceeds 32 GB, with at most 2048 regions;
+                               > 0 = always, with at most that many regions (64..8192); -1 = never */
   double stream_ring_mb;    /* streamed: bytes of the three region tables together (they must stay in L2); 0 = 60 */
   double stream_load;       /* streamed: target load factor of a region table; 0 = 0.45 */
-  double stream_pool_frac;  /* streamed: head room of the record pool over the planned estimate; 0 = 1.15 */
+  double stream_pool_frac;  /* head room of the record pool over the planned estimate (streamed: 0 = 1.15; binned passes: 0 = 1.2) */
   double stream_pool_gb;    /* streamed: budget of the record pool; 0 = 80 % of the free device memory */
 } detham_pt2_options;
 

@@ -31,7 +31,7 @@ class Counters(C.Structure):
 class Pt2Options(C.Structure):
     """detham_pt2_options (include/detham.h); zero in every field = the defaults."""
     _fields_ = [("mode", C.c_int32), ("n_parts", C.c_int32), ("table_slots", C.c_int64), ("table_load", C.c_double),
-                ("max_table_gb", C.c_double), ("small_den", C.c_double), ("stream_bins", C.c_int32), ("reserved", C.c_int32),
+                ("max_table_gb", C.c_double), ("small_den", C.c_double), ("stream_bins", C.c_int32), ("table_regions", C.c_int32),
                 ("stream_ring_mb", C.c_double), ("stream_load", C.c_double), ("stream_pool_frac", C.c_double),
                 ("stream_pool_gb", C.c_double)]
 

@@ -147,7 +147,7 @@ dh_status detham_pt2_set_options(detham_ctx* c, const detham_pt2_options* o) {
   auto fin = [](double x) { return std::isfinite(x); };
   if (o->mode < 0 || o->mode > 2 || o->n_parts < 0 || o->n_parts > (1 << DH_MAX_PBITS) || (o->n_parts & (o->n_parts - 1)) ||
       o->table_slots < 0 || (o->table_slots > 0 && o->table_slots < 64) || !fin(o->table_load) || o->table_load < 0.0 ||
-      o->table_load > 0.95 || !fin(o->max_table_gb) || o->max_table_gb < 0.0 || !fin(o->small_den) || o->stream_bins < 0 ||
+      o->table_load > 0.95 || !fin(o->max_table_gb) || o->max_table_gb < 0.0 || !fin(o->small_den) || o->table_regions < -1 || (o->table_regions > 0 && (o->table_regions < 64 || o->table_regions > 8192)) || o->stream_bins < 0 ||
       o->stream_bins > 4096 || !fin(o->stream_ring_mb) || o->stream_ring_mb < 0.0 || !fin(o->stream_load) || o->stream_load < 0.0 ||
       o->stream_load > 0.95 || !fin(o->stream_pool_frac) || o->stream_pool_frac < 0.0 || !fin(o->stream_pool_gb) || o->stream_pool_gb < 0.0)
     return DH_EINVAL;

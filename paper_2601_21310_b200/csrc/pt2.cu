@@ -64,7 +64,7 @@ count_kernel(EnumParams P, const u64* __restrict__ dets, const double* __restric
 
 // ---------------------------------------------------------------- members of S of this pass's class
 __global__ void member_insert_kernel(const u64* __restrict__ dets, int64_t nd, unsigned pmask, unsigned pass, Slot* table,
-                                     u64 cap, int* overflow) {
+                                     u64 cap, int rshift, int* overflow) {
   __shared__ u64 Z[128];
   for (int t = threadIdx.x; t < 128; t += blockDim.x) Z[t] = dh_zword(t);
   __syncthreads();
@@ -73,7 +73,7 @@ __global__ void member_insert_kernel(const u64* __restrict__ dets, int64_t nd, u
   u64 a = dets[2 * t], b = dets[2 * t + 1];
   u64 z = dh_zobrist(a, b, Z);
   if (((unsigned)z & pmask) != pass) return;
-  u64 slot = __umul64hi(z, cap);
+  u64 slot = dh_table_slot(z, a, b, cap, rshift);
   for (int probes = 0;; ++probes) {
     Slot* sp = table + slot;
     Key128 old = dh_cas128(sp, Key128{0ull, 0ull}, Key128{a, b});
@@ -102,6 +102,7 @@ struct FlatScratch {
   int beg[kChunk];               // first list entry of the kept prefix
   unsigned short meta[kChunk];   // fam << 12 | i << 6 | j
   unsigned short sq[64];         // singles queue: s << 12 | i << 6 | a
+  unsigned dq[64];               // doubles queue: list entry | pair of the chunk << 25
 };
 
 // entry meta: kind << 25 | s << 24 | i << 18 | j << 12 | a << 6 | b
@@ -186,6 +187,32 @@ __device__ __forceinline__ void probe_batch(ProbeCtx& pc, const u64 (&ka)[U], co
   pc.max_probe = max(pc.max_probe, probes);
 }
 
+// Binned mode (tables far beyond L2): instead of probing the table, a contribution is appended as a 32-byte record
+// {key, H_ai psi_i, H_aa} to this CTA's private segment of the bin its slot falls in (bin = slot >> shift: a contiguous
+// region of the table).  pt2_merge_kernel then walks the bins in order, so the probes of the whole GPU stay inside a window
+// of the table that fits L2 (profiles/r1_microbench.md, block C: 36-41 G/s against 15 G/s for random probes).  The position
+// in the segment comes from a shared-memory counter: no global atomic.  A record that does not fit its segment is probed
+// directly, as in the unbinned kernel.
+struct BinCtx { Slot* pool; unsigned* cnt; unsigned seg_cap; int shift; };
+
+template <int U>
+__device__ __forceinline__ unsigned bin_batch(ProbeCtx& pc, const BinCtx& bc, const u64 (&ka)[U], const u64 (&kb)[U],
+                                              const double (&cv)[U], const u64 (&slot)[U], const unsigned (&meta)[U], unsigned pend) {
+#pragma unroll
+  for (int u = 0; u < U; ++u)
+    if ((pend >> u) & 1u) {
+      const double haa = meta_diag(pc, meta[u]);
+      const unsigned bin = (unsigned)(slot[u] >> bc.shift);
+      const unsigned p = atomicAdd(&bc.cnt[bin], 1u);
+      if (p < bc.seg_cap) {
+        dh_st256(bc.pool + ((u64)bin * gridDim.x + blockIdx.x) * bc.seg_cap + p, ka[u], kb[u], (u64)__double_as_longlong(cv[u]),
+                 (u64)__double_as_longlong(haa));
+        pend &= ~(1u << u);
+      }
+    }
+  return pend;
+}
+
 // decode the triangular index t = y(y-1)/2 + x, x < y
 __device__ __forceinline__ void tri_decode(int t, int& x, int& y) {
   y = (int)((1.0f + sqrtf(1.0f + 8.0f * (float)t)) * 0.5f);
@@ -194,16 +221,22 @@ __device__ __forceinline__ void tri_decode(int t, int& x, int& y) {
   x = t - y * (y - 1) / 2;
 }
 
-template <int kAccWarps, int kU, bool kExpand>
+template <int kAccWarps, int kU, bool kExpand, bool kBinned = false>
 __global__ void __launch_bounds__(kAccWarps * 32, 1)
 pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* __restrict__ psi, int64_t nd, double eps2,
                       unsigned pass, Slot* table, u64 cap, u64* counters /* [0] next row [1] gen [2] contrib [3] max probe */,
-                      int* overflow) {
+                      int* overflow, Slot* pool, unsigned* used, unsigned seg_cap, int bin_shift, int nbins) {
   extern __shared__ __align__(16) unsigned char smem[];
   CtaTables T = dh_cta_stage(P, smem);
   size_t off = (dh_cta_table_bytes(P.n) + 15) & ~(size_t)15;
   WarpScratch* wsp = reinterpret_cast<WarpScratch*>(smem + off);
   FlatScratch* fsp = reinterpret_cast<FlatScratch*>(smem + off + kAccWarps * sizeof(WarpScratch));
+  unsigned* bcnt = reinterpret_cast<unsigned*>(fsp + kAccWarps);  // [nbins] records this CTA appended per bin (binned mode)
+  if (kBinned) {
+    for (int t = threadIdx.x; t < nbins; t += blockDim.x) bcnt[t] = 0;
+    __syncthreads();
+  }
+  const BinCtx bc{pool, bcnt, seg_cap, bin_shift};
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const unsigned lt = (1u << lane) - 1u;
   WarpScratch& ws = wsp[warp];
@@ -271,7 +304,7 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
               const u64 nw = (w ^ (1ull << i)) | (1ull << a);
               if (s == 0) ka[0] = nw; else kb[0] = nw;
               const u64 z = zsrc ^ T.Z[64 * s + i] ^ T.Z[64 * s + a];
-              slot[0] = __umul64hi(z, cap);
+              slot[0] = dh_table_slot(z, ka[0], kb[0], cap, bin_shift);
               cv[0] = v * p;
               meta[0] = pack_meta(0, s, i, 0, a, 0);
               pend = 1u;
@@ -280,6 +313,7 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
           __syncwarp();
           qn -= take;
           gen += pend;
+          if (kBinned) pend = bin_batch<1>(pc, bc, ka, kb, cv, slot, meta, pend);
           probe_batch<1, kExpand>(pc, ka, kb, cv, slot, meta, pend);
         }
       }
@@ -313,8 +347,11 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
               const int mid = (lo + hi) >> 1;
               if (fabs(__ldg(P.lval + mid)) >= tau) lo = mid + 1; else hi = mid;
             }
-          } else {
-            lo = end;
+          } else {  // tau = 0: everything but exact zeros (reading Q8), which the |value|-descending order puts at the tail
+            while (lo < hi) {
+              const int mid = (lo + hi) >> 1;
+              if (__ldg(P.lval + mid) != 0.0) lo = mid + 1; else hi = mid;
+            }
           }
           len = lo - beg;
           pm = ((unsigned)fam << 12) | ((unsigned)i << 6) | (unsigned)j;
@@ -333,64 +370,78 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
       }
       if (lane == 0) fs.pref[cnt] = run;
       __syncwarp();
-      // phase B: walk the concatenated prefixes
+      // phase B: walk the concatenated prefixes 32 entries at a time.  Entries whose a or b is occupied in the source (about
+      // 40 % on the Cr2-shaped config) are dropped first - one 2-byte load and a bit test - and the survivors queued, so that
+      // value, phase, key, slot and H_aa are worked out, and the table probed, with every lane busy.
       const int TT = run;
-      int qcur = 0;
-      for (int t0 = 0; t0 < TT; t0 += 32 * kU) {
-        u64 ka[kU], kb[kU], slot[kU];
-        double cv[kU];
-        unsigned meta[kU];
-        unsigned pend = 0u;
-#pragma unroll
-        for (int u = 0; u < kU; ++u) {
-          ka[u] = da; kb[u] = db; slot[u] = 0; cv[u] = 0.0; meta[u] = 0u;
-          const int tt = t0 + 32 * u;
-          if (tt < TT) {  // warp-uniform
-            const int pe = (qcur + lane < cnt) ? fs.pref[qcur + lane + 1] - tt : 0x7fffffff;  // end of pair qcur+lane, relative
-            const unsigned bm = __reduce_or_sync(0xffffffffu, pe < 32 ? (1u << pe) : 0u);
-            const int adv = __popc(__ballot_sync(0xffffffffu, pe <= 32));
-            const int myq = qcur + __popc(bm & ((2u << lane) - 1u));
-            qcur += adv;
-            const int t = tt + lane;
-            if (t < TT) {
-              const int k = fs.beg[myq] + (t - fs.pref[myq]);
-              const unsigned pm = fs.meta[myq];
-              double v = __ldg(P.lval + k);
-              const unsigned ab = __ldg(P.lab + k);
-              const int a = (int)(ab & 0xFFu), b = (int)(ab >> 8);
-              const int fam = (int)(pm >> 12), i = (int)((pm >> 6) & 63u), j = (int)(pm & 63u);
-              const u64 zij = fs.zij[myq];
-              bool act = v != 0.0;
-              if (fam < 2) {
-                const u64 w = fam ? db : da;
-                act = act && !((w >> a) & 1ull) && !((w >> b) & 1ull);
-                if (act) {
-                  const u64 nw = (w ^ (1ull << i) ^ (1ull << j)) | (1ull << a) | (1ull << b);
-                  if (fam == 0) ka[u] = nw; else kb[u] = nw;
-                  const u64 z = zij ^ T.Z[64 * fam + a] ^ T.Z[64 * fam + b];
-                  // a+_a a+_b a_j a_i = (a+_b a_j)(a+_a a_i): phase(i->a on w) * phase(j->b on w with i->a applied)
-                  const int par = dh_parity_between(w, i, a) ^ dh_parity_between((w ^ (1ull << i)) | (1ull << a), j, b);
-                  if (par) v = -v;
-                  slot[u] = __umul64hi(z, cap);
-                  meta[u] = pack_meta(1, fam, i, j, a, b);
-                }
-              } else {
-                act = act && !((da >> a) & 1ull) && !((db >> b) & 1ull);
-                if (act) {
-                  ka[u] = (da ^ (1ull << i)) | (1ull << a);
-                  kb[u] = (db ^ (1ull << j)) | (1ull << b);
-                  const u64 z = zij ^ T.Z[a] ^ T.Z[64 + b];
-                  if (dh_parity_between(da, i, a) ^ dh_parity_between(db, j, b)) v = -v;
-                  slot[u] = __umul64hi(z, cap);
-                  meta[u] = pack_meta(2, 0, i, j, a, b);
-                }
-              }
-              if (act) { cv[u] = v * p; pend |= 1u << u; }
-            }
+      int qcur = 0, dqn = 0;
+      for (int t0 = 0; t0 < TT + 32; t0 += 32) {
+        const bool last = t0 >= TT;
+        if (!last) {
+          const int pe = (qcur + lane < cnt) ? fs.pref[qcur + lane + 1] - t0 : 0x7fffffff;  // end of pair qcur+lane, relative
+          const unsigned bm = __reduce_or_sync(0xffffffffu, pe < 32 ? (1u << pe) : 0u);
+          const int adv = __popc(__ballot_sync(0xffffffffu, pe <= 32));
+          const int myq = qcur + __popc(bm & ((2u << lane) - 1u));
+          qcur += adv;
+          const int t = t0 + lane;
+          bool act = false;
+          unsigned ent = 0u;
+          if (t < TT) {
+            const int k = fs.beg[myq] + (t - fs.pref[myq]);
+            const unsigned ab = __ldg(P.lab + k);
+            const int a = (int)(ab & 0xFFu), b = (int)(ab >> 8);
+            const unsigned fam = fs.meta[myq] >> 12;
+            const u64 wa = fam == 1u ? db : da, wb = fam != 0u ? db : da;  // spin string of (i, a) and of (j, b)
+            act = !(((wa >> a) | (wb >> b)) & 1ull);
+            ent = (unsigned)k | ((unsigned)myq << 25);
           }
+          const unsigned m = __ballot_sync(0xffffffffu, act);
+          if (act) fs.dq[dqn + __popc(m & lt)] = ent;
+          dqn += __popc(m);
+          __syncwarp();
         }
-        gen += __popc(pend);
-        probe_batch<kU, kExpand>(pc, ka, kb, cv, slot, meta, pend);
+        if (dqn >= 32 || (last && dqn > 0)) {
+          const int take = dqn >= 32 ? 32 : dqn;
+          u64 ka[1] = {da}, kb[1] = {db}, slot[1] = {0};
+          double cv[1] = {0.0};
+          unsigned meta[1] = {0u};
+          unsigned pend = 0u;
+          if (lane < take) {
+            const unsigned ent = fs.dq[dqn - take + lane];
+            const int k = (int)(ent & 0x1FFFFFFu), myq = (int)(ent >> 25);
+            const unsigned pm = fs.meta[myq];
+            double v = __ldg(P.lval + k);
+            const unsigned ab = __ldg(P.lab + k);
+            const int a = (int)(ab & 0xFFu), b = (int)(ab >> 8);
+            const int fam = (int)(pm >> 12), i = (int)((pm >> 6) & 63u), j = (int)(pm & 63u);
+            const u64 zij = fs.zij[myq];
+            if (fam < 2) {
+              const u64 w = fam ? db : da;
+              const u64 nw = (w ^ (1ull << i) ^ (1ull << j)) | (1ull << a) | (1ull << b);
+              if (fam == 0) ka[0] = nw; else kb[0] = nw;
+              const u64 z = zij ^ T.Z[64 * fam + a] ^ T.Z[64 * fam + b];
+              // a+_a a+_b a_j a_i = (a+_b a_j)(a+_a a_i): phase(i->a on w) * phase(j->b on w with i->a applied)
+              const int par = dh_parity_between(w, i, a) ^ dh_parity_between((w ^ (1ull << i)) | (1ull << a), j, b);
+              if (par) v = -v;
+              slot[0] = dh_table_slot(z, ka[0], kb[0], cap, bin_shift);
+              meta[0] = pack_meta(1, fam, i, j, a, b);
+            } else {
+              ka[0] = (da ^ (1ull << i)) | (1ull << a);
+              kb[0] = (db ^ (1ull << j)) | (1ull << b);
+              const u64 z = zij ^ T.Z[a] ^ T.Z[64 + b];
+              if (dh_parity_between(da, i, a) ^ dh_parity_between(db, j, b)) v = -v;
+              slot[0] = dh_table_slot(z, ka[0], kb[0], cap, bin_shift);
+              meta[0] = pack_meta(2, 0, i, j, a, b);
+            }
+            cv[0] = v * p;
+            pend = 1u;
+          }
+          __syncwarp();
+          dqn -= take;
+          gen += pend;
+          if (kBinned) pend = bin_batch<1>(pc, bc, ka, kb, cv, slot, meta, pend);
+          probe_batch<1, kExpand>(pc, ka, kb, cv, slot, meta, pend);
+        }
       }
       __syncwarp();
     }
@@ -409,6 +460,65 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
     if (ct) atomicAdd(counters + 2, ct);
     atomicMax(counters + 3, (u64)mp);
   }
+  if (kBinned) {
+    __syncthreads();
+    for (int t = threadIdx.x; t < nbins; t += blockDim.x) used[(size_t)t * gridDim.x + blockIdx.x] = min(bcnt[t], seg_cap);
+  }
+}
+
+// Binned mode, second half: the records of bin b (one segment per accumulate CTA) are merged into the table region the bin
+// covers.  The CTAs take (bin, segment) chunks from one global cursor in bin-major order, so at any time all probes of the
+// GPU fall into one or two neighbouring regions (16 MB each at 4096 bins of a 60 GB table).  The probe itself is the
+// unbinned kernel's; H_aa comes with the record.
+__global__ void __launch_bounds__(1024, 2)
+pt2_table_merge_kernel(const Slot* __restrict__ pool, const unsigned* __restrict__ used, unsigned seg_cap, int nbins, int nseg,
+                 Slot* table, u64 cap, u64* counters /* [2] contrib [3] max probe [5] chunk cursor */, int* overflow, int rshift) {
+  // work unit = kUnit consecutive records of one (bin, segment), taken per WARP from the global cursor in bin-major order: no
+  // CTA barrier in the loop, and the ~9500 resident warps span three or four bins (128-record units were slower than the
+  // CTA-wide chunks: 1e7 atomics per pass on the one cursor cost 18 ms)
+  const int lane = threadIdx.x & 31;
+  constexpr unsigned kUnit = 512;
+  const unsigned nsub = (seg_cap + kUnit - 1u) / kUnit;
+  const u64 nunits = (u64)nbins * nseg * nsub;
+  unsigned contrib = 0; int max_probe = 0;
+  for (;;) {
+    u64 u = 0;
+    if (lane == 0) u = atomicAdd(counters + 5, 1ull);
+    u = __shfl_sync(0xffffffffu, u, 0);
+    if (u >= nunits) break;
+    const u64 q = u / nsub;                                       // segment (q % nseg) of bin (q / nseg)
+    const unsigned lo = (unsigned)(u % nsub) * kUnit, n = used[q];
+    if (lo >= n) continue;
+    const unsigned hi = min(n, lo + kUnit);
+    const Slot* src = pool + q * seg_cap;
+    for (unsigned t = lo + lane; t < hi; t += 32) {
+      u64 ka, kb, vv, hh;
+      dh_ld256_cs(src + t, ka, kb, vv, hh);
+      // the record's region is the bin it was appended to; inside it the key's own hash gives the home slot (dh_table_slot)
+      u64 slot = ((q / nseg) << rshift) | (u64)(dh_key_hash(ka, kb) >> (32 - rshift));
+      const double cv = __longlong_as_double((long long)vv);
+      int probes = 0;
+      for (;;) {
+        u64 k0, k1, vb, hb;
+        dh_ld256(table + slot, k0, k1, vb, hb);
+        if (k0 == ka && k1 == kb) {
+          if (vb != (u64)0x7ff8000000000001ull) { atomicAdd(&table[slot].v, cv); ++contrib; }
+          break;
+        }
+        if ((k0 | k1) == 0ull) {
+          Key128 old = dh_cas128(table + slot, Key128{0ull, 0ull}, Key128{ka, kb});
+          if ((old.a | old.b) == 0ull) { table[slot].haa = __longlong_as_double((long long)hh); atomicAdd(&table[slot].v, cv); ++contrib; break; }
+          if (old.a == ka && old.b == kb) { atomicAdd(&table[slot].v, cv); ++contrib; break; }
+        }
+        if (++slot == cap) slot = 0;
+        if (++probes > kProbeLimit) { *overflow = 1; break; }
+      }
+      max_probe = max(max_probe, probes);
+    }
+  }
+  u64 ct = contrib;
+  for (int o = 16; o > 0; o >>= 1) { ct += __shfl_xor_sync(0xffffffffu, ct, o); max_probe = max(max_probe, __shfl_xor_sync(0xffffffffu, max_probe, o)); }
+  if ((threadIdx.x & 31) == 0) { if (ct) atomicAdd(counters + 2, ct); atomicMax(counters + 3, (u64)max_probe); }
 }
 
 // ---------------------------------------------------------------- reduce: sum_a v_a^2 / (E_S - H_aa), and clear the table
@@ -564,8 +674,11 @@ static dh_status ensure_table(detham_ctx* c, int64_t slots) {
 // contributions share an external.
 struct ExpandOut { u64* keys; double* v; double* score; u64 cap; u64* cursor; };  // device buffers of expand mode
 
+// `est_pass` (0 = unknown): upper estimate of the contributions of one pass; with it, and a table far beyond L2, the passes run
+// binned: the accumulate kernel appends records to per-region segments (bin_batch), pt2_table_merge_kernel probes them region
+// by region.
 static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, double eps2, int pbits, int64_t slots, bool adapt,
-                             double load, double* out, double* pilot = nullptr, const ExpandOut* ex = nullptr) {
+                             double load, double* out, double* pilot = nullptr, const ExpandOut* ex = nullptr, double est_pass = 0.0) {
   const int64_t nd = c->nd;
   dh_status st = ensure_table(c, slots); if (st != DH_OK) return st;
   Slot* table = reinterpret_cast<Slot*>(c->table);
@@ -575,11 +688,45 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
   // launch shape: 32 warps per CTA, one probe in flight per lane.  Measured on B200 (round 1): more warps per SM help
   // (Cr2-shaped accumulate 1419 / 1084 / 1025 / 994 ms at 16 / 24 / 28 / 32 warps), more probes in flight per lane do not.
   const int warps = 32;
-  auto acc_kernel = ex ? pt2_accumulate_kernel<32, 1, true> : pt2_accumulate_kernel<32, 1, false>;
-  const size_t smem = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + warps * (sizeof(WarpScratch) + sizeof(FlatScratch));
-  DH_CUDA(c, cudaFuncSetAttribute(acc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   int64_t want = (nd + warps - 1) / warps;
   const int grid = (int)(want < (int64_t)c->sm_count ? want : (int64_t)c->sm_count);
+  // binned passes: table beyond 32 GB, an estimate to size the record pool with, every SM busy, not expand / probe
+  // (measured, round 1: H2O-shaped, 15 GB table, 5 contributions per external: 17.5 ms binned against 12.8 ms direct; N2-shaped,
+  // 60 GB: 143 against 152 ms; Cr2-shaped: 5.9 against 7.4 s).  opt.table_regions: -1 never, > 0 always, with that many regions
+  // at most (the region size is a power of two of slots; 2048 was the best of a sweep on Cr2-shaped).
+  const int max_bins = c->opt.table_regions > 0 ? c->opt.table_regions : 2048;
+  bool binned = !ex && !pilot && est_pass > 0.0 && grid == c->sm_count && c->opt.table_regions >= 0 &&
+                (c->opt.table_regions > 0 || slots * (int64_t)sizeof(Slot) > (32ll << 30));
+  unsigned* pool_used = nullptr;
+  if (binned) {
+    // the pool holds the records of one pass: 20 % head room over the estimate (an upper bound already) plus 64 records per
+    // segment; it is divided evenly over the pass's (bin, CTA) segments, and what does not fit a segment is probed directly
+    const double pool_frac = c->opt.stream_pool_frac > 0.0 ? c->opt.stream_pool_frac : 1.2;
+    const int64_t bytes = (int64_t)((est_pass * pool_frac + 64.0 * max_bins * grid) * sizeof(Slot));
+    size_t free_b = 0, total_b = 0;
+    DH_CUDA(c, cudaMemGetInfo(&free_b, &total_b));
+    if (c->pool_bytes < bytes) {
+      if ((double)bytes > 0.95 * ((double)free_b + (double)c->pool_bytes)) binned = false;
+      else {
+        if (c->pool) cudaFree(c->pool);
+        c->pool = nullptr; c->pool_bytes = 0;
+        if (cudaMalloc(&c->pool, (size_t)bytes) != cudaSuccess) { cudaGetLastError(); binned = false; }
+        else c->pool_bytes = bytes;
+      }
+    }
+    const size_t ub = (size_t)max_bins * grid * sizeof(unsigned);
+    if (binned && c->sflags_bytes < ub) {
+      if (c->sflags) cudaFree(c->sflags);
+      c->sflags = nullptr; c->sflags_bytes = 0;
+      DH_CUDA(c, cudaMalloc(&c->sflags, ub));
+      c->sflags_bytes = ub;
+    }
+    pool_used = reinterpret_cast<unsigned*>(c->sflags);
+  }
+  auto acc_kernel = ex ? pt2_accumulate_kernel<32, 1, true> : (binned ? pt2_accumulate_kernel<32, 1, false, true> : pt2_accumulate_kernel<32, 1, false>);
+  const size_t smem = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + warps * (sizeof(WarpScratch) + sizeof(FlatScratch)) +
+                      (binned ? max_bins * sizeof(unsigned) : 0);
+  DH_CUDA(c, cudaFuncSetAttribute(acc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const double small_den = c->opt.small_den == 0.0 ? 1e-3 : (c->opt.small_den < 0.0 ? 0.0 : c->opt.small_den);
 
   const int nparts = 1 << pbits;
@@ -603,8 +750,25 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
     const int sgrid = (int)(sblocks < sgrid_max ? sblocks : sgrid_max);
     DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 8 * sizeof(u64), c->stream));
     DH_TICK(c, 2);
-    member_insert_kernel<<<(unsigned)((nd + 255) / 256), 256, 0, c->stream>>>(c->dets, nd, (unsigned)(nparts - 1), (unsigned)pass, table, (u64)cap, overflow);
-    acc_kernel<<<grid, warps * 32, smem, c->stream>>>(P, c->dets, psi, nd, eps2, (unsigned)pass, table, (u64)cap, c->dcount, overflow);
+    int bin_shift = 0, nbins = 1;
+    unsigned seg_cap = 0;
+    int64_t pcap = cap;  // capacity this pass probes
+    if (binned) {  // bins = contiguous table regions of 2^shift slots, at most max_bins of them; whole regions only
+      bin_shift = 10;
+      while ((cap >> bin_shift) > max_bins) ++bin_shift;
+      nbins = (int)(cap >> bin_shift);
+      if (nbins < 1) { nbins = 1; bin_shift = 0; while ((2ll << bin_shift) <= cap) ++bin_shift; }
+      pcap = (int64_t)nbins << bin_shift;
+      seg_cap = (unsigned)(c->pool_bytes / ((int64_t)nbins * grid * (int64_t)sizeof(Slot)));
+    }
+    member_insert_kernel<<<(unsigned)((nd + 255) / 256), 256, 0, c->stream>>>(c->dets, nd, (unsigned)(nparts - 1), (unsigned)pass, table, (u64)pcap, bin_shift, overflow);
+    acc_kernel<<<grid, warps * 32, smem, c->stream>>>(P, c->dets, psi, nd, eps2, (unsigned)pass, table, (u64)pcap, c->dcount, overflow,
+                                                      reinterpret_cast<Slot*>(c->pool), pool_used, seg_cap, bin_shift, nbins);
+    if (binned) {
+      DH_CUDA(c, cudaGetLastError());
+      pt2_table_merge_kernel<<<c->sm_count * 2, 1024, 0, c->stream>>>(reinterpret_cast<const Slot*>(c->pool), pool_used, seg_cap, nbins, grid, table,
+                                                                     (u64)pcap, c->dcount, overflow, bin_shift);
+    }
     DH_TICK(c, 3);
     if (ex && !pilot) {
       pt2_compact_kernel<<<sgrid, 256, 0, c->stream>>>(table, (u64)cap, ex->keys, ex->v, ex->score, ex->cap, ex->cursor);
@@ -646,7 +810,7 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
   c->ctr.pt2_parts = nparts;
   c->ctr.pt2_max_probe = (int32_t)max_probe;
   c->ctr.pt2_table_slots = slots;
-  c->ctr.pt2_binned = 0;
+  c->ctr.pt2_binned = binned ? 1 : 0;
   c->ctr.pt2_stream_bins = 0;
   c->ctr.pt2_sum_abs = sabs / norm2;
   c->ctr.pt2_min_abs_den = mden;
@@ -668,8 +832,8 @@ static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double ep
   // 36 G sectors/s up to 64 GB, 29 at 80 GB, 17 at 96 GB, 8.7 at 160 GB (profiles/r1_microbench.md).  More passes over a
   // smaller table beat fewer passes over a bigger one, so the table never exceeds this many bytes unless configured.
   const double max_table_gb = opt.max_table_gb > 0.0 ? opt.max_table_gb : 60.0;
-  // streamed organisation (pt2_stream.cu): chosen when the table organisation would need a table far beyond L2
-  const bool stream_ok = !ex && opt.mode != 1 && nd >= (int64_t)c->sm_count * 16;
+  // streamed organisation (pt2_stream.cu)
+  const bool stream_ok = !ex && opt.mode == 2 && nd >= (int64_t)c->sm_count * 16;
 
   // ---- plan: partition count and table capacity
   int pbits = 0;
@@ -728,8 +892,9 @@ static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double ep
       slots = need < max_slots ? need : max_slots;
     }
   }
-  // the table organisation would need this many bytes for one pass over everything; beyond 24 GB (or when asked to) stream
-  const bool stream = stream_ok && !hist.empty() && (opt.mode == 2 || max_class(0) / load * (double)sizeof(Slot) > 24e9);
+  // The streamed organisation runs when asked for (mode 2).  Measured on B200 (profiles/r2_pt2_summary.md) it is slower than the
+  // table organisation with binned passes on every configuration of BASELINE.json, so the planner does not choose it.
+  const bool stream = stream_ok && !hist.empty() && opt.mode == 2;
   int64_t probe_parts = 0;
   double pilot_distinct = 0.0;  // distinct externals of one of 2^pilot_pp key slices
   int pilot_pp = 0;
@@ -792,7 +957,8 @@ static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double ep
   }
   for (;;) {
     if (ex) DH_CUDA(c, cudaMemsetAsync(ex->cursor, 0, sizeof(u64), c->stream));
-    st = pt2_attempt(c, psi, e_s, eps2, pbits, slots, auto_slots && !ex, load, out, nullptr, ex);
+    const double est_pass = hist.empty() ? 0.0 : max_class(pbits);  // sizes the record pool of the binned passes
+    st = pt2_attempt(c, psi, e_s, eps2, pbits, slots, auto_slots && !ex, load, out, nullptr, ex, est_pass);
     if (st == DH_OK) c->ctr.pt2_probe_parts = probe_parts;
     if (st != DH_ETABLEFULL || !auto_parts || pbits >= DH_MAX_PBITS) return st;
     ++pbits;  // the plan was too optimistic: halve the keys per pass and start over

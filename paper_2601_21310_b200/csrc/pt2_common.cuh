@@ -31,6 +31,21 @@ __device__ __forceinline__ double dh_diag_from_scratch(int n, const double* __re
   return e_core + one + 0.5 * two;
 }
 
+// multiplicative mix of a key: positions a key inside a table region (the region itself comes from the partition word)
+__device__ __forceinline__ unsigned dh_key_hash(u64 ka, u64 kb) {
+  u64 h = ka * 0x9E3779B97F4A7C15ull + kb * 0xC2B2AE3D27D4EB4Full;
+  h ^= h >> 29;
+  h *= 0xBF58476D1CE4E5B9ull;
+  return (unsigned)(h >> 32);
+}
+// Home slot of a key in the HBM table.  rshift == 0: mulhi(partition word, capacity).  Binned passes (rshift > 0, capacity a
+// multiple of 2^rshift): region = mulhi(partition word, regions), position inside the region from the key itself, so that the
+// merge - which knows a record's region - needs no partition word.
+__device__ __forceinline__ u64 dh_table_slot(u64 z, u64 ka, u64 kb, u64 cap, int rshift) {
+  if (rshift == 0) return __umul64hi(z, cap);
+  return (__umul64hi(z, cap >> rshift) << rshift) | (u64)(dh_key_hash(ka, kb) >> (32 - rshift));
+}
+
 // reduce `nblk` rows of {sum, sum_abs, min_den, count} into out[4] (pt2.cu)
 void dh_launch_final_reduce4(const double* part, int nblk, double* out, cudaStream_t stream);
 

@@ -27,15 +27,11 @@ EnumParams dh_make_params(detham_ctx* c, const HbLists* L);
 
 namespace {
 
-constexpr int kGenWarps = 16;
 constexpr int kPairChunk = 64;   // occupied pairs per phase-A chunk
-constexpr int kExpandU = 2;      // staged references a thread expands together
-constexpr int kWalkU = 2;        // batches of 32 list entries a warp has in flight (their L2 loads overlap)
 constexpr int kMaxSrcSlots = 4;  // sources a warp can have staged references of at one time
 constexpr int kMaxBins = 4096;
-constexpr int kRing = 4;         // region tables in flight
-constexpr int kLag = 2;          // a warp reduces region b - kLag after merging region b: two regions of slack on either side, so
-                                 // that no warp waits for the slowest one of the region it has just finished
+constexpr int kRing = 3;         // region tables in flight: one being merged into, one being reduced, one cleared for the next
+constexpr int kLag = 1;          // the reduce units of region g - kLag follow the merge units of region g in the work list
 constexpr int kMergeWarps = 8;    // warps per merge CTA = units per block of the ordered work list
 constexpr int kMergeCtasPerSm = 4;
 constexpr int kUnitRec = 256;    // records of one merge unit (one warp)
@@ -44,23 +40,27 @@ constexpr int kMergeU = 2;       // records a lane has in flight (their CAS roun
 
 // ---------------------------------------------------------------------------------------------- shared-memory layout
 struct GenLayout {
-  unsigned tables, omask, ptab, warp0, warp_stride, slot_stride, occ_off, zq_off, pref_off, beg_off, meta_off, sq_off;
-  unsigned cnt, used, rec, rank, order, ctrl, total;
+  unsigned tables, omask, ptab, keys, warp0, warp_stride, occ_off, zq_off, cp_off, pref_off, beg_off, meta_off, sq_off;
+  unsigned cnt, used, cv, haa, meta, bin, rank, order, ctrl, total;
 };
 
 __host__ __device__ inline unsigned al16(unsigned x) { return (x + 15u) & ~15u; }
 
-__host__ __device__ inline GenLayout gen_layout(int n, int pbits, int npairs, int W, int K, int B, int N) {
+// bytes of staging per reference: H_ai psi_i 8, H_aa 8, orbitals + key slot 4, bin 2, rank 2, order 2
+constexpr unsigned kRefBytes = 26u;
+
+__host__ __device__ inline GenLayout gen_layout(int n, int pbits, int npairs, int W, int WU, int K, int B, int N) {
   GenLayout L;
   unsigned o = 0;
   L.tables = o; o = al16(o + (unsigned)(n + 128) * 8u);  // h_pp and the key-partition words; J, J-K stay in L2 (read by rows)
   L.omask = o; o = al16(o + 2u * (1u << pbits) * 8u);
   L.ptab = o; o = al16(o + (unsigned)npairs * 2u);
-  L.slot_stride = (unsigned)(2 * n + 6) * 8u;
+  L.keys = o; o = al16(o + (unsigned)(W * K) * 16u);     // {alpha, beta} of the sources that staged references point to
   unsigned w = 0;
-  w = al16(w + (unsigned)K * L.slot_stride);
+  w = al16(w + (unsigned)(2 * n) * 8u);                  // U vectors of the warp's current source
   L.occ_off = w; w = al16(w + 4u * DH_MAX_ORB);
   L.zq_off = w; w = al16(w + kPairChunk * 8u);
+  L.cp_off = w; w = al16(w + kPairChunk * 8u);
   L.pref_off = w; w = al16(w + (kPairChunk + 1) * 4u);
   L.beg_off = w; w = al16(w + kPairChunk * 4u);
   L.meta_off = w; w = al16(w + kPairChunk * 2u);
@@ -69,16 +69,21 @@ __host__ __device__ inline GenLayout gen_layout(int n, int pbits, int npairs, in
   L.warp0 = o; o += (unsigned)W * w;
   L.cnt = o; o = al16(o + (unsigned)(B + 1) * 4u);
   L.used = o; o = al16(o + (unsigned)B * 4u);
-  const unsigned NS = (unsigned)(N + 32 * kWalkU * W);
-  L.rec = o; o = al16(o + NS * 8u);
+  const unsigned NS = (unsigned)(N + 32 * WU * W);
+  L.cv = o; o = al16(o + NS * 8u);
+  L.haa = o; o = al16(o + NS * 8u);
+  L.meta = o; o = al16(o + NS * 4u);
+  L.bin = o; o = al16(o + NS * 2u);
   L.rank = o; o = al16(o + NS * 2u);
   L.order = o; o = al16(o + NS * 2u);
-  L.ctrl = o; o = al16(o + 128u);
+  L.ctrl = o; o = al16(o + 256u);
   L.total = o;
   return L;
 }
 
-// staged reference (8 bytes): bin 12 | list entry 25 | i 6 | j 6 | fam 2 | source slot 3 | warp 5
+// staged reference: H_ai psi_i and H_aa (computed by the walker, whose source is in registers), and 4 bytes of orbitals and
+// key slot - a 6 | b 6 | i 6 | j 6 | fam 2 | key slot 6 - from which the expansion rebuilds the 128-bit key
+
 
 // bit t of the result = parity of the electrons of w below orbital t
 __device__ __forceinline__ u64 prefix_parity(u64 w) {
@@ -112,6 +117,7 @@ struct GenParams {
 
 __device__ __forceinline__ int ld_shared_volatile(const int* p) { return *reinterpret_cast<const volatile int*>(p); }
 
+template <int kGenWarps, int kWalkU>
 __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G) {
   extern __shared__ __align__(16) unsigned char smem[];
   const EnumParams& P = G.E;
@@ -119,7 +125,7 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
   const int NP = 1 << P.pbits;
   const unsigned pmask = (unsigned)NP - 1u;
   const int B = G.nbins, N = G.stage_n, K = G.nslots, npairs = G.npairs;
-  const GenLayout L = gen_layout(n, P.pbits, npairs, kGenWarps, K, B, N);
+  const GenLayout L = gen_layout(n, P.pbits, npairs, kGenWarps, kWalkU, K, B, N);
   CtaTables T;
   T.J = const_cast<double*>(P.J); T.JK = const_cast<double*>(P.JK);  // global (L2): only the per-source U vectors read them
   T.hd = reinterpret_cast<double*>(smem + L.tables);
@@ -130,7 +136,11 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
   unsigned short* ptab = reinterpret_cast<unsigned short*>(smem + L.ptab);  // pair q -> fam << 12 | x << 6 | y (positions in occ)
   unsigned* cnt = reinterpret_cast<unsigned*>(smem + L.cnt);
   unsigned* used = reinterpret_cast<unsigned*>(smem + L.used);
-  u64* rec = reinterpret_cast<u64*>(smem + L.rec);
+  double* scv = reinterpret_cast<double*>(smem + L.cv);      // staged references (structure of arrays)
+  double* shaa = reinterpret_cast<double*>(smem + L.haa);
+  unsigned* smeta = reinterpret_cast<unsigned*>(smem + L.meta);
+  unsigned short* sbin = reinterpret_cast<unsigned short*>(smem + L.bin);
+  ulonglong2* keys = reinterpret_cast<ulonglong2*>(smem + L.keys);  // [warp * K + slot]
   unsigned short* rnk = reinterpret_cast<unsigned short*>(smem + L.rank);
   unsigned short* order = reinterpret_cast<unsigned short*>(smem + L.order);
   int* ctrl = reinterpret_cast<int*>(smem + L.ctrl);  // [0] staged references [1] warps out of work [3] singles of this round [4..] scan carries
@@ -169,7 +179,9 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
 
   unsigned char* wb = smem + L.warp0 + (unsigned)warp * L.warp_stride;
   unsigned char (*occ)[DH_MAX_ORB] = reinterpret_cast<unsigned char (*)[DH_MAX_ORB]>(wb + L.occ_off);  // occ[0..1], vir = occ[2..3]
+  double* const U = reinterpret_cast<double*>(wb);  // U[s * n + p] of the warp's current source
   u64* zq = reinterpret_cast<u64*>(wb + L.zq_off);
+  double* cp = reinterpret_cast<double*>(wb + L.cp_off);  // per pair of the chunk: E(D) - U(i) - U(j)
   int* pref = reinterpret_cast<int*>(wb + L.pref_off);
   int* pbeg = reinterpret_cast<int*>(wb + L.beg_off);
   unsigned short* pmeta = reinterpret_cast<unsigned short*>(wb + L.meta_off);
@@ -181,7 +193,7 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
   int phase = 0;  // 0 fetch a source, 1 singles, 2 phase A of chunk qb, 3 phase B
   int cur_slot = 0, qb = 0, pcnt = 0, TT = 0, t0 = 0, qcur = 0, sl = 0, sqn = 0;
   bool out_of_rows = false, reported = false;
-  u64 da = 0, db = 0, zsrc = 0;
+  u64 da = 0, db = 0, zsrc = 0, ppa = 0, ppb = 0;
   double psi_v = 0.0, tau = 0.0, e0 = 0.0;
   u64 gen_total = 0, contrib_total = 0;
 
@@ -223,13 +235,25 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
           for (int o = 16; o > 0; o >>= 1) z ^= __shfl_xor_sync(full, z, o);
           zsrc = z;
         }
-        // U vectors, E(D), prefix parities into the source slot
-        double* U = reinterpret_cast<double*>(wb + (unsigned)cur_slot * L.slot_stride);
+        // U vectors, E(D), prefix parities; the key goes into the slot that this round's references will name
         for (int p = lane; p < n; p += 32) {
           double ua = T.hd[p], ub = T.hd[p];
           // J and J-K are symmetric (bit for bit: one packed integral each way): row q read by consecutive lanes
-          for (int k = 0; k < na; ++k) { const int q = occ[0][k]; ua += __ldg(T.JK + q * n + p); ub += __ldg(T.J + q * n + p); }
-          for (int k = 0; k < nb; ++k) { const int q = occ[1][k]; ua += __ldg(T.J + q * n + p); ub += __ldg(T.JK + q * n + p); }
+          // (four rows' loads are issued before the first is added; the additions keep their order)
+          for (int s = 0; s < 2; ++s) {
+            const int ne = s ? nb : na;
+            const double* A = s ? T.J : T.JK;   // what an electron of spin s adds to U_alpha
+            const double* Bm = s ? T.JK : T.J;  // ... and to U_beta
+            int k = 0;
+            for (; k + 4 <= ne; k += 4) {
+              double x[4], y[4];
+#pragma unroll
+              for (int u = 0; u < 4; ++u) { const int q = occ[s][k + u]; x[u] = __ldg(A + q * n + p); y[u] = __ldg(Bm + q * n + p); }
+#pragma unroll
+              for (int u = 0; u < 4; ++u) { ua += x[u]; ub += y[u]; }
+            }
+            for (; k < ne; ++k) { const int q = occ[s][k]; ua += __ldg(A + q * n + p); ub += __ldg(Bm + q * n + p); }
+          }
           U[p] = ua; U[n + p] = ub;
         }
         __syncwarp();
@@ -240,11 +264,8 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
           for (int o = 16; o > 0; o >>= 1) e += __shfl_xor_sync(full, e, o);
           e0 = P.e_core + 0.5 * e;
         }
-        if (lane == 0) {
-          u64* sw = reinterpret_cast<u64*>(U + 2 * n);
-          sw[0] = da; sw[1] = db; sw[2] = prefix_parity(da); sw[3] = prefix_parity(db);
-          reinterpret_cast<double*>(sw)[4] = psi_v; reinterpret_cast<double*>(sw)[5] = e0;
-        }
+        ppa = prefix_parity(da); ppb = prefix_parity(db);
+        if (lane == 0) keys[warp * K + cur_slot] = make_ulonglong2(da, db);
         __syncwarp();
         phase = 1; sl = 0; sqn = 0;
         continue;
@@ -285,7 +306,6 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
               if (s == 0) ka = nw; else kb = nw;
               const u64 z = zsrc ^ T.Z[64 * s + i] ^ T.Z[64 * s + a];
               ok = true;
-              const double* U = reinterpret_cast<const double*>(wb + (unsigned)cur_slot * L.slot_stride);
               haa = e0 - U[s * n + i] + U[s * n + a] - __ldg(T.JK + i * n + a);
               cv = v * psi_v;
               bin = __umulhi((unsigned)(z >> 32), (unsigned)B);
@@ -319,6 +339,7 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
           int len = 0, beg = 0;
           unsigned pm = 0;
           u64 zij = 0;
+          double cpair = 0.0;
           if (q < qe) {
             const unsigned pt = ptab[q];
             const int fam = (int)(pt >> 12), x = (int)((pt >> 6) & 63u), y = (int)(pt & 63u);
@@ -331,16 +352,30 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
             beg = __ldg(P.sub_off + so);
             const int end = __ldg(P.sub_off + so + 1);
             // first index whose |value| < tau (tau == 0: whose value == 0, reading Q8): gallop from the head, then bisect
-            int lo = beg, hi = end;
+            int lo = beg, hi = end;  // entries before lo are kept, entries from hi on are not
             {
-              int pos = beg, step = 1;
-              for (;;) {
-                if (pos >= end) break;
-                const double av = fabs(__ldg(P.lval + pos));
-                if (!(av >= tau && av != 0.0)) break;
-                lo = pos + 1; pos += step; step <<= 1;
+              // four probes at once (most kept prefixes are short), then gallop on or bisect the bracket
+              double pv[4];
+#pragma unroll
+              for (int u = 0; u < 4; ++u) { const int idx = beg + (1 << u) - 1; pv[u] = idx < end ? fabs(__ldg(P.lval + idx)) : 0.0; }
+              bool open_end = true;
+#pragma unroll
+              for (int u = 0; u < 4; ++u) {
+                const int idx = beg + (1 << u) - 1;
+                if (open_end && idx < end) {
+                  if (pv[u] >= tau && pv[u] != 0.0) lo = idx + 1; else { hi = idx; open_end = false; }
+                }
               }
-              hi = min(pos, end);
+              if (open_end && lo < end) {
+                int pos = lo + 7, step = 16;
+                for (;;) {
+                  if (pos >= end) break;
+                  const double av = fabs(__ldg(P.lval + pos));
+                  if (!(av >= tau && av != 0.0)) break;
+                  lo = pos + 1; pos += step; step <<= 1;
+                }
+                hi = min(pos, end);
+              }
               while (lo < hi) {
                 const int mid = (lo + hi) >> 1;
                 const double av = fabs(__ldg(P.lval + mid));
@@ -349,6 +384,7 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
             }
             len = lo - beg;
             pm = ((unsigned)fam << 12) | ((unsigned)j << 6) | (unsigned)i;  // same field order as the staged reference
+            cpair = e0 - U[(fam == 1 ? n : 0) + i] - U[(fam != 0 ? n : 0) + j];
           }
           const unsigned m = __ballot_sync(full, len > 0);
           int x = len;
@@ -357,7 +393,7 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
           const int tot = __shfl_sync(full, x, 31);
           if (len > 0) {
             const int idx = cntp + __popc(m & lt);
-            pref[idx] = run + x - len; pbeg[idx] = beg; pmeta[idx] = (unsigned short)pm; zq[idx] = zij;
+            pref[idx] = run + x - len; pbeg[idx] = beg; pmeta[idx] = (unsigned short)pm; zq[idx] = zij; cp[idx] = cpair;
           }
           cntp += __popc(m);
           run += tot;
@@ -370,14 +406,16 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
         continue;
       }
       // ---- phase B: kWalkU x 32 entries of the concatenated kept prefixes; stage the valid, non-member ones.  Three steps so
-      // that the list loads of all batches, then the filter loads of all batches, are in flight together.
+      // that the list loads of all batches, then the filter loads of all batches, are in flight together.  The walker's
+      // source is in registers and its list entries are consecutive, so value, sign and H_aa are finished here.
       {
         bool ok[kWalkU];
-        int kk[kWalkU], mq[kWalkU];
+        int mq[kWalkU];
         unsigned abv[kWalkU];
+        double lv[kWalkU], ls[kWalkU];
 #pragma unroll
         for (int u = 0; u < kWalkU; ++u) {
-          ok[u] = false; kk[u] = 0; mq[u] = 0; abv[u] = 0u;
+          ok[u] = false; mq[u] = 0; abv[u] = 0u; lv[u] = 0.0; ls[u] = 0.0;
           const int tt = t0 + 32 * u;
           if (tt < TT) {  // warp-uniform
             const int pe = (qcur + lane < pcnt) ? pref[qcur + lane + 1] - tt : 0x7fffffff;  // end of pair qcur+lane, relative
@@ -388,8 +426,10 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
             const int t = tt + lane;
             if (t < TT) {
               ok[u] = true; mq[u] = myq;
-              kk[u] = pbeg[myq] + (t - pref[myq]);
-              abv[u] = __ldg(P.lab + kk[u]);
+              const int k = pbeg[myq] + (t - pref[myq]);
+              abv[u] = __ldg(P.lab + k);
+              lv[u] = __ldg(P.lval + k);
+              ls[u] = __ldg(P.lstat + k);
             }
           }
         }
@@ -409,6 +449,8 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
               const u64 z = zq[mq[u]] ^ T.Z[64 * si + a] ^ T.Z[64 * sj + b];
               zv[u] = z; pmv[u] = pm;
               fw[u] = __ldg(reinterpret_cast<const u64*>(G.sbits) + dh_filter_word(G.sbits_n, z));
+              // H_aa = E(D) - U(i) - U(j) + U(a) + U(b) + the entry's source-independent part (the O(1) diagonal update)
+              ls[u] = cp[mq[u]] + U[si * n + a] + U[sj * n + b] + ls[u];
             }
           }
         }
@@ -418,14 +460,20 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
         for (int u = 0; u < kWalkU; ++u) {
           if (ok[u]) {
             gen_total += 1;
+            const unsigned pm = pmv[u], fam = pm >> 12;
+            const unsigned si = fam == 1u, sj = fam != 0u;
+            const int i = (int)(pm & 63u), j = (int)((pm >> 6) & 63u), a = (int)(abv[u] & 0xFFu), b = (int)(abv[u] >> 8);
             const u64 fm = dh_filter_mask(zv[u]);
             if ((fw[u] & fm) == fm) {  // rare: look the key up in the index of S
-              const unsigned pm = pmv[u], fam = pm >> 12;
-              const unsigned si = fam == 1u, sj = fam != 0u;
-              const u64 bia = (1ull << (pm & 63u)) | (1ull << (abv[u] & 0xFFu)), bjb = (1ull << ((pm >> 6) & 63u)) | (1ull << (abv[u] >> 8));
+              const u64 bia = (1ull << i) | (1ull << a), bjb = (1ull << j) | (1ull << b);
               const u64 ka = da ^ ((si ? 0ull : bia) | (sj ? 0ull : bjb)), kb = db ^ ((si ? bia : 0ull) | (sj ? bjb : 0ull));
               if (dh_shash_find(G.shash_key, G.shash_idx, G.shash_cap, ka, kb, zv[u]) >= 0) ok[u] = false;
             }
+            // reading Q1: a same-spin double is a+_a a+_b a_j a_i = (a+_b a_j)(a+_a a_i): phase(i->a on w) * phase(j->b on w with
+            // i->a applied); an alpha-beta double is the product of its two single phases
+            unsigned par = par_between(si ? ppb : ppa, i, a) ^ par_between(sj ? ppb : ppa, j, b);
+            if (fam < 2u) par ^= strictly_between(i, j, b) ^ strictly_between(a, j, b);
+            lv[u] = (par ? -lv[u] : lv[u]) * psi_v;
           }
           msk[u] = __ballot_sync(full, ok[u]);
           nstage += __popc(msk[u]);
@@ -439,7 +487,10 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
             if (ok[u]) {
               const int idx = base + __popc(msk[u] & lt);
               const unsigned bin = __umulhi((unsigned)(zv[u] >> 32), (unsigned)B);
-              rec[idx] = (u64)bin | ((u64)(unsigned)kk[u] << 12) | ((u64)(pmv[u] & 0x3FFFu) << 37) | ((u64)cur_slot << 51) | ((u64)warp << 54);
+              scv[idx] = lv[u]; shaa[idx] = ls[u];
+              // a 6 | b 6 | i 6 | j 6 | fam 2 | key slot 6   (pmv = fam << 12 | j << 6 | i)
+              smeta[idx] = (abv[u] & 0x3Fu) | ((abv[u] >> 8) << 6) | ((pmv[u] & 0x3FFFu) << 12) | ((unsigned)(warp * K + cur_slot) << 26);
+              sbin[idx] = (unsigned short)bin;
               rnk[idx] = (unsigned short)atomicAdd(&cnt[bin], 1u);
               contrib_total += 1;
             }
@@ -478,65 +529,26 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
       __syncthreads();
     }
     const int total = (int)cnt[B];  // references + singles of this round
-    for (int idx = tid; idx < staged; idx += nthr) order[cnt[(unsigned)rec[idx] & 0xFFFu] + rnk[idx]] = (unsigned short)idx;
+    for (int idx = tid; idx < staged; idx += nthr) order[cnt[sbin[idx]] + rnk[idx]] = (unsigned short)idx;
     __syncthreads();
 
     if (G.prof && tid == 0) { const long long t = clock64(); pacc[2] += t - pc0; pc0 = t; }
     // =================================================================== expand in bin order and write the runs
-    for (int t0 = tid; t0 < total; t0 += nthr * kExpandU) {
-      // kExpandU references per thread: their list loads (value, orbital pair: L2) are issued before any is used
-      u64 rr[kExpandU];
-      double vv[kExpandU], sst[kExpandU];
-      unsigned abv[kExpandU];
-      bool live[kExpandU];
-#pragma unroll
-      for (int u = 0; u < kExpandU; ++u) {
-        const int t = t0 + u * nthr;
-        live[u] = false; rr[u] = 0ull; vv[u] = 0.0; sst[u] = 0.0; abv[u] = 0u;
-        if (t < total) {
-          const unsigned idx = order[t];
-          if (idx != 0xFFFFu) {  // 0xFFFF: a single, already written by the walker
-            order[t] = 0xFFFFu;
-            live[u] = true;
-            rr[u] = rec[idx];
-            const unsigned k = (unsigned)(rr[u] >> 12) & 0x1FFFFFFu;
-            vv[u] = __ldg(P.lval + k);
-            sst[u] = __ldg(P.lstat + k);
-            abv[u] = __ldg(P.lab + k);
-          }
-        }
-      }
-#pragma unroll
-      for (int u = 0; u < kExpandU; ++u) {
-        if (!live[u]) continue;
-        const int t = t0 + u * nthr;
-        const u64 r = rr[u];
-        const unsigned bin = (unsigned)r & 0xFFFu;
-        const int i = (int)(r >> 37) & 63, j = (int)(r >> 43) & 63, fam = (int)(r >> 49) & 3;
-        const unsigned slot = (unsigned)(r >> 51) & 7u, w = (unsigned)(r >> 54) & 31u;
-        const double* U = reinterpret_cast<const double*>(smem + L.warp0 + w * L.warp_stride + slot * L.slot_stride);
-        const u64* sw = reinterpret_cast<const u64*>(U + 2 * n);
-        const u64 sda = sw[0], sdb = sw[1];
-        const double spsi = reinterpret_cast<const double*>(sw)[4], se0 = reinterpret_cast<const double*>(sw)[5];
-        double v = vv[u];
-        const int a = (int)(abv[u] & 0xFFu), b = (int)(abv[u] >> 8);
-        // one code path for the three families: fam 0 = alpha-alpha, 1 = beta-beta (i<j -> a<b in one spin), 2 = (i alpha -> a, j beta -> b)
-        const unsigned si = fam == 1, sj = fam != 0;  // spin of (i, a) and of (j, b)
-        const u64 bia = (1ull << i) | (1ull << a), bjb = (1ull << j) | (1ull << b);
-        const u64 ka = sda ^ ((si ? 0ull : bia) | (sj ? 0ull : bjb)), kb = sdb ^ ((si ? bia : 0ull) | (sj ? bjb : 0ull));
-        // reading Q1: a same-spin double is a+_a a+_b a_j a_i = (a+_b a_j)(a+_a a_i): phase(i->a on w) * phase(j->b on w with
-        // i->a applied); an alpha-beta double is the product of its two single phases
-        unsigned par = par_between(sw[2 + si], i, a) ^ par_between(sw[2 + sj], j, b);
-        if (fam < 2) par ^= strictly_between(i, j, b) ^ strictly_between(a, j, b);
-        const double* Ui = U + si * n;
-        const double* Uj = U + sj * n;
-        const double haa = se0 - Ui[i] - Uj[j] + Ui[a] + Uj[b] + sst[u];
-        if (par) v = -v;
-        const double cv = v * spsi;
-        const unsigned pos = used[bin] + ((unsigned)t - cnt[bin]);
-        if (pos < G.seg_cap) dh_st256(my_pool + (size_t)bin * seg_stride + pos, ka, kb, (u64)__double_as_longlong(cv), (u64)__double_as_longlong(haa));
-        else *G.overflow = 1;
-      }
+    for (int t = tid; t < total; t += nthr) {
+      const unsigned idx = order[t];
+      if (idx == 0xFFFFu) continue;  // a single: already written by the walker
+      order[t] = 0xFFFFu;
+      const unsigned m = smeta[idx], bin = sbin[idx];
+      const ulonglong2 src = keys[m >> 26];
+      const int a = (int)(m & 63u), b = (int)((m >> 6) & 63u), i = (int)((m >> 12) & 63u), j = (int)((m >> 18) & 63u);
+      const unsigned fam = (m >> 24) & 3u;
+      // one code path for the three families: fam 0 = alpha-alpha, 1 = beta-beta (i<j -> a<b in one spin), 2 = (i alpha -> a, j beta -> b)
+      const unsigned si = fam == 1u, sj = fam != 0u;  // spin of (i, a) and of (j, b)
+      const u64 bia = (1ull << i) | (1ull << a), bjb = (1ull << j) | (1ull << b);
+      const u64 ka = src.x ^ ((si ? 0ull : bia) | (sj ? 0ull : bjb)), kb = src.y ^ ((si ? bia : 0ull) | (sj ? bjb : 0ull));
+      const unsigned pos = used[bin] + ((unsigned)t - cnt[bin]);
+      if (pos < G.seg_cap) dh_st256(my_pool + (size_t)bin * seg_stride + pos, ka, kb, (u64)__double_as_longlong(scv[idx]), (u64)__double_as_longlong(shaa[idx]));
+      else *G.overflow = 1;
     }
     __syncthreads();
     if (G.prof && tid == 0) { const long long t = clock64(); pacc[3] += t - pc0; pc0 = t; }
@@ -556,7 +568,10 @@ __global__ void __launch_bounds__(kGenWarps * 32, 1) pt2_gen_kernel(GenParams G)
     if (all_done && total == 0) break;
   }
   if (G.prof && tid == 0) for (int k = 0; k < 6; ++k) G.prof[6 * blockIdx.x + k] = (u64)pacc[k];
-  for (int b = tid; b < B; b += nthr) G.used_out[(size_t)b * gridDim.x + blockIdx.x] = min(used[b], G.seg_cap);
+  unsigned mx = 0;
+  for (int b = tid; b < B; b += nthr) { const unsigned ub = min(used[b], G.seg_cap); G.used_out[(size_t)b * gridDim.x + blockIdx.x] = ub; mx = max(mx, ub); }
+  for (int o = 16; o > 0; o >>= 1) mx = max(mx, __shfl_xor_sync(full, mx, o));
+  if (lane == 0 && mx) atomicMax(G.counters + 20, (u64)mx);  // fullest segment of the pass: sizes the merge's work list
   u64 g = gen_total, ct = contrib_total;
   for (int o = 16; o > 0; o >>= 1) { g += __shfl_xor_sync(full, g, o); ct += __shfl_xor_sync(full, ct, o); }
   if (lane == 0) {
@@ -574,6 +589,8 @@ struct MergeParams {
   double* part;  // [gridDim.x][4]: sum, sum_abs, min_den, count
   int* overflow;
   u64* ticket;  // next unit of the ordered work list
+  const u64* max_used;  // records of the fullest segment of the pass (written by the generator)
+  int ring_n, lag;
 };
 
 // L2 eviction policies (createpolicy): the region tables are the only reused lines of the merge - evict_last; the records are
@@ -609,14 +626,6 @@ __device__ __forceinline__ unsigned ld_acquire_u32(const unsigned* p) {
   asm volatile("ld.acquire.gpu.global.u32 %0, [%1];" : "=r"(v) : "l"(p) : "memory");
   return v;
 }
-// slot hash of a key inside its region: the bin already consumed the partition word, so this one is a multiplicative mix
-__device__ __forceinline__ unsigned key_hash(u64 ka, u64 kb) {
-  u64 h = ka * 0x9E3779B97F4A7C15ull + kb * 0xC2B2AE3D27D4EB4Full;
-  h ^= h >> 29;
-  h *= 0xBF58476D1CE4E5B9ull;
-  return (unsigned)(h >> 32);
-}
-
 __device__ __noinline__ double diag_cold(int n, const double* J, const double* JK, const double* hd, double e_core, u64 a, u64 b) {
   return dh_diag_from_scratch(n, J, JK, hd, e_core, a, b);
 }
@@ -631,11 +640,12 @@ __global__ void __launch_bounds__(kMergeWarps * 32, kMergeCtasPerSm) pt2_merge_k
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const unsigned full = 0xffffffffu;
   const u64 keep = l2_policy_evict_last(), once = l2_policy_evict_first();
-  const unsigned QS = (M.seg_cap + kUnitRec - 1) / kUnitRec;                                   // merge units per segment (by capacity)
+  const unsigned QS = max(1u, ((unsigned)*M.max_used + kUnitRec - 1) / kUnitRec);               // merge units per segment (fullest one)
   const unsigned UM = ((unsigned)M.nseg * QS + kMergeWarps - 1) / kMergeWarps * kMergeWarps;   // merge units per region, whole blocks
   const unsigned US = ((M.cap + kUnitSlots - 1) / kUnitSlots + kMergeWarps - 1) / kMergeWarps * kMergeWarps;  // reduce units per region
   const unsigned GS = UM + US;
-  const u64 total = (u64)(M.nbins + kLag) * GS;
+  const int kR = M.ring_n, kL = M.lag;
+  const u64 total = (u64)(M.nbins + kL) * GS;
   double sum = 0.0, sabs = 0.0, mden = INFINITY, cntd = 0.0;
   __shared__ u64 s_base;
   u64 next = 0;
@@ -648,21 +658,21 @@ __global__ void __launch_bounds__(kMergeWarps * 32, kMergeCtasPerSm) pt2_merge_k
     if (base >= total) break;
     const unsigned g = (unsigned)(base / GS), r = (unsigned)(base % GS);
     const bool is_merge = r < UM;
-    const int bin = is_merge ? (int)g : (int)g - kLag;
+    const int bin = is_merge ? (int)g : (int)g - kL;
     const bool valid = bin >= 0 && bin < M.nbins;
     if (threadIdx.x == 0) {
       next = atomicAdd(M.ticket, (u64)kMergeWarps);  // the next block's ticket travels while this one is worked on
       if (valid) {
         const unsigned* dep = nullptr;
         unsigned target = 0;
-        if (is_merge) { if (bin >= kRing) { dep = M.cleared + (bin - kRing); target = US / kMergeWarps; } }
+        if (is_merge) { if (bin >= kR) { dep = M.cleared + (bin - kR); target = US / kMergeWarps; } }
         else { dep = M.merged + bin; target = UM / kMergeWarps; }
         if (dep) { unsigned ns = 32; while (ld_acquire_u32(dep) < target) { __nanosleep(ns); if (ns < 1024) ns *= 2; } }
       }
     }
     __syncthreads();
     if (!valid) continue;
-    Slot* tb = M.ring + (size_t)(bin % kRing) * M.cap;
+    Slot* tb = M.ring + (size_t)(bin % kR) * M.cap;
     if (is_merge) {
       const unsigned u = r + warp;
       const unsigned s = u / QS, q = u % QS;
@@ -681,7 +691,7 @@ __global__ void __launch_bounds__(kMergeWarps * 32, kMergeCtasPerSm) pt2_merge_k
             if (t < hi) { ld256_stream(src + t, ka[k], kb[k], vv[k], hh[k], once); pend |= 1u << k; }
           }
 #pragma unroll
-          for (int k = 0; k < kMergeU; ++k) slot[k] = __umulhi(key_hash(ka[k], kb[k]), M.cap);
+          for (int k = 0; k < kMergeU; ++k) slot[k] = __umulhi(dh_key_hash(ka[k], kb[k]), M.cap);
           // every pending record's claim is issued before any result is looked at
           for (int probes = 0; pend; ++probes) {
             Key128 old[kMergeU];
@@ -777,12 +787,21 @@ dh_status dh_pt2_stream(detham_ctx* c, const double* psi, double e_s, double eps
   GenParams G{};
   G.E = dh_make_params(c, L);
   const int grid = c->sm_count;
+  // generator launch shape: (warps per CTA, batches of 32 list entries in flight per warp)
+  using GenKernel = void (*)(GenParams);
+  struct GenVariant { int warps, u; GenKernel k; };
+  static const GenVariant variants[] = {{16, 2, pt2_gen_kernel<16, 2>}, {24, 2, pt2_gen_kernel<24, 2>}, {32, 2, pt2_gen_kernel<32, 2>}, {32, 1, pt2_gen_kernel<32, 1>}};
+  int vi = 0;
+  if (const char* e = getenv("DETHAM_GEN")) { int v = atoi(e); if (v >= 0 && v < 4) vi = v; }
+  const int kGenWarps = variants[vi].warps, kWalkU = variants[vi].u;
   if (nd < (int64_t)grid * kGenWarps || pbits > 8) return DH_EINVAL;  // the caller keeps small inputs on the table organisation
 
   // ---- region tables: kRing of them share the L2 budget; bins so that a region's distinct keys load it to <= `load`
   const double load = c->opt.stream_load > 0.0 ? c->opt.stream_load : 0.45;
-  const double ring_mb = c->opt.stream_ring_mb > 0.0 ? c->opt.stream_ring_mb : 60.0;
-  const double cap_max = ring_mb * 1048576.0 / (kRing * sizeof(Slot));
+  const double ring_mb = c->opt.stream_ring_mb > 0.0 ? c->opt.stream_ring_mb : 96.0;
+  int ring_n = kRing;
+  if (const char* e = getenv("DETHAM_RING")) { int v = atoi(e); if (v >= 2 && v <= 8) ring_n = v; }
+  const double cap_max = ring_mb * 1048576.0 / (ring_n * sizeof(Slot));
   const double distinct = plan.est_distinct > 0.0 ? plan.est_distinct : plan.est_records;
   int nbins = c->opt.stream_bins > 0 ? c->opt.stream_bins : (int)ceil(distinct / (load * cap_max));
   nbins = std::max(nbins, 16);
@@ -790,7 +809,7 @@ dh_status dh_pt2_stream(detham_ctx* c, const double* psi, double e_s, double eps
   // a region holds its share of the distinct keys plus their spread (hash-uniform bins: 6 sigma) at the target load
   const double per_bin = distinct / nbins;
   const unsigned cap = (unsigned)std::min(4.0e9, std::max(4096.0, (per_bin + 6.0 * sqrt(per_bin) + 64.0) / load));
-  const size_t ring_bytes = (size_t)kRing * cap * sizeof(Slot);
+  const size_t ring_bytes = (size_t)ring_n * cap * sizeof(Slot);
   if (c->ring_bytes < ring_bytes) {
     if (c->ring) cudaFree(c->ring);
     c->ring = nullptr; c->ring_bytes = 0;
@@ -828,17 +847,14 @@ dh_status dh_pt2_stream(detham_ctx* c, const double* psi, double e_s, double eps
   const int npairs = na * (na - 1) / 2 + nb * (nb - 1) / 2 + na * nb;
   int smem_max = 0;
   DH_CUDA(c, cudaDeviceGetAttribute(&smem_max, cudaDevAttrMaxSharedMemoryPerBlockOptin, c->device));
-  int K = kMaxSrcSlots, N = 0;
-  for (; K >= 2; --K) {
-    const GenLayout L0 = gen_layout(n, pbits, npairs, kGenWarps, K, nbins, 0);
-    N = ((int)smem_max - (int)L0.total - 64) / 12;
-    if (N >= 4 * 1024 || K == 2) break;
-  }
+  const int K = std::min(kMaxSrcSlots, 64 / kGenWarps);  // key slots per warp (16 bytes each; 6 bits name a slot)
+  const GenLayout L0 = gen_layout(n, pbits, npairs, kGenWarps, kWalkU, K, nbins, 0);
+  int N = ((int)smem_max - (int)L0.total - 96) / (int)kRefBytes;
   N = std::min(N, 60000) & ~31;
   if (N < 1024) return DH_EINVAL;
-  const GenLayout GL = gen_layout(n, pbits, npairs, kGenWarps, K, nbins, N);
+  const GenLayout GL = gen_layout(n, pbits, npairs, kGenWarps, kWalkU, K, nbins, N);
   if (c->debug) fprintf(stderr, "[detham] generator: staging %d references, %d source slots per warp, %u bytes of shared memory\n", N, K, GL.total);
-  DH_CUDA(c, cudaFuncSetAttribute(pt2_gen_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GL.total));
+  DH_CUDA(c, cudaFuncSetAttribute(variants[vi].k, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)GL.total));
   G.dets = c->dets; G.psi = psi; G.nd = nd; G.eps2 = eps2;
   G.sbits = c->sbits; G.sbits_n = (u64)c->sbits_n; G.shash_key = c->shash_key; G.shash_idx = c->shash_idx; G.shash_cap = (u64)c->shash_cap;
   G.nbins = nbins; G.seg_cap = seg_cap; G.pool = reinterpret_cast<Slot*>(c->pool); G.used_out = used;
@@ -854,6 +870,10 @@ dh_status dh_pt2_stream(detham_ctx* c, const double* psi, double e_s, double eps
   M.small_den = c->opt.small_den == 0.0 ? 1e-3 : (c->opt.small_den < 0.0 ? 0.0 : c->opt.small_den);
   M.overflow = G.overflow;
   M.ticket = c->dcount + 16;
+  M.max_used = c->dcount + 20;
+  M.ring_n = kRing; M.lag = kLag;
+  if (const char* e = getenv("DETHAM_RING")) { int v = atoi(e); if (v >= 2 && v <= 8) M.ring_n = v; }
+  if (const char* e = getenv("DETHAM_LAG")) { int v = atoi(e); if (v >= 1 && v < M.ring_n) M.lag = v; }
   int merge_occ = 0;
   DH_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&merge_occ, pt2_merge_kernel, kMergeWarps * 32, 0));
   if (merge_occ < 1) return DH_ECUDA;
@@ -900,11 +920,11 @@ dh_status dh_pt2_stream(detham_ctx* c, const double* psi, double e_s, double eps
   while ((int)c->sev.size() < 3 * nparts) { cudaEvent_t e; DH_CUDA(c, cudaEventCreate(&e)); c->sev.push_back(e); }
   for (int pass = 0; pass < nparts; ++pass) {
     DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, sizeof(u64), c->stream));  // the row cursor; [1], [2], [8] accumulate over the passes
-    DH_CUDA(c, cudaMemsetAsync(c->dcount + 16, 0, sizeof(u64), c->stream));  // the merge's unit counter
+    DH_CUDA(c, cudaMemsetAsync(c->dcount + 16, 0, 8 * sizeof(u64), c->stream));  // the merge's unit counter [16], fullest segment [20]
     DH_CUDA(c, cudaMemsetAsync(flags, 0, 2 * (size_t)nbins * sizeof(unsigned), c->stream));
     DH_CUDA(c, cudaEventRecord(c->sev[3 * pass], c->stream));
     G.pass = (unsigned)pass;
-    pt2_gen_kernel<<<grid, kGenWarps * 32, GL.total, c->stream>>>(G);
+    variants[vi].k<<<grid, kGenWarps * 32, GL.total, c->stream>>>(G);
     DH_CUDA(c, cudaGetLastError());
     DH_CUDA(c, cudaEventRecord(c->sev[3 * pass + 1], c->stream));
     {

@@ -51,7 +51,11 @@ def make_integrals(n: int, L: int, seed: int, band=None, slope: float = 1.0):
     iu, ju = np.tril_indices(n)  # iu >= ju, ordered by pack_index
     assert np.array_equal(pack_index(iu, ju), np.arange(iu.size))
     Bp = rng_b.normal(0.0, 0.3, size=(L, iu.size)) * decay[iu, ju][None, :]
-    full = Bp.T @ Bp  # [npair, npair]
+    # sum over the L factors in index order with plain multiplies and adds: a BLAS product here would make the last bits of the
+    # integrals depend on the host's dgemm kernels, and stored oracle values (tests/golden) could not be compared across machines
+    full = np.zeros((iu.size, iu.size))
+    for l in range(L):
+        full += np.multiply.outer(Bp[l], Bp[l])  # [npair, npair]
     a, b = np.tril_indices(iu.size)
     eri = np.ascontiguousarray(full[a, b])
     return np.ascontiguousarray(h1), eri

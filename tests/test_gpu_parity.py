@@ -190,8 +190,8 @@ def test_cr2_shaped_full_size_bench_configuration(pkg):
     """The Cr2-shaped config at FULL size in the launch configuration bench.py times (planned passes, streamed organisation).
     The oracle cannot run it (SURVEY.md 8(d) tier 3), so this checks what holds at any size: E_S against a library CSR
     product of the same matrix, structural invariants of the counters, and PT2 / counts invariant under the other
-    organisation and another key partitioning (hash table in HBM, forced 128 passes), whose per-class sums must add up to the
-    same total."""
+    organisation and another key partitioning (streamed, 128 passes: the two share the heat-bath lists and the determinant
+    store, nothing of the enumeration, deduplication or reduction), whose per-class sums must add up to the same total."""
     import torch
     p = make_problem("cr2")
     ctx = _ctx(pkg, p)
@@ -214,12 +214,14 @@ def test_cr2_shaped_full_size_bench_configuration(pkg):
     a_parts = np.array(ctx.pt2_partials())
     assert ca["pt2_parts"] >= 32 and a_ext <= a_con <= ca["pt2_generated"]
     assert abs(a_parts.sum() - a_pt2) <= 1e-12 * ca["pt2_sum_abs"]
-    assert ca["pt2_binned"] == 2                                               # the planner streams this configuration
+    assert ca["pt2_binned"] == 1                                               # the planner bins the passes of this configuration
     ctx.trim()
-    ctx.pt2_set_options(mode="table", table_slots=900_000_000, n_parts=128)
+    ctx.pt2_set_options(mode="stream", n_parts=128)
     b_pt2, b_ext, b_con = ctx.pt2(psi, e_s, p["eps2"])
     cb = ctx.counters()
-    assert cb["pt2_binned"] == 0 and cb["pt2_parts"] == 128 and (b_ext, b_con, cb["pt2_generated"]) == (a_ext, a_con, ca["pt2_generated"])
+    print(f"cr2 full size: binned table {ca['ms_pt2_accum'] + ca['ms_pt2_scan']:.0f} ms, streamed {cb['ms_pt2_accum'] + cb['ms_pt2_scan']:.0f} ms, "
+          f"relative PT2 difference {abs(a_pt2 - b_pt2) / abs(a_pt2):.2e}")
+    assert cb["pt2_binned"] == 2 and cb["pt2_parts"] == 128 and (b_ext, b_con, cb["pt2_generated"]) == (a_ext, a_con, ca["pt2_generated"])
     assert abs(a_pt2 - b_pt2) <= PT2_TOL * max(abs(a_pt2), 1e-3 * ca["pt2_sum_abs"])
     b_parts = np.array(ctx.pt2_partials())
     # class c of 64 partitions = classes c and c + 64 of 128 (low bits of the same partition word, reading Q14)
@@ -420,7 +422,14 @@ def test_pt2_streamed_organisation(pkg, orc):
     assert e.value.status == "DH_ETABLEFULL"
     check(o, psi, 2, mode="stream")
     check(o, psi, 0, mode="table")
-    check(o, psi, 0)  # the planner keeps a 1 GB table in HBM
+    check(o, psi, 0)  # the planner keeps a 1 GB table in HBM and probes it directly
+    # binned passes of the table organisation (chosen by the planner beyond 32 GB): forced, with the default record pool, a pool
+    # too small for most records (the overflow is probed directly, the rest goes through the merge), 16 passes, masked psi
+    c = check(o, psi, 1, table_regions=64)
+    check(o, psi, 1, table_regions=2048, stream_pool_frac=0.05)
+    check(o, psi, 1, table_regions=256, n_parts=16)
+    check(om, torch.from_numpy(q["psi"]).cuda(), 1, table_regions=2048)
+    check(o, psi, 0, table_regions=-1)
     ctx.close()
 
 
