@@ -144,6 +144,7 @@ def main():
     ap.add_argument("--eps2", type=float, default=None, help="override the config's PT2 threshold (scaling sweep, configs[3])")
     ap.add_argument("--n-parts", type=int, default=0, help="pt2 key partitions (0 = planned by the library)")
     ap.add_argument("--table-slots", type=int, default=0)
+    ap.add_argument("--pt2-mode", default="auto", choices=["auto", "table", "stream"], help="pt2 organisation (detham_pt2_options.mode)")
     ap.add_argument("--no-cpu-baseline", action="store_true")
     ap.add_argument("--no-e2e", action="store_true")
     ap.add_argument("--widened", action="store_true",
@@ -180,7 +181,7 @@ def main():
         p["eps2"] = args.eps2
     nd = len(p["psi"])
     ctx = pkg.create(p["n"], p["na"], p["nb"], p["h1"], p["eri"], p["e_core"])
-    ctx.pt2_config(args.table_slots, args.n_parts)
+    ctx.pt2_set_options(mode=args.pt2_mode, table_slots=args.table_slots, n_parts=args.n_parts)
     dets_dev = torch.from_numpy(p["dets"].view(np.int64)).cuda()
     psi_dev = torch.from_numpy(p["psi"]).cuda()
     flush = torch.empty(256 << 20, dtype=torch.uint8, device="cuda")
@@ -198,6 +199,10 @@ def main():
             dist.barrier()
         torch.cuda.synchronize()
 
+    # the metric's numerator is a property of the INPUT, counted once outside the timed region: the screened connection lists of
+    # all sources at ham_build's screen plus at pt2's screen (exactly what the oracle sample counts; detham_count_screened)
+    ctx.set_subspace(dets_dev)
+    elements = ctx.count_screened(p["eps"]) + ctx.count_screened(p["eps2"], psi_dev)
     for _ in range(args.warmup):
         step()
     sampler = ClockSampler(local_rank)
@@ -223,7 +228,6 @@ def main():
         total_ms = float(t.item())
     ms_per_step = total_ms / args.steps
     c = phases[-1]
-    elements = c["build_generated"] + c["pt2_generated"]
     value = world * elements / (ms_per_step * 1e-3)
 
     # ---- roofline of the dominant kernel (pt2_accumulate_kernel), algorithmic bytes per SURVEY.md 8(d)
@@ -237,15 +241,17 @@ def main():
     b_energy = 12.0 * c["nnz"] + 8.0 * (nd + 1) + 16.0 * nd
     b_pt2 = 32.0 * c["pt2_contrib"] + 32.0 * c["pt2_external"] + 24.0 * nd
     path_gbs = (b_energy + b_pt2) / ((t_energy + t_pt2) * 1e-3) / 1e9
-    # binned mode: one key partition's accumulate step is the append + merge pair, timed together (ms_pt2_accum)
-    acc_name = "pt2_accumulate_kernel<binned> + pt2_merge_kernel" if c["pt2_binned"] else "pt2_accumulate_kernel"
+    # one key partition's accumulate step = the pair of kernels that moves every contribution once, timed together (ms_pt2_accum +
+    # ms_pt2_scan for the streamed organisation, whose second kernel also reduces)
+    acc_name = {0: "pt2_accumulate_kernel", 1: "pt2_accumulate_kernel<binned> + pt2_table_merge_kernel",
+                2: "pt2_gen_kernel + pt2_merge_kernel"}[int(c["pt2_binned"])]
+    if c["pt2_binned"] == 2:
+        acc_ms = statistics.mean(x["ms_pt2_accum"] + x["ms_pt2_scan"] for x in phases) / parts
+        achieved = bytes_accum_launch / (acc_ms * 1e-3) / 1e9
     roofline = {"bound": "hbm", "kernel": acc_name, "achieved": achieved, "peak": peak, "unit": "GB/s",
                 "frac": achieved / peak, "traffic": None, "peak_source": peak_src,
                 "bytes_per_launch": bytes_accum_launch, "launch_ms": acc_ms, "launches_per_step": parts,
                 "energy_plus_pt2_GBps": path_gbs, "energy_plus_pt2_frac": path_gbs / peak,
-                # what random 32-byte read-modify-writes can reach on this GPU (profiles/r1_microbench.md): 15 G/s for
-                # duplicates, 10.8-12.5 G/s for first touches, x 32 algorithmic bytes each
-                "pattern_ceiling_GBps": [32 * 10.8, 32 * 15.0],
                 "contributions_per_sec": c["pt2_contrib"] / (statistics.mean(x["ms_pt2_accum"] for x in phases) * 1e-3)}
     traffic_file = os.path.join(ROOT, "profiles", "traffic.json")
     if os.path.exists(traffic_file):
@@ -263,13 +269,14 @@ def main():
                                               "ms_pt2_accum", "ms_pt2_scan")},
            "counters": {k: c[k] for k in ("nnz", "build_generated", "pt2_generated", "pt2_contrib", "pt2_external",
                                           "pt2_parts", "pt2_probe_parts", "pt2_max_probe", "pt2_table_slots", "pt2_sum_abs", "pt2_min_abs_den",
-                                          "pt2_binned")},
+                                          "pt2_binned", "pt2_stream_bins")},
            "results": {"E_S": e_s, "PT2": pt2}, "es_pt2_wall_ms": mean("ms_build_count") + mean("ms_build_fill") + t_energy + t_pt2,
            "stored_nnz_per_sec": c["nnz"] / ((mean("ms_build_count") + mean("ms_build_fill")) * 1e-3),
            # kernels of libdetham.so per step: store 2 (validate, index insert), ham_build 5 (enumerate, row scan, segment copy,
-           # two row sorts), energy 2, pt2 3 (plan histogram, norm + reduce) + 4 per key partition (member insert, accumulate,
-           # scan, reduce) + 4 when the planner probed one slice
-           "gpu_launches": 2 + 5 + 2 + 3 + (5 if c["pt2_binned"] else 4) * parts + (4 if c["pt2_probe_parts"] else 0)}
+           # two row sorts), energy 2, pt2 3 (plan histogram, norm + reduce) + per key partition 4 (member insert, accumulate,
+           # scan, reduce), 5 with binned passes (+ merge), 3 streamed (generate, merge + reduce, reduce) + 4 when the planner
+           # probed one slice
+           "gpu_launches": 2 + 5 + 2 + 3 + {0: 4, 1: 5, 2: 3}[int(c["pt2_binned"])] * parts + (4 if c["pt2_probe_parts"] else 0)}
 
     # ---- the widened rows, timed on the same workload after the hot path: median of 3, CUDA events
     if args.widened and rank == 0:

@@ -46,7 +46,8 @@ typedef enum {
 /* Counters of the most recent calls (metrics). */
 typedef struct {
   int64_t nnz;              /* stored entries of H_SS (diagonal included) */
-  int64_t build_generated;  /* excitations that passed the magnitude screen in ham_build (looked up in S) */
+  int64_t build_generated;  /* candidates ham_build looked up in S: the doubles that passed the screen and every single (singles are
+                               looked up first and evaluated only when they are in S) */
   int64_t pt2_generated;    /* excitations that passed the screen in pt2 (members of S included) */
   int64_t pt2_contrib;      /* contributions H_ai psi_i added to externals a not in S */
   int64_t pt2_external;     /* distinct externals */
@@ -73,6 +74,8 @@ typedef struct {
                                passes, 2 = streamed (records partitioned by key region, deduplicated in L2-resident region tables;
                                no table in HBM) */
   int64_t pt2_stream_bins;  /* streamed organisation: key regions per pass (0 otherwise); pt2_table_slots = slots of one region table */
+  int64_t build_pairs;      /* 1 if the last ham_build went by excitation degree (pairs of S), 0 if it walked the heat-bath lists;
+                               build_generated then counts the Slater-Condon elements evaluated */
 } detham_counters;
 
 /* Options of pt2 (SURVEY.md section 5 "config / flag system").  Zero in every field = the defaults. */
@@ -114,6 +117,11 @@ dh_status detham_set_subspace(detham_ctx* ctx, const uint64_t* dets, int64_t n_d
  * {(i, H_ii)} U {(j, H_ij) : D_j in S, D_j a single or double excitation of D_i, |H_ij| >= eps, H_ij != 0}, columns
  * ascending (reading Q4).  eps >= 0.  *nnz_out (host, may be NULL) receives the number of stored entries. */
 dh_status detham_ham_build(detham_ctx* ctx, double eps, int64_t* nnz_out);
+
+/* Choose how ham_build finds the connections inside S: 0 = the library chooses; 1 = walk the heat-bath lists of every source and
+ * look the screened excitations up in S; 2 = by excitation degree: pairs of S whose bit strings differ by at most
+ * a double excitation (|S| <= 2^31).  Both give the same CSR, bit for bit off the diagonal. */
+dh_status detham_build_config(detham_ctx* ctx, int method);
 
 /* Device pointers of the CSR built last: row_ptr int64 [n_dets+1], col int32 [nnz], val fp64 [nnz].  Valid until the next
  * detham_ham_build / detham_set_subspace / detham_destroy.  DH_EINVAL if no CSR exists. */
@@ -157,6 +165,13 @@ dh_status detham_trim(detham_ctx* ctx);
  * Result  dE = (1 / psi^T psi) sum_a v_a^2 / (e_s - H_aa).  psi: DEVICE fp64 [n_dets]; outputs HOST (counts may be NULL). */
 dh_status detham_pt2(detham_ctx* ctx, const double* psi, double e_s, double eps2, double* pt2_out,
                      int64_t* n_external_out, int64_t* n_contrib_out);
+
+/* Size of the screened connected set (Eq. 1 with the screen of Eq. 14), summed over the sources:
+ *   psi == NULL: sum_i |{ x' : x' a single or double excitation of D_i, |H_x'i| >= thr, H != 0 }|   (the screen of ham_build)
+ *   psi != NULL (DEVICE fp64 [n_dets]): the same with tau_i = thr / |psi_i|, rows with psi_i == 0 skipped (the screen of pt2).
+ * Members of S and externals alike; every single is evaluated.  A property of the input, independent of how ham_build and pt2
+ * are organised: the benchmark's "Hamiltonian elements" are count(NULL, eps) + count(psi, eps2).  *n_out: HOST. */
+dh_status detham_count_screened(detham_ctx* ctx, const double* psi, double thr, int64_t* n_out);
 
 /* expand (Alg. 1 "Subspace Expansion"): the perturbative set of Eq. 14
  *   P = { a not in S : max_i |H_ai psi_i| >= eps2 },

@@ -12,8 +12,8 @@ _lib = None
 STATUS = {0: "DH_OK", 1: "DH_EINVAL", 2: "DH_EUNSORTED", 3: "DH_EPOPCOUNT", 4: "DH_ENOMEM", 5: "DH_ETABLEFULL", 6: "DH_ECUDA"}
 
 # every symbol include/detham.h declares
-SYMBOLS = ["detham_create", "detham_set_subspace", "detham_ham_build", "detham_csr", "detham_csr_copy", "detham_energy", "detham_residual", "detham_ediag",
-           "detham_pt2_config", "detham_pt2_set_options", "detham_trim", "detham_pt2", "detham_expand", "detham_hsp_build", "detham_hsp_csr", "detham_hsp_csr_copy", "detham_pt2_partials", "detham_solve_host", "detham_connections",
+SYMBOLS = ["detham_create", "detham_set_subspace", "detham_ham_build", "detham_build_config", "detham_csr", "detham_csr_copy", "detham_energy", "detham_residual", "detham_ediag",
+           "detham_pt2_config", "detham_pt2_set_options", "detham_trim", "detham_count_screened", "detham_pt2", "detham_expand", "detham_hsp_build", "detham_hsp_csr", "detham_hsp_csr_copy", "detham_pt2_partials", "detham_solve_host", "detham_connections",
            "detham_diagonals", "detham_get_counters", "detham_destroy", "detham_strerror", "detham_last_cuda_error"]
 
 
@@ -25,7 +25,7 @@ class Counters(C.Structure):
                 ("ms_build_fill", C.c_double), ("ms_energy", C.c_double), ("ms_pt2_plan", C.c_double),
                 ("ms_pt2_accum", C.c_double), ("ms_pt2_scan", C.c_double),
                 ("hsp_nnz", C.c_int64), ("hsp_generated", C.c_int64), ("ms_hsp_build", C.c_double),
-                ("ms_hsp_fill", C.c_double), ("pt2_binned", C.c_int64), ("pt2_stream_bins", C.c_int64)]
+                ("ms_hsp_fill", C.c_double), ("pt2_binned", C.c_int64), ("pt2_stream_bins", C.c_int64), ("build_pairs", C.c_int64)]
 
 
 class Pt2Options(C.Structure):
@@ -57,6 +57,7 @@ def load_library():
     L.detham_create.argtypes = [C.POINTER(vp), C.c_int, C.c_int, C.c_int, vp, vp, C.c_double, vp]
     L.detham_set_subspace.argtypes = [vp, vp, C.c_int64]
     L.detham_ham_build.argtypes = [vp, C.c_double, ip]
+    L.detham_build_config.argtypes = [vp, C.c_int]
     L.detham_csr.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
     L.detham_csr_copy.argtypes = [vp, vp, vp, vp]
     L.detham_energy.argtypes = [vp, vp, dp, dp, vp]
@@ -65,6 +66,7 @@ def load_library():
     L.detham_pt2_config.argtypes = [vp, C.c_int64, C.c_int]
     L.detham_pt2_set_options.argtypes = [vp, C.POINTER(Pt2Options)]
     L.detham_trim.argtypes = [vp]
+    L.detham_count_screened.argtypes = [vp, vp, C.c_double, ip]
     L.detham_pt2.argtypes = [vp, vp, C.c_double, C.c_double, dp, ip, ip]
     L.detham_expand.argtypes = [vp, vp, C.c_double, vp, vp, vp, vp, C.c_int64, ip]
     L.detham_hsp_build.argtypes = [vp, vp, C.c_double, vp, C.c_int64, ip]
@@ -132,6 +134,10 @@ class Detham:
         self._check(self._L.detham_set_subspace(self._h, ptr, m))
         self.n_dets = m
         self._last_external = 0
+
+    def build_config(self, method=0):
+        """How ham_build finds connections: 0 library's choice, 1 heat-bath list walk, 2 by excitation degree (pairs of S)."""
+        self._check(self._L.detham_build_config(self._h, int(method)))
 
     def ham_build(self, eps):
         nnz = C.c_int64(0)
@@ -238,6 +244,12 @@ class Detham:
                 raise DethamError(1, f"unknown pt2 option {k}")
             setattr(o, k, v)
         self._check(self._L.detham_pt2_set_options(self._h, C.byref(o)))
+
+    def count_screened(self, thr, psi=None):
+        """Size of the screened connection lists summed over the sources (psi None: tau = thr; else tau_i = thr / |psi_i|)."""
+        n = C.c_int64(0)
+        self._check(self._L.detham_count_screened(self._h, psi.data_ptr() if psi is not None else None, float(thr), C.byref(n)))
+        return n.value
 
     def trim(self):
         self._check(self._L.detham_trim(self._h))

@@ -23,7 +23,7 @@ void free_all(detham_ctx* c) {
   f(c->h1); f(c->eri); f(c->J); f(c->JK); f(c->hd);
   for (auto& L : c->lists) { f(L.sub_off); f(L.val); f(L.ab); f(L.stat); }
   f(c->dets_owned); f(c->psi_owned); f(c->shash_key); f(c->shash_idx); f(c->sbits);
-  f(c->row_ptr); f(c->col); f(c->val); f(c->row_cnt); f(c->sp_row_ptr); f(c->sp_col); f(c->sp_val); f(c->phash_key); f(c->phash_idx); f(c->acol); f(c->aval); f(c->segs); f(c->table); f(c->pool); f(c->ring); f(c->sflags); f(c->red); f(c->dcount); f(c->hist);
+  f(c->row_ptr); f(c->col); f(c->val); f(c->row_cnt); f(c->sp_row_ptr); f(c->sp_col); f(c->sp_val); f(c->phash_key); f(c->phash_idx); f(c->acol); f(c->aval); f(c->segs); f(c->table); f(c->pool); f(c->ring); f(c->sflags); f(c->pair_galpha); f(c->pair_gstart); f(c->pair_diag); f(c->red); f(c->dcount); f(c->hist);
   if (c->pinned) cudaFreeHost(c->pinned);
   for (auto& e : c->ev) if (e) cudaEventDestroy(e);
   for (auto& e : c->sev) cudaEventDestroy(e);
@@ -100,6 +100,12 @@ dh_status detham_ham_build(detham_ctx* c, double eps, int64_t* nnz_out) {
   dh_status st = dh_ham_build(c, eps);
   if (st == DH_OK && nnz_out) *nnz_out = c->nnz;
   return st;
+}
+
+dh_status detham_build_config(detham_ctx* c, int method) {
+  if (!c || method < 0 || method > 2) return DH_EINVAL;
+  c->build_method = method;
+  return DH_OK;
 }
 
 dh_status detham_csr(detham_ctx* c, const int64_t** row_ptr, const int32_t** col, const double** val) {
@@ -179,6 +185,11 @@ dh_status detham_pt2(detham_ctx* c, const double* psi, double e_s, double eps2, 
   if (n_external_out) *n_external_out = c->ctr.pt2_external;
   if (n_contrib_out) *n_contrib_out = c->ctr.pt2_contrib;
   return DH_OK;
+}
+
+dh_status detham_count_screened(detham_ctx* c, const double* psi, double thr, int64_t* n_out) {
+  if (!c || !c->dets || !(thr >= 0.0) || !n_out) return DH_EINVAL;
+  return dh_count_screened(c, psi, thr, n_out);
 }
 
 dh_status detham_expand(detham_ctx* c, const double* psi, double eps2, uint64_t* keys_out, double* score_out, double* v_out,

@@ -78,6 +78,12 @@ struct detham_ctx {
   void* segs = nullptr;    // arena segments
   int64_t seg_cap = 0;
 
+  // ham_build by excitation degree (pair_build.cu): alpha groups of the sorted S, diagonals
+  u64* pair_galpha = nullptr; int64_t pair_group_cap = 0;
+  int* pair_gstart = nullptr; int64_t pair_gstart_cap = 0;
+  double* pair_diag = nullptr; int64_t pair_diag_cap = 0;
+  int build_method = 0;  // detham_build_config: 0 choose, 1 list walk, 2 excitation degree
+
   // CSR H_SP (row f3) and the lookup index of the caller's P it was built against
   int64_t* sp_row_ptr = nullptr;
   int* sp_col = nullptr;
@@ -132,6 +138,7 @@ inline double dh_elapsed(detham_ctx* c, int a, int b) { float ms = 0.f; cudaEven
 dh_status dh_build_jk(detham_ctx* c);
 dh_status dh_get_lists(detham_ctx* c, int pbits, const HbLists** out);
 dh_status dh_ham_build(detham_ctx* c, double eps);
+dh_status dh_pair_build(detham_ctx* c, double eps);
 dh_status dh_hsp_build(detham_ctx* c, const double* psi, double eps2, const u64* pkeys, int64_t m);
 dh_status dh_energy(detham_ctx* c, const double* psi, double* e_out, double* n2_out, double* y_out);
 dh_status dh_expand(detham_ctx* c, const double* psi, double eps2, u64* keys_out, double* score_out, double* v_out, double* haa_out,
@@ -139,6 +146,7 @@ dh_status dh_expand(detham_ctx* c, const double* psi, double eps2, u64* keys_out
 dh_status dh_ediag(detham_ctx* c, const double* v0, double tol, int max_iter, double* e_out, int* iters_out);
 dh_status dh_residual(detham_ctx* c, const double* psi, double e_s, double* r_out, double* internal_out);
 dh_status dh_pt2(detham_ctx* c, const double* psi, double e_s, double eps2, double* out);
+dh_status dh_count_screened(detham_ctx* c, const double* psi, double thr, int64_t* n_out);
 dh_status dh_connections(detham_ctx* c, int64_t row, double tau, std::vector<u64>& keys, std::vector<double>& h);
 dh_status dh_diagonals(detham_ctx* c, const u64* dets, int64_t m, double* out);
 dh_status dh_build_shash(detham_ctx* c);

@@ -19,8 +19,11 @@ __device__ __forceinline__ double member_flag() { return __longlong_as_double(0x
 
 
 // ---------------------------------------------------------------- class histogram (pass planning)
+// kExact = false: pass planning - singles are counted without being evaluated (an upper bound is all the planner needs).
+// kExact = true: the exact number of screen-passing excitations (detham_count_screened): every single is evaluated.
+template <bool kExact>
 struct CountSink {
-  static constexpr bool kLookupFirst = true;  // singles are counted (upper bound) without being evaluated
+  static constexpr bool kLookupFirst = !kExact;
   static constexpr bool kLazySign = true;     // only counts
   unsigned* hist;
   __device__ __forceinline__ bool pre(u64, u64, u64 z) { atomicAdd(hist + ((unsigned)z & (kFine - 1)), 1u); return false; }
@@ -29,6 +32,7 @@ struct CountSink {
   }
 };
 
+template <bool kExact>
 __global__ void __launch_bounds__(kWarpsPerCta * 32)
 count_kernel(EnumParams P, const u64* __restrict__ dets, const double* __restrict__ psi, int64_t nd, int64_t stride,
              double eps2, u64* counters, u64* __restrict__ hist) {
@@ -41,16 +45,16 @@ count_kernel(EnumParams P, const u64* __restrict__ dets, const double* __restric
   __syncthreads();
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   WarpScratch& ws = wsp[warp];
-  CountSink sink{sh};
+  CountSink<kExact> sink{sh};
   for (;;) {
     u64 row = 0;
     if (lane == 0) row = atomicAdd(counters, 1ull);
     row = __shfl_sync(0xffffffffu, row, 0) * (u64)stride;  // every stride-th source (stride 1 = exact histogram)
     if ((int64_t)row >= nd) break;
-    const double p = psi[row];
+    const double p = psi ? psi[row] : 1.0;  // no amplitudes: the amplitude-free screen of ham_build (tau = eps2)
     const u64 da = dets[2 * row], db = dets[2 * row + 1];
     u64 zsrc = 0;
-    if (lane == 0) { zsrc = dh_zobrist(da, db, T.Z); atomicAdd(sh + ((unsigned)zsrc & (kFine - 1)), 1u); }
+    if (lane == 0) { zsrc = dh_zobrist(da, db, T.Z); if (!kExact) atomicAdd(sh + ((unsigned)zsrc & (kFine - 1)), 1u); }
     zsrc = __shfl_sync(0xffffffffu, zsrc, 0);
     if (p == 0.0) continue;
     const double tau = eps2 == 0.0 ? 0.0 : __ddiv_rn(eps2, fabs(p));
@@ -105,11 +109,6 @@ struct FlatScratch {
   unsigned dq[64];               // doubles queue: list entry | pair of the chunk << 25
 };
 
-// entry meta: kind << 25 | s << 24 | i << 18 | j << 12 | a << 6 | b
-__device__ __forceinline__ unsigned pack_meta(int kind, int s, int i, int j, int a, int b) {
-  return ((unsigned)kind << 25) | ((unsigned)s << 24) | ((unsigned)i << 18) | ((unsigned)j << 12) | ((unsigned)a << 6) | (unsigned)b;
-}
-
 struct ProbeCtx {
   Slot* table; u64 cap;
   const CtaTables* T; const WarpScratch* ws; int n;
@@ -117,11 +116,6 @@ struct ProbeCtx {
   unsigned contrib; int max_probe;
   int* overflow;
 };
-
-__device__ __forceinline__ double meta_diag(const ProbeCtx& pc, unsigned m) {
-  return dh_excited_diag(*pc.T, *pc.ws, pc.n, pc.e0, (int)(m >> 25), (int)((m >> 24) & 1u), (int)((m >> 18) & 63u),
-                         (int)((m >> 12) & 63u), (int)((m >> 6) & 63u), (int)(m & 63u));
-}
 
 // v_a += H_ai psi_i; in expand mode (row f2) the slot's second payload word holds max_i |H_ai psi_i| (Eq. 14's score)
 // instead of H_aa: the bit patterns of non-negative doubles order like the values, so an unsigned RED.MAX does it.
@@ -135,7 +129,7 @@ __device__ __forceinline__ void slot_add(Slot* sp, double cv) {
 // before any result is used.  A slot is {key, v, H_aa}; members of S carry the NaN flag in v and absorb nothing.
 template <int U, bool kExpand>
 __device__ __forceinline__ void probe_batch(ProbeCtx& pc, const u64 (&ka)[U], const u64 (&kb)[U], const double (&cv)[U],
-                                            u64 (&slot)[U], const unsigned (&meta)[U], unsigned pend) {
+                                            u64 (&slot)[U], const double (&haa)[U], unsigned pend) {
   if (!pend) return;
   int probes = 0;
   for (;;) {
@@ -169,7 +163,7 @@ __device__ __forceinline__ void probe_batch(ProbeCtx& pc, const u64 (&ka)[U], co
       for (int u = 0; u < U; ++u)
         if ((cas >> u) & 1u) {
           if ((k0[u] | k1[u]) == 0ull) {  // claimed: this thread also records H_aa
-            if (!kExpand) pc.table[slot[u]].haa = meta_diag(pc, meta[u]);
+            if (!kExpand) pc.table[slot[u]].haa = haa[u];
             slot_add<kExpand>(pc.table + slot[u], cv[u]); ++pc.contrib;
             pend &= ~(1u << u);
           } else if (k0[u] == ka[u] && k1[u] == kb[u]) {  // lost the race to the same key, or came here through the half-zero check
@@ -197,16 +191,15 @@ struct BinCtx { Slot* pool; unsigned* cnt; unsigned seg_cap; int shift; };
 
 template <int U>
 __device__ __forceinline__ unsigned bin_batch(ProbeCtx& pc, const BinCtx& bc, const u64 (&ka)[U], const u64 (&kb)[U],
-                                              const double (&cv)[U], const u64 (&slot)[U], const unsigned (&meta)[U], unsigned pend) {
+                                              const double (&cv)[U], const u64 (&slot)[U], const double (&haa)[U], unsigned pend) {
 #pragma unroll
   for (int u = 0; u < U; ++u)
     if ((pend >> u) & 1u) {
-      const double haa = meta_diag(pc, meta[u]);
       const unsigned bin = (unsigned)(slot[u] >> bc.shift);
       const unsigned p = atomicAdd(&bc.cnt[bin], 1u);
       if (p < bc.seg_cap) {
         dh_st256(bc.pool + ((u64)bin * gridDim.x + blockIdx.x) * bc.seg_cap + p, ka[u], kb[u], (u64)__double_as_longlong(cv[u]),
-                 (u64)__double_as_longlong(haa));
+                 (u64)__double_as_longlong(haa[u]));
         pend &= ~(1u << u);
       }
     }
@@ -293,7 +286,7 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
           const int take = qn >= 32 ? 32 : qn;
           u64 ka[1] = {da}, kb[1] = {db}, slot[1] = {0};
           double cv[1] = {0.0};
-          unsigned meta[1] = {0u};
+          double haa[1] = {0.0};
           unsigned pend = 0u;
           if (lane < take) {
             const unsigned code = fs.sq[qn - take + lane];
@@ -306,15 +299,15 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
               const u64 z = zsrc ^ T.Z[64 * s + i] ^ T.Z[64 * s + a];
               slot[0] = dh_table_slot(z, ka[0], kb[0], cap, bin_shift);
               cv[0] = v * p;
-              meta[0] = pack_meta(0, s, i, 0, a, 0);
+              if (!kExpand) haa[0] = dh_excited_diag(T, ws, n, pc.e0, 0, s, i, 0, a, 0);
               pend = 1u;
             }
           }
           __syncwarp();
           qn -= take;
           gen += pend;
-          if (kBinned) pend = bin_batch<1>(pc, bc, ka, kb, cv, slot, meta, pend);
-          probe_batch<1, kExpand>(pc, ka, kb, cv, slot, meta, pend);
+          if (kBinned) pend = bin_batch<1>(pc, bc, ka, kb, cv, slot, haa, pend);
+          probe_batch<1, kExpand>(pc, ka, kb, cv, slot, haa, pend);
         }
       }
     }
@@ -404,7 +397,7 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
           const int take = dqn >= 32 ? 32 : dqn;
           u64 ka[1] = {da}, kb[1] = {db}, slot[1] = {0};
           double cv[1] = {0.0};
-          unsigned meta[1] = {0u};
+          double haa[1] = {0.0};
           unsigned pend = 0u;
           if (lane < take) {
             const unsigned ent = fs.dq[dqn - take + lane];
@@ -424,23 +417,25 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
               const int par = dh_parity_between(w, i, a) ^ dh_parity_between((w ^ (1ull << i)) | (1ull << a), j, b);
               if (par) v = -v;
               slot[0] = dh_table_slot(z, ka[0], kb[0], cap, bin_shift);
-              meta[0] = pack_meta(1, fam, i, j, a, b);
             } else {
               ka[0] = (da ^ (1ull << i)) | (1ull << a);
               kb[0] = (db ^ (1ull << j)) | (1ull << b);
               const u64 z = zij ^ T.Z[a] ^ T.Z[64 + b];
               if (dh_parity_between(da, i, a) ^ dh_parity_between(db, j, b)) v = -v;
               slot[0] = dh_table_slot(z, ka[0], kb[0], cap, bin_shift);
-              meta[0] = pack_meta(2, 0, i, j, a, b);
             }
             cv[0] = v * p;
+            if (!kExpand) {  // O(1) diagonal update: the source's U vectors plus the entry's source-independent part (lists.cu)
+              const int si = fam == 1, sj = fam != 0;
+              haa[0] = pc.e0 - ws.U[si][i] - ws.U[sj][j] + ws.U[si][a] + ws.U[sj][b] + __ldg(P.lstat + k);
+            }
             pend = 1u;
           }
           __syncwarp();
           dqn -= take;
           gen += pend;
-          if (kBinned) pend = bin_batch<1>(pc, bc, ka, kb, cv, slot, meta, pend);
-          probe_batch<1, kExpand>(pc, ka, kb, cv, slot, meta, pend);
+          if (kBinned) pend = bin_batch<1>(pc, bc, ka, kb, cv, slot, haa, pend);
+          probe_batch<1, kExpand>(pc, ka, kb, cv, slot, haa, pend);
         }
       }
       __syncwarp();
@@ -860,11 +855,11 @@ static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double ep
     const int64_t ns = (nd + stride - 1) / stride;
     int64_t want = (ns + kWarpsPerCta - 1) / kWarpsPerCta;
     const int grid = (int)(want < (int64_t)c->sm_count * 4 ? want : (int64_t)c->sm_count * 4);
-    DH_CUDA(c, cudaFuncSetAttribute(count_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+    DH_CUDA(c, cudaFuncSetAttribute(count_kernel<false>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
     DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 8 * sizeof(u64), c->stream));
     DH_CUDA(c, cudaMemsetAsync(c->hist, 0, kFine * sizeof(u64), c->stream));
     DH_TICK(c, 0);
-    count_kernel<<<grid, kWarpsPerCta * 32, smem, c->stream>>>(P0, c->dets, psi, nd, stride, eps2, c->dcount, reinterpret_cast<u64*>(c->hist));
+    count_kernel<false><<<grid, kWarpsPerCta * 32, smem, c->stream>>>(P0, c->dets, psi, nd, stride, eps2, c->dcount, reinterpret_cast<u64*>(c->hist));
     DH_CUDA(c, cudaGetLastError());
     DH_TICK(c, 1);
     hist.assign(kFine, 0);
@@ -964,6 +959,29 @@ static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double ep
     ++pbits;  // the plan was too optimistic: halve the keys per pass and start over
     if (auto_slots) slots = max_slots;
   }
+}
+
+// Exact size of the screened connection lists, summed over the sources: an input property (it does not depend on how ham_build
+// or pt2 go about their work), the numerator of the benchmark's elements/s.
+dh_status dh_count_screened(detham_ctx* c, const double* psi, double thr, int64_t* n_out) {
+  const HbLists* L0 = nullptr;
+  dh_status st = dh_get_lists(c, 0, &L0); if (st != DH_OK) return st;
+  EnumParams P0 = dh_make_params(c, L0);
+  const size_t smem = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + kWarpsPerCta * sizeof(WarpScratch) + kFine * sizeof(unsigned);
+  int64_t want = (c->nd + kWarpsPerCta - 1) / kWarpsPerCta;
+  const int grid = (int)(want < (int64_t)c->sm_count * 4 ? want : (int64_t)c->sm_count * 4);
+  DH_CUDA(c, cudaFuncSetAttribute(count_kernel<true>, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
+  DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 8 * sizeof(u64), c->stream));
+  DH_CUDA(c, cudaMemsetAsync(c->hist, 0, kFine * sizeof(u64), c->stream));
+  count_kernel<true><<<grid, kWarpsPerCta * 32, smem, c->stream>>>(P0, c->dets, psi, c->nd, 1, thr, c->dcount, reinterpret_cast<u64*>(c->hist));
+  DH_CUDA(c, cudaGetLastError());
+  std::vector<u64> hist(kFine);
+  DH_CUDA(c, cudaMemcpyAsync(hist.data(), c->hist, kFine * sizeof(u64), cudaMemcpyDeviceToHost, c->stream));
+  DH_CUDA(c, cudaStreamSynchronize(c->stream));
+  u64 n = 0;
+  for (u64 x : hist) n += x;
+  *n_out = (int64_t)n;
+  return DH_OK;
 }
 
 dh_status dh_pt2(detham_ctx* c, const double* psi, double e_s, double eps2, double* out) {

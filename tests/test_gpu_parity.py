@@ -332,6 +332,20 @@ def test_invalid_subspaces_are_errors(pkg):
     ctx.close()
 
 
+def test_count_screened_is_the_size_of_the_connection_lists(pkg, orc):
+    """detham_count_screened (the benchmark's numerator) against the oracle's connection lists, with and without amplitudes."""
+    p = make_problem("tiny", n_dets=300)
+    p["psi"] = p["psi"].copy(); p["psi"][5] = 0.0
+    ctx = _ctx(pkg, p)
+    for thr in (0.0, 1e-3, 5e-2):
+        want = sum(len(orc.connections(p["n"], p["h1"], p["eri"], p["e_core"], d, thr)[1]) for d in p["dets"])
+        assert ctx.count_screened(thr) == want
+        want = sum(len(orc.connections(p["n"], p["h1"], p["eri"], p["e_core"], d, thr / abs(x) if thr > 0 else 0.0)[1])
+                   for d, x in zip(p["dets"], p["psi"]) if x != 0.0)
+        assert ctx.count_screened(thr, _psi(p)) == want
+    ctx.close()
+
+
 def test_table_overflow_is_reported(pkg):
     p = make_problem("tiny", n_dets=500)
     ctx = _ctx(pkg, p)
@@ -449,6 +463,21 @@ def test_ham_build_repeated_with_different_eps(pkg, orc):
     ref = orc.ham_build(q["n"], q["h1"], q["eri"], q["e_core"], q["dets"], 1e-4)
     assert nnz == len(ref[1])
     _check_csr(ctx, ref)
+    ctx.close()
+
+
+@pytest.mark.parametrize("name,n_dets,eps", [("tiny", None, 0.0), ("tiny", 700, 1e-3), ("tiny", 33, 0.0), ("h2o", 6000, 1e-5), ("n2", 3000, 1e-5)])
+def test_ham_build_both_organisations(pkg, orc, name, n_dets, eps):
+    """ham_build by walking the heat-bath lists (method 1) and by excitation degree over pairs of S (method 2): the same CSR as
+    the oracle's from both, off-diagonal values bit for bit."""
+    p = make_problem(name, n_dets=n_dets)
+    ref = orc.ham_build(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"], eps)
+    ctx = _ctx(pkg, p)
+    for method in (1, 2, 0):
+        ctx.build_config(method)
+        assert ctx.ham_build(eps) == len(ref[1])
+        _check_csr(ctx, ref)
+        assert ctx.counters()["build_pairs"] == (1 if method == 2 else 0)
     ctx.close()
 
 

@@ -86,6 +86,22 @@ def test_p3_csr_bitwise_symmetric(orc, eps):
         assert np.all(np.abs(off) >= eps) and np.all(off != 0.0)
 
 
+def test_p3b_ham_build_row_subset_equals_rows_of_the_full_build(orc):
+    """orc_ham_build(rows=keep) (used by bench.py's bounded oracle sample and by the masked GPU tests) is loop bookkeeping
+    only: the kept rows are the same rows of the full build, bit for bit; the other rows are empty."""
+    p = make_problem("tiny", n_dets=500)
+    rp, col, val = orc.ham_build(p["n"], p["h1"], p["eri"], 0.0, p["dets"], 1e-3)
+    keep = np.array([0, 3, 4, 77, 250, 499])
+    srp, scol, sval = orc.ham_build(p["n"], p["h1"], p["eri"], 0.0, p["dets"], 1e-3, rows=keep)
+    assert len(srp) == 501 and srp[-1] == len(scol) == sum(rp[r + 1] - rp[r] for r in keep)
+    for r in range(500):
+        a, b = srp[r], srp[r + 1]
+        if r in keep:
+            assert np.array_equal(scol[a:b], col[rp[r]:rp[r + 1]]) and np.array_equal(sval[a:b], val[rp[r]:rp[r + 1]])
+        else:
+            assert a == b
+
+
 # ---------------------------------------------------------------- P4 / P5: eps=0 == unscreened, closed-form counts
 @pytest.mark.parametrize("name", ["tiny", "h2o", "n2", "cr2"])
 def test_p5_visit_count_closed_form(orc, name):
