@@ -82,6 +82,8 @@ struct detham_ctx {
   u64* pair_galpha = nullptr; int64_t pair_group_cap = 0;
   int* pair_gstart = nullptr; int64_t pair_gstart_cap = 0;
   double* pair_diag = nullptr; int64_t pair_diag_cap = 0;
+  u64* pair_akey = nullptr; int64_t pair_akey_cap = 0;   // arena tags: row << 32 | place in the row (values in acol / aval)
+  int* pair_bused = nullptr; int64_t pair_bused_cap = 0;  // entries used of every arena block
   int build_method = 0;  // detham_build_config: 0 choose, 1 list walk, 2 excitation degree
 
   // CSR H_SP (row f3) and the lookup index of the caller's P it was built against

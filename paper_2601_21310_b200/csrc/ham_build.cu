@@ -457,9 +457,10 @@ static dh_status build_csr(detham_ctx* c, const CsrTarget& T, const double* psi 
 dh_status dh_ham_build(detham_ctx* c, double eps) {
   // Two organisations with identical results.  By excitation degree (pair_build.cu) the cost grows like the number of pairs of
   // determinants whose alpha strings are within a double excitation of each other; walking the heat-bath lists it grows like
-  // |S| x (screened excitations per source).  Measured on B200 (profiles/r2_summary.md): the list walk wins on the H2O- and
-  // N2-shaped configurations, the pairs on the Cr2-shaped one (1e5 screened excitations per source, 98 % of them not in S).
-  const bool pairs = c->build_method == 2 || (c->build_method == 0 && c->nd >= (1ll << 19) && c->nd <= (4ll << 20) && c->n >= 40);
+  // |S| x (screened excitations per source).  Measured on B200 (profiles/r2_summary.md), list walk against pairs: H2O-shaped
+  // |S| = 2e4 3.9 / 5.6 ms, N2-shaped 1e5 33.7 / 21.2 ms, Cr2-shaped 1e6 1565 / 583 ms (1e5 screened excitations per source,
+  // 98 % of them not in S): pairs from 2^16 determinants on.
+  const bool pairs = c->build_method == 2 || (c->build_method == 0 && c->nd >= (1ll << 16) && c->nd <= (4ll << 20));
   if (pairs) return dh_pair_build(c, eps);
   c->ctr.build_pairs = 0;
   CsrTarget T{&c->row_ptr, &c->col, &c->val, &c->nnz, &c->csr_cap, &c->row_cap,

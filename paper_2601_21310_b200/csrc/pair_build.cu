@@ -10,6 +10,8 @@
 //
 // Values are the very expressions of the list walker (lists.cu, enumerate.cuh) - one packed integral or the difference of two
 // for doubles, the ordered sum of reading Q7 for singles - so both organisations give the same bits.
+#include <algorithm>
+
 #include "pt2_common.cuh"
 
 EnumParams dh_make_params(detham_ctx* c, const HbLists* L);
@@ -17,6 +19,7 @@ EnumParams dh_make_params(detham_ctx* c, const HbLists* L);
 namespace {
 
 constexpr int kPairWarps = 8;
+constexpr int kArenaBlk = 1024;  // arena entries a warp reserves at a time
 
 __global__ void group_flag_kernel(const u64* __restrict__ dets, int64_t nd, int* __restrict__ flag) {
   const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -92,16 +95,17 @@ __device__ double pair_element(const EnumParams& P, u64 ar, u64 br, u64 xa, u64 
   return dh_double_parity(ar, br, 1, s, i, j, a, b) ? -v : v;
 }
 
-// kFill = false: count the kept entries of every row (row_cnt).  kFill = true: write them at row_ptr[row] + running count.
+// One pass: every kept entry goes to an arena (blocks of kArenaBlk entries per warp) tagged with its row and its place in the row,
+// and the rows are counted; after the row scan a scatter moves the entries to their CSR positions.  If the arena is too small the
+// pass still counts exactly and is run again with the exact size.
 // Pairs within reach are queued per warp as (row of the block, column) in the order they are found and evaluated 32 at a time,
 // so that the Slater-Condon evaluation (a few hundred instructions, two to ~40 integral loads) runs with every lane busy; an
 // entry's place in its row is the row's running count plus its rank among the batch's kept entries of the same row.
-template <bool kFill>
 __global__ void __launch_bounds__(kPairWarps * 32)
 pair_kernel(EnumParams P, const u64* __restrict__ dets, int64_t nd, double eps, const u64* __restrict__ galpha,
             const int* __restrict__ gstart, int ngroups, const double* __restrict__ diag, int* __restrict__ row_cnt,
-            const int64_t* __restrict__ row_ptr, int* __restrict__ col, double* __restrict__ val,
-            u64* counters /* [0] next block of rows [1] elements evaluated */) {
+            u64* __restrict__ akey, int* __restrict__ acol, double* __restrict__ aval, int* __restrict__ bused, int64_t arena_cap,
+            u64* counters /* [0] next block of rows [1] elements evaluated [2] arena cursor */, int* overflow) {
   __shared__ int s_qcol[kPairWarps][64];
   __shared__ unsigned char s_qrow[kPairWarps][64];
   __shared__ int s_cnt[kPairWarps][32];
@@ -111,6 +115,7 @@ pair_kernel(EnumParams P, const u64* __restrict__ dets, int64_t nd, double eps, 
   unsigned char* qrow = s_qrow[warp];
   int* cnt = s_cnt[warp];
   u64 evaluated = 0;
+  int64_t wpos = 0, wend = 0;  // this warp's window in the arena (wpos < 0: arena exhausted, count only)
   for (;;) {
     u64 blk = 0;
     if (lane == 0) blk = atomicAdd(counters, 1ull);
@@ -120,7 +125,6 @@ pair_kernel(EnumParams P, const u64* __restrict__ dets, int64_t nd, double eps, 
     const int64_t row = row0 + lane;
     const bool have = row < nd;
     const u64 ar = have ? dets[2 * row] : 0ull, br = have ? dets[2 * row + 1] : 0ull;
-    const int64_t base = (kFill && have) ? row_ptr[row] : 0;
     cnt[lane] = 0;
     int qn = 0;
     __syncwarp();
@@ -130,7 +134,6 @@ pair_kernel(EnumParams P, const u64* __restrict__ dets, int64_t nd, double eps, 
       const int r = mine ? (int)qrow[lane] : 0;
       const int j = mine ? qcol[lane] : 0;
       const u64 a_row = __shfl_sync(full, ar, r), b_row = __shfl_sync(full, br, r);
-      const int64_t rbase = __shfl_sync(full, base, r);
       bool keep = false;
       double v = 0.0;
       if (mine) {
@@ -144,12 +147,29 @@ pair_kernel(EnumParams P, const u64* __restrict__ dets, int64_t nd, double eps, 
         }
       }
       const unsigned peers = __match_any_sync(full, keep ? r : 64 + lane);  // kept entries of the same row
+      const unsigned km = __ballot_sync(full, keep);
+      if (km) {  // warp-uniform: room in the arena for this batch
+        const int nk = __popc(km);
+        if (wpos >= 0 && wpos + nk > wend) {
+          if (lane == 0 && wend > 0) bused[(wend - 1) / kArenaBlk] = (int)(wpos - (wend - kArenaBlk));
+          u64 nb = 0;
+          if (lane == 0) nb = atomicAdd(counters + 2, (u64)kArenaBlk);
+          nb = __shfl_sync(full, nb, 0);
+          if ((int64_t)nb + kArenaBlk > arena_cap) { wpos = -1; if (lane == 0) *overflow = 1; }
+          else { wpos = (int64_t)nb; wend = wpos + kArenaBlk; }
+        }
+      }
       if (keep) {
         const int at = cnt[r];
-        if (kFill) { const int64_t pos = rbase + at + __popc(peers & lt); col[pos] = j; val[pos] = v; }
+        const int k = at + __popc(peers & lt);
+        if (wpos >= 0) {
+          const int64_t e = wpos + __popc(km & lt);
+          akey[e] = ((u64)(unsigned)(row0 + r) << 32) | (u64)(unsigned)k; acol[e] = j; aval[e] = v;
+        }
         __syncwarp(peers);
         if ((peers & lt) == 0u) cnt[r] = at + __popc(peers);
       }
+      if (km && wpos >= 0) wpos += __popc(km);
       __syncwarp();
       const int rest = qn - take;
       const int mr = lane < rest ? (int)qrow[take + lane] : 0, mc = lane < rest ? qcol[take + lane] : 0;
@@ -178,18 +198,42 @@ pair_kernel(EnumParams P, const u64* __restrict__ dets, int64_t nd, double eps, 
           hm &= hm - 1;
           const int dmax = 4 - __shfl_sync(full, da, hh);
           const int js = __shfl_sync(full, gs, hh), je = __shfl_sync(full, ge, hh);
-          for (int c0 = js; c0 < je; c0 += 32) {
-            const int j = c0 + lane;
-            const u64 bj = j < je ? __ldg(dets + 2 * (int64_t)j + 1) : 0ull;
-            for (int r = r0; r < r1; ++r) {  // every row of the run against these 32 columns
+          const int M = je - js, R = r1 - r0;
+          if (M <= 32 && R > 1) {
+            // a small group against a run of several rows: the lanes cover the R x M cross product (row-major, so that a
+            // row's columns still come in ascending order), instead of M of 32 lanes once per row
+            const u64 bj = lane < M ? __ldg(dets + 2 * (int64_t)(js + lane) + 1) : 0ull;
+            const unsigned inv = (65536u + (unsigned)M - 1u) / (unsigned)M;  // t / M == (t * inv) >> 16 for t < 1024, M <= 32
+            const int T = R * M;
+            for (int t0 = 0; t0 < T; t0 += 32) {
+              const int t = t0 + lane;
+              const int q = (int)(((unsigned)t * inv) >> 16), mm = t - q * M;
+              const int r = r0 + (t < T ? q : 0);
               const u64 b_row = __shfl_sync(full, br, r);
-              const bool hit = j < je && __popcll(b_row ^ bj) <= dmax;
+              const u64 b_col = __shfl_sync(full, bj, t < T ? mm : 0);
+              const bool hit = t < T && __popcll(b_row ^ b_col) <= dmax;
               const unsigned m = __ballot_sync(full, hit);
               if (m) {  // warp-uniform
-                if (hit) { const int idx = qn + __popc(m & lt); qrow[idx] = (unsigned char)r; qcol[idx] = j; }
+                if (hit) { const int idx = qn + __popc(m & lt); qrow[idx] = (unsigned char)r; qcol[idx] = js + mm; }
                 qn += __popc(m);
                 __syncwarp();
                 if (qn >= 32) flush(32);
+              }
+            }
+          } else {
+            for (int c0 = js; c0 < je; c0 += 32) {
+              const int j = c0 + lane;
+              const u64 bj = j < je ? __ldg(dets + 2 * (int64_t)j + 1) : 0ull;
+              for (int r = r0; r < r1; ++r) {  // every row of the run against these 32 columns
+                const u64 b_row = __shfl_sync(full, br, r);
+                const bool hit = j < je && __popcll(b_row ^ bj) <= dmax;
+                const unsigned m = __ballot_sync(full, hit);
+                if (m) {  // warp-uniform
+                  if (hit) { const int idx = qn + __popc(m & lt); qrow[idx] = (unsigned char)r; qcol[idx] = j; }
+                  qn += __popc(m);
+                  __syncwarp();
+                  if (qn >= 32) flush(32);
+                }
               }
             }
           }
@@ -197,11 +241,24 @@ pair_kernel(EnumParams P, const u64* __restrict__ dets, int64_t nd, double eps, 
       }
     }
     if (qn > 0) flush(qn);
-    if (!kFill && have) row_cnt[row] = cnt[lane];
+    if (have) row_cnt[row] = cnt[lane];
     __syncwarp();
   }
+  if (lane == 0 && wpos >= 0 && wend > 0) bused[(wend - 1) / kArenaBlk] = (int)(wpos - (wend - kArenaBlk));
   for (int o = 16; o > 0; o >>= 1) evaluated += __shfl_xor_sync(full, evaluated, o);
   if (lane == 0 && evaluated) atomicAdd(counters + 1, evaluated);
+}
+
+// arena -> CSR: entry e of a block's used part goes to row_ptr[row] + place in the row
+__global__ void pair_scatter_kernel(const u64* __restrict__ akey, const int* __restrict__ acol, const double* __restrict__ aval,
+                                    const int* __restrict__ bused, int64_t n_arena, const int64_t* __restrict__ row_ptr,
+                                    int* __restrict__ col, double* __restrict__ val) {
+  for (int64_t e = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; e < n_arena; e += (int64_t)gridDim.x * blockDim.x) {
+    if ((int)(e % kArenaBlk) >= bused[e / kArenaBlk]) continue;
+    const u64 key = akey[e];
+    const int64_t dst = row_ptr[key >> 32] + (int64_t)(key & 0xffffffffull);
+    col[dst] = acol[e]; val[dst] = aval[e];
+  }
 }
 
 }  // namespace
@@ -250,20 +307,50 @@ dh_status dh_pair_build(detham_ctx* c, double eps) {
   group_fill_kernel<<<nb256, 256, 0, c->stream>>>(c->dets, nd, c->row_cnt, c->row_ptr, c->pair_galpha, c->pair_gstart);
   pair_diag_kernel<<<(unsigned)((nd + 127) / 128), 128, 0, c->stream>>>(c->n, c->J, c->JK, c->hd, c->e_core, c->dets, nd, c->pair_diag);
   DH_CUDA(c, cudaGetLastError());
-  // ---- count, scan, fill
+  // ---- one pass into the arena (sized from the previous build; a guess the first time), row scan, scatter
   const int64_t nblk = (nd + 31) / 32;
   int64_t want = (nblk + kPairWarps - 1) / kPairWarps;
   const int grid = (int)(want < (int64_t)c->sm_count * 8 ? want : (int64_t)c->sm_count * 8);
-  DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 8 * sizeof(u64), c->stream));
-  pair_kernel<false><<<grid, kPairWarps * 32, 0, c->stream>>>(P, c->dets, nd, eps, c->pair_galpha, c->pair_gstart, (int)ng, c->pair_diag,
-                                                             c->row_cnt, nullptr, nullptr, nullptr, c->dcount);
-  excl_scan_kernel<<<1, 1024, 0, c->stream>>>(c->row_cnt, nd, c->row_ptr);
-  DH_CUDA(c, cudaGetLastError());
-  DH_TICK(c, 1);
-  DH_CUDA(c, cudaMemcpyAsync(h, c->row_ptr + nd, sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
-  DH_CUDA(c, cudaMemcpyAsync(h + 1, c->dcount, 2 * sizeof(u64), cudaMemcpyDeviceToHost, c->stream));
-  DH_CUDA(c, cudaStreamSynchronize(c->stream));
-  const int64_t nnz = h[0];
+  const int64_t slack = (int64_t)grid * kPairWarps * kArenaBlk;  // every warp may leave one block partly used
+  int* overflow = reinterpret_cast<int*>(c->dcount + 8);
+  int64_t want_arena = c->arena_cap;
+  if (want_arena <= 0) {  // first build of the context: room for 1024 entries per row if a quarter of the free memory allows it
+    size_t free_b = 0, total_b = 0;
+    DH_CUDA(c, cudaMemGetInfo(&free_b, &total_b));
+    const int64_t by_mem = (int64_t)(free_b / 4 / 20);  // 20 bytes per arena entry (tag, column, value)
+    want_arena = std::max<int64_t>(nd * 64 + slack, std::min<int64_t>(nd * 1024 + slack, by_mem));
+  }
+  int64_t nnz = 0, n_arena = 0;
+  double ms_pass = 0.0;
+  for (int attempt = 0;; ++attempt) {
+    if (c->arena_cap < want_arena) {
+      if (c->acol) cudaFree(c->acol);
+      if (c->aval) cudaFree(c->aval);
+      c->acol = nullptr; c->aval = nullptr; c->arena_cap = 0;
+      DH_CUDA(c, cudaMalloc(&c->acol, want_arena * sizeof(int)));
+      DH_CUDA(c, cudaMalloc(&c->aval, want_arena * sizeof(double)));
+      c->arena_cap = want_arena;
+    }
+    st = grow(reinterpret_cast<void**>(&c->pair_akey), &c->pair_akey_cap, c->arena_cap, sizeof(u64)); if (st != DH_OK) return st;
+    st = grow(reinterpret_cast<void**>(&c->pair_bused), &c->pair_bused_cap, c->arena_cap / kArenaBlk + 1, sizeof(int)); if (st != DH_OK) return st;
+    DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 16 * sizeof(u64), c->stream));
+    if (attempt > 0) DH_TICK(c, 0);
+    pair_kernel<<<grid, kPairWarps * 32, 0, c->stream>>>(P, c->dets, nd, eps, c->pair_galpha, c->pair_gstart, (int)ng, c->pair_diag, c->row_cnt,
+                                                        c->pair_akey, c->acol, c->aval, c->pair_bused, c->arena_cap, c->dcount, overflow);
+    excl_scan_kernel<<<1, 1024, 0, c->stream>>>(c->row_cnt, nd, c->row_ptr);
+    DH_CUDA(c, cudaGetLastError());
+    DH_TICK(c, 1);
+    DH_CUDA(c, cudaMemcpyAsync(h, c->row_ptr + nd, sizeof(int64_t), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(c, cudaMemcpyAsync(h + 1, c->dcount, 3 * sizeof(u64), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(c, cudaMemcpyAsync(h + 5, overflow, sizeof(int), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(c, cudaStreamSynchronize(c->stream));
+    ms_pass += dh_elapsed(c, 0, 1);
+    nnz = h[0];
+    n_arena = h[3];
+    if (!*reinterpret_cast<int*>(h + 5)) break;
+    if (attempt >= 1) return DH_ENOMEM;  // cannot happen: the second attempt is sized from the exact count
+    want_arena = nnz + nnz / 32 + slack;  // a block is closed when the next batch of <= 32 entries does not fit
+  }
   if (c->csr_cap < nnz) {
     if (c->col) cudaFree(c->col);
     if (c->val) cudaFree(c->val);
@@ -274,13 +361,12 @@ dh_status dh_pair_build(detham_ctx* c, double eps) {
     c->csr_cap = cap;
   }
   DH_TICK(c, 2);
-  DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 8 * sizeof(u64), c->stream));
-  pair_kernel<true><<<grid, kPairWarps * 32, 0, c->stream>>>(P, c->dets, nd, eps, c->pair_galpha, c->pair_gstart, (int)ng, c->pair_diag,
-                                                            c->row_cnt, c->row_ptr, c->col, c->val, c->dcount);
+  pair_scatter_kernel<<<c->sm_count * 16, 256, 0, c->stream>>>(c->pair_akey, c->acol, c->aval, c->pair_bused, n_arena, c->row_ptr, c->col, c->val);
   DH_CUDA(c, cudaGetLastError());
   DH_TICK(c, 3);
   DH_CUDA(c, cudaEventSynchronize(c->ev[3]));
-  c->ctr.ms_build_count = dh_elapsed(c, 0, 1);
+  (void)ms_pass;
+  c->ctr.ms_build_count = ms_pass;
   c->ctr.ms_build_fill = dh_elapsed(c, 2, 3);
   c->ctr.build_generated = h[2];  // elements evaluated (pairs of S within a double excitation of each other)
   c->ctr.nnz = nnz;
