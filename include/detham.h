@@ -135,6 +135,27 @@ dh_status detham_csr_copy(detham_ctx* ctx, int64_t* row_ptr, int32_t* col, doubl
  * psi: DEVICE fp64 [n_dets].  y_out: DEVICE fp64 [n_dets] or NULL.  e_out, norm2_out: HOST (norm2_out may be NULL). */
 dh_status detham_energy(detham_ctx* ctx, const double* psi, double* e_out, double* norm2_out, double* y_out);
 
+/* energy for callers that may not allocate (code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc):
+ * the same per-row arithmetic as detham_energy (Eq. 11) on a CSR the caller passes, with the partial sums in a
+ * file-scope device array of the library (128 KB, held by every GPU that loads the library until exit) instead of a buffer of
+ * a context.  The call needs no context, allocates nothing (no cudaMalloc, cudaFree or allocating library routine), does not
+ * synchronise, and launches two kernels on `stream` (a cudaStream_t; NULL = the default stream) of the CURRENT device.
+ *   row_ptr DEVICE int64 [n_dets+1], col DEVICE int32 [nnz], val DEVICE fp64 [nnz], psi DEVICE fp64 [n_dets]: borrowed inputs,
+ *     e.g. from detham_csr; n_dets >= 1; nnz (the number of stored entries) only chooses the threads per row.
+ *   y_out DEVICE fp64 [n_dets] or NULL: y = H psi.
+ *   out3 DEVICE fp64 [3]: {psi^T H psi, psi^T psi, E_S = their quotient}, written on `stream`.
+ * Sums are taken per block of 1024 rows and then over the blocks in a fixed order: the result is reproducible and does not
+ * depend on the GPU, but differs from detham_energy's in the last bits (another order of the same additions).
+ * Errors: DH_EINVAL for a NULL pointer, n_dets < 1, or n_dets > DETHAM_ENERGY_STATIC_MAX_ROWS (nothing is launched);
+ * DH_ECUDA for a CUDA failure; detham_energy_static_error() gives the text for the calling thread ("" after a success).
+ * Every call on a device shares the one array, which keeps the last call's contents: each entry read is written first by the
+ * same call, so nothing is cleared, but calls that OVERLAP on the GPU (different streams, or replays of captured graphs in
+ * flight together) race on it - run them in stream order. */
+#define DETHAM_ENERGY_STATIC_MAX_ROWS 8388608 /* 2^23 determinants */
+dh_status detham_energy_static(const int64_t* row_ptr, const int32_t* col, const double* val, const double* psi,
+                               int64_t n_dets, int64_t nnz, double* y_out, double* out3, void* stream);
+const char* detham_energy_static_error(void);
+
 /* residual: r = H_SS psi - e_s psi, the vector that Eq. 12 contracts with grad psi,
  * and the internal term of Eq. 13 (first sum) on the CSR built last (reading Q4: the screened
  * operator): *internal_out = (1 / psi^T psi) sum_{i in S} r_i^2 / (e_s - H_ii); a row with r_i == 0 contributes 0.

@@ -12,7 +12,7 @@ _lib = None
 STATUS = {0: "DH_OK", 1: "DH_EINVAL", 2: "DH_EUNSORTED", 3: "DH_EPOPCOUNT", 4: "DH_ENOMEM", 5: "DH_ETABLEFULL", 6: "DH_ECUDA"}
 
 # every symbol include/detham.h declares
-SYMBOLS = ["detham_create", "detham_set_subspace", "detham_ham_build", "detham_build_config", "detham_csr", "detham_csr_copy", "detham_energy", "detham_residual", "detham_ediag",
+SYMBOLS = ["detham_create", "detham_set_subspace", "detham_ham_build", "detham_build_config", "detham_csr", "detham_csr_copy", "detham_energy", "detham_energy_static", "detham_energy_static_error", "detham_residual", "detham_ediag",
            "detham_pt2_config", "detham_pt2_set_options", "detham_trim", "detham_count_screened", "detham_pt2", "detham_expand", "detham_hsp_build", "detham_hsp_csr", "detham_hsp_csr_copy", "detham_pt2_partials", "detham_solve_host", "detham_connections",
            "detham_diagonals", "detham_get_counters", "detham_destroy", "detham_strerror", "detham_last_cuda_error"]
 
@@ -61,6 +61,9 @@ def load_library():
     L.detham_csr.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
     L.detham_csr_copy.argtypes = [vp, vp, vp, vp]
     L.detham_energy.argtypes = [vp, vp, dp, dp, vp]
+    L.detham_energy_static.argtypes = [vp, vp, vp, vp, C.c_int64, C.c_int64, vp, vp, vp]
+    L.detham_energy_static_error.argtypes = []
+    L.detham_energy_static_error.restype = C.c_char_p
     L.detham_residual.argtypes = [vp, vp, C.c_double, vp, dp]
     L.detham_ediag.argtypes = [vp, vp, C.c_double, C.c_int, dp, C.POINTER(C.c_int)]
     L.detham_pt2_config.argtypes = [vp, C.c_int64, C.c_int]
@@ -84,7 +87,7 @@ def load_library():
     L.detham_last_cuda_error.argtypes = [vp]
     L.detham_last_cuda_error.restype = C.c_char_p
     for name in SYMBOLS:
-        if name not in ("detham_destroy", "detham_strerror", "detham_last_cuda_error"):
+        if name not in ("detham_destroy", "detham_strerror", "detham_last_cuda_error", "detham_energy_static_error"):
             getattr(L, name).restype = C.c_int
     _lib = L
     return L
@@ -312,6 +315,43 @@ class Detham:
             self.close()
         except Exception:
             pass
+
+
+ENERGY_STATIC_MAX_ROWS = 8388608  # DETHAM_ENERGY_STATIC_MAX_ROWS of include/detham.h
+
+
+def energy_static(row_ptr, col, val, psi, n_dets=None, nnz=None, want_y=False, out=None, y=None, stream=None):
+    """detham_energy_static: the energy step on a caller-held CSR with the scratch in a static device array of the library - the
+    C call allocates nothing, needs no context and does not synchronise.  row_ptr / col / val: torch CUDA tensors, or raw device
+    pointers (e.g. Detham.csr_pointers()) with `n_dets` and `nnz` given.  `out` (float64 [3] CUDA) and `y` are created here unless
+    passed in.  Returns out = {psi^T H psi, psi^T psi, E_S} (device; read it after synchronising), and y if want_y."""
+    import torch
+    if not torch.cuda.is_available():
+        raise DethamError(6, "no CUDA device: the detham hot path has no CPU fallback")
+    L = load_library()
+    assert psi.is_cuda and psi.dtype == torch.float64 and psi.is_contiguous()
+    ptrs = []
+    for t, dt in ((row_ptr, torch.int64), (col, torch.int32), (val, torch.float64)):
+        if isinstance(t, int):
+            ptrs.append(t)
+        else:
+            assert t.is_cuda and t.dtype == dt and t.is_contiguous()
+            ptrs.append(t.data_ptr())
+    if n_dets is None:
+        n_dets = psi.numel()
+    if nnz is None:
+        nnz = val.numel()
+    if out is None:
+        out = torch.empty(3, dtype=torch.float64, device=psi.device)
+    if want_y and y is None:
+        y = torch.empty_like(psi)
+    assert out.is_cuda and out.dtype == torch.float64 and out.numel() >= 3
+    sp = C.c_void_p(stream.cuda_stream) if stream is not None else C.c_void_p(torch.cuda.current_stream().cuda_stream)
+    st = L.detham_energy_static(ptrs[0], ptrs[1], ptrs[2], psi.data_ptr(), int(n_dets), int(nnz),
+                                y.data_ptr() if want_y else None, out.data_ptr(), sp)
+    if st != 0:
+        raise DethamError(st, L.detham_strerror(st).decode(), L.detham_energy_static_error().decode())
+    return (out, y) if want_y else out
 
 
 def create(n_orb, n_alpha, n_beta, h1, eri, e_core=0.0, stream=None) -> Detham:

@@ -8,7 +8,7 @@ PKG = os.path.dirname(os.path.abspath(__file__))
 ROOT = os.path.dirname(PKG)
 CSRC = os.path.join(PKG, "csrc")
 SO = os.path.join(PKG, "libdetham.so")
-SOURCES = ["api.cu", "lists.cu", "ham_build.cu", "pair_build.cu", "energy.cu", "ediag.cu", "pt2.cu", "pt2_stream.cu", "expand.cu"]
+SOURCES = ["api.cu", "lists.cu", "ham_build.cu", "pair_build.cu", "energy.cu", "energy_static.cu", "ediag.cu", "pt2.cu", "pt2_stream.cu", "expand.cu"]
 HEADERS = ["common.cuh", "enumerate.cuh", "pt2_common.cuh"]
 
 
