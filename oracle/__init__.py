@@ -60,6 +60,8 @@ def lib():
         L.orc_expand.argtypes = [C.c_int, dp, dp, C.c_double, up, C.c_int64, dp, C.c_double, up, dp, dp, dp, C.c_int64]
         L.orc_hsp_build.restype = C.c_void_p
         L.orc_hsp_build.argtypes = [C.c_int, dp, dp, C.c_double, up, C.c_int64, dp, C.c_double, up, C.c_int64]
+        L.orc_complete_sum.restype = None
+        L.orc_complete_sum.argtypes = [C.c_int, dp, dp, C.c_double, up, C.c_int64, dp, up, C.c_int64, dp]
         L.orc_num_threads.restype = C.c_int
         _lib = L
     return _lib
@@ -181,6 +183,15 @@ def expand(n, h1, eri, e_core, dets, psi, eps2):
     if m:
         lib().orc_expand(n, _d(h1), _d(eri), e_core, _u(dets), dets.shape[0], _d(psi), eps2, _u(keys), _d(score), _d(v), _d(haa), m)
     return keys, score, v, haa
+
+
+def complete_sum(n, h1, eri, e_core, dets, psi, pkeys):
+    """v_a = sum over ALL i in V of H_ai psi_i (the full <x|H|Psi_V> of Eq. 13) for the sorted key list `pkeys`."""
+    h1, eri, dets, psi, pkeys = _f64(h1), _f64(eri), _u64(dets), _f64(psi), _u64(pkeys)
+    v = np.zeros(pkeys.shape[0])
+    if pkeys.shape[0]:
+        lib().orc_complete_sum(n, _d(h1), _d(eri), e_core, _u(dets), dets.shape[0], _d(psi), _u(pkeys), pkeys.shape[0], _d(v))
+    return v
 
 
 def hsp_build(n, h1, eri, e_core, dets, psi, eps2, pkeys):

@@ -444,6 +444,27 @@ void* orc_hsp_build(int n, const double* h1, const double* eri_, double e_core, 
   return out;
 }
 
+// The complete-the-sum variant of the perturbative amplitude (reading Q9's alternative): Eq. 13
+// writes the numerator of the external term as <x|H|Psi_V>, the FULL projection.  For a GIVEN sorted key list P
+// (the members Eq. 14 selected) this returns v_a = sum_{i in V} H_ai psi_i over ALL i, screened or not, by the plain definition:
+// element() on every pair (a, i), added in ascending i in long double.  O(|P| |V|) element tests.
+void orc_complete_sum(int n, const double* h1, const double* eri_, double e_core, const u64* dets, int64_t nd, const double* psi,
+                      const u64* pkeys, int64_t m, double* v_out) {
+  Integrals I{n, h1, eri_, e_core};
+  const Det* S = reinterpret_cast<const Det*>(dets);
+  const Det* Pk = reinterpret_cast<const Det*>(pkeys);
+#pragma omp parallel for schedule(dynamic, 64)
+  for (int64_t a = 0; a < m; ++a) {
+    long double v = 0.0L;
+    for (int64_t i = 0; i < nd; ++i) {
+      if (psi[i] == 0.0) continue;
+      if (__builtin_popcountll(Pk[a].a ^ S[i].a) + __builtin_popcountll(Pk[a].b ^ S[i].b) > 4) continue;  // more than a double: 0
+      v += (long double)(element(I, Pk[a], S[i]) * psi[i]);
+    }
+    v_out[a] = (double)v;
+  }
+}
+
 int orc_num_threads(void) {
 #ifdef _OPENMP
   return omp_get_max_threads();

@@ -351,6 +351,39 @@ def test_p13_expand_dense_brute_force(orc, eps2):
     assert np.isclose(r["pt2"], np.sum(v ** 2 / (-3.0 - haa)) / (psi @ psi), rtol=1e-12)
 
 
+def test_p13b_complete_sum_dense_brute_force(orc):
+    """The complete-the-sum amplitude v_a = sum over ALL i in V of H_ai psi_i (the full <x|H|Psi_V> of Eq. 13) for
+    the members of P that Eq. 14 selected: rows of the dense matrix times psi.  It differs from the screened sum of expand()
+    exactly by the couplings below the screen, and equals it at eps2 = 0."""
+    n, na, nb = 7, 3, 3
+    h1, eri = small_integrals(n, 61)
+    dets = full_space(n, na, nb)
+    H = orc.dense(n, h1, eri, 0.0, dets)
+    rng = np.random.default_rng(18)
+    idx = np.sort(rng.choice(len(dets), size=150, replace=False))
+    psi = rng.standard_normal(150) * np.exp(-rng.random(150) * 4)
+    psi[11] = 0.0
+    pos = {tuple(d): k for k, d in enumerate(dets.tolist())}
+    for eps2 in (0.0, 2e-2):
+        keys, score, v, haa = orc.expand(n, h1, eri, 0.0, dets[idx], psi, eps2)
+        rows = np.array([pos[tuple(k)] for k in keys.tolist()])
+        full = H[np.ix_(rows, idx)] @ psi
+        vc = orc.complete_sum(n, h1, eri, 0.0, dets[idx], psi, keys)
+        assert np.allclose(vc, full, rtol=1e-12, atol=1e-14)
+        if eps2 == 0.0:
+            assert np.allclose(vc, v, rtol=1e-12, atol=1e-14)
+        else:
+            tau = np.where(psi != 0, eps2 / np.abs(np.where(psi != 0, psi, 1.0)), np.inf)
+            below = (np.abs(H[np.ix_(rows, idx)]) < tau[None, :]) * H[np.ix_(rows, idx)]
+            assert np.allclose(vc - v, below @ psi, rtol=1e-10, atol=1e-13)
+            assert np.max(np.abs(vc - v)) > 1e-6  # the two readings really differ on this input
+    # a key list that is not the output of expand (a subset, and a member of V itself: H_ii psi_i + its couplings)
+    sub = np.vstack([keys[::3], dets[idx][5:6]])
+    sub = sub[np.lexsort((sub[:, 1], sub[:, 0]))]
+    rows = np.array([pos[tuple(k)] for k in sub.tolist()])
+    assert np.allclose(orc.complete_sum(n, h1, eri, 0.0, dets[idx], psi, sub), H[np.ix_(rows, idx)] @ psi, rtol=1e-12, atol=1e-14)
+
+
 # ---------------------------------------------------------------- P14: H_VP in CSR and the Proxy Hamiltonian of Eq. 8
 @pytest.mark.parametrize("eps2", [0.0, 1e-3, 2e-2])
 def test_p14_hsp_dense_brute_force(orc, eps2):
