@@ -163,10 +163,14 @@ const char* detham_energy_static_error(void);
 dh_status detham_residual(detham_ctx* ctx, const double* psi, double e_s, double* r_out, double* internal_out);
 
 /* ediag: E_diag = lambda_min(H_SS) of the CSR built last, by Lanczos on the device
- * (SpMV = the energy kernel).  v0: DEVICE fp64 [n_dets] start vector (psi is a good one) or NULL (all ones); stops when the
- * smallest Ritz value moves by less than tol * |value| between two steps, when the Krylov space closes, or after max_iter
- * steps.  e_out, iters_out (may be NULL): HOST.  Delta_opt of the paper = E_S - *e_out >= 0. */
-dh_status detham_ediag(detham_ctx* ctx, const double* v0, double tol, int max_iter, double* e_out, int* iters_out);
+ * (SpMV = the energy kernel).  v0: DEVICE fp64 [n_dets] start vector (psi is a good one) or NULL (all ones).  With r the residual
+ * norm ||H y - theta y|| of the smallest Ritz pair (an eigenvalue lies within r of theta), the iteration stops when
+ * r <= tol |theta| or when the Krylov space closes; otherwise after max_iter steps with *converged_out = 0 (the value is then an
+ * upper bound of lambda_min only).  theta itself converges like r^2 / gap, so tol = 1e-8 already gives ~1e-12 on the value.
+ * e_out, iters_out, resid_out (= r), converged_out (1 / 0): HOST, all but e_out may be NULL.  Delta_opt of the paper =
+ * E_S - *e_out >= 0. */
+dh_status detham_ediag(detham_ctx* ctx, const double* v0, double tol, int max_iter, double* e_out, int* iters_out,
+                       double* resid_out, int* converged_out);
 
 /* Configure pt2: table_slots = hash-table capacity in 32-byte slots (0 = choose from free device memory);
  * n_parts = number of key partitions / passes, a power of two <= 1024 (0 = choose so that every partition fits).
@@ -214,6 +218,15 @@ dh_status detham_expand(detham_ctx* ctx, const double* psi, double eps2, uint64_
  * m < 2^31, may be 0.  *nnz_out (HOST, may be NULL).  The CSR is owned by the context (detham_hsp_csr / detham_hsp_csr_copy),
  * valid until the next detham_hsp_build / detham_set_subspace / detham_destroy. */
 dh_status detham_hsp_build(detham_ctx* ctx, const double* psi, double eps2, const uint64_t* pkeys, int64_t m, int64_t* nnz_out);
+
+/* complete_sum (the complete-the-sum variant; Eq. 13, PAPER.md:189 writes the external numerator as
+ * <x|H|Psi_V>, the full projection, while Eq. 14 / PAPER.md:227 generate only the couplings above the screen - DESIGN.md reading
+ * Q9): for `pkeys` - DEVICE uint64 [m][2], strictly ascending, same electron counts as S (DH_EUNSORTED / DH_EPOPCOUNT otherwise),
+ * normally the keys detham_expand selected - v_out[k] = sum over ALL i in S of H_{P_k, i} psi_i, screened or not (a key that is
+ * itself a member of S includes its diagonal term).  One unscreened enumeration of every source with psi_i != 0, so the cost is
+ * that of pt2 at eps2 = 0.  psi: DEVICE fp64 [n_dets]; v_out: DEVICE fp64 [m], overwritten; m < 2^31, may be 0.  The additions
+ * are atomic: their order, hence the last bits, vary from run to run.  Synchronises the stream. */
+dh_status detham_complete_sum(detham_ctx* ctx, const double* psi, const uint64_t* pkeys, int64_t m, double* v_out);
 /* Device pointers of H_SP: row_ptr int64 [n_dets+1], col int32 [nnz], val fp64 [nnz].  DH_EINVAL if none exists. */
 dh_status detham_hsp_csr(detham_ctx* ctx, const int64_t** row_ptr, const int32_t** col, const double** val);
 /* Copy H_SP into caller buffers (each HOST or DEVICE, detected; any may be NULL to skip).  Synchronises the stream. */

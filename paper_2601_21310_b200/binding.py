@@ -13,7 +13,7 @@ STATUS = {0: "DH_OK", 1: "DH_EINVAL", 2: "DH_EUNSORTED", 3: "DH_EPOPCOUNT", 4: "
 
 # every symbol include/detham.h declares
 SYMBOLS = ["detham_create", "detham_set_subspace", "detham_ham_build", "detham_build_config", "detham_csr", "detham_csr_copy", "detham_energy", "detham_energy_static", "detham_energy_static_error", "detham_residual", "detham_ediag",
-           "detham_pt2_config", "detham_pt2_set_options", "detham_trim", "detham_count_screened", "detham_pt2", "detham_expand", "detham_hsp_build", "detham_hsp_csr", "detham_hsp_csr_copy", "detham_pt2_partials", "detham_solve_host", "detham_connections",
+           "detham_pt2_config", "detham_pt2_set_options", "detham_trim", "detham_count_screened", "detham_pt2", "detham_expand", "detham_hsp_build", "detham_complete_sum", "detham_hsp_csr", "detham_hsp_csr_copy", "detham_pt2_partials", "detham_solve_host", "detham_connections",
            "detham_diagonals", "detham_get_counters", "detham_destroy", "detham_strerror", "detham_last_cuda_error"]
 
 
@@ -65,7 +65,7 @@ def load_library():
     L.detham_energy_static_error.argtypes = []
     L.detham_energy_static_error.restype = C.c_char_p
     L.detham_residual.argtypes = [vp, vp, C.c_double, vp, dp]
-    L.detham_ediag.argtypes = [vp, vp, C.c_double, C.c_int, dp, C.POINTER(C.c_int)]
+    L.detham_ediag.argtypes = [vp, vp, C.c_double, C.c_int, dp, C.POINTER(C.c_int), dp, C.POINTER(C.c_int)]
     L.detham_pt2_config.argtypes = [vp, C.c_int64, C.c_int]
     L.detham_pt2_set_options.argtypes = [vp, C.POINTER(Pt2Options)]
     L.detham_trim.argtypes = [vp]
@@ -73,6 +73,7 @@ def load_library():
     L.detham_pt2.argtypes = [vp, vp, C.c_double, C.c_double, dp, ip, ip]
     L.detham_expand.argtypes = [vp, vp, C.c_double, vp, vp, vp, vp, C.c_int64, ip]
     L.detham_hsp_build.argtypes = [vp, vp, C.c_double, vp, C.c_int64, ip]
+    L.detham_complete_sum.argtypes = [vp, vp, vp, C.c_int64, vp]
     L.detham_hsp_csr.argtypes = [vp, C.POINTER(vp), C.POINTER(vp), C.POINTER(vp)]
     L.detham_hsp_csr_copy.argtypes = [vp, vp, vp, vp]
     L.detham_pt2_partials.argtypes = [vp, dp, C.c_int, C.POINTER(C.c_int)]
@@ -180,13 +181,19 @@ class Detham:
         return r, out.value
 
     def ediag(self, v0=None, tol=1e-12, max_iter=500):
-        """(E_diag = lambda_min(H_SS), Lanczos steps taken)."""
+        """(E_diag = lambda_min(H_SS), Lanczos steps taken).  `self.ediag_residual` = residual norm of the Ritz pair returned,
+        `self.ediag_converged` = whether the stopping rule of include/detham.h was met (False: max_iter reached; a warning is
+        issued, the value is an upper bound only)."""
         import torch
         if v0 is not None:
             assert v0.is_cuda and v0.dtype == torch.float64 and v0.is_contiguous() and v0.numel() == self.n_dets
-        e, it = C.c_double(0), C.c_int(0)
+        e, it, res, conv = C.c_double(0), C.c_int(0), C.c_double(0), C.c_int(0)
         self._check(self._L.detham_ediag(self._h, v0.data_ptr() if v0 is not None else None, float(tol), int(max_iter),
-                                         C.byref(e), C.byref(it)))
+                                         C.byref(e), C.byref(it), C.byref(res), C.byref(conv)))
+        self.ediag_residual, self.ediag_converged = res.value, bool(conv.value)
+        if not self.ediag_converged:
+            import warnings
+            warnings.warn(f"detham_ediag: not converged after {it.value} steps (residual {res.value:.3g})")
         return e.value, it.value
 
     def expand(self, psi, eps2):
@@ -223,6 +230,15 @@ class Detham:
         self._check(self._L.detham_hsp_build(self._h, psi.data_ptr(), float(eps2), ptr if m else None, m, C.byref(nnz)))
         self.hsp_nnz = nnz.value
         return nnz.value
+
+    def complete_sum(self, psi, pkeys):
+        """v_a = sum over ALL i in S of H_ai psi_i (the full <x|H|Psi_V> of Eq. 13) for the sorted CUDA key tensor `pkeys` [m, 2]."""
+        import torch
+        assert psi.is_cuda and psi.dtype == torch.float64 and psi.is_contiguous() and psi.numel() == self.n_dets
+        ptr, m = _dev_u64(pkeys) if pkeys.numel() else (None, 0)
+        v = torch.empty(m, dtype=torch.float64, device="cuda")
+        self._check(self._L.detham_complete_sum(self._h, psi.data_ptr(), ptr, m, v.data_ptr() if m else None))
+        return v
 
     def hsp_csr(self):
         """(row_ptr int64 [|S|+1], col int32 [nnz], val fp64 [nnz]) of H_SP as new torch CUDA tensors."""

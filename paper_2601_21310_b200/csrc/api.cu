@@ -23,7 +23,7 @@ void free_all(detham_ctx* c) {
   f(c->h1); f(c->eri); f(c->J); f(c->JK); f(c->hd);
   for (auto& L : c->lists) { f(L.sub_off); f(L.val); f(L.ab); f(L.stat); }
   f(c->dets_owned); f(c->psi_owned); f(c->shash_key); f(c->shash_idx); f(c->sbits);
-  f(c->row_ptr); f(c->col); f(c->val); f(c->row_cnt); f(c->sp_row_ptr); f(c->sp_col); f(c->sp_val); f(c->phash_key); f(c->phash_idx); f(c->acol); f(c->aval); f(c->segs); f(c->table); f(c->pool); f(c->ring); f(c->sflags); f(c->pair_galpha); f(c->pair_gstart); f(c->pair_diag); f(c->pair_akey); f(c->pair_bused); f(c->red); f(c->dcount); f(c->hist);
+  f(c->row_ptr); f(c->col); f(c->val); f(c->row_cnt); f(c->sp_row_ptr); f(c->sp_col); f(c->sp_val); f(c->phash_key); f(c->phash_idx); f(c->acol); f(c->aval); f(c->segs); f(c->table); f(c->pool); f(c->ring); f(c->sflags); f(c->pair_galpha); f(c->pair_gstart); f(c->pair_diag); f(c->pair_akey); f(c->pair_bused); f(c->red); f(c->dcount); f(c->hist); f(c->scratch); f(c->perm);
   if (c->pinned) cudaFreeHost(c->pinned);
   for (auto& e : c->ev) if (e) cudaEventDestroy(e);
   for (auto& e : c->sev) cudaEventDestroy(e);
@@ -134,9 +134,10 @@ dh_status detham_residual(detham_ctx* c, const double* psi, double e_s, double* 
   return dh_residual(c, psi, e_s, r_out, internal_out);
 }
 
-dh_status detham_ediag(detham_ctx* c, const double* v0, double tol, int max_iter, double* e_out, int* iters_out) {
+dh_status detham_ediag(detham_ctx* c, const double* v0, double tol, int max_iter, double* e_out, int* iters_out, double* resid_out,
+                       int* converged_out) {
   if (!c || !e_out || c->nnz < 0 || !(tol > 0.0) || max_iter < 1) return DH_EINVAL;
-  return dh_ediag(c, v0, tol, max_iter, e_out, iters_out);
+  return dh_ediag(c, v0, tol, max_iter, e_out, iters_out, resid_out, converged_out);
 }
 
 dh_status detham_pt2_config(detham_ctx* c, int64_t table_slots, int n_parts) {
@@ -169,6 +170,7 @@ dh_status detham_trim(detham_ctx* c) {
   f(c->pool); c->pool_bytes = 0;
   f(c->ring); c->ring_bytes = 0;
   f(c->sflags); c->sflags_bytes = 0;
+  f(c->scratch); c->scratch_bytes = 0;
   for (int k = 1; k <= DH_MAX_PBITS; ++k) {
     HbLists& L = c->lists[k];
     f(L.sub_off); f(L.val); f(L.ab); f(L.stat);
@@ -196,6 +198,11 @@ dh_status detham_expand(detham_ctx* c, const double* psi, double eps2, uint64_t*
                         double* haa_out, int64_t cap, int64_t* n_out) {
   if (!c || !c->dets || !psi || !(eps2 >= 0.0) || !n_out || cap < 0 || (cap > 0 && !keys_out)) return DH_EINVAL;
   return dh_expand(c, psi, eps2, reinterpret_cast<u64*>(keys_out), score_out, v_out, haa_out, cap, n_out);
+}
+
+dh_status detham_complete_sum(detham_ctx* c, const double* psi, const uint64_t* pkeys, int64_t m, double* v_out) {
+  if (!c || !c->dets || !psi || m < 0 || m >= (1ll << 31) || (m > 0 && (!pkeys || !v_out || !is_device_ptr(pkeys)))) return DH_EINVAL;
+  return dh_complete_sum(c, psi, reinterpret_cast<const u64*>(pkeys), m, v_out);
 }
 
 dh_status detham_hsp_build(detham_ctx* c, const double* psi, double eps2, const uint64_t* pkeys, int64_t m, int64_t* nnz_out) {

@@ -116,6 +116,10 @@ struct detham_ctx {
   double* red = nullptr;      // device reduction buffer
   int64_t red_cap = 0;
   u64* dcount = nullptr;      // device counters [64]
+  int* perm = nullptr;        // pt2: sources in key-class order
+  int64_t perm_cap = 0;
+  void* scratch = nullptr;    // grow-only work space of ediag / expand / connections (dh_scratch), freed by detham_trim
+  size_t scratch_bytes = 0;
   void* pinned = nullptr;     // pinned host scratch (4 KB)
   int64_t* hist = nullptr;    // device int64 [1024] class histogram
 
@@ -142,10 +146,12 @@ dh_status dh_get_lists(detham_ctx* c, int pbits, const HbLists** out);
 dh_status dh_ham_build(detham_ctx* c, double eps);
 dh_status dh_pair_build(detham_ctx* c, double eps);
 dh_status dh_hsp_build(detham_ctx* c, const double* psi, double eps2, const u64* pkeys, int64_t m);
+dh_status dh_complete_sum(detham_ctx* c, const double* psi, const u64* pkeys, int64_t m, double* v_out);
 dh_status dh_energy(detham_ctx* c, const double* psi, double* e_out, double* n2_out, double* y_out);
 dh_status dh_expand(detham_ctx* c, const double* psi, double eps2, u64* keys_out, double* score_out, double* v_out, double* haa_out,
                     int64_t cap, int64_t* n_out);
-dh_status dh_ediag(detham_ctx* c, const double* v0, double tol, int max_iter, double* e_out, int* iters_out);
+dh_status dh_ediag(detham_ctx* c, const double* v0, double tol, int max_iter, double* e_out, int* iters_out, double* resid_out,
+                   int* converged_out);
 dh_status dh_residual(detham_ctx* c, const double* psi, double e_s, double* r_out, double* internal_out);
 dh_status dh_pt2(detham_ctx* c, const double* psi, double e_s, double eps2, double* out);
 dh_status dh_count_screened(detham_ctx* c, const double* psi, double thr, int64_t* n_out);
@@ -154,6 +160,8 @@ dh_status dh_diagonals(detham_ctx* c, const u64* dets, int64_t m, double* out);
 dh_status dh_build_shash(detham_ctx* c);
 dh_status dh_validate_subspace(detham_ctx* c, const u64* dets, int64_t nd);
 dh_status dh_ensure_red(detham_ctx* c, int64_t n);
+// the context's work space, at least `bytes` long and 256-byte aligned; contents do not survive a call that asks for more
+dh_status dh_scratch(detham_ctx* c, size_t bytes, void** p);
 
 // ---------------------------------------------------------------- device helpers
 #ifdef __CUDACC__

@@ -63,12 +63,15 @@ int sturm_count(const std::vector<double>& a, const std::vector<double>& b, doub
   return cnt;
 }
 
-double tridiag_min(const std::vector<double>& a, const std::vector<double>& b) {
+// smallest eigenvalue of the tridiagonal; `upper` (if finite) is a known upper bound of it - the previous step's value, since
+// the smallest Ritz value never increases from one Lanczos step to the next (Cauchy interlacing)
+double tridiag_min(const std::vector<double>& a, const std::vector<double>& b, double upper) {
   double lo = INFINITY, hi = -INFINITY;
   for (size_t k = 0; k < a.size(); ++k) {  // Gershgorin
     const double r = (k > 0 ? fabs(b[k - 1]) : 0.0) + (k + 1 < a.size() ? fabs(b[k]) : 0.0);
     lo = fmin(lo, a[k] - r); hi = fmax(hi, a[k] + r);
   }
+  if (isfinite(upper) && upper < hi && upper > lo && sturm_count(a, b, upper) >= 1) hi = upper;
   for (int it = 0; it < 200 && hi - lo > 4e-16 * fmax(fabs(lo), fabs(hi)); ++it) {
     const double mid = 0.5 * (lo + hi);
     if (sturm_count(a, b, mid) >= 1) hi = mid; else lo = mid;
@@ -76,18 +79,57 @@ double tridiag_min(const std::vector<double>& a, const std::vector<double>& b) {
   return 0.5 * (lo + hi);
 }
 
+// |last component| of the normalised eigenvector of the tridiagonal for its eigenvalue theta, by the twisted factorisation:
+// with the pivots of T - theta I taken from the top (dp) and from the bottom (dm), gamma_r = dp_r + dm_r - (a_r - theta) is
+// smallest where the eigenvector is largest; from z_r = 1 the components follow downwards through dp and upwards through dm, both
+// in the stable direction.  (A plain top-down pivot sequence meets its near-zero pivot wherever the vector is large - at
+// convergence that is far from the last component - and everything after it is wrong.)  beta_k times this number is the residual
+// norm ||H y - theta y|| of the Ritz vector y.
+double ritz_last_component(const std::vector<double>& a, const std::vector<double>& b, double theta) {
+  const int k = (int)a.size();
+  if (k == 1) return 1.0;
+  std::vector<double> dp(k), dm(k), z(k);
+  for (int j = 0; j < k; ++j) {
+    dp[j] = a[j] - theta - (j == 0 ? 0.0 : b[j - 1] * b[j - 1] / dp[j - 1]);
+    if (dp[j] == 0.0) dp[j] = 1e-300;
+  }
+  for (int j = k - 1; j >= 0; --j) {
+    dm[j] = a[j] - theta - (j == k - 1 ? 0.0 : b[j] * b[j] / dm[j + 1]);
+    if (dm[j] == 0.0) dm[j] = 1e-300;
+  }
+  int r = 0;
+  double best = INFINITY;
+  for (int j = 0; j < k; ++j) {
+    const double g = fabs(dp[j] + dm[j] - (a[j] - theta));
+    if (g < best) { best = g; r = j; }
+  }
+  z[r] = 1.0;
+  for (int j = r - 1; j >= 0; --j) z[j] = -b[j] * z[j + 1] / dp[j];
+  for (int j = r; j < k - 1; ++j) z[j + 1] = -b[j] * z[j] / dm[j + 1];
+  double norm2 = 0.0;
+  for (int j = 0; j < k; ++j) norm2 += z[j] * z[j];
+  return fabs(z[k - 1]) / sqrt(norm2);
+}
+
 }  // namespace
 
-dh_status dh_ediag(detham_ctx* c, const double* v0, double tol, int max_iter, double* e_out, int* iters_out) {
+// Stopping rule: with r_k = beta_k |s_k| the residual norm of the smallest Ritz pair (theta_k, y_k), an eigenvalue of H_SS lies
+// within r_k of theta_k.  The iteration stops when r_k <= tol |theta_k|, or when the Krylov space closes (beta_k ~ 0: exact);
+// otherwise max_iter is reached and *converged_out = 0.  A rule on the movement of theta alone (the first version) takes a start
+// vector close to an excited eigenvector for convergence: theta then stagnates for tens of steps while the ground-state
+// component grows from rounding level, but r_k stays above the bound all the while.  The price is about twice the steps, since
+// theta itself converges like r_k^2 / gap.
+dh_status dh_ediag(detham_ctx* c, const double* v0, double tol, int max_iter, double* e_out, int* iters_out, double* resid_out,
+                   int* converged_out) {
   const int64_t nd = c->nd;
   const int grid = (int)((nd + 255) / 256 < (int64_t)c->sm_count * 8 ? (nd + 255) / 256 : (int64_t)c->sm_count * 8);
-  double* buf = nullptr;  // v_prev, v, w, y
-  DH_CUDA(c, cudaMalloc(&buf, (size_t)4 * nd * sizeof(double)));
-  double* part = nullptr;
-  DH_CUDA(c, cudaMalloc(&part, (size_t)(2 * grid + 2) * sizeof(double)));
+  // v_prev, v, w, y and the partial sums, in the context's work space (no allocation from the second call on)
+  void* ws = nullptr;
+  dh_status st = dh_scratch(c, ((size_t)4 * nd + 2 * grid + 2) * sizeof(double), &ws); if (st != DH_OK) return st;
+  double* buf = static_cast<double*>(ws);
+  double* part = buf + 4 * nd;
   double *vprev = buf, *v = buf + nd, *w = buf + 2 * nd, *y = buf + 3 * nd;
   double* h = reinterpret_cast<double*>(c->pinned);
-  auto cleanup = [&]() { cudaFree(buf); cudaFree(part); };
   auto norm2_of = [&](const double* x, double* out) -> dh_status {  // x^T x through the update kernel's reduction (alpha = beta = 0)
     lanczos_update_kernel<<<grid, 256, 0, c->stream>>>(x, x, nullptr, 0.0, 0.0, nd, w, part);
     sum2_kernel<<<1, 256, 0, c->stream>>>(part, grid, part + 2 * grid);
@@ -97,40 +139,42 @@ dh_status dh_ediag(detham_ctx* c, const double* v0, double tol, int max_iter, do
     *out = h[0];
     return DH_OK;
   };
-  dh_status st;
   // start vector: the caller's (e.g. psi: already close to the ground vector of H_SS), else all ones
   if (v0) DH_CUDA(c, cudaMemcpyAsync(y, v0, nd * sizeof(double), cudaMemcpyDeviceToDevice, c->stream));
   else fill_kernel<<<grid, 256, 0, c->stream>>>(y, 1.0, nd);
   double n2 = 0.0;
-  st = norm2_of(y, &n2); if (st != DH_OK) { cleanup(); return st; }
-  if (!(n2 > 0.0) || !isfinite(n2)) { cleanup(); return DH_EINVAL; }
+  st = norm2_of(y, &n2); if (st != DH_OK) return st;
+  if (!(n2 > 0.0) || !isfinite(n2)) return DH_EINVAL;
   scale_kernel<<<grid, 256, 0, c->stream>>>(y, 1.0 / sqrt(n2), nd, v);
   std::vector<double> a, b;
-  double beta = 0.0, theta = 0.0, theta_prev = INFINITY;
-  int it = 0;
+  double beta = 0.0, theta = 0.0, theta_prev = INFINITY, resid = INFINITY;
+  int it = 0, converged = 0;
   for (; it < max_iter; ++it) {
     double alpha = 0.0, vv = 0.0;
-    st = dh_spmv(c, v, y, &alpha, &vv); if (st != DH_OK) { cleanup(); return st; }  // alpha = v^T H v (v is normalised)
+    st = dh_spmv(c, v, y, &alpha, &vv); if (st != DH_OK) return st;  // alpha = v^T H v (v is normalised)
     alpha /= vv;
     a.push_back(alpha);
-    theta = tridiag_min(a, b);
-    if (it > 0 && fabs(theta - theta_prev) <= tol * fmax(fabs(theta), 1e-300)) { ++it; break; }
-    theta_prev = theta;
+    theta = tridiag_min(a, b, theta_prev);
     lanczos_update_kernel<<<grid, 256, 0, c->stream>>>(y, v, it > 0 ? vprev : nullptr, alpha, beta, nd, w, part);
     sum2_kernel<<<1, 256, 0, c->stream>>>(part, grid, part + 2 * grid);
     DH_CUDA(c, cudaGetLastError());
     DH_CUDA(c, cudaMemcpyAsync(h, part + 2 * grid, sizeof(double), cudaMemcpyDeviceToHost, c->stream));
     DH_CUDA(c, cudaStreamSynchronize(c->stream));
     beta = sqrt(h[0]);
-    if (!(beta > 1e-14 * fmax(fabs(alpha), 1.0))) { ++it; break; }  // invariant subspace reached: theta is exact
+    const double scale = fmax(fabs(theta), 1e-300);
+    if (!(beta > 1e-14 * fmax(fabs(alpha), 1.0))) { resid = beta; converged = 1; ++it; break; }  // invariant subspace: theta is exact
+    resid = beta * ritz_last_component(a, b, theta);
+    theta_prev = theta;
+    if (resid <= tol * scale) { converged = 1; ++it; break; }
     b.push_back(beta);
     double* t = vprev; vprev = v; v = t;           // v_prev <- v
     scale_kernel<<<grid, 256, 0, c->stream>>>(w, 1.0 / beta, nd, v);  // v <- w / beta
     DH_CUDA(c, cudaGetLastError());
   }
   DH_CUDA(c, cudaStreamSynchronize(c->stream));
-  cleanup();
   *e_out = theta;
   if (iters_out) *iters_out = it;
+  if (resid_out) *resid_out = resid;
+  if (converged_out) *converged_out = converged;
   return DH_OK;
 }

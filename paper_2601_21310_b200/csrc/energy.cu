@@ -109,6 +109,17 @@ dh_status dh_ensure_red(detham_ctx* c, int64_t n) {
   return DH_OK;
 }
 
+dh_status dh_scratch(detham_ctx* c, size_t bytes, void** p) {
+  if (c->scratch_bytes < bytes) {
+    if (c->scratch) cudaFree(c->scratch);
+    c->scratch = nullptr; c->scratch_bytes = 0;
+    DH_CUDA(c, cudaMalloc(&c->scratch, bytes));
+    c->scratch_bytes = bytes;
+  }
+  *p = c->scratch;
+  return DH_OK;
+}
+
 dh_status dh_energy(detham_ctx* c, const double* psi, double* e_out, double* n2_out, double* y_out) {
   const int64_t nd = c->nd;
   const double avg = (double)c->nnz / (double)nd;

@@ -1,11 +1,14 @@
-// Sorting of the deduplicated externals of expand mode (row f2) by their 128-bit key: two stable LSD radix-sort passes
-// (low word, then high word) over (word, index) pairs with CUB, then one gather.  A library sort is used here on purpose:
-// this is the "next" row's post-processing, not the hot path.
-#include <cub/device/device_radix_sort.cuh>
-
+// Sorting of the deduplicated externals of expand mode (row f2) by their 128-bit key: a stable LSD radix sort of (word, index)
+// pairs, 8 bits per pass, over the beta word and then the alpha word (only the n_orb bits that can be set), then one gather.
+// Per pass: digit histogram per tile of 4096 elements, one exclusive scan over (digit, tile), stable scatter.  Own kernels: no
+// library sort on this row.
 #include "common.cuh"
 
 namespace {
+
+constexpr int kSortThreads = 1024;  // 32 warps
+constexpr int kSortRounds = 4;      // elements per thread, taken in rounds of 1024 consecutive elements
+constexpr int kSortTile = kSortThreads * kSortRounds;
 
 __global__ void iota_kernel(unsigned* idx, int64_t m) {
   for (int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x; t < m; t += (int64_t)gridDim.x * blockDim.x) idx[t] = (unsigned)t;
@@ -25,35 +28,119 @@ __global__ void gather_kernel(const u64* __restrict__ keys, const double* __rest
   }
 }
 
+// hist[digit * ntiles + tile] = number of elements of the tile with that digit
+__global__ void __launch_bounds__(kSortThreads)
+radix_hist_kernel(const u64* __restrict__ w, int64_t m, int shift, unsigned* __restrict__ hist, int ntiles) {
+  __shared__ unsigned s_hist[256];
+  if (threadIdx.x < 256) s_hist[threadIdx.x] = 0;
+  __syncthreads();
+  const int64_t base = (int64_t)blockIdx.x * kSortTile;
+#pragma unroll
+  for (int r = 0; r < kSortRounds; ++r) {
+    const int64_t e = base + r * kSortThreads + threadIdx.x;
+    if (e < m) atomicAdd(&s_hist[(unsigned)(w[e] >> shift) & 255u], 1u);
+  }
+  __syncthreads();
+  if (threadIdx.x < 256) hist[(int64_t)threadIdx.x * ntiles + blockIdx.x] = s_hist[threadIdx.x];
+}
+
+// in-place exclusive scan of `len` counters by one CTA: per-thread chunk sums, a scan of the 1024 sums, per-thread rescan
+__global__ void __launch_bounds__(1024)
+radix_scan_kernel(unsigned* __restrict__ x, int64_t len) {
+  __shared__ unsigned s_sum[1024];
+  const int64_t chunk = (len + 1023) / 1024;
+  const int64_t b = (int64_t)threadIdx.x * chunk, e = b + chunk < len ? b + chunk : len;
+  unsigned sum = 0;
+  for (int64_t k = b; k < e; ++k) sum += x[k];
+  s_sum[threadIdx.x] = sum;
+  __syncthreads();
+  for (int o = 1; o < 1024; o <<= 1) {  // inclusive Hillis-Steele
+    const unsigned add = threadIdx.x >= o ? s_sum[threadIdx.x - o] : 0u;
+    __syncthreads();
+    s_sum[threadIdx.x] += add;
+    __syncthreads();
+  }
+  unsigned run = s_sum[threadIdx.x] - sum;
+  for (int64_t k = b; k < e; ++k) { const unsigned c = x[k]; x[k] = run; run += c; }
+}
+
+// stable scatter of one tile: an element goes to (start of its digit for this tile) + (elements of the tile with the same digit
+// before it).  Rounds of 1024 consecutive elements; inside a round the order is (warp, lane).
+__global__ void __launch_bounds__(kSortThreads)
+radix_scatter_kernel(const u64* __restrict__ w_in, const unsigned* __restrict__ i_in, int64_t m, int shift,
+                     const unsigned* __restrict__ offs, int ntiles, u64* __restrict__ w_out, unsigned* __restrict__ i_out) {
+  __shared__ unsigned short s_cnt[32][256];
+  __shared__ unsigned s_base[256], s_tot[256];
+  const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
+  const unsigned lt = (1u << lane) - 1u;
+  if (threadIdx.x < 256) s_base[threadIdx.x] = offs[(int64_t)threadIdx.x * ntiles + blockIdx.x];
+  const int64_t base = (int64_t)blockIdx.x * kSortTile;
+  for (int r = 0; r < kSortRounds; ++r) {
+    for (int k = threadIdx.x; k < 32 * 256 / 2; k += kSortThreads) reinterpret_cast<unsigned*>(&s_cnt[0][0])[k] = 0u;
+    __syncthreads();
+    const int64_t e = base + r * kSortThreads + threadIdx.x;
+    const bool valid = e < m;
+    const u64 key = valid ? w_in[e] : 0ull;
+    const unsigned idx = valid ? i_in[e] : 0u;
+    const unsigned d = (unsigned)(key >> shift) & 255u;
+    const unsigned peers = __match_any_sync(0xffffffffu, valid ? d : 256u);
+    const unsigned rank = __popc(peers & lt);
+    if (valid && rank == 0) s_cnt[warp][d] = (unsigned short)__popc(peers);
+    __syncthreads();
+    if (threadIdx.x < 256) {  // exclusive prefix over the warps, per digit
+      unsigned run = 0;
+      for (int q = 0; q < 32; ++q) { const unsigned c = s_cnt[q][threadIdx.x]; s_cnt[q][threadIdx.x] = (unsigned short)run; run += c; }
+      s_tot[threadIdx.x] = run;
+    }
+    __syncthreads();
+    if (valid) {
+      const int64_t pos = (int64_t)s_base[d] + s_cnt[warp][d] + rank;
+      w_out[pos] = key;
+      i_out[pos] = idx;
+    }
+    __syncthreads();
+    if (threadIdx.x < 256) s_base[threadIdx.x] += s_tot[threadIdx.x];
+  }
+}
+
+inline size_t align256(size_t x) { return (x + 255) & ~(size_t)255; }
+
 }  // namespace
 
+// bytes of work space dh_sort_externals needs for m elements
+size_t dh_sort_work_bytes(int64_t m) {
+  const int64_t ntiles = (m + kSortTile - 1) / kSortTile;
+  return 2 * align256((size_t)m * sizeof(u64)) + 2 * align256((size_t)m * sizeof(unsigned)) + align256((size_t)256 * ntiles * sizeof(unsigned)) + 256;
+}
+
+// keys_tmp [m][2], v_tmp, score_tmp (unsorted, may be NULL) -> keys_out, v_out, score_out sorted by (alpha, beta); `work`: device
+// buffer of dh_sort_work_bytes(m) bytes
 dh_status dh_sort_externals(detham_ctx* c, u64* keys_tmp, double* v_tmp, double* score_tmp, int64_t m, u64* keys_out, double* v_out,
-                            double* score_out) {
+                            double* score_out, void* work) {
   if (m >= (1ll << 32)) return DH_EINVAL;
   const int grid = c->sm_count * 8;
-  u64 *w0 = nullptr, *w1 = nullptr; unsigned *i0 = nullptr, *i1 = nullptr; void* tmp = nullptr;
-  auto cleanup = [&]() { cudaFree(w0); cudaFree(w1); cudaFree(i0); cudaFree(i1); cudaFree(tmp); };
-  auto body = [&]() -> dh_status {
-    DH_CUDA(c, cudaMalloc(&w0, m * sizeof(u64)));
-    DH_CUDA(c, cudaMalloc(&w1, m * sizeof(u64)));
-    DH_CUDA(c, cudaMalloc(&i0, m * sizeof(unsigned)));
-    DH_CUDA(c, cudaMalloc(&i1, m * sizeof(unsigned)));
-    size_t tmp_bytes = 0;
-    DH_CUDA(c, cub::DeviceRadixSort::SortPairs(nullptr, tmp_bytes, w0, w1, i0, i1, m, 0, 64, c->stream));
-    DH_CUDA(c, cudaMalloc(&tmp, tmp_bytes));
-    iota_kernel<<<grid, 256, 0, c->stream>>>(i0, m);
-    for (int word = 1; word >= 0; --word) {  // beta (low) word first, alpha (high) word last: order = (alpha, beta)
-      pick_word_kernel<<<grid, 256, 0, c->stream>>>(keys_tmp, i0, word, m, w0);
-      DH_CUDA(c, cudaGetLastError());
-      DH_CUDA(c, cub::DeviceRadixSort::SortPairs(tmp, tmp_bytes, w0, w1, i0, i1, m, 0, 64, c->stream));
-      unsigned* t = i0; i0 = i1; i1 = t;
-    }
-    gather_kernel<<<grid, 256, 0, c->stream>>>(keys_tmp, v_tmp, score_tmp, i0, m, keys_out, v_out, score_out);
+  const int ntiles = (int)((m + kSortTile - 1) / kSortTile);
+  char* p = static_cast<char*>(work);
+  u64* w0 = reinterpret_cast<u64*>(p); p += align256((size_t)m * sizeof(u64));
+  u64* w1 = reinterpret_cast<u64*>(p); p += align256((size_t)m * sizeof(u64));
+  unsigned* i0 = reinterpret_cast<unsigned*>(p); p += align256((size_t)m * sizeof(unsigned));
+  unsigned* i1 = reinterpret_cast<unsigned*>(p); p += align256((size_t)m * sizeof(unsigned));
+  unsigned* hist = reinterpret_cast<unsigned*>(p);
+  iota_kernel<<<grid, 256, 0, c->stream>>>(i0, m);
+  for (int word = 1; word >= 0; --word) {  // beta (low) word first, alpha (high) word last: order = (alpha, beta)
+    pick_word_kernel<<<grid, 256, 0, c->stream>>>(keys_tmp, i0, word, m, w0);
     DH_CUDA(c, cudaGetLastError());
-    DH_CUDA(c, cudaStreamSynchronize(c->stream));
-    return DH_OK;
-  };
-  dh_status st = body();
-  cleanup();
-  return st;
+    for (int shift = 0; shift < c->n; shift += 8) {  // bits at or above n_orb are zero in every key
+      radix_hist_kernel<<<ntiles, kSortThreads, 0, c->stream>>>(w0, m, shift, hist, ntiles);
+      radix_scan_kernel<<<1, 1024, 0, c->stream>>>(hist, (int64_t)256 * ntiles);
+      radix_scatter_kernel<<<ntiles, kSortThreads, 0, c->stream>>>(w0, i0, m, shift, hist, ntiles, w1, i1);
+      DH_CUDA(c, cudaGetLastError());
+      u64* tw = w0; w0 = w1; w1 = tw;
+      unsigned* ti = i0; i0 = i1; i1 = ti;
+    }
+  }
+  gather_kernel<<<grid, 256, 0, c->stream>>>(keys_tmp, v_tmp, score_tmp, i0, m, keys_out, v_out, score_out);
+  DH_CUDA(c, cudaGetLastError());
+  DH_CUDA(c, cudaStreamSynchronize(c->stream));
+  return DH_OK;
 }

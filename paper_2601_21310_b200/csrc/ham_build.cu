@@ -154,6 +154,70 @@ build_kernel(EnumParams P, const u64* __restrict__ dets, const double* __restric
   if (lane == 0 && gen) atomicAdd(counters + 1, gen);
 }
 
+// Sink of the complete-the-sum pass (row f2, the alternative of reading Q9): every excitation of the source that is a key of
+// P adds H_ai psi_i to v[position of a in P]; nothing is stored.
+struct CompleteSink {
+  static constexpr bool kLookupFirst = true;
+  static constexpr bool kLazySign = true;   // the phase of a double is worked out for the keys of P only
+  u64 da, db;
+  const u64* keys; const int* idx; u64 cap;
+  double* v;
+  double psi_i;
+  u64 generated;
+  int pre_tok;
+  __device__ __forceinline__ bool pre(u64 ka, u64 kb, u64 z) {
+    ++generated;
+    pre_tok = dh_shash_find(keys, idx, cap, ka, kb, z);
+    return pre_tok >= 0;
+  }
+  __device__ __forceinline__ void emit(bool act, u64 ka, u64 kb, u64 z, double H, int kind, int s, int i, int j, int a, int b) {
+    if (!act) return;
+    int tok = pre_tok;
+    if (kind != 0) {
+      ++generated;
+      tok = dh_shash_find(keys, idx, cap, ka, kb, z);
+      if (tok >= 0 && dh_double_parity(da, db, kind, s, i, j, a, b)) H = -H;
+    }
+    if (tok >= 0) atomicAdd(v + tok, H * psi_i);
+  }
+};
+
+// v[a] += sum_i H_ai psi_i over EVERY single and double excitation of every source with psi_i != 0 (tau = 0: the whole lists)
+__global__ void __launch_bounds__(kBuildWarps * 32, 2)
+complete_kernel(EnumParams P, const u64* __restrict__ dets, const double* __restrict__ psi, int64_t nd, const u64* __restrict__ hkeys,
+                const int* __restrict__ hidx, u64 hcap, double* __restrict__ v, u64* counters /* [0] next row [1] looked up */) {
+  extern __shared__ __align__(16) unsigned char smem[];
+  CtaTables T = dh_cta_stage(P, smem);
+  WarpScratch* wsp = reinterpret_cast<WarpScratch*>(smem + ((dh_cta_table_bytes(P.n) + 15) & ~(size_t)15));
+  const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
+  WarpScratch& ws = wsp[warp];
+  CompleteSink sink{0ull, 0ull, hkeys, hidx, hcap, v, 0.0, 0ull, -1};
+  for (;;) {
+    u64 row = 0;
+    if (lane == 0) row = atomicAdd(counters, 1ull);
+    row = __shfl_sync(0xffffffffu, row, 0);
+    if ((int64_t)row >= nd) break;
+    const double p = psi[row];
+    if (p == 0.0) continue;
+    const u64 da = dets[2 * row], db = dets[2 * row + 1];
+    dh_fill_occ(P, ws, da, db, lane);
+    const double e0 = dh_fill_U(P, T, ws, lane);
+    sink.da = da; sink.db = db; sink.psi_i = p;
+    u64 zsrc = 0;
+    if (lane == 0) {
+      zsrc = dh_zobrist(da, db, T.Z);
+      const int self = dh_shash_find(hkeys, hidx, hcap, da, db, zsrc);  // a key list may hold members of S: the sum runs over i = a too
+      if (self >= 0) atomicAdd(v + self, e0 * p);
+    }
+    zsrc = __shfl_sync(0xffffffffu, zsrc, 0);
+    dh_enumerate(P, T, ws, da, db, 0.0, zsrc, 0u, sink, lane);
+    __syncwarp();
+  }
+  u64 gen = sink.generated;
+  for (int o = 16; o > 0; o >>= 1) gen += __shfl_xor_sync(0xffffffffu, gen, o);
+  if (lane == 0 && gen) atomicAdd(counters + 1, gen);
+}
+
 // arena segments -> CSR positions, one warp per segment
 __global__ void __launch_bounds__(256)
 copy_segs_kernel(const Seg* __restrict__ segs, int64_t nseg, const int64_t* __restrict__ row_ptr, const int* __restrict__ acol,
@@ -471,8 +535,9 @@ dh_status dh_ham_build(detham_ctx* c, double eps) {
 // H_SP (row f3; "constructs the sparse Hamiltonian blocks H_VV and H_VP in CSR format", Eq. 8 PAPER.md:126,
 // Eq. S3): rows = determinants of S, columns = positions in the caller's sorted, deduplicated key list P
 // (detham_expand's output or any sorted subset of it), values H_{P_k, i} of the couplings the screen of Eq. 14 generates.
-dh_status dh_hsp_build(detham_ctx* c, const double* psi, double eps2, const u64* pkeys, int64_t m) {
-  dh_status st = m > 0 ? dh_validate_subspace(c, pkeys, m) : DH_OK;  // strictly ascending, electron counts, high bits clear
+// open-addressing index of the caller's sorted key list P (validated: strictly ascending, electron counts, high bits clear)
+static dh_status build_p_index(detham_ctx* c, const u64* pkeys, int64_t m) {
+  dh_status st = m > 0 ? dh_validate_subspace(c, pkeys, m) : DH_OK;
   if (st != DH_OK) return st;
   int64_t cap = 1024;
   while (cap < 2 * m) cap <<= 1;
@@ -489,8 +554,36 @@ dh_status dh_hsp_build(detham_ctx* c, const double* psi, double eps2, const u64*
     shash_insert_kernel<<<(unsigned)((m + 255) / 256), 256, 0, c->stream>>>(pkeys, m, c->phash_key, c->phash_idx, (u64)cap, nullptr, 0ull);
     DH_CUDA(c, cudaGetLastError());
   }
+  return DH_OK;
+}
+
+dh_status dh_hsp_build(detham_ctx* c, const double* psi, double eps2, const u64* pkeys, int64_t m) {
+  dh_status st = build_p_index(c, pkeys, m);
+  if (st != DH_OK) return st;
   c->sp_cols = m;
   CsrTarget T{&c->sp_row_ptr, &c->sp_col, &c->sp_val, &c->sp_nnz, &c->sp_csr_cap, &c->sp_row_cap,
               c->phash_key, c->phash_idx, c->phash_cap, nullptr, 0};
   return build_csr(c, T, psi, eps2);
+}
+
+// The complete-the-sum amplitude (row f2; Eq. 13: <x|H|Psi_V>, the full projection): v_out[k] = sum over ALL i in S of
+// H_{P_k, i} psi_i for the caller's sorted key list P.  One unscreened enumeration of every source, looked up in the index of P,
+// accumulated with RED.ADD.F64 (the order of the additions varies from run to run).
+dh_status dh_complete_sum(detham_ctx* c, const double* psi, const u64* pkeys, int64_t m, double* v_out) {
+  dh_status st = build_p_index(c, pkeys, m);
+  if (st != DH_OK) return st;
+  if (m == 0) return DH_OK;
+  const HbLists* L = nullptr;
+  st = dh_get_lists(c, 0, &L); if (st != DH_OK) return st;
+  EnumParams P = make_params(c, L);
+  const size_t smem = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + kBuildWarps * sizeof(WarpScratch);
+  st = set_smem(c, complete_kernel, smem); if (st != DH_OK) return st;
+  int64_t want = (c->nd + kBuildWarps - 1) / kBuildWarps;
+  const int grid = (int)(want < (int64_t)c->sm_count * 2 ? want : (int64_t)c->sm_count * 2);
+  DH_CUDA(c, cudaMemsetAsync(v_out, 0, (size_t)m * sizeof(double), c->stream));
+  DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 16 * sizeof(u64), c->stream));
+  complete_kernel<<<grid, kBuildWarps * 32, smem, c->stream>>>(P, c->dets, psi, c->nd, c->phash_key, c->phash_idx, (u64)c->phash_cap, v_out, c->dcount);
+  DH_CUDA(c, cudaGetLastError());
+  DH_CUDA(c, cudaStreamSynchronize(c->stream));
+  return DH_OK;
 }

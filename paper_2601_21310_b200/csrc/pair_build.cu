@@ -59,6 +59,16 @@ __global__ void pair_diag_kernel(int n, const double* __restrict__ J, const doub
   if (t < m) out[t] = dh_diag_from_scratch(n, J, JK, hd, e_core, dets[2 * t], dets[2 * t + 1]);
 }
 
+// position in [js, je) of the determinant with beta string `b` (the determinants of an alpha group are sorted by beta), or -1
+__device__ __forceinline__ int dh_find_beta(const u64* __restrict__ dets, int js, int je, u64 b) {
+  int lo = js, hi = je;
+  while (hi - lo > 1) {  // invariant: beta[lo] <= b if it is there at all
+    const int mid = (lo + hi) >> 1;
+    if (__ldg(dets + 2 * (int64_t)mid + 1) <= b) lo = mid; else hi = mid;
+  }
+  return (lo < je && __ldg(dets + 2 * (int64_t)lo + 1) == b) ? lo : -1;
+}
+
 // Single-excitation element i -> a in the spin string `ws` of the SOURCE (the other string is `wo`): the ordered sum of reading
 // Q7 - h_ia, then ((ia|qq) - (iq|qa)) over same-spin occupied q ascending, then (ia|qq) over other-spin occupied q ascending -
 // exactly dh_single_value_occ's additions, with the occupied orbitals taken from the words instead of a list.
@@ -193,13 +203,45 @@ pair_kernel(EnumParams P, const u64* __restrict__ dets, int64_t nd, double eps, 
         const u64 a_run = __shfl_sync(full, ar, r0);
         const int da = __popcll(a_run ^ ah);
         unsigned hm = __ballot_sync(full, hq < ngroups && da <= 4);
+        if (!hm) continue;
+        const unsigned hm4 = __ballot_sync(full, hq < ngroups && da == 4);
+        if (hm == hm4) {
+          // Every group of this chunk within reach is an alpha DOUBLE away (the common case: ~1500 such groups per run against ~50
+          // an alpha single away): only the determinant with the row's own beta string connects, so each lane looks that one
+          // string up in its group (sorted by beta) instead of the warp scanning the group.  At most one hit per lane and row;
+          // lane order = ascending group = ascending column.
+          for (int r = r0; r < r1; ++r) {
+            const u64 b_row = __shfl_sync(full, br, r);
+            int found = -1;
+            if ((hm4 >> lane) & 1u) found = dh_find_beta(dets, gs, ge, b_row);
+            const unsigned m = __ballot_sync(full, found >= 0);
+            if (m) {  // warp-uniform
+              if (found >= 0) { const int idx = qn + __popc(m & lt); qrow[idx] = (unsigned char)r; qcol[idx] = found; }
+              qn += __popc(m);
+              __syncwarp();
+              if (qn >= 32) flush(32);
+            }
+          }
+          continue;
+        }
         while (hm) {  // groups within reach of this run, ascending
           const int hh = __ffs(hm) - 1;
           hm &= hm - 1;
           const int dmax = 4 - __shfl_sync(full, da, hh);
           const int js = __shfl_sync(full, gs, hh), je = __shfl_sync(full, ge, hh);
           const int M = je - js, R = r1 - r0;
-          if (M <= 32 && R > 1) {
+          if (dmax == 0) {
+            // an alpha double in a chunk that also holds closer groups: kept in group order; the lanes are the rows of the run
+            int found = -1;
+            if (lane >= r0 && lane < r1) found = dh_find_beta(dets, js, je, br);
+            const unsigned m = __ballot_sync(full, found >= 0);
+            if (m) {  // warp-uniform
+              if (found >= 0) { const int idx = qn + __popc(m & lt); qrow[idx] = (unsigned char)lane; qcol[idx] = found; }
+              qn += __popc(m);
+              __syncwarp();
+              if (qn >= 32) flush(32);
+            }
+          } else if (M <= 32 && R > 1) {
             // a small group against a run of several rows: the lanes cover the R x M cross product (row-major, so that a
             // row's columns still come in ascending order), instead of M of 32 lanes once per row
             const u64 bj = lane < M ? __ldg(dets + 2 * (int64_t)(js + lane) + 1) : 0ull;

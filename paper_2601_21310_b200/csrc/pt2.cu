@@ -66,6 +66,27 @@ count_kernel(EnumParams P, const u64* __restrict__ dets, const double* __restric
   for (int t = threadIdx.x; t < kFine; t += blockDim.x) if (sh[t]) atomicAdd(hist + t, (u64)sh[t]);
 }
 
+// ---------------------------------------------------------------- sources ordered by key class
+// The sub-list a source reads for an occupied pair (i, j) in pass p is that of class p ^ class(source) ^ z(i) ^ z(j): the 32 warps
+// of a CTA, which take consecutive sources, share sub-lists (and so L1 lines) only if their sources are of one class.  perm =
+// the sources sorted by class (counting sort; the order inside a class does not matter).
+__global__ void class_count_kernel(const u64* __restrict__ dets, int64_t nd, unsigned pmask, unsigned* __restrict__ hist) {
+  __shared__ u64 Z[128];
+  for (int t = threadIdx.x; t < 128; t += blockDim.x) Z[t] = dh_zword(t);
+  __syncthreads();
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nd) return;
+  atomicAdd(hist + ((unsigned)dh_zobrist(dets[2 * t], dets[2 * t + 1], Z) & pmask), 1u);
+}
+__global__ void class_fill_kernel(const u64* __restrict__ dets, int64_t nd, unsigned pmask, unsigned* __restrict__ cursor, int* __restrict__ perm) {
+  __shared__ u64 Z[128];
+  for (int t = threadIdx.x; t < 128; t += blockDim.x) Z[t] = dh_zword(t);
+  __syncthreads();
+  const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
+  if (t >= nd) return;
+  perm[atomicAdd(cursor + ((unsigned)dh_zobrist(dets[2 * t], dets[2 * t + 1], Z) & pmask), 1u)] = (int)t;
+}
+
 // ---------------------------------------------------------------- members of S of this pass's class
 __global__ void member_insert_kernel(const u64* __restrict__ dets, int64_t nd, unsigned pmask, unsigned pass, Slot* table,
                                      u64 cap, int rshift, int* overflow) {
@@ -218,7 +239,8 @@ template <int kAccWarps, int kU, bool kExpand, bool kBinned = false>
 __global__ void __launch_bounds__(kAccWarps * 32, 1)
 pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* __restrict__ psi, int64_t nd, double eps2,
                       unsigned pass, Slot* table, u64 cap, u64* counters /* [0] next row [1] gen [2] contrib [3] max probe */,
-                      int* overflow, Slot* pool, unsigned* used, unsigned seg_cap, int bin_shift, int nbins) {
+                      int* overflow, Slot* pool, unsigned* used, unsigned seg_cap, int bin_shift, int nbins,
+                      const int* __restrict__ perm /* order in which the sources are taken, or NULL */) {
   extern __shared__ __align__(16) unsigned char smem[];
   CtaTables T = dh_cta_stage(P, smem);
   size_t off = (dh_cta_table_bytes(P.n) + 15) & ~(size_t)15;
@@ -249,6 +271,7 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
     int ovf = 0;
     if (lane == 0) ovf = *reinterpret_cast<volatile int*>(overflow);
     if (__shfl_sync(0xffffffffu, ovf, 0)) break;  // warp-uniform by construction
+    if (perm) row = (u64)perm[row];
     const double p = psi[row];
     if (p == 0.0) continue;  // reading Q6: a source with zero amplitude generates nothing
     const double tau = eps2 == 0.0 ? 0.0 : __ddiv_rn(eps2, fabs(p));
@@ -718,6 +741,31 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
     }
     pool_used = reinterpret_cast<unsigned*>(c->sflags);
   }
+  // sources in class order (see class_count_kernel); not for a single pass, where every source reads the same lists
+  const int* perm = nullptr;
+  if (pbits >= 1 && nd >= 4096 && nd < (1ll << 31)) {
+    const int np = 1 << pbits;
+    if (c->perm_cap < nd) {
+      if (c->perm) cudaFree(c->perm);
+      c->perm = nullptr; c->perm_cap = 0;
+      DH_CUDA(c, cudaMalloc(&c->perm, nd * sizeof(int)));
+      c->perm_cap = nd;
+    }
+    unsigned* chist = reinterpret_cast<unsigned*>(c->hist);  // [kFine] u64 = room for 2 * kFine counters
+    std::vector<unsigned> hh(np);
+    DH_CUDA(c, cudaMemsetAsync(chist, 0, np * sizeof(unsigned), c->stream));
+    class_count_kernel<<<(unsigned)((nd + 255) / 256), 256, 0, c->stream>>>(c->dets, nd, (unsigned)(np - 1), chist);
+    DH_CUDA(c, cudaGetLastError());
+    DH_CUDA(c, cudaMemcpyAsync(hh.data(), chist, np * sizeof(unsigned), cudaMemcpyDeviceToHost, c->stream));
+    DH_CUDA(c, cudaStreamSynchronize(c->stream));
+    unsigned run = 0;
+    for (int k = 0; k < np; ++k) { const unsigned t = hh[k]; hh[k] = run; run += t; }
+    DH_CUDA(c, cudaMemcpyAsync(chist, hh.data(), np * sizeof(unsigned), cudaMemcpyHostToDevice, c->stream));
+    class_fill_kernel<<<(unsigned)((nd + 255) / 256), 256, 0, c->stream>>>(c->dets, nd, (unsigned)(np - 1), chist, c->perm);
+    DH_CUDA(c, cudaGetLastError());
+    DH_CUDA(c, cudaStreamSynchronize(c->stream));  // hh is a host temporary
+    perm = c->perm;
+  }
   auto acc_kernel = ex ? pt2_accumulate_kernel<32, 1, true> : (binned ? pt2_accumulate_kernel<32, 1, false, true> : pt2_accumulate_kernel<32, 1, false>);
   const size_t smem = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + warps * (sizeof(WarpScratch) + sizeof(FlatScratch)) +
                       (binned ? max_bins * sizeof(unsigned) : 0);
@@ -758,7 +806,7 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
     }
     member_insert_kernel<<<(unsigned)((nd + 255) / 256), 256, 0, c->stream>>>(c->dets, nd, (unsigned)(nparts - 1), (unsigned)pass, table, (u64)pcap, bin_shift, overflow);
     acc_kernel<<<grid, warps * 32, smem, c->stream>>>(P, c->dets, psi, nd, eps2, (unsigned)pass, table, (u64)pcap, c->dcount, overflow,
-                                                      reinterpret_cast<Slot*>(c->pool), pool_used, seg_cap, bin_shift, nbins);
+                                                      reinterpret_cast<Slot*>(c->pool), pool_used, seg_cap, bin_shift, nbins, perm);
     if (binned) {
       DH_CUDA(c, cudaGetLastError());
       pt2_table_merge_kernel<<<c->sm_count * 2, 1024, 0, c->stream>>>(reinterpret_cast<const Slot*>(c->pool), pool_used, seg_cap, nbins, grid, table,
@@ -829,6 +877,9 @@ static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double ep
   const double max_table_gb = opt.max_table_gb > 0.0 ? opt.max_table_gb : 60.0;
   // streamed organisation (pt2_stream.cu)
   const bool stream_ok = !ex && opt.mode == 2 && nd >= (int64_t)c->sm_count * 16;
+
+  // a large work space left by expand / ediag would be counted against the table: give it back first
+  if (!ex && c->scratch_bytes > ((size_t)256 << 20)) { cudaFree(c->scratch); c->scratch = nullptr; c->scratch_bytes = 0; }
 
   // ---- plan: partition count and table capacity
   int pbits = 0;
@@ -988,37 +1039,46 @@ dh_status dh_pt2(detham_ctx* c, const double* psi, double e_s, double eps2, doub
   return pt2_run(c, psi, e_s, eps2, out, nullptr);
 }
 
+size_t dh_sort_work_bytes(int64_t m);  // expand.cu
 dh_status dh_sort_externals(detham_ctx* c, u64* keys_tmp, double* v_tmp, double* score_tmp, int64_t m, u64* keys_out, double* v_out,
-                            double* score_out);  // expand.cu
+                            double* score_out, void* work);  // expand.cu
 
 // Subspace expansion (row f2): the perturbative set P of Eq. 14 (Alg. 1 "Subspace Expansion"),
 // sorted ascending and deduplicated, with score_a = max_i |H_ai psi_i|, v_a = sum_i H_ai psi_i and H_aa.
 dh_status dh_expand(detham_ctx* c, const double* psi, double eps2, u64* keys_out, double* score_out, double* v_out, double* haa_out,
                     int64_t cap, int64_t* n_out) {
   u64* cursor = c->dcount + 16;
-  u64* keys_tmp = nullptr; double* v_tmp = nullptr; double* score_tmp = nullptr;
+  // unsorted keys / sums / scores and the sort's buffers live in the context's work space (kept for the next call; detham_trim
+  // or a later pt2 that needs the memory releases it)
   const int64_t tcap = cap > 0 ? cap : 1;
-  DH_CUDA(c, cudaMalloc(&keys_tmp, (size_t)tcap * 2 * sizeof(u64)));
-  auto cleanup = [&]() { cudaFree(keys_tmp); if (v_tmp) cudaFree(v_tmp); if (score_tmp) cudaFree(score_tmp); };
-  if (v_out && cudaMalloc(&v_tmp, (size_t)tcap * sizeof(double)) != cudaSuccess) { cleanup(); cudaGetLastError(); return DH_ENOMEM; }
-  if (score_out && cudaMalloc(&score_tmp, (size_t)tcap * sizeof(double)) != cudaSuccess) { cleanup(); cudaGetLastError(); return DH_ENOMEM; }
+  auto al = [](size_t x) { return (x + 255) & ~(size_t)255; };
+  const size_t kb = al((size_t)tcap * 2 * sizeof(u64)), vb = v_out ? al((size_t)tcap * sizeof(double)) : 0, sb = score_out ? al((size_t)tcap * sizeof(double)) : 0;
+  void* ws = nullptr;
+  {
+    dh_status st0 = dh_scratch(c, kb + vb + sb + dh_sort_work_bytes(tcap), &ws);
+    if (st0 != DH_OK) { cudaGetLastError(); return DH_ENOMEM; }
+  }
+  char* wp = static_cast<char*>(ws);
+  u64* keys_tmp = reinterpret_cast<u64*>(wp);
+  double* v_tmp = v_out ? reinterpret_cast<double*>(wp + kb) : nullptr;
+  double* score_tmp = score_out ? reinterpret_cast<double*>(wp + kb + vb) : nullptr;
+  void* sort_work = wp + kb + vb + sb;
   ExpandOut ex{keys_tmp, v_tmp, score_tmp, (u64)cap, cursor};
   double dummy = 0.0;
   dh_status st = pt2_run(c, psi, 0.0, eps2, &dummy, &ex);
-  if (st != DH_OK) { cleanup(); return st; }
+  if (st != DH_OK) return st;
   u64* hp = reinterpret_cast<u64*>(c->pinned);
   DH_CUDA(c, cudaMemcpyAsync(hp, cursor, sizeof(u64), cudaMemcpyDeviceToHost, c->stream));
   DH_CUDA(c, cudaStreamSynchronize(c->stream));
   const int64_t m = (int64_t)hp[0];
   *n_out = m;
   c->ctr.pt2_external = m;
-  if (m > cap) { cleanup(); return DH_EINVAL; }  // *n_out tells the caller how much room it takes
+  if (m > cap) return DH_EINVAL;  // *n_out tells the caller how much room it takes
   if (m > 0) {
-    st = dh_sort_externals(c, keys_tmp, v_tmp, score_tmp, m, keys_out, v_out, score_out);
+    st = dh_sort_externals(c, keys_tmp, v_tmp, score_tmp, m, keys_out, v_out, score_out, sort_work);
     if (st == DH_OK && haa_out) st = dh_diagonals(c, keys_out, m, haa_out);
   }
   if (st == DH_OK) DH_CUDA(c, cudaStreamSynchronize(c->stream));
-  cleanup();
   return st;
 }
 
@@ -1029,10 +1089,11 @@ dh_status dh_connections(detham_ctx* c, int64_t row, double tau, std::vector<u64
   const int64_t n = c->n, na = c->na, nb = c->nb;
   auto c2 = [](int64_t x) { return x * (x - 1) / 2; };
   int64_t cap = na * (n - na) + nb * (n - nb) + c2(na) * c2(n - na) + c2(nb) * c2(n - nb) + na * nb * (n - na) * (n - nb) + 32;
-  u64* dk = nullptr; double* dh = nullptr; int* dn = nullptr;
-  DH_CUDA(c, cudaMalloc(&dk, cap * 2 * sizeof(u64)));
-  DH_CUDA(c, cudaMalloc(&dh, cap * sizeof(double)));
-  DH_CUDA(c, cudaMalloc(&dn, sizeof(int)));
+  void* ws = nullptr;
+  st = dh_scratch(c, (size_t)cap * 24 + 256, &ws); if (st != DH_OK) return st;
+  u64* dk = static_cast<u64*>(ws);
+  double* dh = reinterpret_cast<double*>(dk + 2 * cap);
+  int* dn = reinterpret_cast<int*>(dh + cap);
   size_t smem = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + sizeof(WarpScratch);
   DH_CUDA(c, cudaFuncSetAttribute(connections_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   connections_kernel<<<1, 32, smem, c->stream>>>(P, c->dets, row, tau, dk, dh, dn);
@@ -1045,7 +1106,6 @@ dh_status dh_connections(detham_ctx* c, int64_t row, double tau, std::vector<u64
     DH_CUDA(c, cudaMemcpy(keys.data(), dk, 2 * (size_t)m * sizeof(u64), cudaMemcpyDeviceToHost));
     DH_CUDA(c, cudaMemcpy(h.data(), dh, (size_t)m * sizeof(double), cudaMemcpyDeviceToHost));
   }
-  cudaFree(dk); cudaFree(dh); cudaFree(dn);
   return DH_OK;
 }
 

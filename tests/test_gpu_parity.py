@@ -526,11 +526,29 @@ def test_ediag_lanczos(pkg, orc, name, n_dets, eps):
     ref = orc.ham_build(p["n"], p["h1"], p["eri"], p["e_core"], p["dets"], eps)
     lam = orc.ediag(*ref)
     e1, it1 = ctx.ediag(_psi(p))
-    e2, it2 = ctx.ediag(None)
     assert abs(e1 - lam) <= 1e-9 * abs(lam), (e1, lam, it1)
+    assert ctx.ediag_converged
+    e2, it2 = ctx.ediag(None)
     assert abs(e2 - lam) <= 1e-9 * abs(lam), (e2, lam, it2)
+    assert ctx.ediag_converged and ctx.ediag_residual <= 1e-12 * abs(lam)  # the stopping rule at the default tol
     e_var, _ = ctx.energy(_psi(p))
     assert e_var >= e1 - 1e-9 * abs(e1)  # Delta_opt >= 0
+    if len(p["psi"]) > 1:
+        # max_iter reached: flagged, and the Ritz value is still an upper bound of lambda_min
+        with pytest.warns(UserWarning, match="not converged"):
+            e3, it3 = ctx.ediag(None, tol=1e-14, max_iter=3)
+        assert it3 == 3 and not ctx.ediag_converged and e3 >= lam - 1e-12 * abs(lam)
+        # a start vector that is almost an excited eigenvector: the Ritz value stagnates there for a step or two, which the old
+        # rule on the movement of the value took for convergence; the residual-based rule goes on to lambda_min
+        import scipy.sparse as sp
+        import torch
+        rp, col, val = ref
+        nd = len(rp) - 1
+        if nd <= 2000:
+            w, U = np.linalg.eigh(sp.csr_matrix((val, col, rp), shape=(nd, nd)).toarray())
+            v0 = U[:, 3] + 1e-9 * U[:, 0]
+            e4, it4 = ctx.ediag(torch.from_numpy(np.ascontiguousarray(v0)).cuda(), tol=1e-12, max_iter=2000)
+            assert ctx.ediag_converged and abs(e4 - lam) <= 1e-9 * abs(lam), (e4, w[3], lam, it4)
     ctx.close()
 
 
@@ -554,6 +572,48 @@ def test_expand_perturbative_set(pkg, orc, name, n_dets, eps2, parts):
     g_pt2, g_ext, g_con = ctx.pt2(_psi(p), e_s, eps2)
     assert (g_ext, g_con) == (o["n_external"], o["n_contrib"]) and g_ext == len(okeys)
     assert abs(g_pt2 - o["pt2"]) <= PT2_TOL * abs(o["pt2"])
+    ctx.close()
+
+
+@pytest.mark.parametrize("name,n_dets,eps2,zero", [("tiny", None, 1e-3, False), ("tiny", 600, 1e-4, True), ("h2o", 600, 1e-5, True),
+                                                   ("tiny", 1, 0.0, False), ("tiny", 300, 0.0, False)])
+def test_complete_sum(pkg, orc, name, n_dets, eps2, zero):
+    """SURVEY.md 8(f) f2, the complete-the-sum variant: v_a = sum over ALL i of H_ai psi_i (Eq. 13's <x|H|Psi_V>) for
+    the keys expand selected, for a subset, for a list that holds a member of S, and for an empty list.  The sum is accumulated
+    atomically, so the bar is the PT2 one (relative 1e-9) with an absolute floor of 1e-12 of the largest amplitude."""
+    import torch
+    p = make_problem(name, n_dets=n_dets)
+    if n_dets == 1:
+        p["psi"] = np.array([1.0])
+    if zero:
+        p["psi"] = p["psi"].copy(); p["psi"][::5] = 0.0
+    ctx = _ctx(pkg, p)
+    psi = _psi(p)
+    keys, _, v_scr, _ = ctx.expand(psi, eps2)
+    okeys = keys.cpu().numpy().view(np.uint64)
+    args = (p["n"], p["h1"], p["eri"], p["e_core"], p["dets"], p["psi"])
+
+    def check(k_dev, k_host):
+        got = ctx.complete_sum(psi, k_dev).cpu().numpy()
+        ref = orc.complete_sum(*args, k_host)
+        # atomic accumulation: the error of an entry is a few ulp of sum_i |H_ai psi_i|, itself at most ~1e3 of the largest entry
+        assert np.allclose(got, ref, rtol=PT2_TOL, atol=1e-12 * (np.max(np.abs(ref)) if len(ref) else 0.0)), np.max(np.abs(got - ref))
+        return got
+
+    full = check(keys, okeys)
+    if eps2 == 0.0:
+        assert np.allclose(full, v_scr.cpu().numpy(), rtol=1e-10, atol=1e-14)      # nothing is below the screen
+    elif len(okeys) > 10:
+        assert np.max(np.abs(full - v_scr.cpu().numpy())) > 0.0                   # the two readings differ
+    if len(okeys) > 4:
+        check(keys[::3].contiguous(), okeys[::3])
+        mixed = np.vstack([okeys[::4], p["dets"][:1]])
+        mixed = np.unique(mixed, axis=0)
+        mixed = mixed[np.lexsort((mixed[:, 1], mixed[:, 0]))]
+        check(torch.from_numpy(mixed.view(np.int64)).cuda(), mixed)
+        with pytest.raises(pkg.DethamError):
+            ctx.complete_sum(psi, keys.flip(0).contiguous())
+    assert ctx.complete_sum(psi, keys[:0]).numel() == 0
     ctx.close()
 
 
