@@ -119,11 +119,15 @@ pair_kernel(EnumParams P, const u64* __restrict__ dets, int64_t nd, double eps, 
   __shared__ int s_qcol[kPairWarps][64];
   __shared__ unsigned char s_qrow[kPairWarps][64];
   __shared__ int s_cnt[kPairWarps][32];
+  __shared__ int s_tg[kPairWarps][64];            // pending look-ups: alpha group ...
+  __shared__ unsigned char s_tr[kPairWarps][64];  // ... and row of the block whose beta string is looked up in it
   const int lane = threadIdx.x & 31, warp = threadIdx.x >> 5;
   const unsigned full = 0xffffffffu, lt = (1u << lane) - 1u;
   int* qcol = s_qcol[warp];
   unsigned char* qrow = s_qrow[warp];
   int* cnt = s_cnt[warp];
+  int* tg = s_tg[warp];
+  unsigned char* tr = s_tr[warp];
   u64 evaluated = 0;
   int64_t wpos = 0, wend = 0;  // this warp's window in the arena (wpos < 0: arena exhausted, count only)
   for (;;) {
@@ -188,6 +192,29 @@ pair_kernel(EnumParams P, const u64* __restrict__ dets, int64_t nd, double eps, 
       qn = rest;
       __syncwarp();
     };
+    // run the first `take` pending look-ups, one per lane; the hits join the evaluation queue in look-up order
+    int tn = 0;
+    auto tflush = [&](int take) {
+      const bool mine = lane < take;
+      const int r = mine ? (int)tr[lane] : 0;
+      const int g = mine ? tg[lane] : 0;
+      const u64 b_row = __shfl_sync(full, br, r);
+      int found = -1;
+      if (mine) found = dh_find_beta(dets, __ldg(gstart + g), __ldg(gstart + g + 1), b_row);
+      const unsigned m = __ballot_sync(full, found >= 0);
+      if (m) {  // warp-uniform
+        if (found >= 0) { const int idx = qn + __popc(m & lt); qrow[idx] = (unsigned char)r; qcol[idx] = found; }
+        qn += __popc(m);
+        __syncwarp();
+        if (qn >= 32) flush(32);
+      }
+      const int rest = tn - take;
+      const int mr = lane < rest ? (int)tr[take + lane] : 0, mg = lane < rest ? tg[take + lane] : 0;
+      __syncwarp();
+      if (lane < rest) { tr[lane] = (unsigned char)mr; tg[lane] = mg; }
+      tn = rest;
+      __syncwarp();
+    };
     // runs of equal alpha among the 32 rows (S is sorted by alpha first)
     const u64 prev = __shfl_up_sync(full, ar, 1);
     const unsigned runs = __ballot_sync(full, have && (lane == 0 || ar != prev));
@@ -207,23 +234,38 @@ pair_kernel(EnumParams P, const u64* __restrict__ dets, int64_t nd, double eps, 
         const unsigned hm4 = __ballot_sync(full, hq < ngroups && da == 4);
         if (hm == hm4) {
           // Every group of this chunk within reach is an alpha DOUBLE away (the common case: ~1500 such groups per run against ~50
-          // an alpha single away): only the determinant with the row's own beta string connects, so each lane looks that one
-          // string up in its group (sorted by beta) instead of the warp scanning the group.  At most one hit per lane and row;
-          // lane order = ascending group = ascending column.
-          for (int r = r0; r < r1; ++r) {
-            const u64 b_row = __shfl_sync(full, br, r);
-            int found = -1;
-            if ((hm4 >> lane) & 1u) found = dh_find_beta(dets, gs, ge, b_row);
-            const unsigned m = __ballot_sync(full, found >= 0);
-            if (m) {  // warp-uniform
-              if (found >= 0) { const int idx = qn + __popc(m & lt); qrow[idx] = (unsigned char)r; qcol[idx] = found; }
-              qn += __popc(m);
+          // an alpha single away): only the determinant with the row's own beta string connects, so that one string is looked
+          // up in the group (sorted by beta) instead of the warp scanning the group.
+          if (r1 - r0 >= 8) {
+            // a long run: the lanes are its rows, one group at a time (ascending)
+            for (unsigned gm = hm4; gm;) {
+              const int hh = __ffs(gm) - 1;
+              gm &= gm - 1;
+              const int js = __shfl_sync(full, gs, hh), je = __shfl_sync(full, ge, hh);
+              int found = -1;
+              if (lane >= r0 && lane < r1) found = dh_find_beta(dets, js, je, br);
+              const unsigned m = __ballot_sync(full, found >= 0);
+              if (m) {  // warp-uniform
+                if (found >= 0) { const int idx = qn + __popc(m & lt); qrow[idx] = (unsigned char)lane; qcol[idx] = found; }
+                qn += __popc(m);
+                __syncwarp();
+                if (qn >= 32) flush(32);
+              }
+            }
+          } else {
+            // a short run: (row, group) look-ups are queued and run 32 at a time, whatever run and chunk they come from.  A row's
+            // look-ups enter the queue in ascending group order and leave it in that order, so its columns stay ascending.
+            const int k = __popc(hm4);
+            for (int r = r0; r < r1; ++r) {
+              if ((hm4 >> lane) & 1u) { const int idx = tn + __popc(hm4 & lt); tg[idx] = hq; tr[idx] = (unsigned char)r; }
+              tn += k;
               __syncwarp();
-              if (qn >= 32) flush(32);
+              if (tn >= 32) tflush(32);
             }
           }
           continue;
         }
+        while (tn > 0) tflush(tn < 32 ? tn : 32);  // the groups below are handled at once: what was found before them goes first
         while (hm) {  // groups within reach of this run, ascending
           const int hh = __ffs(hm) - 1;
           hm &= hm - 1;
@@ -282,6 +324,7 @@ pair_kernel(EnumParams P, const u64* __restrict__ dets, int64_t nd, double eps, 
         }
       }
     }
+    while (tn > 0) tflush(tn < 32 ? tn : 32);
     if (qn > 0) flush(qn);
     if (have) row_cnt[row] = cnt[lane];
     __syncwarp();

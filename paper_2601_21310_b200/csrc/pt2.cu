@@ -486,7 +486,7 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
 
 // Binned mode, second half: the records of bin b (one segment per accumulate CTA) are merged into the table region the bin
 // covers.  The CTAs take (bin, segment) chunks from one global cursor in bin-major order, so at any time all probes of the
-// GPU fall into one or two neighbouring regions (16 MB each at 4096 bins of a 60 GB table).  The probe itself is the
+// GPU fall into one or two neighbouring regions (32 MB each at the default 2048 regions of a 60 GB table).  The probe itself is the
 // unbinned kernel's; H_aa comes with the record.
 __global__ void __launch_bounds__(1024, 2)
 pt2_table_merge_kernel(const Slot* __restrict__ pool, const unsigned* __restrict__ used, unsigned seg_cap, int nbins, int nseg,
@@ -938,7 +938,7 @@ static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double ep
       slots = need < max_slots ? need : max_slots;
     }
   }
-  // The streamed organisation runs when asked for (mode 2).  Measured on B200 (profiles/r2_pt2_summary.md) it is slower than the
+  // The streamed organisation runs when asked for (mode 2).  Measured on B200 (profiles/r2_summary.md) it is slower than the
   // table organisation with binned passes on every configuration of BASELINE.json, so the planner does not choose it.
   const bool stream = stream_ok && !hist.empty() && opt.mode == 2;
   int64_t probe_parts = 0;
@@ -968,6 +968,13 @@ static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double ep
         while (pb2 < pbits && uniq_class(pb2) > load * (double)max_slots) ++pb2;
         pbits = pb2;
         int64_t need = (int64_t)(uniq_class(pbits) / load);
+        // beyond 32 GB the passes run binned and the probes stay in L2, where longer chains cost little while every slot less is 64
+        // bytes of DRAM traffic less per pass (fetch + scan): measured on Cr2-shaped, load 0.5 / 0.6 / 0.7 / 0.8: accumulate 5999 /
+        // 6004 / 6202 / 6527 ms, scan 810 / 679 / 591 / 534 ms
+        if (opt.table_load <= 0.0 && opt.table_regions >= 0 && need * (int64_t)sizeof(Slot) > (32ll << 30)) {
+          const int64_t denser = (int64_t)(uniq_class(pbits) / 0.6);
+          if (denser * (int64_t)sizeof(Slot) > (32ll << 30)) need = denser;
+        }
         slots = need < max_slots ? need : max_slots;
         if (slots < 1024) slots = 1024;
       }

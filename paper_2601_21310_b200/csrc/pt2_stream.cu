@@ -787,20 +787,19 @@ dh_status dh_pt2_stream(detham_ctx* c, const double* psi, double e_s, double eps
   GenParams G{};
   G.E = dh_make_params(c, L);
   const int grid = c->sm_count;
-  // generator launch shape: (warps per CTA, batches of 32 list entries in flight per warp)
+  // generator launch shape: 16 warps per CTA, two batches of 32 list entries in flight per warp (24 x 2, 32 x 2 and 32 x 1 were
+  // measured too: slower, the staging arrays of 32 warps spill)
   using GenKernel = void (*)(GenParams);
   struct GenVariant { int warps, u; GenKernel k; };
-  static const GenVariant variants[] = {{16, 2, pt2_gen_kernel<16, 2>}, {24, 2, pt2_gen_kernel<24, 2>}, {32, 2, pt2_gen_kernel<32, 2>}, {32, 1, pt2_gen_kernel<32, 1>}};
-  int vi = 0;
-  if (const char* e = getenv("DETHAM_GEN")) { int v = atoi(e); if (v >= 0 && v < 4) vi = v; }
+  static const GenVariant variants[] = {{16, 2, pt2_gen_kernel<16, 2>}};
+  const int vi = 0;
   const int kGenWarps = variants[vi].warps, kWalkU = variants[vi].u;
   if (nd < (int64_t)grid * kGenWarps || pbits > 8) return DH_EINVAL;  // the caller keeps small inputs on the table organisation
 
   // ---- region tables: kRing of them share the L2 budget; bins so that a region's distinct keys load it to <= `load`
   const double load = c->opt.stream_load > 0.0 ? c->opt.stream_load : 0.45;
   const double ring_mb = c->opt.stream_ring_mb > 0.0 ? c->opt.stream_ring_mb : 96.0;
-  int ring_n = kRing;
-  if (const char* e = getenv("DETHAM_RING")) { int v = atoi(e); if (v >= 2 && v <= 8) ring_n = v; }
+  const int ring_n = kRing;
   const double cap_max = ring_mb * 1048576.0 / (ring_n * sizeof(Slot));
   const double distinct = plan.est_distinct > 0.0 ? plan.est_distinct : plan.est_records;
   int nbins = c->opt.stream_bins > 0 ? c->opt.stream_bins : (int)ceil(distinct / (load * cap_max));
@@ -872,8 +871,6 @@ dh_status dh_pt2_stream(detham_ctx* c, const double* psi, double e_s, double eps
   M.ticket = c->dcount + 16;
   M.max_used = c->dcount + 20;
   M.ring_n = kRing; M.lag = kLag;
-  if (const char* e = getenv("DETHAM_RING")) { int v = atoi(e); if (v >= 2 && v <= 8) M.ring_n = v; }
-  if (const char* e = getenv("DETHAM_LAG")) { int v = atoi(e); if (v >= 1 && v < M.ring_n) M.lag = v; }
   int merge_occ = 0;
   DH_CUDA(c, cudaOccupancyMaxActiveBlocksPerMultiprocessor(&merge_occ, pt2_merge_kernel, kMergeWarps * 32, 0));
   if (merge_occ < 1) return DH_ECUDA;
@@ -899,8 +896,7 @@ dh_status dh_pt2_stream(detham_ctx* c, const double* psi, double e_s, double eps
     DH_CUDA(c, cudaDeviceGetAttribute(&max_persist, cudaDevAttrMaxPersistingL2CacheSize, c->device));
     DH_CUDA(c, cudaDeviceGetAttribute(&max_window, cudaDevAttrMaxAccessPolicyWindowSize, c->device));
     DH_CUDA(c, cudaDeviceGetLimit(&persist_before, cudaLimitPersistingL2CacheSize));
-    const char* e = getenv("DETHAM_PERSIST");
-    if (!(e && e[0] == '0') && max_persist > 0 && max_window > 0) {
+    if (max_persist > 0 && max_window > 0) {
       persist_bytes = std::min(ring_bytes, std::min((size_t)max_persist, (size_t)max_window));
       if (cudaDeviceSetLimit(cudaLimitPersistingL2CacheSize, persist_bytes) != cudaSuccess) { cudaGetLastError(); persist_bytes = 0; }
     }
