@@ -4,4 +4,4 @@ Argument marshalling only: every step of the hot path (heat-bath lists, excitati
 elements, CSR H_SS, SpMV/energy, PT2 hash accumulation and reduction) runs in the CUDA kernels of libdetham.so.
 PyTorch is used for device memory and streams.  There is no CPU fallback: a missing library or device raises.
 """
-from .binding import (Detham, DethamError, load_library, create, energy_static, ENERGY_STATIC_MAX_ROWS, SYMBOLS, STATUS)  # noqa: F401
+from .binding import (Detham, DethamError, load_library, use_checked_library, create, energy_static, ENERGY_STATIC_MAX_ROWS, SYMBOLS, STATUS)  # noqa: F401

@@ -44,6 +44,15 @@ class DethamError(RuntimeError):
         super().__init__(f"{self.status}: {text}" + (f" [{cuda}]" if cuda else ""))
 
 
+def use_checked_library():
+    """Make this process load libdetham_checked.so (the same sources built with -DDETHAM_CHECKED: device asserts at every
+    computed index).  Call before the first context is created."""
+    global _SO
+    if _lib is not None:
+        raise RuntimeError("the library is already loaded")
+    _SO = os.path.join(_PKG, "libdetham_checked.so")
+
+
 def load_library():
     """dlopen the in-tree libdetham.so (built by paper_2601_21310_b200.build).  Fails loudly if it is missing."""
     global _lib

@@ -81,6 +81,7 @@ struct detham_ctx {
   // ham_build by excitation degree (pair_build.cu): alpha groups of the sorted S, diagonals
   u64* pair_galpha = nullptr; int64_t pair_group_cap = 0;
   int* pair_gstart = nullptr; int64_t pair_gstart_cap = 0;
+  u64* pair_tsig = nullptr; int64_t pair_tsig_cap = 0;   // OR / AND of the beta strings of every 32 consecutive determinants
   double* pair_diag = nullptr; int64_t pair_diag_cap = 0;
   u64* pair_akey = nullptr; int64_t pair_akey_cap = 0;   // arena tags: row << 32 | place in the row (values in acol / aval)
   int* pair_bused = nullptr; int64_t pair_bused_cap = 0;  // entries used of every arena block
@@ -236,6 +237,16 @@ __device__ __forceinline__ int dh_shash_find(const u64* __restrict__ keys, const
 // membership pre-filter of the determinant store: false = certainly not in S (one 8-byte L2 load).  A blocked Bloom filter:
 // `nbits` (a power of two, >= 64 per determinant) bits seen as 64-bit words; a determinant sets two bits of the word its
 // partition word selects.  About 0.1-0.2 % of the non-members pass, so a warp of candidates rarely diverges into the index.
+// Bounds checks of the checked build (libdetham_checked.so, -DDETHAM_CHECKED; paper_2601_21310_b200/build.py): device asserts at
+// every computed index into a queue, arena, pool, table or output array.  compute-sanitizer is not available on the GPU pool
+// this was developed on; tests/test_gpu_parity.py::test_checked_build runs the small cases through this build instead.
+#ifdef DETHAM_CHECKED
+#include <assert.h>
+#define DH_CHECK(cond) assert(cond)
+#else
+#define DH_CHECK(cond) ((void)0)
+#endif
+
 __device__ __forceinline__ u64 dh_filter_mask(u64 z) { return (1ull << ((z >> 10) & 63ull)) | (1ull << ((z >> 16) & 63ull)); }
 __device__ __forceinline__ u64 dh_filter_word(u64 nbits, u64 z) { return z >> (__clzll((long long)nbits) + 7); }
 __device__ __forceinline__ bool dh_maybe_member(const unsigned* __restrict__ bits, u64 nbits, u64 z) {

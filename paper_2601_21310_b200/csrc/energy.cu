@@ -17,7 +17,7 @@ spmv_energy_kernel(const int64_t* __restrict__ row_ptr, const int* __restrict__ 
     const bool live = row < nd;
     const int64_t b = live ? row_ptr[row] : 0, e = live ? row_ptr[row + 1] : 0;
     double acc = 0.0;
-    for (int64_t k = b + sub; k < e; k += TPR) acc = fma(val[k], __ldg(psi + col[k]), acc);
+    for (int64_t k = b + sub; k < e; k += TPR) { DH_CHECK(col[k] >= 0 && col[k] < nd); acc = fma(val[k], __ldg(psi + col[k]), acc); }
 #pragma unroll
     for (int o = TPR / 2; o > 0; o >>= 1) acc += __shfl_xor_sync(0xffffffffu, acc, o, TPR);
     if (sub == 0 && live) {

@@ -95,6 +95,7 @@ radix_scatter_kernel(const u64* __restrict__ w_in, const unsigned* __restrict__ 
     __syncthreads();
     if (valid) {
       const int64_t pos = (int64_t)s_base[d] + s_cnt[warp][d] + rank;
+      DH_CHECK(pos >= 0 && pos < m);
       w_out[pos] = key;
       i_out[pos] = idx;
     }

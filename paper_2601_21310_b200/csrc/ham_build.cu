@@ -87,7 +87,7 @@ struct BuildSink {
       seg_start = wpos; seg_local = count;
     }
     if (wpos >= 0) {
-      if (has) { const int64_t pos = wpos + __popc(hit & ((1u << lane) - 1u)); acol[pos] = tok; aval[pos] = H; }
+      if (has) { const int64_t pos = wpos + __popc(hit & ((1u << lane) - 1u)); DH_CHECK(pos >= 0 && pos < arena_cap); acol[pos] = tok; aval[pos] = H; }
       wpos += h;
     }
     count += h;
@@ -227,6 +227,7 @@ copy_segs_kernel(const Seg* __restrict__ segs, int64_t nseg, const int64_t* __re
   for (int64_t s = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5); s < nseg; s += nw) {
     const Seg g = segs[s];
     const int64_t dst = row_ptr[g.row] + g.local;
+    DH_CHECK(dst + g.cnt <= row_ptr[g.row + 1]);
     for (int t = lane; t < g.cnt; t += 32) { col[dst + t] = acol[g.off + t]; val[dst + t] = aval[g.off + t]; }
   }
 }

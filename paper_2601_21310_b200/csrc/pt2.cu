@@ -157,7 +157,7 @@ __device__ __forceinline__ void probe_batch(ProbeCtx& pc, const u64 (&ka)[U], co
     u64 k0[U], k1[U], vb[U], hb[U];
 #pragma unroll
     for (int u = 0; u < U; ++u)
-      if ((pend >> u) & 1u) dh_ld256(pc.table + slot[u], k0[u], k1[u], vb[u], hb[u]);
+      if ((pend >> u) & 1u) { DH_CHECK(slot[u] < pc.cap); dh_ld256(pc.table + slot[u], k0[u], k1[u], vb[u], hb[u]); }
     unsigned cas = 0;
 #pragma unroll
     for (int u = 0; u < U; ++u)
@@ -208,7 +208,7 @@ __device__ __forceinline__ void probe_batch(ProbeCtx& pc, const u64 (&ka)[U], co
 // of the table that fits L2 (profiles/r1_microbench.md, block C: 36-41 G/s against 15 G/s for random probes).  The position
 // in the segment comes from a shared-memory counter: no global atomic.  A record that does not fit its segment is probed
 // directly, as in the unbinned kernel.
-struct BinCtx { Slot* pool; unsigned* cnt; unsigned seg_cap; int shift; };
+struct BinCtx { Slot* pool; unsigned* cnt; unsigned seg_cap; int shift; unsigned nbins; };
 
 template <int U>
 __device__ __forceinline__ unsigned bin_batch(ProbeCtx& pc, const BinCtx& bc, const u64 (&ka)[U], const u64 (&kb)[U],
@@ -217,6 +217,7 @@ __device__ __forceinline__ unsigned bin_batch(ProbeCtx& pc, const BinCtx& bc, co
   for (int u = 0; u < U; ++u)
     if ((pend >> u) & 1u) {
       const unsigned bin = (unsigned)(slot[u] >> bc.shift);
+      DH_CHECK(bin < bc.nbins);
       const unsigned p = atomicAdd(&bc.cnt[bin], 1u);
       if (p < bc.seg_cap) {
         dh_st256(bc.pool + ((u64)bin * gridDim.x + blockIdx.x) * bc.seg_cap + p, ka[u], kb[u], (u64)__double_as_longlong(cv[u]),
@@ -251,7 +252,7 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
     for (int t = threadIdx.x; t < nbins; t += blockDim.x) bcnt[t] = 0;
     __syncthreads();
   }
-  const BinCtx bc{pool, bcnt, seg_cap, bin_shift};
+  const BinCtx bc{pool, bcnt, seg_cap, bin_shift, (unsigned)nbins};
   const int warp = threadIdx.x >> 5, lane = threadIdx.x & 31;
   const unsigned lt = (1u << lane) - 1u;
   WarpScratch& ws = wsp[warp];
@@ -271,7 +272,7 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
     int ovf = 0;
     if (lane == 0) ovf = *reinterpret_cast<volatile int*>(overflow);
     if (__shfl_sync(0xffffffffu, ovf, 0)) break;  // warp-uniform by construction
-    if (perm) row = (u64)perm[row];
+    if (perm) { row = (u64)perm[row]; DH_CHECK((int64_t)row < nd); }
     const double p = psi[row];
     if (p == 0.0) continue;  // reading Q6: a source with zero amplitude generates nothing
     const double tau = eps2 == 0.0 ? 0.0 : __ddiv_rn(eps2, fabs(p));
@@ -301,6 +302,7 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
             code = ((unsigned)s << 12) | ((unsigned)i << 6) | (unsigned)a;
           }
           const unsigned m = __ballot_sync(0xffffffffu, in);
+          DH_CHECK(qn + __popc(m) <= 64);
           if (in) fs.sq[qn + __popc(m & lt)] = (unsigned short)code;
           qn += __popc(m);
           __syncwarp();
@@ -412,6 +414,7 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
             ent = (unsigned)k | ((unsigned)myq << 25);
           }
           const unsigned m = __ballot_sync(0xffffffffu, act);
+          DH_CHECK(dqn + __popc(m) <= 64);
           if (act) fs.dq[dqn + __popc(m & lt)] = ent;
           dqn += __popc(m);
           __syncwarp();
@@ -518,6 +521,7 @@ pt2_table_merge_kernel(const Slot* __restrict__ pool, const unsigned* __restrict
       int probes = 0;
       for (;;) {
         u64 k0, k1, vb, hb;
+        DH_CHECK(slot < cap);
         dh_ld256(table + slot, k0, k1, vb, hb);
         if (k0 == ka && k1 == kb) {
           if (vb != (u64)0x7ff8000000000001ull) { atomicAdd(&table[slot].v, cv); ++contrib; }
@@ -832,7 +836,8 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
     if (pilot) { pilot[0] = reinterpret_cast<double*>(hp + 8)[3]; pilot[1] = ms_accum + ms_scan; return DH_OK; }
     if (adapt && pass == 0 && nparts > 1) {
       const double u0 = reinterpret_cast<double*>(hp + 8)[3] + (double)nd / nparts;  // distinct externals + members of one class
-      const double need = (u0 + 8.0 * sqrt(u0) + 1024.0) / load;
+      // binned passes probe in L2, where a load of 0.6 costs nothing (see the planner's note in pt2_run)
+      const double need = (u0 + 8.0 * sqrt(u0) + 1024.0) / ((binned && c->opt.table_load <= 0.0) ? 0.6 : load);
       if (need < (double)cap) cap = (int64_t)need;
     }
   }

@@ -701,6 +701,7 @@ __global__ void __launch_bounds__(kMergeWarps * 32, kMergeCtasPerSm) pt2_merge_k
 #pragma unroll
             for (int k = 0; k < kMergeU; ++k)
               if ((pend >> k) & 1u) {
+                DH_CHECK(slot[k] < M.cap);
                 Slot* sp = tb + slot[k];
                 if ((old[k].a | old[k].b) == 0ull) {  // claimed: this thread also records H_aa
                   st_f64_hint(&sp->haa, __longlong_as_double((long long)hh[k]), keep);

@@ -723,6 +723,59 @@ def test_n2_sweep_large_points_masked(pkg, orc, n_dets):
     _masked_parity(pkg, orc, p, 400, 11, parts=(0, 16))
 
 
+_CHECKED_SCRIPT = r"""
+import sys, numpy as np, torch
+sys.path.insert(0, sys.argv[1])
+import paper_2601_21310_b200 as pkg
+pkg.use_checked_library()
+from synth_inputs import make_problem
+out = []
+for name, nd, eps, eps2 in (("tiny", None, 0.0, 0.0), ("tiny", 700, 1e-3, 1e-4), ("h2o", 5000, 1e-5, 1e-6), ("n2", 3000, 1e-5, 1e-6)):
+    p = make_problem(name, n_dets=nd)
+    ctx = pkg.create(p["n"], p["na"], p["nb"], p["h1"], p["eri"], p["e_core"])
+    ctx.set_subspace(p["dets"])
+    psi = torch.from_numpy(np.ascontiguousarray(p["psi"])).cuda()
+    nnz = []
+    for method in (1, 2):
+        ctx.build_config(method)
+        nnz.append(ctx.ham_build(eps))
+    assert nnz[0] == nnz[1]
+    e, _ = ctx.energy(psi)
+    ctx.residual(psi, e)
+    ctx.ediag(psi, tol=1e-8, max_iter=200)
+    res = []
+    for opts in ({}, {"n_parts": 8}, {"table_regions": 64}, {"table_regions": 256, "n_parts": 4}, {"mode": "stream"}):
+        if opts.get("mode") == "stream" and len(p["psi"]) < 2400:
+            continue
+        ctx.pt2_set_options(**opts)
+        res.append(ctx.pt2(psi, e - 1.0, eps2))
+    ctx.pt2_set_options()
+    assert all(r[1:] == res[0][1:] for r in res), res
+    keys, score, v, haa = ctx.expand(psi, max(eps2, 1e-5))
+    ctx.complete_sum(psi, keys[: min(len(keys), 20000)].contiguous())
+    ctx.hsp_build(psi, max(eps2, 1e-5), keys)
+    rp, col, val = ctx.csr()
+    pkg.energy_static(rp, col, val, psi)
+    torch.cuda.synchronize()
+    out.append((name, nnz[0], res[0][1], int(keys.shape[0])))
+    ctx.close()
+print("checked build ok", out)
+"""
+
+
+def test_checked_build(pkg):
+    """The small cases through libdetham_checked.so (-DDETHAM_CHECKED: a device assert at every computed index into a queue, arena,
+    pool, table or output array), in a process of its own: a failed assert kills the CUDA context.  Stands in for
+    compute-sanitizer, which the GPU pool this was developed on does not allow."""
+    import os
+    import subprocess
+    import sys
+    root = os.path.dirname(os.path.dirname(os.path.abspath(__file__)))
+    assert os.path.exists(os.path.join(root, "paper_2601_21310_b200", "libdetham_checked.so"))  # built by __graft_entry__.build()
+    r = subprocess.run([sys.executable, "-c", _CHECKED_SCRIPT, root], capture_output=True, text=True, timeout=1200)
+    assert r.returncode == 0 and "checked build ok" in r.stdout, (r.stdout[-2000:], r.stderr[-4000:])
+
+
 def test_against_stored_oracle_values(pkg):
     """The CUDA path against tests/golden/tiny_oracle.json (written by the oracle alone, tests/golden/make_golden.py)."""
     import json
