@@ -23,7 +23,7 @@ void free_all(detham_ctx* c) {
   f(c->h1); f(c->eri); f(c->J); f(c->JK); f(c->hd);
   for (auto& L : c->lists) { f(L.sub_off); f(L.val); f(L.ab); f(L.stat); }
   f(c->dets_owned); f(c->psi_owned); f(c->shash_key); f(c->shash_idx); f(c->sbits);
-  f(c->row_ptr); f(c->col); f(c->val); f(c->row_cnt); f(c->sp_row_ptr); f(c->sp_col); f(c->sp_val); f(c->phash_key); f(c->phash_idx); f(c->acol); f(c->aval); f(c->segs); f(c->table); f(c->pool); f(c->ring); f(c->sflags); f(c->pair_galpha); f(c->pair_gstart); f(c->pair_tsig); f(c->pair_diag); f(c->pair_akey); f(c->pair_bused); f(c->red); f(c->dcount); f(c->hist); f(c->scratch); f(c->perm);
+  f(c->row_ptr); f(c->col); f(c->val); f(c->row_cnt); f(c->sp_row_ptr); f(c->sp_col); f(c->sp_val); f(c->phash_key); f(c->phash_idx); f(c->acol); f(c->aval); f(c->segs); f(c->table); f(c->pool); f(c->ring); f(c->sflags); f(c->pair_galpha); f(c->pair_gstart); f(c->pair_diag); f(c->pair_akey); f(c->pair_bused); f(c->red); f(c->dcount); f(c->hist); f(c->scratch); f(c->perm);
   if (c->pinned) cudaFreeHost(c->pinned);
   for (auto& e : c->ev) if (e) cudaEventDestroy(e);
   for (auto& e : c->sev) cudaEventDestroy(e);

@@ -81,7 +81,6 @@ struct detham_ctx {
   // ham_build by excitation degree (pair_build.cu): alpha groups of the sorted S, diagonals
   u64* pair_galpha = nullptr; int64_t pair_group_cap = 0;
   int* pair_gstart = nullptr; int64_t pair_gstart_cap = 0;
-  u64* pair_tsig = nullptr; int64_t pair_tsig_cap = 0;   // OR / AND of the beta strings of every 32 consecutive determinants
   double* pair_diag = nullptr; int64_t pair_diag_cap = 0;
   u64* pair_akey = nullptr; int64_t pair_akey_cap = 0;   // arena tags: row << 32 | place in the row (values in acol / aval)
   int* pair_bused = nullptr; int64_t pair_bused_cap = 0;  // entries used of every arena block

@@ -53,19 +53,6 @@ __global__ void group_fill_kernel(const u64* __restrict__ dets, int64_t nd, cons
   if (t == nd) gstart[pre[nd]] = (int)nd;
 }
 
-// Signatures of the beta strings of every 32 consecutive determinants ("tile"): tsig[2t] = OR, tsig[2t + 1] = AND.  A string b is
-// at least popc(b & ~OR) + popc(AND & ~b) bits away from every string of the tile, which lets the scan of a large alpha group skip
-// most of its tiles (the group is sorted by beta, so neighbours share their high bits).
-__global__ void tile_sig_kernel(const u64* __restrict__ dets, int64_t nd, u64* __restrict__ tsig) {
-  const int lane = threadIdx.x & 31;
-  const int64_t tile = (int64_t)blockIdx.x * (blockDim.x >> 5) + (threadIdx.x >> 5);
-  if (tile * 32 >= nd) return;
-  const int64_t j = tile * 32 + lane;
-  u64 o = j < nd ? dets[2 * j + 1] : 0ull, a = j < nd ? dets[2 * j + 1] : ~0ull;
-  for (int k = 16; k > 0; k >>= 1) { o |= __shfl_xor_sync(0xffffffffu, o, k); a &= __shfl_xor_sync(0xffffffffu, a, k); }
-  if (lane == 0) { tsig[2 * tile] = o; tsig[2 * tile + 1] = a; }
-}
-
 __global__ void pair_diag_kernel(int n, const double* __restrict__ J, const double* __restrict__ JK, const double* __restrict__ hd,
                                  double e_core, const u64* __restrict__ dets, int64_t m, double* __restrict__ out) {
   const int64_t t = (int64_t)blockIdx.x * blockDim.x + threadIdx.x;
@@ -126,7 +113,7 @@ __device__ double pair_element(const EnumParams& P, u64 ar, u64 br, u64 xa, u64 
 // entry's place in its row is the row's running count plus its rank among the batch's kept entries of the same row.
 __global__ void __launch_bounds__(kPairWarps * 32)
 pair_kernel(EnumParams P, const u64* __restrict__ dets, int64_t nd, double eps, const u64* __restrict__ galpha,
-            const int* __restrict__ gstart, int ngroups, const u64* __restrict__ tsig, const double* __restrict__ diag, int* __restrict__ row_cnt,
+            const int* __restrict__ gstart, int ngroups, const double* __restrict__ diag, int* __restrict__ row_cnt,
             u64* __restrict__ akey, int* __restrict__ acol, double* __restrict__ aval, int* __restrict__ bused, int64_t arena_cap,
             u64* counters /* [0] next block of rows [1] elements evaluated [2] arena cursor */, int* overflow) {
   __shared__ int s_qcol[kPairWarps][64];
@@ -318,32 +305,6 @@ pair_kernel(EnumParams P, const u64* __restrict__ dets, int64_t nd, double eps, 
                 if (qn >= 32) flush(32);
               }
             }
-          } else if (M > 64) {
-            // a large group: 32 tiles of 32 columns at a time, a lane per tile; only the tiles whose signature leaves room for a
-            // string within dmax bits of the row's are read.  Per row the tiles, and the columns inside one, stay ascending.
-            const int t_end = (je - 1) >> 5;
-            for (int T0 = js >> 5; T0 <= t_end; T0 += 32) {
-              const int tt = T0 + lane;
-              const ulonglong2 sg = tt <= t_end ? __ldg(reinterpret_cast<const ulonglong2*>(tsig) + tt) : make_ulonglong2(0ull, ~0ull);
-              for (int r = r0; r < r1; ++r) {
-                const u64 b_row = __shfl_sync(full, br, r);
-                const bool ok = tt <= t_end && __popcll(b_row & ~sg.x) + __popcll(sg.y & ~b_row) <= dmax;
-                for (unsigned tm = __ballot_sync(full, ok); tm;) {
-                  const int j = ((T0 + __ffs(tm) - 1) << 5) + lane;
-                  tm &= tm - 1;
-                  const bool in = j >= js && j < je;
-                  const u64 bj = in ? __ldg(dets + 2 * (int64_t)j + 1) : 0ull;
-                  const bool hit = in && __popcll(b_row ^ bj) <= dmax;
-                  const unsigned m = __ballot_sync(full, hit);
-                  if (m) {  // warp-uniform
-                    if (hit) { const int idx = qn + __popc(m & lt); DH_CHECK(idx < 64); qrow[idx] = (unsigned char)r; qcol[idx] = j; }
-                    qn += __popc(m);
-                    __syncwarp();
-                    if (qn >= 32) flush(32);
-                  }
-                }
-              }
-            }
           } else {
             for (int c0 = js; c0 < je; c0 += 32) {
               const int j = c0 + lane;
@@ -430,9 +391,6 @@ dh_status dh_pair_build(detham_ctx* c, double eps) {
     DH_CUDA(c, cudaMalloc(&c->pair_gstart, (ng + 1) * sizeof(int)));
     c->pair_gstart_cap = ng + 1;
   }
-  const int64_t ntile = (nd + 31) / 32;
-  st = grow(reinterpret_cast<void**>(&c->pair_tsig), &c->pair_tsig_cap, 2 * ntile, sizeof(u64)); if (st != DH_OK) return st;
-  tile_sig_kernel<<<(unsigned)((ntile + 7) / 8), 256, 0, c->stream>>>(c->dets, nd, c->pair_tsig);
   group_fill_kernel<<<nb256, 256, 0, c->stream>>>(c->dets, nd, c->row_cnt, c->row_ptr, c->pair_galpha, c->pair_gstart);
   pair_diag_kernel<<<(unsigned)((nd + 127) / 128), 128, 0, c->stream>>>(c->n, c->J, c->JK, c->hd, c->e_core, c->dets, nd, c->pair_diag);
   DH_CUDA(c, cudaGetLastError());
@@ -464,7 +422,7 @@ dh_status dh_pair_build(detham_ctx* c, double eps) {
     st = grow(reinterpret_cast<void**>(&c->pair_bused), &c->pair_bused_cap, c->arena_cap / kArenaBlk + 1, sizeof(int)); if (st != DH_OK) return st;
     DH_CUDA(c, cudaMemsetAsync(c->dcount, 0, 16 * sizeof(u64), c->stream));
     if (attempt > 0) DH_TICK(c, 0);
-    pair_kernel<<<grid, kPairWarps * 32, 0, c->stream>>>(P, c->dets, nd, eps, c->pair_galpha, c->pair_gstart, (int)ng, c->pair_tsig, c->pair_diag, c->row_cnt,
+    pair_kernel<<<grid, kPairWarps * 32, 0, c->stream>>>(P, c->dets, nd, eps, c->pair_galpha, c->pair_gstart, (int)ng, c->pair_diag, c->row_cnt,
                                                         c->pair_akey, c->acol, c->aval, c->pair_bused, c->arena_cap, c->dcount, overflow);
     excl_scan_kernel<<<1, 1024, 0, c->stream>>>(c->row_cnt, nd, c->row_ptr);
     DH_CUDA(c, cudaGetLastError());

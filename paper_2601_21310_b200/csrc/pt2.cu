@@ -801,10 +801,12 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
     unsigned seg_cap = 0;
     int64_t pcap = cap;  // capacity this pass probes
     if (binned) {  // bins = contiguous table regions of 2^shift slots, at most max_bins of them; whole regions only
+      // the regions cover `cap` rounded UP to whole regions where the allocation allows it (rounding down would raise the load)
       bin_shift = 10;
-      while ((cap >> bin_shift) > max_bins) ++bin_shift;
-      nbins = (int)(cap >> bin_shift);
-      if (nbins < 1) { nbins = 1; bin_shift = 0; while ((2ll << bin_shift) <= cap) ++bin_shift; }
+      while (((cap + (1ll << bin_shift) - 1) >> bin_shift) > max_bins) ++bin_shift;
+      nbins = (int)((cap + (1ll << bin_shift) - 1) >> bin_shift);
+      if (((int64_t)nbins << bin_shift) > slots) nbins = (int)(slots >> bin_shift);
+      if (nbins < 1) { nbins = 1; bin_shift = 0; while ((2ll << bin_shift) <= slots) ++bin_shift; }
       pcap = (int64_t)nbins << bin_shift;
       seg_cap = (unsigned)(c->pool_bytes / ((int64_t)nbins * grid * (int64_t)sizeof(Slot)));
     }
@@ -821,7 +823,8 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
       pt2_compact_kernel<<<sgrid, 256, 0, c->stream>>>(table, (u64)cap, ex->keys, ex->v, ex->score, ex->cap, ex->cursor);
       DH_CUDA(c, cudaMemsetAsync(results + 4 * pass, 0, 4 * sizeof(double), c->stream));
     } else {
-      pt2_scan_kernel<<<sgrid, 256, 0, c->stream>>>(table, (u64)cap, e_s, c->n, c->J, c->JK, c->hd, c->e_core, small_den, part);
+      // binned passes may probe up to a whole region beyond `cap`: the scan covers what was probed
+      pt2_scan_kernel<<<sgrid, 256, 0, c->stream>>>(table, (u64)(pcap > cap ? pcap : cap), e_s, c->n, c->J, c->JK, c->hd, c->e_core, small_den, part);
       final_reduce4_kernel<<<1, 256, 0, c->stream>>>(part, sgrid, results + 4 * pass);
     }
     DH_CUDA(c, cudaGetLastError());
@@ -837,7 +840,7 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
     if (adapt && pass == 0 && nparts > 1) {
       const double u0 = reinterpret_cast<double*>(hp + 8)[3] + (double)nd / nparts;  // distinct externals + members of one class
       // binned passes probe in L2, where a load of 0.6 costs nothing (see the planner's note in pt2_run)
-      const double need = (u0 + 8.0 * sqrt(u0) + 1024.0) / ((binned && c->opt.table_load <= 0.0) ? 0.6 : load);
+      const double need = (u0 + 8.0 * sqrt(u0) + 1024.0) / ((binned && c->opt.table_load <= 0.0 && u0 > 1e7) ? 0.6 : load);
       if (need < (double)cap) cap = (int64_t)need;
     }
   }
