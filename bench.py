@@ -127,6 +127,21 @@ def run_reference(args, p):
             "e2e": {"value": value, "unit": UNIT, "h2d_bytes_per_step": 0, "d2h_bytes_per_step": 0}, "gpu_launches": 0}
 
 
+def max_over_ranks(value, dist=None, device="cuda"):
+    """The replicas' times are combined as the contract says: the maximum over the ranks (a collective only when N > 1)."""
+    if dist is None:
+        return value
+    import torch
+    t = torch.tensor([value], dtype=torch.float64, device=device)
+    dist.all_reduce(t, op=dist.ReduceOp.MAX)
+    return float(t.item())
+
+
+def aggregate_value(elements_per_rank, world, ms_per_step):
+    """Whole-job throughput of N replicas (weak scaling): every rank processes the same workload."""
+    return world * elements_per_rank / (ms_per_step * 1e-3)
+
+
 def workload_config(p):
     return {"workload": f"{p['name']}-shaped synthetic: n_orb={p['n']}, N_alpha+N_beta={p['na']}+{p['nb']}, |S|={len(p['psi'])}, "
                         f"eps={p['eps']:g}, eps2={p['eps2']:g}",
@@ -225,14 +240,10 @@ def main():
         phases.append(ctx.counters())
     barrier()
     clocks = sampler.stop()
-    total_ms = sum(step_ms)
-    if dist is not None:
-        t = torch.tensor([total_ms], dtype=torch.float64, device="cuda")
-        dist.all_reduce(t, op=dist.ReduceOp.MAX)
-        total_ms = float(t.item())
+    total_ms = max_over_ranks(sum(step_ms), dist)
     ms_per_step = total_ms / args.steps
     c = phases[-1]
-    value = world * elements / (ms_per_step * 1e-3)
+    value = aggregate_value(elements, world, ms_per_step)
 
     # ---- roofline of the dominant kernel (pt2_accumulate_kernel), algorithmic bytes per SURVEY.md 8(d)
     peak, peak_src = load_peaks()
@@ -267,7 +278,7 @@ def main():
             pass
 
     out = {"metric": METRIC, "value": value, "unit": UNIT, "n_gpus": world, "steps": args.steps, "warmup": args.warmup,
-           "ms_per_step": ms_per_step, "step_ms": [round(x, 3) for x in step_ms], "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
+           "ms_per_step": ms_per_step, "step_ms": [round(x, 3) for x in step_ms], "ms_per_step_median": statistics.median(step_ms), "higher_is_better": True, "scaling": "weak", "vs_baseline": None, "dtype": "f64",
            "data": "synthetic", "config": workload_config(p), "clocks": clocks, "roofline": roofline,
            "phases_ms": {k: mean(k) for k in ("ms_store", "ms_build_count", "ms_build_fill", "ms_energy", "ms_pt2_plan",
                                               "ms_pt2_accum", "ms_pt2_scan")},
@@ -335,11 +346,7 @@ def main():
             t1.record()
             torch.cuda.synchronize()
             e2e_ms.append(t0.elapsed_time(t1))
-        e2e_total = sum(e2e_ms) / len(e2e_ms)
-        if dist is not None:
-            t = torch.tensor([e2e_total], dtype=torch.float64, device="cuda")
-            dist.all_reduce(t, op=dist.ReduceOp.MAX)
-            e2e_total = float(t.item())
+        e2e_total = max_over_ranks(sum(e2e_ms) / len(e2e_ms), dist)
         out["e2e"] = {"value": world * elements / (e2e_total * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 24 * nd,
                       "d2h_bytes_per_step": 32, "ms_per_step": e2e_total}
 

@@ -83,3 +83,32 @@ def test_reference_arm_under_torchrun_two_ranks():
     assert d["impl"] == "reference" and d["n_gpus"] == 2 and d["value"] > 0 and d["unit"] == "elements/s"
     assert d["cpu_baseline"]["kind"] == "oracle" and d["e2e"]["h2d_bytes_per_step"] == 0
     assert d["config"]["workload"].startswith("tiny")
+
+
+_GLOO_SCRIPT = r"""
+import os, sys
+sys.path.insert(0, sys.argv[1])
+import torch.distributed as dist
+import bench
+dist.init_process_group("gloo")
+rank, world = dist.get_rank(), dist.get_world_size()
+ms = bench.max_over_ranks(100.0 + 50.0 * rank, dist, device="cpu")      # replica times 100 and 150 ms
+assert ms == 150.0, ms
+assert bench.aggregate_value(1000.0, world, ms) == 2 * 1000.0 / 0.150
+dist.barrier()
+if rank == 0:
+    print("gloo ok", world, ms)
+dist.destroy_process_group()
+"""
+
+
+def test_replica_aggregation_two_ranks_gloo():
+    """the path does not shard - `bench.py --gpus N` runs N replicas; the only cross-rank logic is the
+    barrier and the max-over-ranks time.  That logic on CPU with gloo, world_size 2."""
+    import subprocess
+    import sys
+    cmd = [sys.executable, "-m", "torch.distributed.run", "--nnodes=1", "--nproc-per-node", "2", "--master-addr", "127.0.0.1",
+           "--master-port", "29773", "--no-python", sys.executable, "-c", _GLOO_SCRIPT, ROOT]
+    out = subprocess.run(cmd, capture_output=True, text=True, timeout=600, cwd=ROOT)
+    assert out.returncode == 0, out.stderr[-2000:]
+    assert "gloo ok 2 150.0" in out.stdout
