@@ -287,11 +287,13 @@ def main():
                                           "pt2_binned", "pt2_stream_bins")},
            "results": {"E_S": e_s, "PT2": pt2}, "es_pt2_wall_ms": mean("ms_build_count") + mean("ms_build_fill") + t_energy + t_pt2,
            "stored_nnz_per_sec": c["nnz"] / ((mean("ms_build_count") + mean("ms_build_fill")) * 1e-3),
-           # kernels of libdetham.so per step: store 2 (validate, index insert), ham_build 5 (enumerate, row scan, segment copy,
-           # two row sorts), energy 2, pt2 3 (plan histogram, norm + reduce) + per key partition 4 (member insert, accumulate,
-           # scan, reduce), 5 with binned passes (+ merge), 3 streamed (generate, merge + reduce, reduce) + 4 when the planner
-           # probed one slice
-           "gpu_launches": 2 + 5 + 2 + 3 + {0: 4, 1: 5, 2: 3}[int(c["pt2_binned"])] * parts + (4 if c["pt2_probe_parts"] else 0)}
+           # kernels of libdetham.so per warm step, counted against the ncu launch list (profiles/r2_summary.md): store 2 (validate,
+           # index insert); ham_build 7 by pairs (group flag, 2 scans, group fill, diagonals, pair kernel, scatter) or 5 by the list
+           # walk (enumerate, row scan, segment copy, two row sorts); energy 2; pt2: plan histogram 1, per attempt norm + its
+           # reduction 2 and the class-order permutation 2 when there are several passes, the planner's probe of one key slice 4
+           # (member insert, accumulate, scan, reduce), and per key partition 4, 5 with binned passes (+ merge), 3 streamed
+           "gpu_launches": 2 + (7 if c.get("build_pairs") else 5) + 2 + 1 + (2 + (2 if parts > 1 else 0)) * (2 if c["pt2_probe_parts"] else 1)
+                           + (4 if c["pt2_probe_parts"] else 0) + {0: 4, 1: 5, 2: 3}[int(c["pt2_binned"])] * parts}
 
     # ---- the widened rows, timed on the same workload after the hot path: median of 3, CUDA events
     if args.widened and rank == 0:
@@ -337,7 +339,7 @@ def main():
         dh, ph = dets_pin.numpy().view(np.uint64), psi_pin.numpy()
         ctx.solve_host(dh, ph, p["eps"], p["eps2"])
         e2e_ms = []
-        for _ in range(2):
+        for _ in range(max(2, args.steps)):  # as many end-to-end steps as timed device steps
             flush.fill_(1)
             torch.cuda.synchronize()
             t0, t1 = torch.cuda.Event(enable_timing=True), torch.cuda.Event(enable_timing=True)
@@ -348,7 +350,7 @@ def main():
             e2e_ms.append(t0.elapsed_time(t1))
         e2e_total = max_over_ranks(sum(e2e_ms) / len(e2e_ms), dist)
         out["e2e"] = {"value": world * elements / (e2e_total * 1e-3), "unit": UNIT, "h2d_bytes_per_step": 24 * nd,
-                      "d2h_bytes_per_step": 32, "ms_per_step": e2e_total}
+                      "d2h_bytes_per_step": 32, "ms_per_step": e2e_total, "step_ms": [round(x, 3) for x in e2e_ms]}
 
     if rank == 0 and world == 1 and not args.no_cpu_baseline:
         s = oracle_sample(p, sample_size(p))

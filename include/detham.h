@@ -84,7 +84,8 @@ typedef struct {
                                1 = hash table in HBM; 2 = streamed (DH_EINVAL if |S| < 16 x SM count) */
   int32_t n_parts;          /* key partitions / passes, a power of two <= 1024 (streamed: <= 256); 0 = planned */
   int64_t table_slots;      /* table organisation: capacity in 32-byte slots; 0 = planned from free device memory */
-  double table_load;        /* table organisation: target load factor, 0 = 0.5 */
+  double table_load;        /* table organisation: target load factor; 0 = 0.5, and 0.6 for binned passes of large tables (their
+                               probes are L2 hits, a denser table is less DRAM traffic: measured) */
   double max_table_gb;      /* table organisation: the planner never sizes the table beyond this (random 32-byte accesses lose
                                4x of their rate past ~70 GB on a B200: TLB reach); 0 = 60 */
   double small_den;         /* externals with |E_S - H_aa| below this take H_aa from the key alone instead of the O(1) update from
@@ -94,7 +95,7 @@ typedef struct {
   int32_t table_regions;    /* table organisation, binned passes (contributions appended per table region, then merged region by
                                region so that the probes stay in L2): 0 = when the table exceeds 32 GB, with at most 2048 regions;
                                > 0 = always, with at most that many regions (64..8192); -1 = never */
-  double stream_ring_mb;    /* streamed: bytes of the three region tables together (they must stay in L2); 0 = 60 */
+  double stream_ring_mb;    /* streamed: bytes of the three region tables together (they must stay in L2); 0 = 96 */
   double stream_load;       /* streamed: target load factor of a region table; 0 = 0.45 */
   double stream_pool_frac;  /* head room of the record pool over the planned estimate (streamed: 0 = 1.15; binned passes: 0 = 1.2) */
   double stream_pool_gb;    /* streamed: budget of the record pool; 0 = 80 % of the free device memory */
