@@ -1024,18 +1024,22 @@ static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double ep
     int sp = 0;
     if (!auto_parts) { while ((1 << sp) < opt.n_parts) ++sp; }
     else while (sp < 8 && max_class(sp) * 1.25 * (double)sizeof(Slot) > budget) ++sp;
-    double dscale = 1.15;
+    double dscale = 1.15, boost = 1.0;
     for (int tries = 0; tries < 6; ++tries) {
       const double recs = max_class(sp);
       double distinct = pilot_distinct > 0.0 ? fmin(recs, dscale * pilot_distinct * ldexp(1.0, pilot_pp - sp)) : recs;
-      const StreamPlan plan{sp, recs, distinct};
+      const StreamPlan plan{sp, recs * boost, distinct};
       st = dh_pt2_stream(c, psi, e_s, eps2, plan, out);
       if (c->debug) fprintf(stderr, "[detham] pt2 streamed: %d passes, %.3g records and %.3g distinct keys per pass planned (pool budget %.1f GB) -> status %d\n", 1 << sp, recs, distinct, budget / 1e9, (int)st);
       if (st == DH_OK) { c->ctr.pt2_probe_parts = probe_parts; return st; }
       if (st != DH_ETABLEFULL) break;  // DH_EINVAL / DH_ENOMEM: not a case for this organisation
+      const bool can_grow = distinct < recs || opt.stream_pool_frac <= 0.0 || (auto_parts && sp < 8);
+      if (!can_grow) break;  // nothing left to change: the same attempt would fail the same way
       if (distinct < recs) dscale *= 2.0;   // a region table filled up: the slice probed was not representative
-      else if (auto_parts && sp < 8) ++sp;  // a pool segment filled up
-      else break;
+      // a pool segment filled up (the sources a CTA happens to take differ from run to run; with few sources per CTA one CTA can
+      // get well over its share): more head room, and more passes where the planner may choose them
+      if (opt.stream_pool_frac <= 0.0) boost *= 1.5;  // a configured head room is taken at its word
+      if (auto_parts && sp < 8) ++sp;
     }
     if (st != DH_ETABLEFULL && st != DH_EINVAL && st != DH_ENOMEM) return st;
     if (opt.mode == 2) return st;  // asked for explicitly: report instead of switching organisation
