@@ -60,6 +60,8 @@ def lib():
         L.orc_expand.argtypes = [C.c_int, dp, dp, C.c_double, up, C.c_int64, dp, C.c_double, up, dp, dp, dp, C.c_int64]
         L.orc_hsp_build.restype = C.c_void_p
         L.orc_hsp_build.argtypes = [C.c_int, dp, dp, C.c_double, up, C.c_int64, dp, C.c_double, up, C.c_int64]
+        L.orc_use_lists.restype = C.c_int
+        L.orc_use_lists.argtypes = [C.c_int]
         L.orc_complete_sum.restype = None
         L.orc_complete_sum.argtypes = [C.c_int, dp, dp, C.c_double, up, C.c_int64, dp, up, C.c_int64, dp]
         L.orc_num_threads.restype = C.c_int
@@ -183,6 +185,13 @@ def expand(n, h1, eri, e_core, dets, psi, eps2):
     if m:
         lib().orc_expand(n, _d(h1), _d(eri), e_core, _u(dets), dets.shape[0], _d(psi), eps2, _u(keys), _d(score), _d(v), _d(haa), m)
     return keys, score, v, haa
+
+
+def use_lists(on):
+    """Switch conn(D, tau) in connections / ham_build / pt2 between the plain definition (False, the default every parity test
+    uses) and the paper's CPU algorithm - per-pair lists sorted by magnitude, walked with the early exit - which
+    is only the second timed CPU baseline of bench.py.  Returns the previous setting."""
+    return bool(lib().orc_use_lists(1 if on else 0))
 
 
 def complete_sum(n, h1, eri, e_core, dets, psi, pkeys):

@@ -137,6 +137,103 @@ int64_t connections(const Integrals& I, Det d, double tau, std::vector<Conn>* ou
   return visited;
 }
 
+// ---------------------------------------------------------------------------------------------------------------------------
+// The paper's own CPU algorithm for the doubles: "for each pair of occupied spin-orbitals (i,j), the
+// corresponding pairs of virtual orbitals (a,b) are sorted in descending order of the integral magnitude ... the inner loop over
+// (a,b) terminates immediately once |<ij||ab>| < tau".  A second, faster statement of conn(D, tau), used ONLY as the timed CPU
+// baseline of bench.py (`cpu_lists`) and pinned against connections() above (P15: identical sets, identical values bit for bit).
+// Lists are over ALL orbital pairs (a,b) of the right spins; entries whose a or b is occupied in D are skipped during the walk.
+// Singles are evaluated exactly as above (reading Q5).  Nothing on the CUDA side shares this code.
+struct HbEntry { double v; int a, b; };
+struct HbTables {
+  int n = 0;
+  const double* key_h1 = nullptr; const double* key_eri = nullptr;
+  std::vector<std::vector<HbEntry>> ss;  // [j*(j-1)/2 + i], i < j: same spin, a < b, v = (ia|jb) - (ib|ja)
+  std::vector<std::vector<HbEntry>> os;  // [i*n + j]: i alpha, j beta, v = (ia|jb)
+};
+HbTables g_tab;
+
+void build_tables(const Integrals& I) {
+  const int n = I.n;
+  g_tab.n = n; g_tab.key_h1 = I.h1; g_tab.key_eri = I.eri;
+  g_tab.ss.assign((size_t)n * (n - 1) / 2, {});
+  g_tab.os.assign((size_t)n * n, {});
+  auto by_mag = [](const HbEntry& x, const HbEntry& y) {
+    const double ax = std::fabs(x.v), ay = std::fabs(y.v);
+    if (ax != ay) return ax > ay;
+    return x.a != y.a ? x.a < y.a : x.b < y.b;
+  };
+#pragma omp parallel for schedule(dynamic, 4)
+  for (int j = 1; j < n; ++j)
+    for (int i = 0; i < j; ++i) {
+      auto& L = g_tab.ss[(size_t)j * (j - 1) / 2 + i];
+      for (int a = 0; a < n; ++a) for (int b = a + 1; b < n; ++b) {
+        if (a == i || a == j || b == i || b == j) continue;
+        const double v = eri(I, i, a, j, b) - eri(I, i, b, j, a);
+        if (v != 0.0) L.push_back({v, a, b});
+      }
+      std::sort(L.begin(), L.end(), by_mag);
+    }
+#pragma omp parallel for schedule(dynamic, 4)
+  for (int i = 0; i < n; ++i)
+    for (int j = 0; j < n; ++j) {
+      auto& L = g_tab.os[(size_t)i * n + j];
+      for (int a = 0; a < n; ++a) for (int b = 0; b < n; ++b) {
+        if (a == i || b == j) continue;
+        const double v = eri(I, i, a, j, b);
+        if (v != 0.0) L.push_back({v, a, b});
+      }
+      std::sort(L.begin(), L.end(), by_mag);
+    }
+}
+
+int64_t connections_lists(const Integrals& I, Det d, double tau, std::vector<Conn>* out) {
+  if (g_tab.n != I.n || g_tab.key_h1 != I.h1 || g_tab.key_eri != I.eri) {
+#pragma omp critical(orc_tables)
+    if (g_tab.n != I.n || g_tab.key_h1 != I.h1 || g_tab.key_eri != I.eri) build_tables(I);
+  }
+  const int n = I.n;
+  int64_t visited = 0;
+  auto keep = [&](Det x, double v) {
+    ++visited;
+    if (v != 0.0 && std::fabs(v) >= tau && out) out->push_back({x, v});
+  };
+  for (int i = 0; i < n; ++i) for (int a = 0; a < n; ++a) {
+    if (occ(d.a, i) && !occ(d.a, a)) keep({(d.a ^ (1ull << i)) | (1ull << a), d.b}, single_value(I, d.a, d.b, i, a));
+    if (occ(d.b, i) && !occ(d.b, a)) keep({d.a, (d.b ^ (1ull << i)) | (1ull << a)}, single_value(I, d.b, d.a, i, a));
+  }
+  for (int s = 0; s < 2; ++s) {  // same-spin doubles of the alpha (s = 0) and of the beta (s = 1) string
+    const u64 w = s ? d.b : d.a;
+    for (int j = 1; j < n; ++j) if (occ(w, j))
+      for (int i = 0; i < j; ++i) if (occ(w, i))
+        for (const HbEntry& e : g_tab.ss[(size_t)j * (j - 1) / 2 + i]) {
+          if (std::fabs(e.v) < tau) break;  // the early exit
+          if (occ(w, e.a) || occ(w, e.b)) continue;
+          int ph = single_phase(w, i, e.a);
+          ph *= single_phase((w & ~(1ull << i)) | (1ull << e.a), j, e.b);
+          const u64 nw = (w ^ (1ull << i) ^ (1ull << j)) | (1ull << e.a) | (1ull << e.b);
+          keep(s ? Det{d.a, nw} : Det{nw, d.b}, e.v * ph);
+        }
+  }
+  for (int i = 0; i < n; ++i) if (occ(d.a, i))
+    for (int j = 0; j < n; ++j) if (occ(d.b, j))
+      for (const HbEntry& e : g_tab.os[(size_t)i * n + j]) {
+        if (std::fabs(e.v) < tau) break;
+        if (occ(d.a, e.a) || occ(d.b, e.b)) continue;
+        keep({(d.a ^ (1ull << i)) | (1ull << e.a), (d.b ^ (1ull << j)) | (1ull << e.b)},
+             e.v * (single_phase(d.a, i, e.a) * single_phase(d.b, j, e.b)));
+      }
+  if (out) std::sort(out->begin(), out->end(), [](const Conn& x, const Conn& y) { return x.d < y.d; });
+  return visited;
+}
+
+// which statement of conn(D, tau) orc_ham_build / orc_pt2 / orc_connections use: 0 = the plain definition (default: every parity
+// test), 1 = the lists with early exit (bench.py's second CPU baseline only)
+int g_use_lists = 0;
+inline int64_t conn_dispatch(const Integrals& I, Det d, double tau, std::vector<Conn>* out) {
+  return g_use_lists ? connections_lists(I, d, tau, out) : connections(I, d, tau, out);
+}
+
 // General Slater-Condon element <X|H|Y> found from the two bitstrings alone (used by the dense-matrix pins).
 double element(const Integrals& I, Det x, Det y) {
   int da = __builtin_popcountll(x.a ^ y.a) / 2, db = __builtin_popcountll(x.b ^ y.b) / 2;
@@ -192,7 +289,7 @@ int64_t orc_connections(int n, const double* h1, const double* eri_, double e_co
                         u64* keys_out, double* h_out, int64_t cap, int64_t* visited_out) {
   Integrals I{n, h1, eri_, e_core};
   std::vector<Conn> c;
-  int64_t vis = connections(I, {det[0], det[1]}, tau, &c);
+  int64_t vis = conn_dispatch(I, {det[0], det[1]}, tau, &c);
   if (visited_out) *visited_out = vis;
   for (int64_t k = 0; k < (int64_t)c.size() && k < cap; ++k) {
     keys_out[2 * k] = c[k].d.a; keys_out[2 * k + 1] = c[k].d.b; h_out[k] = c[k].h;
@@ -224,7 +321,7 @@ void* orc_ham_build(int n, const double* h1, const double* eri_, double e_core, 
   for (int64_t k = 0; k < n_do; ++k) {
     const int64_t i = row_list ? row_list[k] : k;
     std::vector<Conn> c;
-    connections(I, S[i], eps, &c);
+    conn_dispatch(I, S[i], eps, &c);
     auto& r = rows[i];
     r.push_back({(int32_t)i, diagonal(I, S[i])});
     for (const Conn& x : c) {
@@ -323,7 +420,7 @@ void orc_pt2(int n, const double* h1, const double* eri_, double e_core, const u
       if (psi[i] == 0.0) continue;  // reading Q6
       double tau = eps2 == 0.0 ? 0.0 : eps2 / std::fabs(psi[i]);
       std::vector<Conn> c;
-      connections(I, S[i], tau, &c);
+      conn_dispatch(I, S[i], tau, &c);
       for (const Conn& x : c) {
         if (std::binary_search(S, S + nd, x.d)) continue;  // P = C \ V
         int cls = (int)(zobrist(x.d) & (u64)(n_parts - 1));
@@ -464,6 +561,10 @@ void orc_complete_sum(int n, const double* h1, const double* eri_, double e_core
     v_out[a] = (double)v;
   }
 }
+
+// 0 = the plain definition (default), 1 = heat-bath lists with early exit in orc_connections, orc_ham_build and
+// orc_pt2.  Returns the previous setting.
+int orc_use_lists(int on) { const int was = g_use_lists; g_use_lists = on ? 1 : 0; return was; }
 
 int orc_num_threads(void) {
 #ifdef _OPENMP

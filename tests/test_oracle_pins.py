@@ -463,3 +463,35 @@ def test_golden_regression_values():
                 assert np.allclose(w, v, rtol=1e-11, atol=1e-15), (tag, k)
             else:
                 assert w == v, (tag, k, v, w)
+
+
+# ---------------------------------------------------------------- P15: the list-based statement of conn(D, tau) (bench.py's second CPU baseline)
+def test_p15_heat_bath_lists_with_early_exit_equal_the_plain_definition(orc):
+    """PAPER.md:223-227 (per-pair lists sorted by |<ij||ab>|, inner loop left at the first entry below tau) gives exactly
+    conn(D, tau) of the plain enumeration: the same keys and the same values bit for bit at every tau, hence the same CSR and the
+    same PT2.  The list statement visits fewer excitations (that is its point) except at tau = 0."""
+    from synth_inputs import make_problem
+    for name, nd in (("tiny", 300), ("h2o", 40)):
+        p = make_problem(name, n_dets=nd)
+        args = (p["n"], p["h1"], p["eri"], p["e_core"])
+        rows = list(range(0, len(p["dets"]), max(1, len(p["dets"]) // 12)))
+        for tau in (0.0, 1e-6, 1e-3, 5e-2, 0.7):
+            for r in rows:
+                assert not orc.use_lists(True)
+                try:
+                    k1, h1v, vis1 = orc.connections(*args, p["dets"][r], tau)
+                finally:
+                    assert orc.use_lists(False)
+                k0, h0v, vis0 = orc.connections(*args, p["dets"][r], tau)
+                assert np.array_equal(k1, k0) and np.array_equal(h1v, h0v), (name, r, tau)
+                assert vis1 <= vis0 and (tau == 0.0 or vis1 < vis0 or len(k0) == vis0)
+        ref = orc.ham_build(*args, p["dets"], 1e-4)
+        o0 = orc.pt2(*args, p["dets"], p["psi"], -3.0, 1e-5)
+        orc.use_lists(True)
+        try:
+            got = orc.ham_build(*args, p["dets"], 1e-4)
+            o1 = orc.pt2(*args, p["dets"], p["psi"], -3.0, 1e-5)
+        finally:
+            orc.use_lists(False)
+        assert all(np.array_equal(a, b) for a, b in zip(got, ref))
+        assert o1["pt2"] == o0["pt2"] and o1["n_external"] == o0["n_external"] and o1["n_contrib"] == o0["n_contrib"]
