@@ -133,7 +133,8 @@ dh_status detham_csr(detham_ctx* ctx, const int64_t** row_ptr, const int32_t** c
 dh_status detham_csr_copy(detham_ctx* ctx, int64_t* row_ptr, int32_t* col, double* val);
 
 /* energy (Eq. 11; the SpMV of Alg. 1 line 14): y = H_SS psi, E_S = psi^T y / psi^T psi.
- * psi: DEVICE fp64 [n_dets].  y_out: DEVICE fp64 [n_dets] or NULL.  e_out, norm2_out: HOST (norm2_out may be NULL). */
+ * psi: DEVICE fp64 [n_dets].  y_out: DEVICE fp64 [n_dets] or NULL.  e_out, norm2_out: HOST (norm2_out may be NULL).
+ * DH_EINVAL if psi^T psi is zero or not finite (y_out is written all the same). */
 dh_status detham_energy(detham_ctx* ctx, const double* psi, double* e_out, double* norm2_out, double* y_out);
 
 /* energy for callers that may not allocate (code under CUDA graph capture, serving loops, harnesses that forbid cudaMalloc):
@@ -188,7 +189,8 @@ dh_status detham_trim(detham_ctx* ctx);
 /* pt2 (Eq. 13 second term, screened per Eq. 14 / PAPER.md:227; readings Q6, Q9, Q10):
  * for every source i with psi_i != 0, tau_i = eps2 / |psi_i| (0 if eps2 == 0); for every single or double excitation a
  * of D_i with |H_ai| >= tau_i, H_ai != 0 and a not in S:  v_a += H_ai psi_i.
- * Result  dE = (1 / psi^T psi) sum_a v_a^2 / (e_s - H_aa).  psi: DEVICE fp64 [n_dets]; outputs HOST (counts may be NULL). */
+ * Result  dE = (1 / psi^T psi) sum_a v_a^2 / (e_s - H_aa).  psi: DEVICE fp64 [n_dets]; outputs HOST (counts may be NULL).
+ * DH_EINVAL if psi^T psi is zero or not finite. */
 dh_status detham_pt2(detham_ctx* ctx, const double* psi, double e_s, double eps2, double* pt2_out,
                      int64_t* n_external_out, int64_t* n_contrib_out);
 

@@ -141,6 +141,7 @@ dh_status dh_energy(detham_ctx* c, const double* psi, double* e_out, double* n2_
   DH_CUDA(c, cudaMemcpyAsync(h, c->red, 2 * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
   DH_CUDA(c, cudaStreamSynchronize(c->stream));
   c->ctr.ms_energy = dh_elapsed(c, 0, 1);
+  if (!(h[1] > 0.0) || !isfinite(h[1])) return DH_EINVAL;  // psi identically zero (or not finite): Eq. 11 has no value
   *e_out = h[0] / h[1];
   if (n2_out) *n2_out = h[1];
   return DH_OK;

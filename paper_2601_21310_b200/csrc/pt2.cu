@@ -4,6 +4,8 @@
 #include <stdio.h>
 #include <stdlib.h>
 
+#include <cmath>
+
 #include "pt2_common.cuh"
 
 EnumParams dh_make_params(detham_ctx* c, const HbLists* L);
@@ -873,6 +875,7 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
   DH_CUDA(c, cudaMemcpyAsync(res.data(), results, res.size() * sizeof(double), cudaMemcpyDeviceToHost, c->stream));
   DH_CUDA(c, cudaStreamSynchronize(c->stream));
   const double norm2 = res[4 * (size_t)nparts];
+  if (!(norm2 > 0.0) || !std::isfinite(norm2)) return DH_EINVAL;  // psi identically zero (or not finite): Eq. 13 has no value
   double sum = 0, sabs = 0, mden = INFINITY, cnt = 0;
   c->partials.assign(nparts, 0.0);
   for (int p = 0; p < nparts; ++p) {

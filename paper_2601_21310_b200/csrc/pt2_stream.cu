@@ -964,6 +964,7 @@ dh_status dh_pt2_stream(detham_ctx* c, const double* psi, double e_s, double eps
     ms_gen += a; ms_merge += b;
   }
   const double norm2 = res[4 * (size_t)nparts];
+  if (!(norm2 > 0.0) || !isfinite(norm2)) return DH_EINVAL;  // psi identically zero (or not finite): Eq. 13 has no value
   double sum = 0, sabs = 0, mden = INFINITY, cnt = 0;
   c->partials.assign(nparts, 0.0);
   for (int p = 0; p < nparts; ++p) {

@@ -324,11 +324,26 @@ def test_invalid_subspaces_are_errors(pkg):
     with pytest.raises(pkg.DethamError) as e:
         ctx.set_subspace(hi)
     assert e.value.status == "DH_EPOPCOUNT"
+    with pytest.raises(pkg.DethamError) as e:
+        ctx.set_subspace(d[:0].copy())                      # the empty subspace is an argument error, not a crash
+    assert e.value.status == "DH_EINVAL"
     with pytest.raises(pkg.DethamError):
         ctx.ham_build(-1.0)
     ctx.set_subspace(d)
     with pytest.raises(pkg.DethamError):
         ctx.ham_build(float("nan"))
+    import torch
+    ctx.ham_build(0.0)
+    zero = torch.zeros(len(d), dtype=torch.float64, device="cuda")
+    with pytest.raises(pkg.DethamError) as e:                # psi identically zero: Eq. 11 / Eq. 13 have no value
+        ctx.energy(zero)
+    assert e.value.status == "DH_EINVAL"
+    with pytest.raises(pkg.DethamError) as e:
+        ctx.pt2(zero, -1.0, 0.0)
+    assert e.value.status == "DH_EINVAL"
+    one = zero.clone(); one[3] = 2.0                        # a single non-zero amplitude is fine
+    e_one, n2 = ctx.energy(one)
+    assert n2 == 4.0 and np.isfinite(e_one) and np.isfinite(ctx.pt2(one, e_one, 0.0)[0])
     ctx.close()
 
 
