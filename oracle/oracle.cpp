@@ -13,7 +13,10 @@
 //   * connected set, Eq. 1: every single and double excitation D' of D with H_{D'D} != 0.
 //   * heat-bath screening, Eq. 14 and the tau rule: the sorted lists + early exit of the
 //     paper reach exactly { D' : |H_{D'D}| >= tau }, so the oracle is that definition: enumerate every
-//     excitation, evaluate it, filter by magnitude.  No sorted lists, no early exit here.
+//     excitation, evaluate it, filter by magnitude.  No sorted lists, no early exit in that statement.  A second statement
+//     that does follow the paper's lists + early exit (connections_lists, off by default, switched on by orc_use_lists) exists
+//     only so that bench.py can time the paper's own CPU algorithm beside the plain one; it is pinned bit for bit against the
+//     plain statement (P15) and no parity test runs with it.
 //   * H_VV in CSR, E_var Eq. 11, PT2 external term Eq. 13.
 //
 // Parity pins (tests/test_oracle_pins.py): P1 explicit second-quantised operator application, P2 dense FCI
