@@ -363,8 +363,8 @@ def main():
         s = oracle_sample(p, sample_size(p))
         out["cpu_baseline"] = {"value": s["elements"] / s["seconds"], "unit": UNIT, "cores": s["threads"], "kind": "oracle",
                                "sample": f"brute-force oracle (no heat-bath lists, no early exit: it visits every orbital-valid "
-                                         f"excitation, so the GPU/CPU ratio overstates the gain over the paper's list-based CPU "
-                                         f"path): {s['sources']} of {nd} sources (ham_build rows + energy + pt2 with psi masked to them) "
+                                         f"excitation; cpu_baseline_lists times the paper's list-based conn on the same sample): "
+                                         f"{s['sources']} of {nd} sources (ham_build rows + energy + pt2 with psi masked to them) "
                                          f"on the full S and integrals, {s['seconds']:.1f} s; host has {os.cpu_count()} cpus"}
         # beside it, the same sample through the paper's own CPU algorithm (sorted per-pair lists, early exit): a fairer picture of
         # what a CPU does with this path than the plain definition, which visits every orbital-valid excitation
