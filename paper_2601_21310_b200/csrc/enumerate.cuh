@@ -67,8 +67,10 @@ __device__ __forceinline__ double dh_fill_U(const EnumParams& P, const CtaTables
   const int n = P.n;
   for (int p = lane; p < n; p += 32) {
     double ua = T.hd[p], ub = T.hd[p];
-    for (int k = 0; k < P.na; ++k) { int q = ws.occ[0][k]; ua += T.JK[p * n + q]; ub += T.J[p * n + q]; }
-    for (int k = 0; k < P.nb; ++k) { int q = ws.occ[1][k]; ua += T.J[p * n + q]; ub += T.JK[p * n + q]; }
+    // J and J-K are symmetric (bit for bit: both triangles come from the same packed integral), so row q is read at column p:
+    // the lanes (p = lane) then touch consecutive words instead of words n apart (a 16-way bank conflict at n = 56)
+    for (int k = 0; k < P.na; ++k) { int q = ws.occ[0][k]; ua += T.JK[q * n + p]; ub += T.J[q * n + p]; }
+    for (int k = 0; k < P.nb; ++k) { int q = ws.occ[1][k]; ua += T.J[q * n + p]; ub += T.JK[q * n + p]; }
     ws.U[0][p] = ua;
     ws.U[1][p] = ub;
   }
