@@ -37,9 +37,26 @@ struct WarpScratch {
 
 __host__ __device__ inline size_t dh_cta_table_bytes(int n) { return (size_t)(2 * n * n + n) * sizeof(double) + 128 * sizeof(u64); }
 
+// kStageJK = false (the pt2 accumulate kernel): J and J-K stay in global memory and are read through L1 - per source they are
+// touched by dh_fill_U (the rows of the occupied orbitals: the same ~20 KB for most sources) and by the few singles - which leaves
+// 50 KB more of the SM's L1 / shared-memory array to the L1 that serves the heat-bath lists; only h_pp and the Zobrist words are
+// staged (dh_cta_light_bytes).
+__host__ __device__ inline size_t dh_cta_light_bytes(int n) { return (size_t)n * sizeof(double) + 128 * sizeof(u64); }
+
+template <bool kStageJK = true>
 __device__ __forceinline__ CtaTables dh_cta_stage(const EnumParams& P, unsigned char* smem) {
   CtaTables T;
   const int n = P.n;
+  if (!kStageJK) {
+    T.J = const_cast<double*>(P.J);
+    T.JK = const_cast<double*>(P.JK);
+    T.hd = reinterpret_cast<double*>(smem);
+    T.Z = reinterpret_cast<u64*>(T.hd + n);
+    for (int t = threadIdx.x; t < n; t += blockDim.x) T.hd[t] = P.hd[t];
+    for (int t = threadIdx.x; t < 128; t += blockDim.x) T.Z[t] = dh_zword(t);
+    __syncthreads();
+    return T;
+  }
   T.J = reinterpret_cast<double*>(smem);
   T.JK = T.J + n * n;
   T.hd = T.JK + n * n;

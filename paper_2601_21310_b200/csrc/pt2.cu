@@ -245,8 +245,8 @@ pt2_accumulate_kernel(EnumParams P, const u64* __restrict__ dets, const double* 
                       int* overflow, Slot* pool, unsigned* used, unsigned seg_cap, int bin_shift, int nbins,
                       const int* __restrict__ perm /* order in which the sources are taken, or NULL */) {
   extern __shared__ __align__(16) unsigned char smem[];
-  CtaTables T = dh_cta_stage(P, smem);
-  size_t off = (dh_cta_table_bytes(P.n) + 15) & ~(size_t)15;
+  CtaTables T = dh_cta_stage<false>(P, smem);
+  size_t off = (dh_cta_light_bytes(P.n) + 15) & ~(size_t)15;
   WarpScratch* wsp = reinterpret_cast<WarpScratch*>(smem + off);
   FlatScratch* fsp = reinterpret_cast<FlatScratch*>(smem + off + kAccWarps * sizeof(WarpScratch));
   unsigned* bcnt = reinterpret_cast<unsigned*>(fsp + kAccWarps);  // [nbins] records this CTA appended per bin (binned mode)
@@ -796,7 +796,7 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
     perm = c->perm;
   }
   auto acc_kernel = ex ? pt2_accumulate_kernel<32, 1, true> : (binned ? pt2_accumulate_kernel<32, 1, false, true> : pt2_accumulate_kernel<32, 1, false>);
-  const size_t smem = ((dh_cta_table_bytes(c->n) + 15) & ~(size_t)15) + warps * (sizeof(WarpScratch) + sizeof(FlatScratch)) +
+  const size_t smem = ((dh_cta_light_bytes(c->n) + 15) & ~(size_t)15) + warps * (sizeof(WarpScratch) + sizeof(FlatScratch)) +
                       (binned ? max_bins * sizeof(unsigned) : 0);
   DH_CUDA(c, cudaFuncSetAttribute(acc_kernel, cudaFuncAttributeMaxDynamicSharedMemorySize, (int)smem));
   const double small_den = c->opt.small_den == 0.0 ? 1e-3 : (c->opt.small_den < 0.0 ? 0.0 : c->opt.small_den);
