@@ -725,7 +725,8 @@ struct ExpandOut { u64* keys; double* v; double* score; u64 cap; u64* cursor; };
 // binned: the accumulate kernel appends records to per-region segments (bin_batch), pt2_table_merge_kernel probes them region
 // by region.
 static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, double eps2, int pbits, int64_t slots, bool adapt,
-                             double load, double* out, double* pilot = nullptr, const ExpandOut* ex = nullptr, double est_pass = 0.0) {
+                             double load, double* out, double* pilot = nullptr, const ExpandOut* ex = nullptr, double est_pass = 0.0,
+                             bool force_binned = false) {
   const int64_t nd = c->nd;
   dh_status st = ensure_table(c, slots); if (st != DH_OK) return st;
   Slot* table = reinterpret_cast<Slot*>(c->table);
@@ -743,7 +744,7 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
   // at most (the region size is a power of two of slots; 2048 was the best of a sweep on Cr2-shaped).
   const int max_bins = c->opt.table_regions > 0 ? c->opt.table_regions : 2048;
   bool binned = !ex && !pilot && est_pass > 0.0 && grid == c->sm_count && c->opt.table_regions >= 0 &&
-                (c->opt.table_regions > 0 || slots * (int64_t)sizeof(Slot) > (32ll << 30));
+                (c->opt.table_regions > 0 || force_binned || slots * (int64_t)sizeof(Slot) > (32ll << 30));
   unsigned* pool_used = nullptr;
   if (binned) {
     // the pool holds the records of one pass: 20 % head room over the estimate (an upper bound already) plus 64 records per
@@ -1048,14 +1049,37 @@ static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double ep
     if (opt.mode == 2) return st;  // asked for explicitly: report instead of switching organisation
     if (c->pool) { cudaFree(c->pool); c->pool = nullptr; c->pool_bytes = 0; }  // make room for the table
   }
+  // A plan whose table is beyond 32 GB runs binned passes if the record pool of a pass fits beside the table.  Where it does not
+  // (many contributions per external: the large N2-shaped sweep points, 9 per external, 4 passes of 6e9 records), more passes of
+  // fewer records do, with a smaller table each: measured 20.5-21 G contributions/s binned against 18-19 G/s direct.
+  bool force_binned = false;
+  if (auto_parts && auto_slots && !ex && !hist.empty() && pilot_distinct > 0.0 && opt.table_regions == 0 &&
+      slots * (int64_t)sizeof(Slot) > (32ll << 30)) {
+    size_t free_b = 0, total_b = 0;
+    DH_CUDA(c, cudaMemGetInfo(&free_b, &total_b));
+    const double avail = 0.9 * ((double)free_b + (double)c->table_slots * sizeof(Slot) + (double)c->pool_bytes);
+    auto uniq = [&](int pb) { const double u = pilot_distinct * ldexp(1.0, pilot_pp - pb); return 1.2 * u + 8.0 * sqrt(u) + 4096.0; };
+    auto need_bytes = [&](int pb, double ld) { return (max_class(pb) * 1.2 + 64.0 * 2048 * c->sm_count + uniq(pb) / ld) * (double)sizeof(Slot); };
+    if (need_bytes(pbits, 0.6) > avail) {
+      for (int pb = pbits + 1; pb <= pbits + 3 && pb <= DH_MAX_PBITS; ++pb)
+        if (need_bytes(pb, 0.6) <= avail) {
+          pbits = pb;
+          slots = (int64_t)(uniq(pb) / 0.6);
+          if (slots < 1024) slots = 1024;
+          force_binned = true;
+          break;
+        }
+    }
+  }
   for (;;) {
     if (ex) DH_CUDA(c, cudaMemsetAsync(ex->cursor, 0, sizeof(u64), c->stream));
     const double est_pass = hist.empty() ? 0.0 : max_class(pbits);  // sizes the record pool of the binned passes
-    st = pt2_attempt(c, psi, e_s, eps2, pbits, slots, auto_slots && !ex, load, out, nullptr, ex, est_pass);
+    st = pt2_attempt(c, psi, e_s, eps2, pbits, slots, auto_slots && !ex, load, out, nullptr, ex, est_pass, force_binned);
     if (st == DH_OK) c->ctr.pt2_probe_parts = probe_parts;
     if (st != DH_ETABLEFULL || !auto_parts || pbits >= DH_MAX_PBITS) return st;
     ++pbits;  // the plan was too optimistic: halve the keys per pass and start over
     if (auto_slots) slots = max_slots;
+    force_binned = false;
   }
 }
 
