@@ -93,7 +93,7 @@ typedef struct {
                                reading Q11); 0 = 1e-3, negative = never */
   int32_t stream_bins;      /* streamed: key regions per pass (<= 4096); 0 = planned so that a region's distinct keys fit its table */
   int32_t table_regions;    /* table organisation, binned passes (contributions appended per table region, then merged region by
-                               region so that the probes stay in L2): 0 = when the table exceeds 32 GB, with at most 2048 regions;
+                               region so that the probes stay in L2): 0 = when the table exceeds 8 GB (and the record pool fits), with at most 2048 regions;
                                > 0 = always, with at most that many regions (64..8192); -1 = never */
   double stream_ring_mb;    /* streamed: bytes of the three region tables together (they must stay in L2); 0 = 96 */
   double stream_load;       /* streamed: target load factor of a region table; 0 = 0.45 */

@@ -14,6 +14,10 @@ namespace {
 
 constexpr int kWarpsPerCta = 8;
 constexpr int kFine = 1 << DH_MAX_PBITS;  // finest class histogram
+// Tables beyond this size run region-binned passes (if the record pool fits).  Round 1 put the line at 32 GB (H2O-shaped, 15 GB:
+// binned 17.5 ms against 12.8 ms direct); with this round's append it is lower: H2O-shaped 11.5 ms binned against 13.7 ms direct,
+// N2-shaped sweep 1e4 (18.5 GB) 17.3 against 23.0 ms.  Below ~8 GB nothing was measured, and a table that small is half L2-resident.
+constexpr int64_t kBinnedTableBytes = 8ll << 30;
 
 // Slot (pt2_common.cuh): one 32-byte sector per external.  Members of S are pre-inserted with v = NaN.
 
@@ -738,13 +742,13 @@ static dh_status pt2_attempt(detham_ctx* c, const double* psi, double e_s, doubl
   const int warps = 32;
   int64_t want = (nd + warps - 1) / warps;
   const int grid = (int)(want < (int64_t)c->sm_count ? want : (int64_t)c->sm_count);
-  // binned passes: table beyond 32 GB, an estimate to size the record pool with, every SM busy, not expand / probe
+  // binned passes: table beyond kBinnedTableBytes, an estimate to size the record pool with, every SM busy, not expand / probe
   // (measured, round 1: H2O-shaped, 15 GB table, 5 contributions per external: 17.5 ms binned against 12.8 ms direct; N2-shaped,
   // 60 GB: 143 against 152 ms; Cr2-shaped: 5.9 against 7.4 s).  opt.table_regions: -1 never, > 0 always, with that many regions
   // at most (the region size is a power of two of slots; 2048 was the best of a sweep on Cr2-shaped).
   const int max_bins = c->opt.table_regions > 0 ? c->opt.table_regions : 2048;
   bool binned = !ex && !pilot && est_pass > 0.0 && grid == c->sm_count && c->opt.table_regions >= 0 &&
-                (c->opt.table_regions > 0 || force_binned || slots * (int64_t)sizeof(Slot) > (32ll << 30));
+                (c->opt.table_regions > 0 || force_binned || slots * (int64_t)sizeof(Slot) > kBinnedTableBytes);
   unsigned* pool_used = nullptr;
   if (binned) {
     // the pool holds the records of one pass: 20 % head room over the estimate (an upper bound already) plus 64 records per
@@ -1005,12 +1009,12 @@ static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double ep
         while (pb2 < pbits && uniq_class(pb2) > load * (double)max_slots) ++pb2;
         pbits = pb2;
         int64_t need = (int64_t)(uniq_class(pbits) / load);
-        // beyond 32 GB the passes run binned and the probes stay in L2, where longer chains cost little while every slot less is 64
+        // beyond that size the passes run binned and the probes stay in L2, where longer chains cost little while every slot less is 64
         // bytes of DRAM traffic less per pass (fetch + scan): measured on Cr2-shaped, load 0.5 / 0.6 / 0.7 / 0.8: accumulate 5999 /
         // 6004 / 6202 / 6527 ms, scan 810 / 679 / 591 / 534 ms
-        if (opt.table_load <= 0.0 && opt.table_regions >= 0 && need * (int64_t)sizeof(Slot) > (32ll << 30)) {
+        if (opt.table_load <= 0.0 && opt.table_regions >= 0 && need * (int64_t)sizeof(Slot) > kBinnedTableBytes) {
           const int64_t denser = (int64_t)(uniq_class(pbits) / 0.6);
-          if (denser * (int64_t)sizeof(Slot) > (32ll << 30)) need = denser;
+          if (denser * (int64_t)sizeof(Slot) > kBinnedTableBytes) need = denser;
         }
         slots = need < max_slots ? need : max_slots;
         if (slots < 1024) slots = 1024;
@@ -1049,12 +1053,12 @@ static dh_status pt2_run(detham_ctx* c, const double* psi, double e_s, double ep
     if (opt.mode == 2) return st;  // asked for explicitly: report instead of switching organisation
     if (c->pool) { cudaFree(c->pool); c->pool = nullptr; c->pool_bytes = 0; }  // make room for the table
   }
-  // A plan whose table is beyond 32 GB runs binned passes if the record pool of a pass fits beside the table.  Where it does not
+  // A plan whose table is beyond kBinnedTableBytes runs binned passes if the record pool of a pass fits beside the table.  Where it does not
   // (many contributions per external: the large N2-shaped sweep points, 9 per external, 4 passes of 6e9 records), more passes of
   // fewer records do, with a smaller table each: measured 20.5-21 G contributions/s binned against 18-19 G/s direct.
   bool force_binned = false;
   if (auto_parts && auto_slots && !ex && !hist.empty() && pilot_distinct > 0.0 && opt.table_regions == 0 &&
-      slots * (int64_t)sizeof(Slot) > (32ll << 30)) {
+      slots * (int64_t)sizeof(Slot) > kBinnedTableBytes) {
     size_t free_b = 0, total_b = 0;
     DH_CUDA(c, cudaMemGetInfo(&free_b, &total_b));
     const double avail = 0.9 * ((double)free_b + (double)c->table_slots * sizeof(Slot) + (double)c->pool_bytes);

@@ -452,7 +452,7 @@ def test_pt2_streamed_organisation(pkg, orc):
     check(o, psi, 2, mode="stream")
     check(o, psi, 0, mode="table")
     check(o, psi, 0)  # the planner keeps a 1 GB table in HBM and probes it directly
-    # binned passes of the table organisation (chosen by the planner beyond 32 GB): forced, with the default record pool, a pool
+    # binned passes of the table organisation (chosen by the planner beyond 8 GB): forced, with the default record pool, a pool
     # too small for most records (the overflow is probed directly, the rest goes through the merge), 16 passes, masked psi
     c = check(o, psi, 1, table_regions=64)
     check(o, psi, 1, table_regions=2048, stream_pool_frac=0.05)
