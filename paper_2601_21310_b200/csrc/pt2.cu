@@ -16,7 +16,8 @@ constexpr int kWarpsPerCta = 8;
 constexpr int kFine = 1 << DH_MAX_PBITS;  // finest class histogram
 // Tables beyond this size run region-binned passes (if the record pool fits).  Round 1 put the line at 32 GB (H2O-shaped, 15 GB:
 // binned 17.5 ms against 12.8 ms direct); with this round's append it is lower: H2O-shaped 11.5 ms binned against 13.7 ms direct,
-// N2-shaped sweep 1e4 (18.5 GB) 17.3 against 23.0 ms.  Below ~8 GB nothing was measured, and a table that small is half L2-resident.
+// N2-shaped sweep 1e4 (18.5 GB) 17.3 against 23.0 ms; H2O-shaped prefixes with 9.3 / 6.2 / 3.9 GB tables 7.0 / 5.0 / 3.4 ms against
+// 8.5 / 6.2 / 4.5 ms.  The line stays at 8 GB, below every table of the BASELINE configurations that is not L2-sized.
 constexpr int64_t kBinnedTableBytes = 8ll << 30;
 
 // Slot (pt2_common.cuh): one 32-byte sector per external.  Members of S are pre-inserted with v = NaN.
